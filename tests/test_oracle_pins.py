@@ -1,0 +1,487 @@
+"""Pins of the oracle (oracle/ctr_oracle.c) to things OTHER than itself: closed forms,
+brute force written independently in numpy here, textbook/library routines, invariants
+and a hand-evaluated example (tests/golden/a2_a3_4x4.json).  CPU only.
+Citations: PAPER.md lines; O*/S* = readings in DESIGN.md."""
+import json
+import math
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+from ctr_inputs import (Ellipse, analytic_sinogram, get_config, make_case, make_phantom,
+                        rasterize, ray_endpoints, scaled_config)
+from ctr_inputs.configs import Config
+
+GOLD = Path(__file__).resolve().parent / "golden"
+
+
+def tiny2d(**kw):
+    base = dict(name="t2", index=90, ndim=2, nx=8, ny=8, nz=1, dx=1.5, dy=1.5, dz=1.0,
+                nviews=12, nu=12, nv=1, du=2.0, dv=1.0, dso=541.0, dsd=949.0)
+    base.update(kw)
+    return Config(**base)
+
+
+def tiny3d(**kw):
+    base = dict(name="t3", index=91, ndim=3, nx=5, ny=4, nz=3, dx=1.5, dy=1.25, dz=2.0,
+                nviews=7, nu=6, nv=5, du=2.5, dv=3.0, dso=100.0, dsd=160.0)
+    base.update(kw)
+    return Config(**base)
+
+
+# ---------------------------------------------------------------- independent brute force
+def box_chords(cfg, lo, hi):
+    """Length of every source->bin segment inside the axis-aligned box [lo,hi] (slab clip)."""
+    out = np.zeros((cfg.nviews, cfg.nv, cfg.nu))
+    for k in range(cfg.nviews):
+        S, D = ray_endpoints(cfg, k)
+        d = D - S
+        amin = np.zeros(d.shape[:-1])
+        amax = np.ones(d.shape[:-1])
+        for ax in range(3):
+            with np.errstate(divide="ignore", invalid="ignore"):
+                a1 = (lo[ax] - S[ax]) / d[..., ax]
+                a2 = (hi[ax] - S[ax]) / d[..., ax]
+            par = d[..., ax] == 0
+            inside = (S[ax] >= lo[ax]) & (S[ax] < hi[ax])
+            en = np.where(par, -np.inf if inside else np.inf, np.minimum(a1, a2))
+            ex = np.where(par, np.inf if inside else -np.inf, np.maximum(a1, a2))
+            amin = np.maximum(amin, en)
+            amax = np.minimum(amax, ex)
+        out[k] = np.maximum(amax - amin, 0.0) * np.linalg.norm(d, axis=-1)
+    return out
+
+
+def image_box(cfg):
+    lo = np.array([cfg.cx - cfg.nx * cfg.dx / 2, cfg.cy - cfg.ny * cfg.dy / 2, cfg.cz - cfg.nz * cfg.dz / 2])
+    hi = lo + np.array([cfg.nx * cfg.dx, cfg.ny * cfg.dy, cfg.nz * cfg.dz])
+    return lo, hi
+
+
+def brute_matrix(cfg):
+    """Dense A[ray, voxel] = |ray ∩ voxel box| for every pair, no traversal."""
+    lo, _ = image_box(cfg)
+    A = np.zeros((cfg.nviews * cfg.nv * cfg.nu, cfg.nz * cfg.ny * cfg.nx))
+    for k in range(cfg.nz):
+        for j in range(cfg.ny):
+            for i in range(cfg.nx):
+                vlo = lo + np.array([i * cfg.dx, j * cfg.dy, k * cfg.dz])
+                vhi = vlo + np.array([cfg.dx, cfg.dy, cfg.dz])
+                A[:, (k * cfg.ny + j) * cfg.nx + i] = box_chords(cfg, vlo, vhi).ravel()
+    return A
+
+
+# ---------------------------------------------------------------- O1/O2: P
+@pytest.mark.parametrize("name", ["c1", "c2"])
+def test_forward_of_ones_is_box_chord(orc, name):
+    """(i) P·1 = chord of each ray through the image box, closed form, to 1e-12."""
+    cfg = get_config(name)
+    got = orc.forward(cfg, np.ones((cfg.ny, cfg.nx)))
+    want = box_chords(cfg, *image_box(cfg))[:, 0, :]
+    assert np.max(np.abs(got - want)) <= 1e-12 * np.max(want)
+    assert want.max() > 0
+
+
+def test_forward_of_ones_3d(orc):
+    cfg = tiny3d()
+    got = orc.forward(cfg, np.ones((cfg.nz, cfg.ny, cfg.nx)))
+    want = box_chords(cfg, *image_box(cfg))
+    assert np.max(np.abs(got - want)) <= 1e-12 * np.max(want)
+
+
+@pytest.mark.parametrize("cfg", [tiny2d(), tiny2d(nx=7, ny=5, dx=1.0, dy=2.0, cx=0.7, cy=-0.4, u_off=0.25),
+                                 tiny2d(nviews=8, nu=11, theta0=0.0)],
+                         ids=["8x8", "7x5-offcentre", "axis-parallel-central-ray"])
+def test_dense_matrix_2d(orc, cfg):
+    """(ii) every p_ij equals the brute-force ray∩pixel length; includes rays parallel to an
+    axis through pixel interiors (odd nu: the central ray at theta = 0, 90, ...)."""
+    A = orc.matrix(cfg)
+    B = brute_matrix(cfg)
+    assert A.shape == B.shape
+    assert np.max(np.abs(A - B)) <= 1e-11
+    assert (B > 0).sum() > 50
+
+
+def test_dense_matrix_3d(orc):
+    cfg = tiny3d()
+    A = orc.matrix(cfg)
+    B = brute_matrix(cfg)
+    assert np.max(np.abs(A - B)) <= 1e-11
+    rng = np.random.default_rng(3)
+    x = rng.random((cfg.nz, cfg.ny, cfg.nx))
+    y = rng.random((cfg.nviews, cfg.nv, cfg.nu))
+    assert np.allclose(orc.forward(cfg, x).ravel(), B @ x.ravel(), rtol=0, atol=1e-11)
+    assert np.allclose(orc.back(cfg, y).ravel(), B.T @ y.ravel(), rtol=0, atol=1e-11)
+
+
+def test_forward_back_equal_dense_matrix_products(orc):
+    cfg = tiny2d()
+    B = brute_matrix(cfg)
+    rng = np.random.default_rng(1)
+    x = rng.standard_normal((cfg.ny, cfg.nx))
+    y = rng.standard_normal((cfg.nviews, cfg.nu))
+    assert np.allclose(orc.forward(cfg, x).ravel(), B @ x.ravel(), rtol=0, atol=1e-11)
+    assert np.allclose(orc.back(cfg, y).ravel(), B.T @ y.ravel(), rtol=0, atol=1e-11)
+
+
+def test_disk_chord_closed_form(orc):
+    """(iii) uniform disk: P(raster) -> 2 rho sqrt(r^2 - d^2) with ~O(h) discretisation error."""
+    errs = []
+    for n, h in [(64, 1.5), (128, 0.75), (256, 0.375)]:
+        cfg = scaled_config("c1", nx=n, ny=n, dx=h, dy=h)
+        r, rho = 30.0, 0.02
+        disk = [Ellipse(3.0, -2.0, 0, r, r, math.inf, 0.0, rho)]
+        img = rasterize(cfg, disk, supersample=8)[0]
+        got = orc.forward(cfg, img)
+        # closed form written out here (not via ctr_inputs): distance of the disk centre to each ray
+        want = np.zeros_like(got)
+        for k in range(cfg.nviews):
+            S, D = ray_endpoints(cfg, k)
+            u = (D[0] - S)[:, :2]
+            u /= np.linalg.norm(u, axis=1, keepdims=True)
+            c = np.array([3.0, -2.0]) - S[:2]
+            dist = np.abs(c[0] * u[:, 1] - c[1] * u[:, 0])
+            want[k] = 2 * rho * np.sqrt(np.maximum(r * r - dist * dist, 0))
+        errs.append(np.linalg.norm(got - want) / np.linalg.norm(want))
+    assert errs[0] < 0.02
+    assert errs[1] < 0.6 * errs[0] and errs[2] < 0.6 * errs[1]
+
+
+@pytest.mark.parametrize("name,tol", [("c1", 0.03), ("c2", 0.008), ("c3", 0.005)])
+def test_ellipse_phantom_analytic(orc, name, tol):
+    """(iii) P(raster of the seeded phantom) vs analytic ellipse line integrals."""
+    cfg = get_config(name)
+    d = make_case(cfg, noisy=False)
+    got = orc.forward(cfg, d["truth"][0].astype(np.float64))
+    want = d["sino"][0].astype(np.float64)
+    assert np.linalg.norm(got - want) / np.linalg.norm(want) < tol
+
+
+def test_rotation_symmetry(orc):
+    """(iv) rotating the image by 90 deg equals shifting the views by nviews/4."""
+    cfg = scaled_config("c1", nviews=32)
+    rng = np.random.default_rng(5)
+    x = rng.random((cfg.ny, cfg.nx))
+    s0 = orc.forward(cfg, x)
+    # rotate the object by +90 deg: new[j][i] = old at (x,y) -> (y,-x)
+    xr = np.rot90(x, k=1)  # counter-clockwise in (row=j=y up, col=i=x) with y increasing by row
+    s1 = orc.forward(cfg, xr)
+    a = np.linalg.norm(s1 - np.roll(s0, cfg.nviews // 4, axis=0))
+    b = np.linalg.norm(s1 - np.roll(s0, -cfg.nviews // 4, axis=0))
+    # dtheta is an fp32 value, so 8*dtheta misses pi/2 by ~1e-8 rad: tolerance 2e-6, not 1e-12
+    assert min(a, b) <= 2e-6 * np.linalg.norm(s0)
+    assert max(a, b) > 1e-3 * np.linalg.norm(s0)
+
+
+def test_arc_detector_directions(orc):
+    """ARC: bin a looks along angle theta + t_a/dsd at distance dsd."""
+    cfg = tiny2d(det_type=1, nu=9, du=1.0239, dsd=949.075)
+    for k in (0, 3, 7):
+        th = cfg.theta0 + cfg.dtheta * k
+        for a in (0, 4, 8):
+            S, D = orc.ray(cfg, k, 0, a)
+            d = D - S
+            beta = (a - 4.0) * float(np.float32(1.0239)) / float(np.float32(949.075))
+            assert abs(np.linalg.norm(d) - float(np.float32(949.075))) < 1e-9
+            assert abs(math.atan2(d[1], d[0]) - math.atan2(math.sin(th + beta), math.cos(th + beta))) < 1e-12
+    A = orc.matrix(cfg)
+    B = brute_matrix(cfg)
+    assert np.max(np.abs(A - B)) <= 1e-11
+
+
+# ---------------------------------------------------------------- O3: P^T
+@pytest.mark.parametrize("name", ["c1", "c2"])
+def test_adjoint_identity(orc, name):
+    """PAPER.md:471 (A3'): <f, P^T y> = <P f, y>; exact transpose -> 1e-12."""
+    cfg = get_config(name)
+    rng = np.random.default_rng(7)
+    x = rng.standard_normal((cfg.ny, cfg.nx))
+    y = rng.standard_normal((cfg.nviews, cfg.nu))
+    px, pty = orc.forward(cfg, x), orc.back(cfg, y)
+    assert abs((px * y).sum() - (x * pty).sum()) <= 1e-12 * np.linalg.norm(px) * np.linalg.norm(y)
+
+
+# ---------------------------------------------------------------- O4: CGLS
+def test_cgls_converges_to_dense_least_squares(orc):
+    """CGLS from x0 = 0 -> the min-norm least-squares solution (textbook)."""
+    cfg = tiny2d()
+    A = brute_matrix(cfg)
+    rng = np.random.default_rng(11)
+    b = A @ rng.random(cfg.nx * cfg.ny) + 0.01 * rng.standard_normal(A.shape[0])
+    x_ls = np.linalg.lstsq(A, b, rcond=None)[0]
+    x = orc.cgls(cfg, b.reshape(cfg.nviews, cfg.nu), np.zeros((cfg.ny, cfg.nx)), 400).ravel()
+    assert np.linalg.norm(A @ x - A @ x_ls) <= 1e-8 * np.linalg.norm(b)
+    assert np.linalg.norm(x - x_ls) <= 1e-6 * np.linalg.norm(x_ls)
+
+
+def test_cgls_first_iterate_and_monotone_residual(orc):
+    cfg = tiny2d()
+    A = brute_matrix(cfg)
+    rng = np.random.default_rng(12)
+    b = rng.random(A.shape[0])
+    x0 = rng.random(A.shape[1])
+    r0 = b - A @ x0
+    s0 = A.T @ r0
+    x1_hand = x0 + (s0 @ s0) / ((A @ s0) @ (A @ s0)) * s0            # App. I steps 1-2, m = 0
+    x1 = orc.cgls(cfg, b.reshape(cfg.nviews, cfg.nu), x0.reshape(cfg.ny, cfg.nx), 1).ravel()
+    assert np.allclose(x1, x1_hand, rtol=0, atol=1e-12)
+    # two iterations against the recurrence typed from App. I (:423-435)
+    a0 = (s0 @ s0) / ((A @ s0) @ (A @ s0))
+    r1 = r0 - a0 * (A @ s0)
+    g1 = A.T @ r1
+    s1 = g1 + (g1 @ g1) / (s0 @ s0) * s0
+    x2_hand = x1_hand + (g1 @ g1) / ((A @ s1) @ (A @ s1)) * s1
+    x2 = orc.cgls(cfg, b.reshape(cfg.nviews, cfg.nu), x0.reshape(cfg.ny, cfg.nx), 2).ravel()
+    assert np.allclose(x2, x2_hand, rtol=0, atol=1e-12)
+    res = [np.linalg.norm(b - A @ orc.cgls(cfg, b.reshape(cfg.nviews, cfg.nu),
+                                           x0.reshape(cfg.ny, cfg.nx), m).ravel()) for m in range(0, 12)]
+    assert all(res[m + 1] <= res[m] * (1 + 1e-12) for m in range(11))
+    # n_iter = 0 is the identity
+    assert np.array_equal(orc.cgls(cfg, b.reshape(cfg.nviews, cfg.nu), x0.reshape(cfg.ny, cfg.nx), 0).ravel(), x0)
+
+
+# ---------------------------------------------------------------- O5-O8: A2 / A3
+def test_hand_evaluated_4x4(orc):
+    gold = json.loads((GOLD / "a2_a3_4x4.json").read_text())
+    f = np.array(gold["image_rows_j_then_cols_i"], dtype=np.float64)
+    n0 = orc.face_mag2(f)                                   # [axis, 0, j, i]
+    for key, val in gold["n0sq"].items():
+        ax, i, j = key.split("_")
+        assert n0[0 if ax == "x" else 1, 0, int(j), int(i)] == pytest.approx(val, abs=1e-13)
+    ones = (n0 > -1).astype(np.float64)
+    g_tv = orc.gradient(f, f, orc.weights(n0, 1.0, mode=1), lam=0.0, eps=0.0)
+    assert g_tv[0, 1, 1] == pytest.approx(gold["a2_tv_at_1_1"], abs=5e-8)
+    w = orc.weights(n0, gold["sigma"], mode=0)
+    for key, val in gold["omega"].items():
+        ax, i, j = key.split("_")
+        assert w[0 if ax == "x" else 1, 0, int(j), int(i)] == pytest.approx(val, abs=5e-9)
+    g_ep = orc.gradient(f, f, w, lam=0.0, eps=0.0)
+    assert g_ep[0, 1, 1] == pytest.approx(gold["a2_eptv_at_1_1"], abs=5e-8)
+    assert ones.all()
+
+
+def test_constant_image_invariants(orc):
+    """north_star invariant: zero TV and unit weights on a constant image (S12)."""
+    for shape, ndim in (((1, 9, 7), 2), ((4, 5, 6), 3)):
+        f = np.full(shape, 0.37)
+        n0 = orc.face_mag2(f, ndim)
+        assert np.all(n0 == 0)
+        w, sig = orc.update_weights(f, 0.9, 1e-6, 0, ndim)
+        assert sig == pytest.approx(float(np.float32(1e-6)))
+        interior = np.ones_like(w, dtype=bool)
+        interior[0, :, :, -1] = False
+        interior[1, :, -1, :] = False
+        if ndim == 3:
+            interior[2, -1, :, :] = False
+        assert np.all(w[interior] == 1.0) and np.all(w[~interior] == 0.0)
+        assert np.all(orc.gradient(f, f, w, 0.02, 1e-6, ndim) == 0)
+        assert orc.energy(f, f, w, 0.02, 1e-6, ndim) == 0.0
+
+
+def test_ramp_has_zero_interior_tv_gradient(orc):
+    j, i = np.mgrid[0:10, 0:12]
+    f = (0.3 * i - 0.2 * j + 1.0)[None]
+    w = np.ones((2,) + f.shape)
+    w[0, :, :, -1] = 0
+    w[1, :, -1, :] = 0
+    g = orc.gradient(f, f, w, 0.0, 0.0)
+    assert np.max(np.abs(g[0, 2:-2, 2:-2])) < 1e-12
+    # on a ramp every interior face magnitude is the Euclidean gradient norm (isotropy, S5)
+    n0 = orc.face_mag2(f)
+    assert np.allclose(n0[0, 0, 2:-2, 2:-2], 0.3 ** 2 + 0.2 ** 2)
+    assert np.allclose(n0[1, 0, 2:-2, 2:-2], 0.3 ** 2 + 0.2 ** 2)
+
+
+def test_one_dimensional_reduction_to_textbook_tv(orc):
+    """With a single row the transverse terms of A3 vanish: N0 = |f_{i+1}-f_i|, J = sum|diff|
+    and (omega = 1) A2 = -(sign(d_i) - sign(d_{i-1})): the textbook 1D TV subgradient."""
+    rng = np.random.default_rng(2)
+    f = rng.standard_normal((1, 1, 40))
+    n0 = orc.face_mag2(f)
+    assert np.allclose(n0[0, 0, 0, :-1], np.diff(f[0, 0]) ** 2, atol=1e-15)
+    assert np.all(n0[1] == 0)
+    w = orc.weights(n0, 1.0, mode=1)
+    # energy: (1/ndim) * sum |d|   (O9, eps = 0)
+    assert orc.energy(f, f, w, 0.0, 0.0) == pytest.approx(np.abs(np.diff(f[0, 0])).sum() / 2, rel=1e-14)
+    sgn = np.sign(np.diff(f[0, 0]))
+    want = -(np.concatenate([sgn, [0]]) - np.concatenate([[0], sgn]))
+    assert np.allclose(orc.gradient(f, f, w, 0.0, 0.0)[0, 0], want, atol=1e-12)
+
+
+def test_gradient_matches_energy_derivative_in_1d(orc):
+    """In 1D A2 IS the derivative of the discrete energy (times ndim, as E carries 1/ndim):
+    central differences of orc_energy pin the sign and indexing of A2 and of lambda(f-v)."""
+    rng = np.random.default_rng(4)
+    f = rng.standard_normal((1, 1, 16))
+    v = rng.standard_normal((1, 1, 16))
+    n0 = orc.face_mag2(f)
+    w = orc.weights(n0, 1.3, mode=0)
+    eps, lam = 0.05, 0.7
+    g = orc.gradient(f, v, w, lam, eps)[0, 0]
+    g_fid = np.float32(lam) * (f - v)[0, 0]
+    h = 1e-6
+    for i in range(16):
+        e = np.zeros_like(f)
+        e[0, 0, i] = h
+        dE_tv = (orc.energy(f + e, v, w, 0.0, eps) - orc.energy(f - e, v, w, 0.0, eps)) / (2 * h)
+        dE_fid = (orc.energy(f + e, v, 0 * w, lam, eps) - orc.energy(f - e, v, 0 * w, lam, eps)) / (2 * h)
+        assert g[i] - g_fid[i] == pytest.approx(2 * dE_tv, abs=1e-6)
+        assert g_fid[i] == pytest.approx(dE_fid, abs=1e-6)
+
+
+def test_flip_and_transpose_equivariance(orc):
+    rng = np.random.default_rng(6)
+    f = rng.random((1, 9, 11))
+    v = rng.random((1, 9, 11))
+    w, sig = orc.update_weights(f, 0.9)
+    g = orc.gradient(f, v, w, 0.3)
+    # left-right flip
+    wf, sf = orc.update_weights(f[:, :, ::-1], 0.9)
+    assert sf == pytest.approx(sig, rel=1e-14)
+    assert np.allclose(orc.gradient(f[:, :, ::-1], v[:, :, ::-1], wf, 0.3), g[:, :, ::-1], atol=1e-13)
+    # transpose swaps the roles of the x- and y-face planes
+    ft, vt = f.transpose(0, 2, 1), v.transpose(0, 2, 1)
+    wt, st = orc.update_weights(ft, 0.9)
+    assert st == pytest.approx(sig, rel=1e-14)
+    assert np.allclose(wt[0], w[1].transpose(0, 2, 1), atol=1e-14)
+    assert np.allclose(orc.gradient(ft, vt, wt, 0.3), g.transpose(0, 2, 1), atol=1e-13)
+
+
+def test_tv_is_eptv_with_unit_weights_and_eptv_le_tv(orc):
+    """TV = EPTV with w = 1, and w < 1 => ||f||_EPTV <= ||f||_TV."""
+    rng = np.random.default_rng(8)
+    f = rng.random((1, 12, 12))
+    w_tv, _ = orc.update_weights(f, 0.9, mode=1)
+    w_ep, sig = orc.update_weights(f, 0.9, mode=0)
+    interior = np.ones_like(w_tv, dtype=bool)
+    interior[0, :, :, -1] = False
+    interior[1, :, -1, :] = False
+    assert np.all(w_tv[interior] == 1.0)
+    assert np.all((w_ep[interior] > 0) & (w_ep[interior] <= 1.0))
+    assert orc.energy(f, f, w_ep, 0.0) <= orc.energy(f, f, w_tv, 0.0)
+    n0 = orc.face_mag2(f)
+    assert np.allclose(w_ep[interior], np.exp(-n0[interior] / sig ** 2), rtol=1e-14)
+
+
+def test_face_mag2_3d_against_direct_numpy(orc):
+    """3D generalisation (S22) of A3, written out with numpy edge padding."""
+    rng = np.random.default_rng(9)
+    f = rng.random((4, 5, 6))
+    n0 = orc.face_mag2(f, 3)
+    fp = np.pad(f, 1, mode="edge")
+    # x-faces: m = mean of the two voxels along x; transverse axes y (axis 1) and z (axis 0)
+    m = 0.5 * (fp[:, :, 1:] + fp[:, :, :-1])          # [nz+2, ny+2, nx+1], face i between i-1+1.. (padded)
+    mx = m[:, :, 1:-1]                                 # faces between voxel i and i+1, i = 0..nx-2
+    d = f[:, :, 1:] - f[:, :, :-1]
+    want = d ** 2
+    for axis in (0, 1):
+        c = mx[1:-1, 1:-1]
+        up = np.take(mx, range(2, mx.shape[axis]), axis=axis)
+        dn = np.take(mx, range(0, mx.shape[axis] - 2), axis=axis)
+        other = 1 - axis
+        up = np.take(up, range(1, up.shape[other] - 1), axis=other)
+        dn = np.take(dn, range(1, dn.shape[other] - 1), axis=other)
+        want = want + 0.5 * (up - c) ** 2 + 0.5 * (c - dn) ** 2
+    assert np.allclose(n0[0, :, :, :-1], want, atol=1e-14)
+    assert np.all(n0[0, :, :, -1] == 0)
+
+
+# ---------------------------------------------------------------- O6: sigma
+@pytest.mark.parametrize("q", [0.5, 0.9, 0.95, 1.0, 1e-9])
+def test_sigma_is_order_statistic(orc, q):
+    rng = np.random.default_rng(10)
+    f = rng.random((1, 13, 17))
+    n0 = orc.face_mag2(f)
+    S = np.sqrt(np.concatenate([n0[0, 0, :, :-1].ravel(), n0[1, 0, :-1, :].ravel()]))
+    assert len(S) == 12 * 17 + 13 * 16
+    k = min(max(math.ceil(float(np.float32(q)) * len(S)), 1), len(S))
+    assert orc.sigma(n0, q, 1e-6) == np.sort(S)[k - 1]
+    assert orc.sigma(n0, q, 10.0) == 10.0  # floor at eps
+
+
+# ---------------------------------------------------------------- O9: Armijo sweep
+def test_armijo_accepts_first_sufficient_decrease(orc):
+    rng = np.random.default_rng(13)
+    v = 0.02 + 0.004 * rng.standard_normal((1, 24, 24))
+    f = v.copy()
+    p = dict(armijo_t0=1e-3, armijo_rho=0.5, armijo_c=1e-4, armijo_max=16, eps=1e-6)
+    lam = 0.02
+    E_prev = None
+    ks = []
+    for sweep in range(6):
+        w, sig = orc.update_weights(f, 0.9)
+        g = orc.gradient(f, v, w, lam)
+        f_new, k, E0, G, t = orc.eptv_step(f, v, w, lam, p)
+        assert G == pytest.approx((g ** 2).sum(), rel=1e-13)
+        assert E0 == pytest.approx(orc.energy(f, v, w, lam), rel=1e-13)
+        assert k >= 0
+        t0, rho, c = (float(np.float32(p[x])) for x in ("armijo_t0", "armijo_rho", "armijo_c"))
+        assert t == pytest.approx(t0 * rho ** k)
+        assert np.allclose(f_new, f - t * g, atol=1e-18)
+        E1 = orc.energy(f_new, v, w, lam)
+        assert E1 <= E0 - c * t * G                                   # the inequality holds at t
+        for kk in range(k):                                           # and fails at every larger t
+            tt = t0 * rho ** kk
+            assert orc.energy(f - tt * g, v, w, lam) > E0 - c * tt * G
+        assert E1 <= E0                                               # monotone within the sweep (S17)
+        ks.append(k)
+        f = f_new
+
+
+def test_armijo_rejects_everything_leaves_f_unchanged(orc):
+    rng = np.random.default_rng(14)
+    v = rng.random((1, 10, 10))
+    f = v + 0.1 * rng.standard_normal(v.shape)
+    w, _ = orc.update_weights(f, 0.9)
+    # a huge first step and only one trial: cannot decrease the energy
+    f_new, k, E0, G, t = orc.eptv_step(f, v, w, 0.02, dict(armijo_t0=1e3, armijo_max=1))
+    assert k == -1 and t == 0.0
+    assert np.array_equal(f_new, f)
+
+
+# ---------------------------------------------------------------- O10: outer loop
+def test_reconstruct_positivity_and_restarted_cgls(orc):
+    cfg = tiny2d()
+    A = brute_matrix(cfg)
+    rng = np.random.default_rng(15)
+    x_true = rng.random(cfg.nx * cfg.ny)
+    b = (A @ x_true).reshape(cfg.nviews, cfg.nu)
+    # n_gd = 0, no clamp: the outer loop is restarted CGLS (S1): identical to chaining orc.cgls,
+    # and it drives the (consistent) system's residual towards the dense least-squares one (= 0)
+    f, w, log = orc.reconstruct(cfg, b, dict(n_outer=30, n_cgls=20, n_gd=0, positivity=0))
+    u = np.zeros((cfg.ny, cfg.nx))
+    res = []
+    for it in range(30):
+        u = orc.cgls(cfg, b, u, 20)
+        res.append(np.linalg.norm(A @ u.ravel() - b.ravel()))
+    assert np.array_equal(f, u)
+    x_ls = np.linalg.lstsq(A, b.ravel(), rcond=None)[0]
+    assert np.linalg.norm(A @ x_ls - b.ravel()) <= 1e-9 * np.linalg.norm(b)
+    assert all(res[i + 1] <= res[i] for i in range(29))
+    assert res[-1] <= 5e-4 * np.linalg.norm(b)
+    # one outer iteration by composition of the pinned parts
+    p = dict(n_outer=1, n_cgls=4, n_gd=3, lam=0.05, positivity=1)
+    f1, w1, log1 = orc.reconstruct(cfg, b - 0.3, p)
+    u = orc.cgls(cfg, b - 0.3, np.zeros((cfg.ny, cfg.nx)), 4)
+    fm = u.copy()
+    for s in range(3):
+        ww, sig = orc.update_weights(fm, 0.9)
+        fm3, k, E0, G, t = orc.eptv_step(fm, u, ww, 0.05, p)
+        assert log1[s, 0] == sig and log1[s, 1] == k and log1[s, 2] == E0
+        fm = fm3[0]
+    assert np.array_equal(f1, np.maximum(fm, 0.0))
+    assert f1.min() >= 0.0 and (fm < 0).any()
+    assert np.array_equal(w1, ww[:, 0])
+
+
+def test_reconstruct_c1_reduces_error_and_stays_positive(orc):
+    """Sanity on the seeded c1 workload: positivity after every outer iteration
+    and a reconstruction closer to the truth than the zero image."""
+    cfg = scaled_config("c1", n_outer=3)
+    d = make_case(cfg)
+    f, w, log = orc.reconstruct(cfg, d["sino"][0], cfg)
+    truth = d["truth"][0]
+    assert f.min() >= 0.0
+    assert np.linalg.norm(f - truth) < 0.5 * np.linalg.norm(truth)
+    assert np.all(log[:, 1] >= 0)
