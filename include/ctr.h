@@ -1,0 +1,150 @@
+/*
+ * ctr.h -- C ABI of libctr: the B200 (sm_100a) hot path of edge-preserving-TV CT
+ * reconstruction (Tian, Jia, Yuan, Pan, Jiang; citations are /root/reference/PAPER.md:<line>).
+ *
+ * The path:
+ *   P   ray-driven projector, p_ij = length of ray i inside pixel j      PAPER.md:85-89 (Eq. 1)
+ *   P^T exact transpose of that matrix, computed in gather form           PAPER.md:193, :471 (A3')
+ *   CGLS with warm start                                                  PAPER.md:149, :414-440 (App. I)
+ *   edge weights w = exp(-(|grad f|/sigma)^2), sigma from the histogram   PAPER.md:106-110 (Eq. 4-5)
+ *   EP-TV gradient, symmetric scheme A2/A3
+ *   Armijo line search along -g, positivity clamp, outer loop
+ *
+ * Conventions common to every call
+ * --------------------------------
+ * - All array arguments named d_* are DEVICE pointers to contiguous fp32, 16-byte aligned, owned by
+ *   the caller for the duration of the (asynchronous) call. Nothing is allocated on the hot path:
+ *   the handle owns the geometry tables and all scratch (sized at ctr_create for `batch`).
+ * - Layouts (x fastest):  image     2D: [batch][ny][nx]        3D: [nz][ny][nx]
+ *                         sinogram  2D: [batch][nviews][nu]    3D: [nviews][nv][nu]
+ *                         weights   [ndim][image]  plane A holds the face between voxel p and p+e_A
+ *                                   at p; border faces (last index along A) hold 0.
+ * - Batched 2D slices are independent problems: every scalar (CGLS a, b; sigma; Armijo k) is per slice.
+ * - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream). Calls only enqueue work
+ *   and return without synchronising, except ctr_create, ctr_destroy and ctr_get_stats.
+ * - Return value: CTR_OK (0) or a negative ctr_status. No exceptions, no exit(), nothing printed.
+ *   On error nothing has been enqueued unless the code is CTR_ECUDA.
+ * - A handle must not be used from two host threads at once (its scratch is shared by all calls).
+ */
+#ifndef CTR_H_
+#define CTR_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ctr_handle ctr_handle; /* opaque */
+
+typedef enum {
+  CTR_OK = 0,
+  CTR_EINVAL = -1, /* NULL / misaligned pointer, non-positive size, dsd <= dso, n_iter < 0, quantile not in (0,1] ... */
+  CTR_EGEOM = -2,  /* source or detector inside the image's circumscribed circle                                   */
+  CTR_ENOMEM = -3, /* device or host allocation failed                                                             */
+  CTR_ECUDA = -4,  /* a CUDA runtime call failed; text in ctr_last_error                                           */
+  CTR_EARCH = -5   /* current device is not compute capability 10.x (sm_100)                                       */
+} ctr_status;
+
+/* Scanner + grid. Geometry of PAPER.md:85-89, :217 and App. III A6 (:484): at view angle th_k the source
+ * sits at -dso (cos th_k, sin th_k, 0), the detector centre at (dsd-dso)(cos th_k, sin th_k, 0), the
+ * detector u-axis is (-sin th_k, cos th_k, 0), the v-axis is +z. Bin (a,b) is at
+ * t_a = (a-(nu-1)/2+u_off) du along u and v_b = (b-(nv-1)/2+v_off) dv along v (FLAT), or at fan angle
+ * t_a/dsd on a circle of radius dsd about the source (ARC, 2D only). Voxel (i,j,k) covers
+ * [X_i,X_i+dx) x [Y_j,Y_j+dy) x [Z_k,Z_k+dz), X_i = cx - nx dx/2 + i dx (likewise Y, Z). Lengths in mm. */
+typedef struct {
+  int32_t ndim;           /* 2 = fan-beam slice(s), 3 = circular cone beam                                      */
+  int32_t nx, ny, nz;     /* nz = 1 for 2D                                                                      */
+  float dx, dy, dz;       /* voxel size, mm (dz ignored in 2D)                                                   */
+  float cx, cy, cz;       /* grid centre minus isocentre, mm                                                     */
+  int32_t nviews;
+  float theta0, dtheta;   /* th_k = theta0 + k dtheta (radians), used when angles == NULL                        */
+  const float* angles;    /* optional HOST array [nviews] overriding theta0/dtheta; copied by ctr_create          */
+  int32_t nu, nv;         /* detector bins; nv = 1 for 2D                                                        */
+  float du, dv;           /* bin pitch, mm (ARC: arc length at radius dsd)                                       */
+  float u_off, v_off;     /* detector centre shift, in bins                                                      */
+  float dso, dsd;         /* source-isocentre and source-detector distances, mm                                  */
+  int32_t det_type;       /* 0 = FLAT, 1 = ARC                                                    */
+  int32_t batch;          /* independent 2D slices sharing this geometry (>= 1); must be 1 when ndim = 3          */
+} ctr_geometry;
+
+/* Iteration schedule and the constants the paper leaves open (readings S13, S14). */
+typedef struct {
+  int32_t n_outer, n_cgls, n_gd;  /* outer iterations; CGLS iterations per outer; GD sweeps per outer            */
+  float lambda;                   /* lambda of (P2), Eq. 8                                           */
+  float sigma_quantile;           /* q in (0,1]: sigma = q-quantile of the face gradient magnitudes */
+  float eps;                      /* |grad f| -> sqrt(N0^2 + eps^2) in A2's denominators and the energy           */
+  float armijo_t0, armijo_rho, armijo_c;
+  int32_t armijo_max;             /* trials t = t0 rho^k, k < armijo_max (<= 32)                                   */
+  int32_t weights_mode;           /* 0 = EP-TV (Eq. 4-5), 1 = plain TV, w = 1                        */
+  int32_t positivity;             /* 1: f <- max(f,0) after the last sweep of every outer iteration  */
+  int32_t warm_start;             /* 0: f^(0) = 0 as in the paper (:171); 1: ctr_reconstruct continues from d_img   */
+} ctr_params;
+
+/* One record per (GD sweep, slice), in execution order: what steered the iteration. */
+typedef struct {
+  double sigma;   /* O6                                   */
+  double e0;      /* energy before the sweep (O9)          */
+  double g2;      /* ||g||^2                               */
+  int32_t k;      /* accepted Armijo index, -1 = none      */
+  int32_t pad;
+} ctr_sweep_stat;
+
+/* Defaults: n_outer 1, n_cgls 10, n_gd 5, lambda 0.01, q 0.90, eps 1e-6, t0 1e-3, rho 0.5, c 1e-4,
+ * armijo_max 16, EP-TV, positivity on, warm_start off. */
+void ctr_default_params(ctr_params* p);
+
+/* Build a handle for `g` on the CURRENT CUDA device: validates the geometry, builds the ray table
+ * and allocates all scratch. Synchronous. *out is NULL on failure. */
+int ctr_create(const ctr_geometry* g, ctr_handle** out);
+/* Frees everything the handle owns (synchronises the device first). NULL is allowed. */
+void ctr_destroy(ctr_handle* h);
+
+/* a1: d_sino = P d_img. d_sino is overwritten; d_img is not modified. */
+int ctr_forward(ctr_handle* h, const float* d_img, float* d_sino, void* stream);
+/* a2: d_img = P^T d_sino, the exact transpose of ctr_forward's matrix (same p_ij, bit for bit), gather
+ * form, no atomics (PAPER.md:193 explains why not scatter). d_img is overwritten. */
+int ctr_back(ctr_handle* h, const float* d_sino, float* d_img, void* stream);
+/* a3: n_iter CGLS iterations on min ||P x - b||^2 from the start value in d_x;
+ * d_x is updated in place to u^(n_iter). n_iter = 0 is a no-op. Zero denominators stop the update (S4). */
+int ctr_cgls(ctr_handle* h, const float* d_b, float* d_x, int n_iter, void* stream);
+/* a4: d_w[ndim][image] = exp(-N0^2/sigma^2) with N0 the face magnitudes of A3 at d_x and
+ * sigma = max(k-th smallest N0, eps), k = ceil(quantile * #interior faces) per slice (exact order
+ * statistic). weights_mode = 1 writes 1 on interior faces. d_sigma (device, [batch]) may be NULL. */
+int ctr_update_weights(ctr_handle* h, const float* d_x, float* d_w, float quantile, float* d_sigma, void* stream);
+/* a5+a6: ONE gradient-descent sweep on lambda/2 ||x - v||^2 + sum w |grad x| with w frozen: gradient of
+ * Eq. 9 / A2, Armijo search (first k with E(x - t_k g) <= E(x) - c t_k ||g||^2), x <- x - t_k g in place
+ * (unchanged if no trial passes). eps and the Armijo constants come from ctr_set_params / the defaults. */
+int ctr_eptv_step(ctr_handle* h, float* d_x, const float* d_v, const float* d_w, float lambda, void* stream);
+/* a8: the whole EPTV algorithm: f = 0; n_outer x { v = CGLS(sino, x0 = f, n_cgls); f = v;
+ * n_gd x (weights, sweep); clamp }. d_img receives f. p = NULL uses the handle's current parameters.
+ * If d_w is not NULL it receives the weights of the last sweep ([ndim][image]). */
+int ctr_reconstruct(ctr_handle* h, const float* d_sino, float* d_img, const ctr_params* p, void* stream);
+int ctr_reconstruct_w(ctr_handle* h, const float* d_sino, float* d_img, float* d_w, const ctr_params* p, void* stream);
+
+/* Replace the handle's parameters (validated: CTR_EINVAL leaves them unchanged). */
+int ctr_set_params(ctr_handle* h, const ctr_params* p);
+/* Synchronises `the stream last used`, then copies up to n_records sweep records of the last
+ * ctr_reconstruct / ctr_eptv_step / ctr_update_weights sequence into HOST memory `buf`, ordered
+ * [sweep][slice]. Returns the number of records available (>= 0) or a negative status. */
+int ctr_get_stats(ctr_handle* h, ctr_sweep_stat* buf, size_t n_records);
+/* Device-side timing of the handle's own launches, by kind, with CUDA events recorded on the launching
+ * stream around every kernel (or short kernel sequence) while enabled. ctr_profile_enable(h, 1) clears
+ * the accumulators and starts recording (at most 32768 intervals; later ones are dropped);
+ * ctr_profile_enable(h, 0) stops. ctr_profile_read synchronises the last stream and returns, per kind,
+ * the summed milliseconds and the interval count in HOST arrays of length CTR_PROF_KINDS. */
+enum { CTR_PROF_FORWARD = 0, CTR_PROF_BACK = 1, CTR_PROF_VECTOR = 2, CTR_PROF_TV = 3, CTR_PROF_LAYOUT = 4, CTR_PROF_KINDS = 5 };
+int ctr_profile_enable(ctr_handle* h, int on);
+int ctr_profile_read(ctr_handle* h, double* ms_by_kind, long long* count_by_kind);
+/* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
+long long ctr_launch_count(const ctr_handle* h);
+
+const char* ctr_strerror(int status);
+/* Text of the last error on this handle ("" if none); valid until the next call on the handle. */
+const char* ctr_last_error(const ctr_handle* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CTR_H_ */

@@ -4,7 +4,7 @@
  * Plain, slow, fp64 CPU restatement of the EP-TV CT reconstruction hot path of
  * Tian, Jia, Yuan, Pan, Jiang, "GPU-based Low Dose CT Reconstruction via
  * Edge-preserving Total Variation Regularization",
- * following the readings O1..O10 / S1..S23 of SURVEY.md section 8(c) (restated in
+ * following the readings O1..O10 / S1..S23 of SURVEY.md section 8(c) and S24 (restated in
  * DESIGN.md).  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
  * --impl reference legs may load this.  It shares no code, header, table or
  * constant with paper_1009_2288_b200/csrc (the CUDA path) and neither includes
@@ -13,7 +13,8 @@
  * Every function cites the passage it follows as PAPER.md:<line>.
  * Pins (tests/test_oracle_pins.py): P against box chords, a brute-force dense
  * matrix and analytic ellipse integrals; P^T against the dense transpose and the
- * adjoint identity; CGLS against numpy.linalg.lstsq; A2/A3 against a hand-evaluated
+ * adjoint identity; CGLS against numpy.linalg.lstsq, hand iterations and the Krylov-subspace
+ * minimiser built without a CG recurrence; A2/A3 against a hand-evaluated
  * 4x4 example and invariants; sigma against a sort; Armijo against its inequality.
  * PARITY UNPINNED: A2 (orc_gradient) beyond those special cases -- it is a
  * definition, not a theorem -- and the composed orc_reconstruct result.
@@ -44,6 +45,7 @@ typedef struct {
   int n_outer, n_cgls, n_gd;
   double lambda, sigma_quantile, eps, armijo_t0, armijo_rho, armijo_c;
   int armijo_max, weights_mode, positivity;
+  int reorth; /* S24: 1 = CGLS with re-orthogonalised gradients (default), 0 = recurrence as printed */
 } orc_params;
 
 /* ------------------------------------------------------------------ O1 geometry
@@ -235,24 +237,42 @@ void orc_matrix_row(const orc_geom* g, int k, int b, int a, double* row /* [nz*n
 
 /* ------------------------------------------------------------------ O4 CGLS
  * PAPER.md:414-440 (Appendix I), steps 1-5, warm start u0 = f^(k), M = n_iter iterations
- * (reading S3); a zero denominator stops the iteration (reading S4).                      */
+ * (reading S3); a zero denominator stops the iteration (reading S4).
+ *
+ * reorth = 0: the five steps exactly as printed.
+ * reorth = 1 (reading S24, used by orc_reconstruct): the same five steps, and after each
+ * g = P^T r the components of g along the earlier gradients P^T r^(0..m) are removed (modified
+ * Gram-Schmidt). In exact arithmetic those components are zero -- the gradients of CG are
+ * mutually orthogonal (Hestenes & Stiefel 1952, the paper's reference for CGLS) --
+ * so both variants define the same iterate: the minimiser of ||P u - y|| over
+ * u0 + span{(P^T P)^i P^T r0, i < M}. In floating point the printed recurrence loses that
+ * orthogonality after the dominant singular direction has converged; from then on its result
+ * moves by ~1e-2 relative under a 1e-14 perturbation of y (fp64, M = 15, measured: DESIGN.md S24),
+ * i.e. it is not a usable reference. With the projection the result is reproducible to ~1e-11.   */
 static double dot(const double* a, const double* b, long n) {
   double s = 0.0;
   for (long i = 0; i < n; ++i) s += a[i] * b[i];
   return s;
 }
 
-void orc_cgls(const orc_geom* g, const double* y, double* u /* in: x0, out: u^(M) */, int n_iter) {
+void orc_cgls(const orc_geom* g, const double* y, double* u /* in: x0, out: u^(M) */, int n_iter, int reorth) {
   const long nvox = (long)g->nx * g->ny * g->nz, nray = (long)g->nviews * g->nv * g->nu;
   double* r = (double*)malloc(nray * sizeof(double));
   double* q = (double*)malloc(nray * sizeof(double));
   double* s = (double*)malloc(nvox * sizeof(double));
   double* gr = (double*)malloc(nvox * sizeof(double));
+  double* basis = reorth ? (double*)malloc((size_t)(n_iter + 1) * nvox * sizeof(double)) : NULL;
+  int nb = 0;                                             /* normalised earlier gradients kept      */
   orc_forward(g, u, q);                                   /* r0 = y - P u0        (:420) */
   for (long i = 0; i < nray; ++i) r[i] = y[i] - q[i];
   orc_back(g, r, gr);                                     /* s0 = P^T r0          (:420) */
   memcpy(s, gr, nvox * sizeof(double));
   double gamma = dot(gr, gr, nvox);                       /* ||P^T r||^2                 */
+  if (reorth && gamma > 0.0) {
+    double inv = 1.0 / sqrt(gamma);
+    for (long i = 0; i < nvox; ++i) basis[i] = gr[i] * inv;
+    nb = 1;
+  }
   for (int m = 0; m < n_iter; ++m) {
     orc_forward(g, s, q);                                 /* P s                         */
     double delta = dot(q, q, nray);
@@ -261,12 +281,24 @@ void orc_cgls(const orc_geom* g, const double* y, double* u /* in: x0, out: u^(M
     for (long i = 0; i < nvox; ++i) u[i] += a * s[i];     /* step 2               (:426) */
     for (long i = 0; i < nray; ++i) r[i] -= a * q[i];     /* step 3               (:429) */
     orc_back(g, r, gr);                                   /* P^T r^(m+1)                 */
+    if (reorth)                                           /* S24: enforce g _|_ earlier gradients */
+      for (int p = 0; p < nb; ++p) {
+        const double* bp = basis + (size_t)p * nvox;
+        double c = dot(bp, gr, nvox);
+        for (long i = 0; i < nvox; ++i) gr[i] -= c * bp[i];
+      }
     double gamma1 = dot(gr, gr, nvox);
+    if (reorth && gamma1 > 0.0) {
+      double inv = 1.0 / sqrt(gamma1);
+      double* bp = basis + (size_t)nb * nvox;
+      for (long i = 0; i < nvox; ++i) bp[i] = gr[i] * inv;
+      ++nb;
+    }
     double b = gamma1 / gamma;                            /* step 4               (:432) */
     for (long i = 0; i < nvox; ++i) s[i] = gr[i] + b * s[i]; /* step 5            (:435) */
     gamma = gamma1;
   }
-  free(r); free(q); free(s); free(gr);
+  free(r); free(q); free(s); free(gr); free(basis);
 }
 
 /* ------------------------------------------------------------------ O5 face magnitudes
@@ -478,7 +510,7 @@ void orc_reconstruct(const orc_geom* g, const double* sino, const orc_params* p,
   memset(f, 0, nvox * sizeof(double));
   memset(w, 0, (size_t)g->ndim * nvox * sizeof(double));
   for (int it = 0; it < p->n_outer; ++it) {
-    orc_cgls(g, sino, f, p->n_cgls);                      /* Step 1 (:171) */
+    orc_cgls(g, sino, f, p->n_cgls, p->reorth);           /* Step 1 (:171), S24 */
     memcpy(v, f, nvox * sizeof(double));
     for (int s = 0; s < p->n_gd; ++s) {                   /* Step 2 (:172) */
       double sig = orc_update_weights(g->ndim, g->nx, g->ny, g->nz, f, p->sigma_quantile, p->eps,

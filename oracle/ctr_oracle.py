@@ -46,7 +46,8 @@ class OrcParams(C.Structure):
     _fields_ = [("n_outer", C.c_int), ("n_cgls", C.c_int), ("n_gd", C.c_int),
                 ("lam", C.c_double), ("sigma_quantile", C.c_double), ("eps", C.c_double),
                 ("armijo_t0", C.c_double), ("armijo_rho", C.c_double), ("armijo_c", C.c_double),
-                ("armijo_max", C.c_int), ("weights_mode", C.c_int), ("positivity", C.c_int)]
+                ("armijo_max", C.c_int), ("weights_mode", C.c_int), ("positivity", C.c_int),
+                ("reorth", C.c_int)]
 
 
 _DP = C.POINTER(C.c_double)
@@ -63,7 +64,7 @@ def lib():
         L.orc_forward.argtypes = [G, _DP, _DP]
         L.orc_back.argtypes = [G, _DP, _DP]
         L.orc_matrix_row.argtypes = [G, i, i, i, _DP]
-        L.orc_cgls.argtypes = [G, _DP, _DP, i]
+        L.orc_cgls.argtypes = [G, _DP, _DP, i, i]
         L.orc_face_mag2.argtypes = [i, i, i, i, _DP, _DP]
         L.orc_sigma.argtypes = [i, i, i, i, _DP, d, d]
         L.orc_sigma.restype = d
@@ -113,9 +114,9 @@ def make_params(p) -> OrcParams:
     op = OrcParams()
     defaults = dict(n_outer=1, n_cgls=1, n_gd=5, lam=0.01, sigma_quantile=0.90, eps=1e-6,
                     armijo_t0=1e-3, armijo_rho=0.5, armijo_c=1e-4, armijo_max=16,
-                    weights_mode=0, positivity=1)
+                    weights_mode=0, positivity=1, reorth=1)
     defaults.update(d)
-    for k in ("n_outer", "n_cgls", "n_gd", "armijo_max", "weights_mode", "positivity"):
+    for k in ("n_outer", "n_cgls", "n_gd", "armijo_max", "weights_mode", "positivity", "reorth"):
         setattr(op, k, int(defaults[k]))
     for k in ("lam", "sigma_quantile", "eps", "armijo_t0", "armijo_rho", "armijo_c"):
         setattr(op, k, _f32(defaults[k]))
@@ -173,11 +174,12 @@ def matrix(g):
     return A
 
 
-def cgls(g, b, x0, n_iter):
+def cgls(g, b, x0, n_iter, reorth=True):
+    """O4. reorth=True: reading S24 (gradients re-orthogonalised); False: recurrence as printed."""
     og = make_geom(g)
     b = _c64(b)
     x = _c64(x0).copy()
-    lib().orc_cgls(C.byref(og), _p(b), _p(x), int(n_iter))
+    lib().orc_cgls(C.byref(og), _p(b), _p(x), int(n_iter), int(bool(reorth)))
     return x
 
 

@@ -1,0 +1,669 @@
+// C ABI of libctr (include/ctr.h): handle management, layout conversion, CGLS and the outer loop.
+#include <math.h>
+#include <stdlib.h>
+
+#include <new>
+
+#include "ctr_common.cuh"
+#include "ctr_internal.h"
+
+using namespace ctr;
+
+namespace ctr {
+
+// ---------------------------------------------------------------------------------------------
+// ABI <-> internal layout. ABI: [B][n] floats. Internal (V = 4): [G][n] float4, lane c = slice 4g+c,
+// missing slices are zero. V = 1 uses the ABI arrays in place (no copies).
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_pack4(const float* __restrict__ src, float* __restrict__ dst, size_t n, int B,
+                                               int planes) {
+  const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
+  const int g = blockIdx.y, pl = blockIdx.z, G = gridDim.y;
+  if (idx >= n) return;
+  float o[4];
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    const int sl = 4 * g + c;
+    o[c] = sl < B ? __ldg(src + ((size_t)pl * B + sl) * n + idx) : 0.0f;
+  }
+  reinterpret_cast<float4*>(dst)[((size_t)pl * G + g) * n + idx] = make_float4(o[0], o[1], o[2], o[3]);
+  (void)planes;
+}
+
+__global__ void __launch_bounds__(256) k_unpack4(const float* __restrict__ src, float* __restrict__ dst, size_t n, int B,
+                                                 int planes) {
+  const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
+  const int g = blockIdx.y, pl = blockIdx.z, G = gridDim.y;
+  if (idx >= n) return;
+  const float4 t = __ldg(reinterpret_cast<const float4*>(src) + ((size_t)pl * G + g) * n + idx);
+  const float o[4] = {t.x, t.y, t.z, t.w};
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    const int sl = 4 * g + c;
+    if (sl < B) dst[((size_t)pl * B + sl) * n + idx] = o[c];
+  }
+  (void)planes;
+}
+
+static int pack(ctr_handle* h, const float* src, float* dst, size_t n, int planes, cudaStream_t st) {
+  dim3 grid((unsigned)((n + 255) / 256), h->d.G, planes);
+  ProfScope prof(h, CTR_PROF_LAYOUT, st);
+  k_pack4<<<grid, 256, 0, st>>>(src, dst, n, h->d.B, planes);
+  CTR_LAUNCHED(h);
+  return CTR_OK;
+}
+static int unpack(ctr_handle* h, const float* src, float* dst, size_t n, int planes, cudaStream_t st) {
+  dim3 grid((unsigned)((n + 255) / 256), h->d.G, planes);
+  ProfScope prof(h, CTR_PROF_LAYOUT, st);
+  k_unpack4<<<grid, 256, 0, st>>>(src, dst, n, h->d.B, planes);
+  CTR_LAUNCHED(h);
+  return CTR_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a3  CGLS vector updates (App. I steps 2, 3, 5), per-slice scalars from device.
+// ---------------------------------------------------------------------------------------------
+template <int V>
+__global__ void __launch_bounds__(256) k_sino_axpy(size_t n, float* __restrict__ r, const float* __restrict__ q, Scal sc) {
+  const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
+  const int g = blockIdx.y;
+  if (idx >= n) return;
+  float rv[V], qv[V];
+  Pack<V>::ldcg(r, (size_t)g * n + idx, rv);
+  Pack<V>::ldcg(q, (size_t)g * n + idx, qv);
+#pragma unroll
+  for (int c = 0; c < V; ++c) rv[c] = fmaf(-sc.a[g * V + c], qv[c], rv[c]);  // r <- r - a P s
+  Pack<V>::st(r, (size_t)g * n + idx, rv);
+}
+
+// s <- g + beta s (App. I step 5, :435; first = 1: s <- g) and store the unit gradient g/||g||
+// as the next basis vector of the re-orthogonalisation (S24).
+template <int V>
+__global__ void __launch_bounds__(256) k_img_supdate(size_t n, float* __restrict__ s, const float* __restrict__ gi,
+                                                     float* __restrict__ bnew, Scal sc, int first) {
+  const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
+  const int g = blockIdx.y;
+  if (idx >= n) return;
+  float sv[V], gv[V], bv[V];
+  Pack<V>::ldcg(gi, (size_t)g * n + idx, gv);
+  if (first) {
+#pragma unroll
+    for (int c = 0; c < V; ++c) sv[c] = gv[c];
+  } else {
+    Pack<V>::ldcg(s, (size_t)g * n + idx, sv);
+#pragma unroll
+    for (int c = 0; c < V; ++c) sv[c] = fmaf(sc.beta[g * V + c], sv[c], gv[c]);
+  }
+  Pack<V>::st(s, (size_t)g * n + idx, sv);
+  if (bnew) {
+#pragma unroll
+    for (int c = 0; c < V; ++c) bv[c] = gv[c] * sc.ginv[g * V + c];
+    Pack<V>::st(bnew, (size_t)g * n + idx, bv);
+  }
+}
+
+template <int V>
+__global__ void __launch_bounds__(256) k_img_uupdate(size_t n, float* __restrict__ u, const float* __restrict__ s, Scal sc) {
+  const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
+  const int g = blockIdx.y;
+  if (idx >= n) return;
+  float uv[V], sv[V];
+  Pack<V>::ldcg(u, (size_t)g * n + idx, uv);
+  Pack<V>::ldcg(s, (size_t)g * n + idx, sv);
+#pragma unroll
+  for (int c = 0; c < V; ++c) uv[c] = fmaf(sc.a[g * V + c], sv[c], uv[c]);  // u <- u + a s
+  Pack<V>::st(u, (size_t)g * n + idx, uv);
+}
+
+// Re-orthogonalisation of the CGLS gradients (S24). In exact arithmetic P^T r^(m+1) is
+// orthogonal to every earlier P^T r^(i) (Hestenes & Stiefel); in fp32 that is lost
+// after ~6 iterations and the iterate then lags the exact one by a whole step. Classical
+// Gram-Schmidt against the stored unit gradients b_i restores it:
+//   pass 1 (k_reorth_dots): c_i = <b_i, g> for NB basis vectors per launch, fp64 accumulation
+//   pass 2 (k_reorth_sub) : g <- g - sum_i c_i b_i, gamma' = ||g||^2, beta = gamma'/gamma (:432)
+#define REORTH_NB 4
+template <int V>
+__global__ void __launch_bounds__(256) k_reorth_dots(size_t n, size_t nimg, const float* __restrict__ gi,
+                                                     const float* __restrict__ basis, int i0, int nb, int Bp, Scal sc,
+                                                     double* part, unsigned* counter) {
+  const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
+  const int g = blockIdx.y;
+  double red[REORTH_NB * V];
+#pragma unroll
+  for (int q = 0; q < REORTH_NB * V; ++q) red[q] = 0.0;
+  if (idx < n) {
+    float gv[V];
+    Pack<V>::ldcg(gi, (size_t)g * n + idx, gv);
+#pragma unroll
+    for (int q = 0; q < REORTH_NB; ++q) {
+      if (q < nb) {
+        float bv[V];
+        Pack<V>::ldcg(basis + (size_t)(i0 + q) * nimg, (size_t)g * n + idx, bv);
+#pragma unroll
+        for (int c = 0; c < V; ++c) red[q * V + c] = (double)bv[c] * (double)gv[c];
+      }
+    }
+  }
+  grid_reduce<REORTH_NB * V>(red, part + (size_t)g * gridDim.x * REORTH_NB * V, counter + g, gridDim.x, blockIdx.x,
+                             threadIdx.x, 256, [&](double(&sum)[REORTH_NB * V]) {
+                               for (int q = 0; q < nb; ++q)
+#pragma unroll
+                                 for (int c = 0; c < V; ++c) sc.coef[(size_t)(i0 + q) * Bp + g * V + c] = (float)sum[q * V + c];
+                             });
+}
+
+template <int V>
+__global__ void __launch_bounds__(256) k_reorth_sub(size_t n, size_t nimg, float* __restrict__ gi,
+                                                    const float* __restrict__ basis, int nb, int Bp, int first, Scal sc,
+                                                    double* part, unsigned* counter) {
+  const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
+  const int g = blockIdx.y;
+  double red[V];
+#pragma unroll
+  for (int c = 0; c < V; ++c) red[c] = 0.0;
+  if (idx < n) {
+    float gv[V];
+    Pack<V>::ldcg(gi, (size_t)g * n + idx, gv);
+    for (int q = 0; q < nb; ++q) {
+      float bv[V];
+      Pack<V>::ldcg(basis + (size_t)q * nimg, (size_t)g * n + idx, bv);
+#pragma unroll
+      for (int c = 0; c < V; ++c) gv[c] = fmaf(-sc.coef[(size_t)q * Bp + g * V + c], bv[c], gv[c]);
+    }
+    if (nb > 0) Pack<V>::st(gi, (size_t)g * n + idx, gv);
+#pragma unroll
+    for (int c = 0; c < V; ++c) red[c] = (double)gv[c] * (double)gv[c];
+  }
+  grid_reduce<V>(red, part + (size_t)g * gridDim.x * V, counter + g, gridDim.x, blockIdx.x, threadIdx.x, 256,
+                 [&](double(&sum)[V]) {
+#pragma unroll
+                   for (int c = 0; c < V; ++c) {
+                     const int sl = g * V + c;
+                     if (!first) {
+                       const double gamma = sc.gamma[sl];
+                       sc.beta[sl] = gamma > 0.0 ? (float)(sum[c] / gamma) : 0.0f;  // S4
+                     }
+                     sc.gamma[sl] = sum[c];
+                     sc.ginv[sl] = sum[c] > 0.0 ? (float)(1.0 / sqrt(sum[c])) : 0.0f;
+                   }
+                 });
+}
+
+static int vec_sino_axpy(ctr_handle* h, float* r, const float* q, cudaStream_t st) {
+  const size_t n = h->d.nray;
+  dim3 grid((unsigned)((n + 255) / 256), h->d.G);
+  ProfScope prof(h, CTR_PROF_VECTOR, st);
+  if (h->d.V == 1) k_sino_axpy<1><<<grid, 256, 0, st>>>(n, r, q, h->sc);
+  else k_sino_axpy<4><<<grid, 256, 0, st>>>(n, r, q, h->sc);
+  CTR_LAUNCHED(h);
+  return CTR_OK;
+}
+static int vec_img_supdate(ctr_handle* h, float* s, const float* g, float* bnew, int first, cudaStream_t st) {
+  const size_t n = h->d.npix;
+  dim3 grid((unsigned)((n + 255) / 256), h->d.G);
+  ProfScope prof(h, CTR_PROF_VECTOR, st);
+  if (h->d.V == 1) k_img_supdate<1><<<grid, 256, 0, st>>>(n, s, g, bnew, h->sc, first);
+  else k_img_supdate<4><<<grid, 256, 0, st>>>(n, s, g, bnew, h->sc, first);
+  CTR_LAUNCHED(h);
+  return CTR_OK;
+}
+static int vec_img_uupdate(ctr_handle* h, float* u, const float* s, cudaStream_t st) {
+  const size_t n = h->d.npix;
+  dim3 grid((unsigned)((n + 255) / 256), h->d.G);
+  ProfScope prof(h, CTR_PROF_VECTOR, st);
+  if (h->d.V == 1) k_img_uupdate<1><<<grid, 256, 0, st>>>(n, u, s, h->sc);
+  else k_img_uupdate<4><<<grid, 256, 0, st>>>(n, u, s, h->sc);
+  CTR_LAUNCHED(h);
+  return CTR_OK;
+}
+// g <- g minus its components along basis[0..nb), then gamma / beta / 1/||g||
+static int vec_reorth(ctr_handle* h, float* g, int nb, int first, cudaStream_t st) {
+  const Dims& d = h->d;
+  const size_t n = d.npix;
+  const int Bp = d.G * d.V;
+  dim3 grid((unsigned)((n + 255) / 256), d.G);
+  ProfScope prof(h, CTR_PROF_VECTOR, st);
+  if (nb > CTR_MAX_BASIS) nb = CTR_MAX_BASIS;
+  for (int i0 = 0; i0 < nb; i0 += REORTH_NB) {
+    const int cnt = nb - i0 < REORTH_NB ? nb - i0 : REORTH_NB;
+    if (d.V == 1) k_reorth_dots<1><<<grid, 256, 0, st>>>(n, h->nimg, g, h->basis, i0, cnt, Bp, h->sc, h->part, h->counters + 4 * d.G);
+    else k_reorth_dots<4><<<grid, 256, 0, st>>>(n, h->nimg, g, h->basis, i0, cnt, Bp, h->sc, h->part, h->counters + 4 * d.G);
+    CTR_LAUNCHED(h);
+  }
+  if (d.V == 1) k_reorth_sub<1><<<grid, 256, 0, st>>>(n, h->nimg, g, h->basis, nb, Bp, first, h->sc, h->part, h->counters + 5 * d.G);
+  else k_reorth_sub<4><<<grid, 256, 0, st>>>(n, h->nimg, g, h->basis, nb, Bp, first, h->sc, h->part, h->counters + 5 * d.G);
+  CTR_LAUNCHED(h);
+  return CTR_OK;
+}
+
+static int op_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st) {
+  return h->d.ndim == 3 ? cone_forward(h, img, out, mode, bs, st) : fan_forward(h, img, out, mode, bs, st);
+}
+static int op_back(ctr_handle* h, const float* sino, float* out, int mode, const float* s, float* u, cudaStream_t st) {
+  return h->d.ndim == 3 ? cone_back(h, sino, out, mode, s, u, st) : fan_back(h, sino, out, mode, s, u, st);
+}
+
+// storage for the unit gradients; grows (synchronously) only when a longer CGLS run is requested
+static int ensure_basis(ctr_handle* h, int n_iter) {
+  int need = n_iter < CTR_MAX_BASIS ? n_iter : CTR_MAX_BASIS;
+  if (need <= h->basis_cap) return CTR_OK;
+  CTR_CUDA(h, cudaDeviceSynchronize());
+  if (h->basis) cudaFree(h->basis);
+  h->basis = nullptr;
+  h->basis_cap = 0;
+  cudaError_t e = cudaMalloc((void**)&h->basis, (size_t)need * h->nimg * sizeof(float));
+  if (e != cudaSuccess) { cudaGetLastError(); return set_err(h, CTR_ENOMEM, "CGLS basis allocation failed"); }
+  h->basis_cap = need;
+  return CTR_OK;
+}
+
+// CGLS on internal-layout arrays (gradients re-orthogonalised, S24). u: in x0 /
+// out u^(M). The last iteration only needs u (its P^T r and s are never used, O4), so it ends with a
+// plain u += a s.
+static int cgls_internal(ctr_handle* h, const float* b, float* u, int n_iter, bool x0_zero, cudaStream_t st) {
+  if (n_iter <= 0) return CTR_OK;
+  int rc;
+  if ((rc = ensure_basis(h, n_iter))) return rc;
+  if (x0_zero) {
+    CTR_CUDA(h, cudaMemcpyAsync(h->r, b, h->nsino * sizeof(float), cudaMemcpyDeviceToDevice, st));  // r0 = y
+  } else if ((rc = op_forward(h, u, h->r, 1, b, st))) return rc;                                    // r0 = y - P u0
+  if ((rc = op_back(h, h->r, h->gimg, 0, nullptr, nullptr, st))) return rc;                         // g0 = P^T r0
+  if ((rc = vec_reorth(h, h->gimg, 0, 1, st))) return rc;                                           // gamma0
+  if ((rc = vec_img_supdate(h, h->s, h->gimg, h->basis, 1, st))) return rc;                         // s0 = g0, b_0
+  for (int m = 0; m < n_iter; ++m) {
+    if ((rc = op_forward(h, h->s, h->q, 2, nullptr, st))) return rc;     // q = P s, a = gamma/||q||^2
+    if (m == n_iter - 1) return vec_img_uupdate(h, u, h->s, st);         // u += a s
+    if ((rc = vec_sino_axpy(h, h->r, h->q, st))) return rc;              // r -= a q
+    if ((rc = op_back(h, h->r, h->gimg, 2, h->s, u, st))) return rc;     // g = P^T r, u += a s
+    if ((rc = vec_reorth(h, h->gimg, m + 1, 0, st))) return rc;          // g _|_ b_0..b_m, gamma', beta
+    float* bnew = (m + 1 < h->basis_cap) ? h->basis + (size_t)(m + 1) * h->nimg : nullptr;
+    if ((rc = vec_img_supdate(h, h->s, h->gimg, bnew, 0, st))) return rc;  // s = g + beta s, b_{m+1}
+  }
+  return CTR_OK;
+}
+
+// double -> float copy for ctr_update_weights' optional sigma output
+__global__ void k_d2f(const double* __restrict__ s, float* __restrict__ o, int n) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) o[i] = (float)s[i];
+}
+
+static bool aligned16(const void* p) { return p && (((uintptr_t)p) & 15u) == 0; }
+
+static int check_params(const ctr_params* p) {
+  if (!p) return CTR_EINVAL;
+  if (p->n_outer < 0 || p->n_cgls < 0 || p->n_gd < 0) return CTR_EINVAL;
+  if (!(p->lambda >= 0.0f) || !(p->sigma_quantile > 0.0f && p->sigma_quantile <= 1.0f)) return CTR_EINVAL;
+  if (!(p->eps >= 0.0f) || !(p->armijo_t0 > 0.0f) || !(p->armijo_rho > 0.0f && p->armijo_rho < 1.0f)) return CTR_EINVAL;
+  if (!(p->armijo_c >= 0.0f) || p->armijo_max < 1 || p->armijo_max > CTR_MAX_ARMIJO) return CTR_EINVAL;
+  if (p->weights_mode != 0 && p->weights_mode != 1) return CTR_EINVAL;
+  return CTR_OK;
+}
+
+static void set_quantile(ctr_handle* h, float q) {
+  const Dims& d = h->d;
+  // number of interior faces per slice / volume (O6)
+  unsigned long long S = 0;
+  S += (unsigned long long)(d.nx - 1) * d.ny * d.nz;
+  S += (unsigned long long)d.nx * (d.ny - 1) * d.nz;
+  if (d.ndim == 3) S += (unsigned long long)d.nx * d.ny * (d.nz - 1);
+  double kk = ceil((double)q * (double)S);
+  unsigned long long k = kk < 1.0 ? 1ull : (unsigned long long)kk;
+  if (k > S) k = S;
+  if (S == 0) k = 0;
+  h->sel_k = k;
+  h->sel_q = q;
+}
+
+}  // namespace ctr
+
+// =============================================================================================
+extern "C" {
+
+void ctr_default_params(ctr_params* p) {
+  if (!p) return;
+  p->n_outer = 1; p->n_cgls = 10; p->n_gd = 5;
+  p->lambda = 0.01f; p->sigma_quantile = 0.90f; p->eps = 1e-6f;
+  p->armijo_t0 = 1e-3f; p->armijo_rho = 0.5f; p->armijo_c = 1e-4f; p->armijo_max = 16;
+  p->weights_mode = 0; p->positivity = 1; p->warm_start = 0;
+}
+
+const char* ctr_strerror(int status) {
+  switch (status) {
+    case CTR_OK: return "ok";
+    case CTR_EINVAL: return "invalid argument";
+    case CTR_EGEOM: return "invalid geometry (source or detector inside the image circle)";
+    case CTR_ENOMEM: return "out of memory";
+    case CTR_ECUDA: return "CUDA error";
+    case CTR_EARCH: return "device is not sm_100 (B200)";
+    default: return "unknown status";
+  }
+}
+
+const char* ctr_last_error(const ctr_handle* h) { return h ? h->err : ""; }
+long long ctr_launch_count(const ctr_handle* h) { return h ? h->launches : 0; }
+
+void ctr_destroy(ctr_handle* h) {
+  if (!h) return;
+  cudaDeviceSynchronize();
+  void* bufs[] = {h->rays, h->rays2, h->views, h->ximg, h->bsino, h->r, h->q, h->s, h->gimg, h->v, h->w, h->n0,
+                  h->part, h->counters, h->hist, h->scal_block, h->stats, h->basis};
+  for (void* b : bufs)
+    if (b) cudaFree(b);
+  if (h->prof_ev) {
+    for (int i = 0; i < 2 * CTR_PROF_MAX; ++i) cudaEventDestroy(h->prof_ev[i]);
+    free(h->prof_ev);
+    free(h->prof_kind);
+  }
+  free(h->g.angles ? (void*)h->g.angles : nullptr);
+  delete h;
+}
+
+int ctr_create(const ctr_geometry* g, ctr_handle** out) {
+  if (!out) return CTR_EINVAL;
+  *out = nullptr;
+  if (!g) return CTR_EINVAL;
+  if (g->ndim != 2 && g->ndim != 3) return CTR_EINVAL;
+  if (g->nx < 1 || g->ny < 1 || g->nz < 1 || g->nviews < 1 || g->nu < 1 || g->nv < 1 || g->batch < 1) return CTR_EINVAL;
+  if (g->ndim == 2 && (g->nz != 1 || g->nv != 1)) return CTR_EINVAL;
+  if (g->ndim == 3 && (g->batch != 1 || g->det_type != 0)) return CTR_EINVAL;
+  if (!(g->dx > 0) || !(g->dy > 0) || !(g->du > 0) || !(g->dso > 0) || !(g->dsd > g->dso)) return CTR_EINVAL;
+  if (g->ndim == 3 && (!(g->dz > 0) || !(g->dv > 0))) return CTR_EINVAL;
+  if (g->det_type != 0 && g->det_type != 1) return CTR_EINVAL;
+  if ((long long)g->nx * g->ny * g->nz >= (1ll << 31) || (long long)g->nviews * g->nu * g->nv >= (1ll << 31)) return CTR_EINVAL;
+  // source and detector must lie outside the circle circumscribing the grid (plus one voxel)
+  {
+    double hx = fabs((double)g->cx) + 0.5 * g->nx * (double)g->dx + g->dx;
+    double hy = fabs((double)g->cy) + 0.5 * g->ny * (double)g->dy + g->dy;
+    double rad = sqrt(hx * hx + hy * hy);
+    if (!(g->dso > rad) || !((double)g->dsd - g->dso > rad)) return CTR_EGEOM;
+  }
+  int dev = 0;
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return CTR_ECUDA;
+  if (prop.major != 10) return CTR_EARCH;
+
+  ctr_handle* h = new (std::nothrow) ctr_handle();
+  if (!h) return CTR_ENOMEM;
+  memset(h, 0, sizeof(*h));
+  h->g = *g;
+  h->g.angles = nullptr;
+  if (g->angles) {
+    float* a = (float*)malloc(sizeof(float) * g->nviews);
+    if (!a) { delete h; return CTR_ENOMEM; }
+    memcpy(a, g->angles, sizeof(float) * g->nviews);
+    h->g.angles = a;
+  }
+  h->device = dev;
+  ctr_default_params(&h->p);
+
+  Dims& d = h->d;
+  d.ndim = g->ndim;
+  d.nx = g->nx; d.ny = g->ny; d.nz = g->nz;
+  d.nviews = g->nviews; d.nu = g->nu; d.nv = g->nv;
+  d.c0x = g->nx / 2; d.c0y = g->ny / 2; d.c0z = g->nz / 2;
+  d.npix = g->nx * g->ny * g->nz;
+  d.nray = g->nviews * g->nu * g->nv;
+  d.B = g->batch;
+  d.V = g->batch > 1 ? 4 : 1;
+  d.G = (g->batch + d.V - 1) / d.V;
+  d.dx = g->dx; d.dy = g->dy; d.dz = g->ndim == 3 ? g->dz : 1.0f;
+  d.xlo = (float)((double)g->cx - g->nx * (double)g->dx / 2.0);
+  d.ylo = (float)((double)g->cy - g->ny * (double)g->dy / 2.0);
+  d.zlo = (float)((double)g->cz - g->nz * (double)d.dz / 2.0);
+  d.dso = g->dso; d.dsd = g->dsd;
+  d.inv_du = 1.0f / g->du;
+  d.inv_dv = g->ndim == 3 ? 1.0f / g->dv : 1.0f;
+  d.boff_u = (float)((g->nu - 1) / 2.0 - (double)g->u_off);
+  d.boff_v = (float)((g->nv - 1) / 2.0 - (double)g->v_off);
+  d.rvox = 0.5f * sqrtf(d.dx * d.dx + d.dy * d.dy + (g->ndim == 3 ? d.dz * d.dz : 0.0f));
+  d.det_type = g->det_type;
+
+  const int Bp = d.G * d.V;
+  h->nimg = (size_t)Bp * d.npix;
+  h->nsino = (size_t)Bp * d.nray;
+  const size_t fb = sizeof(float);
+  cudaError_t e = cudaSuccess;
+  auto A = [&](void** p, size_t bytes) {
+    if (e == cudaSuccess) e = cudaMalloc(p, bytes ? bytes : 16);
+  };
+  A((void**)&h->rays, sizeof(float4) * d.nray);
+  if (d.ndim == 3) A((void**)&h->rays2, sizeof(float4) * d.nray);
+  A((void**)&h->views, sizeof(float2) * d.nviews);
+  A((void**)&h->ximg, h->nimg * fb);
+  A((void**)&h->bsino, h->nsino * fb);
+  A((void**)&h->r, h->nsino * fb);
+  A((void**)&h->q, h->nsino * fb);
+  A((void**)&h->s, h->nimg * fb);
+  A((void**)&h->gimg, h->nimg * fb);
+  A((void**)&h->v, h->nimg * fb);
+  A((void**)&h->w, h->nimg * fb * d.ndim);
+  A((void**)&h->n0, h->nimg * fb * d.ndim);
+  // partial sums: the largest user is the TV trial kernel (TV_KC * V slots per block)
+  {
+    size_t nblk_tv = (size_t)((d.nx + 31) / 32) * ((d.ny + 3) / 4) * d.nz;
+    size_t nblk_p = (size_t)(d.nray + 127) / 128;
+    size_t nblk = nblk_tv > nblk_p ? nblk_tv : nblk_p;
+    h->part_len = (size_t)d.G * nblk * 4 * d.V;
+    A((void**)&h->part, h->part_len * sizeof(double));
+  }
+  A((void**)&h->counters, sizeof(unsigned) * CTR_NCOUNTERS * d.G);
+  A((void**)&h->hist, sizeof(unsigned) * 2048 * Bp);
+  A((void**)&h->stats, sizeof(ctr_sweep_stat) * (size_t)CTR_STAT_SWEEPS * Bp);
+  const size_t scal_bytes = (size_t)Bp * (3 * sizeof(double) + (5 + CTR_MAX_BASIS) * sizeof(float) + 3 * sizeof(unsigned) + 16);
+  A(&h->scal_block, scal_bytes);
+  if (e != cudaSuccess) {
+    int rc = e == cudaErrorMemoryAllocation ? CTR_ENOMEM : CTR_ECUDA;
+    cudaGetLastError();
+    ctr_destroy(h);
+    return rc;
+  }
+  cudaMemset(h->counters, 0, sizeof(unsigned) * CTR_NCOUNTERS * d.G);
+  cudaMemset(h->hist, 0, sizeof(unsigned) * 2048 * Bp);
+  cudaMemset(h->scal_block, 0, scal_bytes);
+  cudaMemset(h->stats, 0, sizeof(ctr_sweep_stat) * (size_t)CTR_STAT_SWEEPS * Bp);
+  {
+    char* p = (char*)h->scal_block;
+    h->sc.gamma = (double*)p; p += sizeof(double) * Bp;
+    h->sc.e0 = (double*)p; p += sizeof(double) * Bp;
+    h->sc.g2 = (double*)p; p += sizeof(double) * Bp;
+    h->sc.a = (float*)p; p += sizeof(float) * Bp;
+    h->sc.beta = (float*)p; p += sizeof(float) * Bp;
+    h->sc.sigma2 = (float*)p; p += sizeof(float) * Bp;
+    h->sc.tacc = (float*)p; p += sizeof(float) * Bp;
+    h->sc.kacc = (int*)p; p += sizeof(int) * Bp;
+    h->sc.sel_prefix = (unsigned*)p; p += sizeof(unsigned) * Bp;
+    h->sc.sel_rank = (unsigned*)p; p += sizeof(unsigned) * Bp;
+    h->sc.ginv = (float*)p; p += sizeof(float) * Bp;
+    h->sc.coef = (float*)p;
+  }
+  set_quantile(h, h->p.sigma_quantile);
+  int rc = d.ndim == 3 ? cone_build_tables(h) : fan_build_tables(h);
+  if (rc != CTR_OK) { ctr_destroy(h); return rc; }
+  *out = h;
+  return CTR_OK;
+}
+
+int ctr_set_params(ctr_handle* h, const ctr_params* p) {
+  if (!h) return CTR_EINVAL;
+  int rc = check_params(p);
+  if (rc) return set_err(h, rc, "ctr_set_params: parameter out of range");
+  h->p = *p;
+  set_quantile(h, p->sigma_quantile);
+  return CTR_OK;
+}
+
+int ctr_forward(ctr_handle* h, const float* d_img, float* d_sino, void* stream) {
+  if (!h) return CTR_EINVAL;
+  if (!aligned16(d_img) || !aligned16(d_sino)) return set_err(h, CTR_EINVAL, "ctr_forward: NULL or misaligned pointer");
+  cudaStream_t st = (cudaStream_t)stream;
+  h->last_stream = st;
+  if (h->d.V == 1) return op_forward(h, d_img, d_sino, 0, nullptr, st);
+  int rc;
+  if ((rc = pack(h, d_img, h->ximg, h->d.npix, 1, st))) return rc;
+  if ((rc = op_forward(h, h->ximg, h->q, 0, nullptr, st))) return rc;
+  return unpack(h, h->q, d_sino, h->d.nray, 1, st);
+}
+
+int ctr_back(ctr_handle* h, const float* d_sino, float* d_img, void* stream) {
+  if (!h) return CTR_EINVAL;
+  if (!aligned16(d_img) || !aligned16(d_sino)) return set_err(h, CTR_EINVAL, "ctr_back: NULL or misaligned pointer");
+  cudaStream_t st = (cudaStream_t)stream;
+  h->last_stream = st;
+  if (h->d.V == 1) return op_back(h, d_sino, d_img, 0, nullptr, nullptr, st);
+  int rc;
+  if ((rc = pack(h, d_sino, h->bsino, h->d.nray, 1, st))) return rc;
+  if ((rc = op_back(h, h->bsino, h->gimg, 0, nullptr, nullptr, st))) return rc;
+  return unpack(h, h->gimg, d_img, h->d.npix, 1, st);
+}
+
+int ctr_cgls(ctr_handle* h, const float* d_b, float* d_x, int n_iter, void* stream) {
+  if (!h) return CTR_EINVAL;
+  if (!aligned16(d_b) || !aligned16(d_x)) return set_err(h, CTR_EINVAL, "ctr_cgls: NULL or misaligned pointer");
+  if (n_iter < 0) return set_err(h, CTR_EINVAL, "ctr_cgls: n_iter < 0");
+  if (n_iter == 0) return CTR_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  h->last_stream = st;
+  if (h->d.V == 1) return cgls_internal(h, d_b, d_x, n_iter, false, st);
+  int rc;
+  if ((rc = pack(h, d_b, h->bsino, h->d.nray, 1, st))) return rc;
+  if ((rc = pack(h, d_x, h->ximg, h->d.npix, 1, st))) return rc;
+  if ((rc = cgls_internal(h, h->bsino, h->ximg, n_iter, false, st))) return rc;
+  return unpack(h, h->ximg, d_x, h->d.npix, 1, st);
+}
+
+int ctr_update_weights(ctr_handle* h, const float* d_x, float* d_w, float quantile, float* d_sigma, void* stream) {
+  if (!h) return CTR_EINVAL;
+  if (!aligned16(d_x) || !aligned16(d_w)) return set_err(h, CTR_EINVAL, "ctr_update_weights: NULL or misaligned pointer");
+  if (!(quantile > 0.0f && quantile <= 1.0f)) return set_err(h, CTR_EINVAL, "ctr_update_weights: quantile not in (0,1]");
+  cudaStream_t st = (cudaStream_t)stream;
+  h->last_stream = st;
+  const float q_saved = h->sel_q;
+  set_quantile(h, quantile);
+  int rc;
+  if (h->d.V == 1) {
+    rc = tv_update_weights(h, d_x, d_w, st);
+  } else {
+    if ((rc = pack(h, d_x, h->ximg, h->d.npix, 1, st))) return rc;
+    if ((rc = tv_update_weights(h, h->ximg, h->w, st))) return rc;
+    rc = unpack(h, h->w, d_w, h->d.npix, h->d.ndim, st);
+  }
+  set_quantile(h, q_saved);
+  if (rc) return rc;
+  if (d_sigma) {
+    // sigma = sqrt(sigma^2) per true slice, from the sweep record just written
+    const int Bp = h->d.G * h->d.V;
+    ctr_sweep_stat* rec = h->stats + (size_t)(h->sweep_count % CTR_STAT_SWEEPS) * Bp;
+    // strided device copy: sigma is the first double of each record
+    CTR_CUDA(h, cudaMemcpy2DAsync(h->part, sizeof(double), rec, sizeof(ctr_sweep_stat), sizeof(double), h->d.B,
+                                  cudaMemcpyDeviceToDevice, st));
+    k_d2f<<<(h->d.B + 127) / 128, 128, 0, st>>>(h->part, d_sigma, h->d.B);
+    CTR_LAUNCHED(h);
+  }
+  return CTR_OK;
+}
+
+int ctr_eptv_step(ctr_handle* h, float* d_x, const float* d_v, const float* d_w, float lambda, void* stream) {
+  if (!h) return CTR_EINVAL;
+  if (!aligned16(d_x) || !aligned16(d_v) || !aligned16(d_w))
+    return set_err(h, CTR_EINVAL, "ctr_eptv_step: NULL or misaligned pointer");
+  if (!(lambda >= 0.0f)) return set_err(h, CTR_EINVAL, "ctr_eptv_step: lambda < 0");
+  cudaStream_t st = (cudaStream_t)stream;
+  h->last_stream = st;
+  if (h->d.V == 1) return tv_sweep(h, d_x, d_v, d_w, lambda, 0, st);
+  int rc;
+  if ((rc = pack(h, d_x, h->ximg, h->d.npix, 1, st))) return rc;
+  if ((rc = pack(h, d_v, h->v, h->d.npix, 1, st))) return rc;
+  if ((rc = pack(h, d_w, h->w, h->d.npix, h->d.ndim, st))) return rc;
+  if ((rc = tv_sweep(h, h->ximg, h->v, h->w, lambda, 0, st))) return rc;
+  return unpack(h, h->ximg, d_x, h->d.npix, 1, st);
+}
+
+int ctr_reconstruct_w(ctr_handle* h, const float* d_sino, float* d_img, float* d_w, const ctr_params* p, void* stream) {
+  if (!h) return CTR_EINVAL;
+  if (!aligned16(d_sino) || !aligned16(d_img) || (d_w && !aligned16(d_w)))
+    return set_err(h, CTR_EINVAL, "ctr_reconstruct: NULL or misaligned pointer");
+  int rc;
+  if (p && (rc = ctr_set_params(h, p))) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  h->last_stream = st;
+  h->sweep_count = 0;
+  const ctr_params& P = h->p;
+  const bool direct = h->d.V == 1;
+  float* f = direct ? d_img : h->ximg;
+  const float* b = d_sino;
+  if (!direct) {
+    if ((rc = pack(h, d_sino, h->bsino, h->d.nray, 1, st))) return rc;
+    b = h->bsino;
+  }
+  if ((rc = ensure_basis(h, P.n_cgls))) return rc;
+  if (!P.warm_start) CTR_CUDA(h, cudaMemsetAsync(f, 0, h->nimg * sizeof(float), st));            // f^(0) = 0 (:171)
+  else if (!direct && (rc = pack(h, d_img, h->ximg, h->d.npix, 1, st))) return rc;
+  for (int it = 0; it < P.n_outer; ++it) {
+    if ((rc = cgls_internal(h, b, f, P.n_cgls, it == 0 && !P.warm_start, st))) return rc;        // Step 1 (:171)
+    if (P.n_gd > 0)
+      CTR_CUDA(h, cudaMemcpyAsync(h->v, f, h->nimg * sizeof(float), cudaMemcpyDeviceToDevice, st));  // v = CGLS result
+    for (int s = 0; s < P.n_gd; ++s) {                                                            // Step 2 (:172)
+      if ((rc = tv_update_weights(h, f, h->w, st))) return rc;
+      if ((rc = tv_sweep(h, f, h->v, h->w, P.lambda, (s == P.n_gd - 1) && P.positivity, st))) return rc;
+    }
+    if (P.n_gd == 0 && P.positivity && (rc = tv_clamp(h, f, st))) return rc;                     // Step 3 (:173)
+  }
+  if (!direct && (rc = unpack(h, h->ximg, d_img, h->d.npix, 1, st))) return rc;
+  if (d_w) {
+    if (direct) CTR_CUDA(h, cudaMemcpyAsync(d_w, h->w, h->nimg * sizeof(float) * h->d.ndim, cudaMemcpyDeviceToDevice, st));
+    else if ((rc = unpack(h, h->w, d_w, h->d.npix, h->d.ndim, st))) return rc;
+  }
+  return CTR_OK;
+}
+
+int ctr_reconstruct(ctr_handle* h, const float* d_sino, float* d_img, const ctr_params* p, void* stream) {
+  return ctr_reconstruct_w(h, d_sino, d_img, nullptr, p, stream);
+}
+
+int ctr_profile_enable(ctr_handle* h, int on) {
+  if (!h) return CTR_EINVAL;
+  if (on && !h->prof_ev) {
+    h->prof_ev = (cudaEvent_t*)calloc(2 * CTR_PROF_MAX, sizeof(cudaEvent_t));
+    h->prof_kind = (unsigned char*)calloc(CTR_PROF_MAX, 1);
+    if (!h->prof_ev || !h->prof_kind) return set_err(h, CTR_ENOMEM, "profiler allocation failed");
+    for (int i = 0; i < 2 * CTR_PROF_MAX; ++i) CTR_CUDA(h, cudaEventCreate(&h->prof_ev[i]));
+  }
+  if (on) h->prof_n = 0;
+  h->prof_on = on ? 1 : 0;
+  return CTR_OK;
+}
+
+int ctr_profile_read(ctr_handle* h, double* ms_by_kind, long long* count_by_kind) {
+  if (!h || !ms_by_kind || !count_by_kind) return CTR_EINVAL;
+  CTR_CUDA(h, cudaStreamSynchronize(h->last_stream));
+  for (int k = 0; k < CTR_PROF_KINDS; ++k) { ms_by_kind[k] = 0.0; count_by_kind[k] = 0; }
+  for (int i = 0; i < h->prof_n; ++i) {
+    float ms = 0.0f;
+    CTR_CUDA(h, cudaEventElapsedTime(&ms, h->prof_ev[2 * i], h->prof_ev[2 * i + 1]));
+    ms_by_kind[h->prof_kind[i]] += ms;
+    count_by_kind[h->prof_kind[i]]++;
+  }
+  return CTR_OK;
+}
+
+int ctr_get_stats(ctr_handle* h, ctr_sweep_stat* buf, size_t n_records) {
+  if (!h) return CTR_EINVAL;
+  CTR_CUDA(h, cudaStreamSynchronize(h->last_stream));
+  const int Bp = h->d.G * h->d.V, B = h->d.B;
+  long long sweeps = h->sweep_count < CTR_STAT_SWEEPS ? h->sweep_count : CTR_STAT_SWEEPS;
+  long long avail = sweeps * B;
+  if (!buf || n_records == 0) return (int)avail;
+  long long first = h->sweep_count - sweeps;
+  size_t done = 0;
+  for (long long sw = first; sw < h->sweep_count && done < n_records; ++sw) {
+    size_t n = (size_t)B < n_records - done ? (size_t)B : n_records - done;
+    CTR_CUDA(h, cudaMemcpy(buf + done, h->stats + (size_t)(sw % CTR_STAT_SWEEPS) * Bp, n * sizeof(ctr_sweep_stat),
+                           cudaMemcpyDeviceToHost));
+    done += n;
+  }
+  return (int)avail;
+}
+
+}  // extern "C"
+

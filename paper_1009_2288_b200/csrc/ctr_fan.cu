@@ -1,0 +1,275 @@
+// 2D fan-beam projector pair for sm_100a: ray-driven P (one thread per ray and slice group)
+// and its exact transpose P^T in gather form (one thread per pixel and slice group).
+// Both evaluate the SAME slab_weights() on the SAME fp32 ray table, so every p_ij is identical
+// bit for bit in the two kernels and <Px,y> = <x,P^T y> holds up to summation order.
+//   P   : PAPER.md:87-89 (Eq. 1), :193 ("each thread responsible for one ray line")
+//   P^T : PAPER.md:193 (why not scatter), :471 (adjoint condition A3'); north_star: exact transpose
+#include "ctr_common.cuh"
+#include "ctr_internal.h"
+
+namespace ctr {
+
+// ------------------------------------------------------------------------------------------------
+// Ray table, built once per handle in fp64 and rounded to fp32.
+// Grid-index coordinates: X' = (x - xlo)/dx - c0x, so grid lines sit at integers -c0x .. nx-c0x.
+//   y-driving (|dy'| >= |dx'|):  x'(y') = x0 + m y',  L = length per unit y' (mm), stored +L
+//   x-driving:                    y'(x') = x0 + m x',  L = length per unit x' (mm), stored -L
+//   K = L/|m| (0 when m = 0).
+// ------------------------------------------------------------------------------------------------
+struct FanGeomD {
+  double dso, dsd, du, u_off, theta0, dtheta, xlo, ylo, dx, dy;
+  int nviews, nu, c0x, c0y, det_type;
+};
+
+__global__ void k_fan_build(FanGeomD g, const float* __restrict__ angles, float4* __restrict__ rays,
+                            float2* __restrict__ views) {
+  int r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= g.nviews * g.nu) return;
+  int k = r / g.nu, b = r - k * g.nu;
+  double th = angles ? (double)angles[k] : g.theta0 + g.dtheta * (double)k;
+  double c = cos(th), s = sin(th);
+  if (b == 0) views[k] = make_float2((float)c, (float)s);
+  double Sx = -g.dso * c, Sy = -g.dso * s;
+  double t = ((double)b - (g.nu - 1) / 2.0 + g.u_off) * g.du;
+  double Dx, Dy;
+  if (g.det_type == 0) {
+    Dx = (g.dsd - g.dso) * c - t * s;
+    Dy = (g.dsd - g.dso) * s + t * c;
+  } else {
+    double beta = t / g.dsd;
+    Dx = Sx + g.dsd * cos(th + beta);
+    Dy = Sy + g.dsd * sin(th + beta);
+  }
+  double sxp = (Sx - g.xlo) / g.dx - g.c0x, syp = (Sy - g.ylo) / g.dy - g.c0y;
+  double ddx = (Dx - Sx) / g.dx, ddy = (Dy - Sy) / g.dy;
+  double m, x0, L;
+  bool xdrv = fabs(ddx) > fabs(ddy);
+  if (!xdrv) {
+    m = ddx / ddy;
+    x0 = sxp - m * syp;
+    L = sqrt(m * m * g.dx * g.dx + g.dy * g.dy);
+  } else {
+    m = ddy / ddx;
+    x0 = syp - m * sxp;
+    L = sqrt(g.dx * g.dx + m * m * g.dy * g.dy);
+  }
+  float mf = (float)m;
+  float K = (mf != 0.0f) ? (float)(L / fabs(m)) : 0.0f;
+  rays[r] = make_float4((float)x0, mf, xdrv ? -(float)L : (float)L, K);
+}
+
+int fan_build_tables(ctr_handle* h) {
+  const ctr_geometry& g = h->g;
+  FanGeomD gd;
+  gd.dso = g.dso; gd.dsd = g.dsd; gd.du = g.du; gd.u_off = g.u_off;
+  gd.theta0 = g.theta0; gd.dtheta = g.dtheta;
+  gd.dx = g.dx; gd.dy = g.dy;
+  gd.xlo = (double)g.cx - g.nx * (double)g.dx / 2.0;
+  gd.ylo = (double)g.cy - g.ny * (double)g.dy / 2.0;
+  gd.nviews = g.nviews; gd.nu = g.nu; gd.c0x = h->d.c0x; gd.c0y = h->d.c0y; gd.det_type = g.det_type;
+  float* d_angles = nullptr;
+  if (g.angles) {
+    CTR_CUDA(h, cudaMalloc(&d_angles, sizeof(float) * g.nviews));
+    CTR_CUDA(h, cudaMemcpy(d_angles, g.angles, sizeof(float) * g.nviews, cudaMemcpyHostToDevice));
+  }
+  int n = g.nviews * g.nu;
+  k_fan_build<<<(n + 127) / 128, 128>>>(gd, d_angles, h->rays, h->views);
+  CTR_LAUNCHED(h);
+  CTR_CUDA(h, cudaDeviceSynchronize());
+  if (d_angles) cudaFree(d_angles);
+  return CTR_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1  P: one thread per (ray, slice group). The thread walks the slabs of the ray's driving axis;
+// per slab it touches at most two cells (|m| <= 1). Lanes of a warp are adjacent bins of one view,
+// so their cells are adjacent in memory when the driving axis is y.
+// MODE 0: out = P x        MODE 1: out = bs - P x   (CGLS r0)
+// MODE 2: out = P x and delta = ||out||^2 per slice -> a = gamma/delta (App. I step 1, :423)
+// ------------------------------------------------------------------------------------------------
+template <int V, int MODE>
+__global__ void __launch_bounds__(128) k_fan_forward(Dims d, const float4* __restrict__ rays,
+                                                     const float* __restrict__ img, float* __restrict__ out,
+                                                     const float* __restrict__ bs, Scal sc, double* part,
+                                                     unsigned* counter) {
+  const int r = blockIdx.x * 128 + threadIdx.x;
+  const int g = blockIdx.y;
+  float acc[V];
+#pragma unroll
+  for (int c = 0; c < V; ++c) acc[c] = 0.0f;
+
+  if (r < d.nray) {
+    const float4 R = __ldg(&rays[r]);
+    const float x0 = R.x, m = R.y, L = fabsf(R.z), K = R.w;
+    const bool xdrv = R.z < 0.0f;
+    const int n_drv = xdrv ? d.nx : d.ny, n_oth = xdrv ? d.ny : d.nx;
+    const int c_drv = xdrv ? d.c0x : d.c0y, c_oth = xdrv ? d.c0y : d.c0x;
+    const int st_drv = xdrv ? 1 : d.nx, st_oth = xdrv ? d.nx : 1;
+    // slabs in which the ray can be inside [-c_oth, n_oth - c_oth) (two cells of margin)
+    int s0 = 0, s1 = n_drv;
+    const float lo = (float)(-c_oth) - 1.0f, hi = (float)(n_oth - c_oth) + 1.0f;
+    if (m != 0.0f) {
+      float t1 = (lo - x0) / m, t2 = (hi - x0) / m;
+      float tmin = fminf(t1, t2), tmax = fmaxf(t1, t2);
+      tmin = fminf(fmaxf(tmin, -1.0e6f), 1.0e6f);
+      tmax = fminf(fmaxf(tmax, -1.0e6f), 1.0e6f);
+      s0 = max(0, (int)floorf(tmin) + c_drv - 2);
+      s1 = min(n_drv, (int)ceilf(tmax) + c_drv + 2);
+    } else if (x0 < lo || x0 > hi) {
+      s1 = 0;
+    }
+    const float* base = img + (size_t)g * d.npix * V;
+    float y = (float)(s0 - c_drv);
+    float oa = fmaf(m, y, x0);
+    for (int s = s0; s < s1; ++s) {
+      const float ob = fmaf(m, y + 1.0f, x0);
+      const SlabW w = slab_weights(oa, ob, L, K);
+      const int ia = cell_of(w.ra) + c_oth, ib = cell_of(w.rb) + c_oth;
+      const size_t row = (size_t)s * st_drv;
+      if ((unsigned)ia < (unsigned)n_oth) {
+        float f[V];
+        Pack<V>::ld(base, row + (size_t)ia * st_oth, f);
+#pragma unroll
+        for (int c = 0; c < V; ++c) acc[c] = fmaf(w.wa, f[c], acc[c]);
+      }
+      if (w.wb != 0.0f && (unsigned)ib < (unsigned)n_oth) {
+        float f[V];
+        Pack<V>::ld(base, row + (size_t)ib * st_oth, f);
+#pragma unroll
+        for (int c = 0; c < V; ++c) acc[c] = fmaf(w.wb, f[c], acc[c]);
+      }
+      oa = ob;
+      y += 1.0f;
+    }
+    const size_t e = (size_t)g * d.nray + r;
+    if (MODE == 1) {
+      float b[V];
+      Pack<V>::ld(bs, e, b);
+#pragma unroll
+      for (int c = 0; c < V; ++c) acc[c] = b[c] - acc[c];
+    }
+    Pack<V>::st(out, e, acc);
+  }
+  if (MODE == 2) {
+    double v[V];
+#pragma unroll
+    for (int c = 0; c < V; ++c) v[c] = (double)acc[c] * (double)acc[c];
+    grid_reduce<V>(v, part + (size_t)g * gridDim.x * V, counter + g, gridDim.x, blockIdx.x, threadIdx.x, 128,
+                   [&](double(&sum)[V]) {
+#pragma unroll
+                     for (int c = 0; c < V; ++c) {
+                       const int sl = g * V + c;
+                       const double gamma = sc.gamma[sl];
+                       sc.a[sl] = (sum[c] > 0.0 && gamma > 0.0) ? (float)(gamma / sum[c]) : 0.0f;  // S4
+                     }
+                   });
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a2  P^T (gather): one thread per (pixel, slice group). For every view the bins whose rays can
+// cross the pixel form a short window around the projection of the pixel centre; the window is a
+// strict superset (half diagonal of the pixel, projected, plus a guard), and slab_weights() gives
+// exactly 0 for rays that miss. Accumulation order is fixed (views ascending, bins ascending).
+// MODE 0: out = P^T y
+// MODE 2: out = g = P^T r and, fused, u += a s (App. I step 2) for the pixel it owns.
+// (gamma, beta come from the re-orthogonalisation pass that follows, ctr_api.cu.)
+// ------------------------------------------------------------------------------------------------
+template <int V, int MODE>
+__global__ void __launch_bounds__(128) k_fan_back(Dims d, const float4* __restrict__ rays,
+                                                  const float2* __restrict__ views,
+                                                  const float* __restrict__ sino, float* __restrict__ out,
+                                                  const float* __restrict__ s_img, float* __restrict__ u_img, Scal sc) {
+  const int i = blockIdx.x * 32 + threadIdx.x;
+  const int j = blockIdx.y * 4 + threadIdx.y;
+  const int g = blockIdx.z;
+  const bool active = (i < d.nx) && (j < d.ny);
+  float acc[V];
+#pragma unroll
+  for (int c = 0; c < V; ++c) acc[c] = 0.0f;
+
+  if (active) {
+    const float fi = (float)(i - d.c0x), fj = (float)(j - d.c0y);
+    const float bi = bias_of(i - d.c0x), bj = bias_of(j - d.c0y);
+    const float px = fmaf((float)i + 0.5f, d.dx, d.xlo), py = fmaf((float)j + 0.5f, d.dy, d.ylo);
+    const float* sg = sino + (size_t)g * d.nray * V;
+    const float rp = d.rvox, sdu = d.dsd * d.inv_du;
+    for (int k = 0; k < d.nviews; ++k) {
+      const float2 cs = __ldg(&views[k]);
+      const float den = fmaf(px, cs.x, fmaf(py, cs.y, d.dso));  // distance along the central ray
+      const float aa = fmaf(py, cs.x, -px * cs.y);              // lateral offset
+      const float ell = sqrtf(fmaf(aa, aa, den * den));
+      float bc, hb;
+      if (d.det_type == 0) {
+        const float inv = 1.0f / (den - rp);
+        bc = fmaf(sdu * aa, 1.0f / den, d.boff_u);
+        hb = rp * sdu * (ell + rp) * inv * inv;
+      } else {
+        bc = fmaf(atan2f(aa, den), sdu, d.boff_u);
+        hb = rp * sdu / (ell - rp);
+      }
+      const int b_lo = max(0, (int)ceilf(bc - hb - 0.02f));
+      const int b_hi = min(d.nu - 1, (int)floorf(bc + hb + 0.02f));
+      const int rbase = k * d.nu;
+      for (int b = b_lo; b <= b_hi; ++b) {
+        const float4 R = __ldg(&rays[rbase + b]);
+        const bool xdrv = R.z < 0.0f;
+        const float sc_ = xdrv ? fi : fj, tgt = xdrv ? bj : bi;
+        const float oa = fmaf(R.y, sc_, R.x);
+        const float ob = fmaf(R.y, sc_ + 1.0f, R.x);
+        const SlabW w = slab_weights(oa, ob, fabsf(R.z), R.w);
+        const float wt = (w.ra == tgt ? w.wa : 0.0f) + (w.rb == tgt ? w.wb : 0.0f);
+        if (wt != 0.0f) {
+          float y[V];
+          Pack<V>::ld(sg, (size_t)(rbase + b), y);
+#pragma unroll
+          for (int c = 0; c < V; ++c) acc[c] = fmaf(wt, y[c], acc[c]);
+        }
+      }
+    }
+    const size_t e = (size_t)g * d.npix + (size_t)j * d.nx + i;
+    Pack<V>::st(out, e, acc);
+    if (MODE == 2) {
+      float sv[V], uv[V];
+      Pack<V>::ldcg(s_img, e, sv);
+      Pack<V>::ldcg(u_img, e, uv);
+#pragma unroll
+      for (int c = 0; c < V; ++c) uv[c] = fmaf(sc.a[g * V + c], sv[c], uv[c]);
+      Pack<V>::st(u_img, e, uv);
+    }
+  }
+}
+
+template <int V>
+static int fan_forward_v(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st) {
+  const Dims& d = h->d;
+  dim3 grid((d.nray + 127) / 128, d.G);
+  unsigned* cnt = h->counters + 0 * d.G;
+  ProfScope prof(h, CTR_PROF_FORWARD, st);
+  if (mode == 0) k_fan_forward<V, 0><<<grid, 128, 0, st>>>(d, h->rays, img, out, bs, h->sc, h->part, cnt);
+  else if (mode == 1) k_fan_forward<V, 1><<<grid, 128, 0, st>>>(d, h->rays, img, out, bs, h->sc, h->part, cnt);
+  else k_fan_forward<V, 2><<<grid, 128, 0, st>>>(d, h->rays, img, out, bs, h->sc, h->part, cnt);
+  CTR_LAUNCHED(h);
+  return CTR_OK;
+}
+
+int fan_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st) {
+  return h->d.V == 1 ? fan_forward_v<1>(h, img, out, mode, bs, st) : fan_forward_v<4>(h, img, out, mode, bs, st);
+}
+
+template <int V>
+static int fan_back_v(ctr_handle* h, const float* sino, float* out, int mode, const float* s, float* u, cudaStream_t st) {
+  const Dims& d = h->d;
+  dim3 grid((d.nx + 31) / 32, (d.ny + 3) / 4, d.G), block(32, 4);
+  ProfScope prof(h, CTR_PROF_BACK, st);
+  if (mode == 0) k_fan_back<V, 0><<<grid, block, 0, st>>>(d, h->rays, h->views, sino, out, s, u, h->sc);
+  else k_fan_back<V, 2><<<grid, block, 0, st>>>(d, h->rays, h->views, sino, out, s, u, h->sc);
+  CTR_LAUNCHED(h);
+  return CTR_OK;
+}
+
+int fan_back(ctr_handle* h, const float* sino, float* out, int mode, const float* s, float* u, cudaStream_t st) {
+  return h->d.V == 1 ? fan_back_v<1>(h, sino, out, mode, s, u, st) : fan_back_v<4>(h, sino, out, mode, s, u, st);
+}
+
+}  // namespace ctr

@@ -1,0 +1,151 @@
+// Host-side internals of libctr: the handle and the launch helpers shared by the .cu files.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/ctr.h"
+
+namespace ctr {
+
+#define CTR_MAX_ARMIJO 32
+#define CTR_STAT_SWEEPS 4096 /* ring capacity, in sweeps */
+#define CTR_PROF_MAX 32768
+#define CTR_MAX_BASIS 64 /* stored CGLS gradients used for re-orthogonalisation */
+#define CTR_NCOUNTERS 8
+
+// Plain-data description of the problem, passed by value to every kernel.
+struct Dims {
+  int ndim;
+  int nx, ny, nz;
+  int nviews, nu, nv;
+  int c0x, c0y, c0z;      // grid line taken as coordinate origin (n/2)
+  int npix;               // voxels per slice / volume
+  int nray;               // rays per slice / volume
+  int G, B, V;            // groups, true batch, slices per group
+  float xlo, ylo, zlo;    // mm, lower corner of the grid
+  float dx, dy, dz;       // mm
+  float dso, dsd;
+  float inv_du, inv_dv;   // 1/pitch
+  float boff_u, boff_v;   // (n-1)/2 - off : bin = coord/pitch + boff
+  float rvox;             // half diagonal of a voxel, mm
+  int det_type;
+};
+
+// Per-slice device scalars (arrays of length Bp = G*V).
+struct Scal {
+  double* gamma;   // ||P^T r||^2
+  float* a;        // CGLS step
+  float* beta;     // CGLS beta
+  float* sigma2;   // sigma^2 of the current sweep
+  double* e0;      // energy at the sweep start
+  double* g2;      // ||g||^2
+  int* kacc;       // accepted Armijo index or -1
+  float* tacc;     // accepted step
+  unsigned* sel_prefix;  // radix-select state
+  unsigned* sel_rank;
+  float* ginv;     // 1/||g|| of the newest CGLS gradient (0 when g = 0)
+  float* coef;     // [CTR_MAX_BASIS][Bp] projections of g on the stored unit gradients
+};
+
+struct TvParams {
+  float lambda, eps, c_armijo;
+  int kmax;
+  int weights_mode;
+  float t[CTR_MAX_ARMIJO];
+};
+
+}  // namespace ctr
+
+struct ctr_handle {
+  ctr_geometry g;
+  ctr_params p;
+  ctr::Dims d;
+  int device;
+  // geometry tables
+  float4* rays;    // [nviews*nv*nu]  (2D: {x0, m, +-L, K}); 3D: see ctr_cone.cu
+  float4* rays2;   // 3D second half of the ray record
+  float2* views;   // [nviews] (cos, sin)
+  // scratch, internal layout [G][n][V]
+  size_t nimg, nsino;  // floats per internal image / sinogram (all groups)
+  float *ximg, *bsino, *r, *q, *s, *gimg, *v, *w, *n0;
+  float* basis;         // [basis_cap][nimg] unit CGLS gradients (S24)
+  int basis_cap;
+  double* part;
+  size_t part_len;
+  unsigned* counters;   // [CTR_NCOUNTERS][G]
+  unsigned* hist;       // [Bp][2048]
+  ctr::Scal sc;
+  void* scal_block;
+  ctr_sweep_stat* stats;     // device ring [CTR_STAT_SWEEPS][Bp]
+  long long sweep_count;     // sweeps recorded since the last reset
+  unsigned long long sel_k;  // rank of the sigma order statistic (1-based), from the current quantile
+  float sel_q;
+  cudaStream_t last_stream;
+  long long launches;
+  // optional event profiler (ctr_profile_*)
+  int prof_on;
+  int prof_n;                 // intervals recorded
+  cudaEvent_t* prof_ev;       // [2 * CTR_PROF_MAX]
+  unsigned char* prof_kind;   // [CTR_PROF_MAX]
+  char err[256];
+};
+
+namespace ctr {
+
+inline int set_err(ctr_handle* h, int code, const char* msg) {
+  if (h) snprintf(h->err, sizeof(h->err), "%s", msg);
+  return code;
+}
+
+inline int cuda_fail(ctr_handle* h, cudaError_t e, const char* where) {
+  if (h) snprintf(h->err, sizeof(h->err), "%s: %s", where, cudaGetErrorString(e));
+  return CTR_ECUDA;
+}
+
+#define CTR_CUDA(h, call)                                         \
+  do {                                                            \
+    cudaError_t e__ = (call);                                     \
+    if (e__ != cudaSuccess) return ctr::cuda_fail(h, e__, #call); \
+  } while (0)
+
+#define CTR_LAUNCHED(h)                                                       \
+  do {                                                                        \
+    (h)->launches++;                                                          \
+    cudaError_t e__ = cudaPeekAtLastError();                                  \
+    if (e__ != cudaSuccess) return ctr::cuda_fail(h, e__, "kernel launch");   \
+  } while (0)
+
+// RAII interval of the event profiler: records an event pair on `st` around a scope when enabled.
+struct ProfScope {
+  ctr_handle* h;
+  cudaStream_t st;
+  int slot;
+  ProfScope(ctr_handle* h_, int kind, cudaStream_t st_) : h(h_), st(st_), slot(-1) {
+    if (h->prof_on && h->prof_n < CTR_PROF_MAX) {
+      slot = h->prof_n++;
+      h->prof_kind[slot] = (unsigned char)kind;
+      cudaEventRecord(h->prof_ev[2 * slot], st);
+    }
+  }
+  ~ProfScope() {
+    if (slot >= 0) cudaEventRecord(h->prof_ev[2 * slot + 1], st);
+  }
+};
+
+// implemented in ctr_fan.cu (2D fan beam, V = 1 or 4)
+int fan_build_tables(ctr_handle* h);
+int fan_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st);
+int fan_back(ctr_handle* h, const float* sino, float* out, int mode, const float* s, float* u, cudaStream_t st);
+// implemented in ctr_cone.cu (3D cone beam, V = 1)
+int cone_build_tables(ctr_handle* h);
+int cone_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st);
+int cone_back(ctr_handle* h, const float* sino, float* out, int mode, const float* s, float* u, cudaStream_t st);
+// implemented in ctr_tv.cu
+int tv_update_weights(ctr_handle* h, const float* f, float* w, cudaStream_t st);
+int tv_sweep(ctr_handle* h, float* f, const float* v, const float* w, float lambda, int clamp, cudaStream_t st);
+int tv_clamp(ctr_handle* h, float* f, cudaStream_t st);
+// implemented in ctr_api.cu
+
+}  // namespace ctr

@@ -1,0 +1,522 @@
+// Edge-preserving TV step for sm_100a (2D slices with V = 1 or 4 slices per element, and 3D volumes
+// with V = 1): face magnitudes A3, exact sigma order statistic, weights, gradient A2, Armijo trials and
+// the descent update (+ positivity clamp).
+//   A3 / weights : PAPER.md:106-110 (Eq. 4-5, sigma from the histogram), :458-463
+//   A2 / gradient: PAPER.md:151-153 (Eq. 9-10), :453
+//   Armijo       : PAPER.md:149;  clamp: PAPER.md:157, :173
+// Readings: S5/S7/S8 faces, S9/S10 sigma = exact q-quantile, S11 eps, S12 replicate border
+// with zero border flux, S14 Armijo constants, S22 3D generalisation.
+#include "ctr_common.cuh"
+#include "ctr_internal.h"
+
+namespace ctr {
+
+#define TV_KC 4 /* Armijo candidates evaluated per pass */
+
+// ---------------------------------------------------------------------------------------------
+// Neighbourhood access. The stencil of A2/A3 around voxel p needs f at p + {-1,0,1}^ndim minus
+// the far corners; we load the full 3x3 (2D) or 3x3x3 (3D) window with per-axis clamped indices
+// (replicate border, S12) so the formulas below need no special cases.
+// ---------------------------------------------------------------------------------------------
+template <int V, int ND>
+struct Window {
+  float c[ND == 3 ? 3 : 1][3][3][V];  // [dz+1][dy+1][dx+1][slice]
+};
+
+template <int V, int ND>
+__device__ __forceinline__ void load_window(const Dims& d, const float* __restrict__ f, int g, int i, int j, int k,
+                                            Window<V, ND>& w) {
+  const float* base = f + (size_t)g * d.npix * V;
+  int xi[3] = {max(i - 1, 0), i, min(i + 1, d.nx - 1)};
+  int yj[3] = {max(j - 1, 0), j, min(j + 1, d.ny - 1)};
+  if (ND == 3) {
+    int zk[3] = {max(k - 1, 0), k, min(k + 1, d.nz - 1)};
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+      for (int b = 0; b < 3; ++b)
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+          Pack<V>::ldcg(base, ((size_t)zk[a] * d.ny + yj[b]) * d.nx + xi[c], w.c[ND == 3 ? a : 0][b][c]);
+  } else {
+#pragma unroll
+    for (int b = 0; b < 3; ++b)
+#pragma unroll
+      for (int c = 0; c < 3; ++c) Pack<V>::ldcg(base, (size_t)yj[b] * d.nx + xi[c], w.c[0][b][c]);
+  }
+}
+
+// N0^2 of the face between window cell q and q + e_A (A3), for slice lane s.
+// q is given as window coordinates (qz,qy,qx) in {0,1,2}; the caller guarantees q+e_A and q +- e_T
+// stay inside the window (true for the faces adjacent to the centre cell).
+template <int V, int ND>
+__device__ __forceinline__ float face_n0sq(const Window<V, ND>& w, int A, int qz, int qy, int qx, int s) {
+  const int ez = (A == 2), ey = (A == 1), ex = (A == 0);
+  const float lo = w.c[qz][qy][qx][s], hi = w.c[qz + ez][qy + ey][qx + ex][s];
+  const float dd = hi - lo;
+  float n0 = dd * dd;
+  const float m0 = 0.5f * (hi + lo);
+#pragma unroll
+  for (int T = 0; T < ND; ++T) {
+    if (T == A) continue;
+    const int tz = (T == 2), ty = (T == 1), tx = (T == 0);
+    const float mp = 0.5f * (w.c[qz + ez + tz][qy + ey + ty][qx + ex + tx][s] + w.c[qz + tz][qy + ty][qx + tx][s]);
+    const float mm = 0.5f * (w.c[qz + ez - tz][qy + ey - ty][qx + ex - tx][s] + w.c[qz - tz][qy - ty][qx - tx][s]);
+    const float a = mp - m0, b = m0 - mm;
+    n0 = fmaf(0.5f * a, a, n0);
+    n0 = fmaf(0.5f * b, b, n0);
+  }
+  return n0;
+}
+
+// thread -> voxel mapping shared by all stencil kernels: block (32,4), grid (nx/32, ny/4 * nz, G)
+struct Vox {
+  int i, j, k, g, tid;
+  bool active;
+  unsigned blk, nblk;
+};
+__device__ __forceinline__ Vox vox_of_thread(const Dims& d) {
+  Vox v;
+  const int nby = (d.ny + 3) / 4;
+  v.i = blockIdx.x * 32 + threadIdx.x;
+  v.k = blockIdx.y / nby;
+  v.j = (blockIdx.y - v.k * nby) * 4 + threadIdx.y;
+  v.g = blockIdx.z;
+  v.tid = threadIdx.y * 32 + threadIdx.x;
+  v.active = v.i < d.nx && v.j < d.ny;
+  v.blk = blockIdx.y * gridDim.x + blockIdx.x;
+  v.nblk = gridDim.x * gridDim.y;
+  return v;
+}
+static dim3 vox_grid(const Dims& d) { return dim3((d.nx + 31) / 32, ((d.ny + 3) / 4) * d.nz, d.G); }
+
+// ---------------------------------------------------------------------------------------------
+// a4.1  faces: N0^2 of the ND faces owned by each voxel (towards +x, +y, +z) -> n0 planes, plus the
+// first radix pass (top 11 of the 31 value bits) of the per-slice histogram over INTERIOR faces.
+// Exact zeros (flat regions) are counted with a ballot instead of hammering one shared bin.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void hist_add(unsigned* hist_s, unsigned bits, int shift, unsigned mask, bool valid) {
+  const unsigned bin = (bits >> shift) & mask;
+  const bool zero = valid && bin == 0;
+  const unsigned zb = __ballot_sync(0xffffffffu, zero);
+  if (valid && bin != 0) atomicAdd(&hist_s[bin], 1u);
+  if ((threadIdx.x & 31) == 0 && zb) atomicAdd(&hist_s[0], (unsigned)__popc(zb));
+}
+
+template <int V, int ND>
+__global__ void __launch_bounds__(128) k_tv_faces(Dims d, const float* __restrict__ f, float* __restrict__ n0,
+                                                  unsigned* __restrict__ hist) {
+  __shared__ unsigned hs[V][2048];
+  const Vox p = vox_of_thread(d);
+  for (int t = p.tid; t < V * 2048; t += 128) (&hs[0][0])[t] = 0;
+  __syncthreads();
+  const int lim[3] = {d.nx - 1, d.ny - 1, d.nz - 1};
+  const int pos[3] = {p.i, p.j, p.k};
+  float val[ND][V];
+  if (p.active) {
+    Window<V, ND> w;
+    load_window<V, ND>(d, f, p.g, p.i, p.j, p.k, w);
+    const int cz = (ND == 3) ? 1 : 0;
+#pragma unroll
+    for (int A = 0; A < ND; ++A)
+#pragma unroll
+      for (int s = 0; s < V; ++s) val[A][s] = pos[A] < lim[A] ? face_n0sq<V, ND>(w, A, cz, 1, 1, s) : 0.0f;
+    const size_t e = (size_t)p.g * d.npix + ((size_t)p.k * d.ny + p.j) * d.nx + p.i;
+#pragma unroll
+    for (int A = 0; A < ND; ++A) Pack<V>::st(n0 + (size_t)A * d.G * d.npix * V, e, val[A]);
+  }
+#pragma unroll
+  for (int A = 0; A < ND; ++A) {
+    const bool valid = p.active && pos[A] < lim[A];
+#pragma unroll
+    for (int s = 0; s < V; ++s) hist_add(hs[s], valid ? __float_as_uint(val[A][s]) : 0u, 20, 2047u, valid);
+  }
+  __syncthreads();
+  for (int t = p.tid; t < V * 2048; t += 128) {
+    const unsigned c = (&hs[0][0])[t];
+    if (c) atomicAdd(&hist[(size_t)(p.g * V + t / 2048) * 2048 + (t & 2047)], c);
+  }
+}
+
+// a4.2  later radix passes over the stored N0^2 planes: only values whose higher bits equal the
+// prefix found so far are counted.
+template <int V, int ND>
+__global__ void __launch_bounds__(128) k_tv_hist(Dims d, const float* __restrict__ n0, unsigned* __restrict__ hist,
+                                                 Scal sc, int shift, unsigned mask, int prefix_shift) {
+  __shared__ unsigned hs[V][1024];
+  const Vox p = vox_of_thread(d);
+  for (int t = p.tid; t < V * 1024; t += 128) (&hs[0][0])[t] = 0;
+  __syncthreads();
+  const int lim[3] = {d.nx - 1, d.ny - 1, d.nz - 1};
+  const int pos[3] = {p.i, p.j, p.k};
+  unsigned pre[V];
+#pragma unroll
+  for (int s = 0; s < V; ++s) pre[s] = sc.sel_prefix[p.g * V + s] >> prefix_shift;
+  const size_t e = (size_t)p.g * d.npix + ((size_t)p.k * d.ny + p.j) * d.nx + p.i;
+#pragma unroll
+  for (int A = 0; A < ND; ++A) {
+    float val[V];
+    const bool inside = p.active && pos[A] < lim[A];
+    if (inside) Pack<V>::ldcg(n0 + (size_t)A * d.G * d.npix * V, e, val);
+#pragma unroll
+    for (int s = 0; s < V; ++s) {
+      const unsigned bits = inside ? __float_as_uint(val[s]) : 0u;
+      const bool valid = inside && (bits >> prefix_shift) == pre[s];
+      hist_add(hs[s], bits, shift, mask, valid);
+    }
+  }
+  __syncthreads();
+  for (int t = p.tid; t < V * 1024; t += 128) {
+    const unsigned c = (&hs[0][0])[t];
+    if (c) atomicAdd(&hist[(size_t)(p.g * V + t / 1024) * 2048 + (t & 1023)], c);
+  }
+}
+
+// a4.3  per slice: find the bin holding the element of rank sel_rank, extend the prefix, clear the
+// histogram. After the last pass the prefix IS the bit pattern of the k-th smallest N0^2 (O6).
+__global__ void __launch_bounds__(256) k_tv_select(Scal sc, unsigned* __restrict__ hist, int nbins, int shift,
+                                                   int first, int final_pass, unsigned long long rank0, float eps2,
+                                                   ctr_sweep_stat* stats, int nslices) {
+  __shared__ unsigned tot[256];
+  __shared__ unsigned found_bin, found_before;
+  const int sl = blockIdx.x, t = threadIdx.x;
+  unsigned* h = hist + (size_t)sl * 2048;
+  const int per = nbins / 256;  // 8 or 4
+  unsigned loc[8], sum = 0;
+  for (int q = 0; q < per; ++q) { loc[q] = h[t * per + q]; sum += loc[q]; }
+  tot[t] = sum;
+  __syncthreads();
+  // inclusive scan over the 256 thread totals (Hillis-Steele; tiny)
+  for (int o = 1; o < 256; o <<= 1) {
+    unsigned add = t >= o ? tot[t - o] : 0u;
+    __syncthreads();
+    tot[t] += add;
+    __syncthreads();
+  }
+  const unsigned rank = first ? (unsigned)rank0 : sc.sel_rank[sl];
+  const unsigned before = tot[t] - sum;
+  if (rank > before && rank <= tot[t]) {
+    unsigned cum = before;
+    for (int q = 0; q < per; ++q) {
+      if (rank <= cum + loc[q]) { found_bin = t * per + q; found_before = cum; break; }
+      cum += loc[q];
+    }
+  }
+  __syncthreads();
+  for (int q = 0; q < per; ++q) h[t * per + q] = 0;
+  if (t == 0) {
+    const unsigned prefix = (first ? 0u : sc.sel_prefix[sl]) | (found_bin << shift);
+    sc.sel_prefix[sl] = prefix;
+    sc.sel_rank[sl] = rank - found_before;
+    if (final_pass) {
+      const float s2 = fmaxf(__uint_as_float(prefix), eps2);
+      sc.sigma2[sl] = s2;
+      if (stats) stats[sl].sigma = sqrt((double)s2);
+    }
+  }
+  (void)nslices;
+}
+
+// a4.4  w = exp(-N0^2/sigma^2) on interior faces, 0 on border faces; TV mode: 1
+template <int V, int ND>
+__global__ void __launch_bounds__(128) k_tv_weights(Dims d, const float* __restrict__ n0, float* __restrict__ w,
+                                                    Scal sc, int mode) {
+  const Vox p = vox_of_thread(d);
+  if (!p.active) return;
+  const int lim[3] = {d.nx - 1, d.ny - 1, d.nz - 1};
+  const int pos[3] = {p.i, p.j, p.k};
+  const size_t e = (size_t)p.g * d.npix + ((size_t)p.k * d.ny + p.j) * d.nx + p.i;
+  float inv[V];
+#pragma unroll
+  for (int s = 0; s < V; ++s) inv[s] = -1.0f / sc.sigma2[p.g * V + s];
+#pragma unroll
+  for (int A = 0; A < ND; ++A) {
+    float val[V], o[V];
+    Pack<V>::ldcg(n0 + (size_t)A * d.G * d.npix * V, e, val);
+#pragma unroll
+    for (int s = 0; s < V; ++s) o[s] = pos[A] < lim[A] ? (mode == 1 ? 1.0f : expf(val[s] * inv[s])) : 0.0f;
+    Pack<V>::st(w + (size_t)A * d.G * d.npix * V, e, o);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a5  gradient g = lambda (f - v) - sum_A (flux_A(p) - flux_A(p - e_A)),
+//     flux_A = w_A d_A / sqrt(N0^2 + eps^2) (A2), plus G = ||g||^2 and E0 (O9).
+// ---------------------------------------------------------------------------------------------
+template <int V, int ND>
+__global__ void __launch_bounds__(128) k_tv_gradient(Dims d, const float* __restrict__ f, const float* __restrict__ v,
+                                                     const float* __restrict__ w, float* __restrict__ gout,
+                                                     TvParams tp, Scal sc, double* part, unsigned* counter) {
+  const Vox p = vox_of_thread(d);
+  double red[2 * V];
+#pragma unroll
+  for (int s = 0; s < 2 * V; ++s) red[s] = 0.0;
+  if (p.active) {
+    Window<V, ND> win;
+    load_window<V, ND>(d, f, p.g, p.i, p.j, p.k, win);
+    const int cz = (ND == 3) ? 1 : 0;
+    const int pos[3] = {p.i, p.j, p.k};
+    const size_t stride[3] = {1, (size_t)d.nx, (size_t)d.nx * d.ny};
+    const size_t e = (size_t)p.g * d.npix + ((size_t)p.k * d.ny + p.j) * d.nx + p.i;
+    const size_t plane = (size_t)d.G * d.npix * V;
+    const float eps2 = tp.eps * tp.eps;
+    float vv[V], gv[V], etv[V];
+    Pack<V>::ldcg(v, e, vv);
+#pragma unroll
+    for (int s = 0; s < V; ++s) {
+      gv[s] = tp.lambda * (win.c[cz][1][1][s] - vv[s]);
+      etv[s] = 0.0f;
+    }
+#pragma unroll
+    for (int A = 0; A < ND; ++A) {
+      float wp[V], wm[V];
+      Pack<V>::ldcg(w + A * plane, e, wp);  // border faces store 0
+      if (pos[A] > 0) Pack<V>::ldcg(w + A * plane, e - stride[A], wm);
+      else {
+#pragma unroll
+        for (int s = 0; s < V; ++s) wm[s] = 0.0f;
+      }
+      const int ez = (A == 2), ey = (A == 1), ex = (A == 0);
+#pragma unroll
+      for (int s = 0; s < V; ++s) {
+        // face towards +A (owned by this voxel) and face towards -A (owned by the neighbour)
+        const float n0p = face_n0sq<V, ND>(win, A, cz, 1, 1, s) + eps2;
+        const float n0m = face_n0sq<V, ND>(win, A, cz - ez, 1 - ey, 1 - ex, s) + eps2;
+        const float dp = win.c[cz + ez][1 + ey][1 + ex][s] - win.c[cz][1][1][s];
+        const float dm = win.c[cz][1][1][s] - win.c[cz - ez][1 - ey][1 - ex][s];
+        const float fp = (wp[s] != 0.0f && n0p > 0.0f) ? wp[s] * dp * rsqrtf(n0p) : 0.0f;
+        const float fm = (wm[s] != 0.0f && n0m > 0.0f) ? wm[s] * dm * rsqrtf(n0m) : 0.0f;
+        gv[s] -= fp - fm;
+        etv[s] = fmaf(wp[s], sqrtf(n0p) - tp.eps, etv[s]);
+      }
+    }
+    Pack<V>::st(gout, e, gv);
+#pragma unroll
+    for (int s = 0; s < V; ++s) {
+      const float df = win.c[cz][1][1][s] - vv[s];
+      red[s] = (double)gv[s] * (double)gv[s];
+      red[V + s] = 0.5 * (double)tp.lambda * (double)df * (double)df + (double)etv[s] / (double)ND;
+    }
+  }
+  grid_reduce<2 * V>(red, part + (size_t)p.g * p.nblk * 2 * V, counter + p.g, p.nblk, p.blk, p.tid, 128,
+                     [&](double(&sum)[2 * V]) {
+#pragma unroll
+                       for (int s = 0; s < V; ++s) {
+                         const int sl = p.g * V + s;
+                         sc.g2[sl] = sum[s];
+                         sc.e0[sl] = sum[V + s];
+                         sc.kacc[sl] = -1;
+                         sc.tacc[sl] = 0.0f;
+                       }
+                     });
+}
+
+// ---------------------------------------------------------------------------------------------
+// a6.1  Armijo trials k0 .. k0+TV_KC-1 in one pass: E(f - t_k g) with w frozen (O9). Slices that
+// already accepted a step contribute nothing; a group whose slices are all done exits at once.
+// ---------------------------------------------------------------------------------------------
+template <int V, int ND>
+__global__ void __launch_bounds__(128) k_tv_trial(Dims d, const float* __restrict__ f, const float* __restrict__ gin,
+                                                  const float* __restrict__ v, const float* __restrict__ w, TvParams tp,
+                                                  int k0, Scal sc, double* part, unsigned* counter) {
+  const Vox p = vox_of_thread(d);
+  bool todo[V], any = false;
+#pragma unroll
+  for (int s = 0; s < V; ++s) { todo[s] = sc.kacc[p.g * V + s] < 0; any |= todo[s]; }
+  if (!any) return;
+  double red[TV_KC * V];
+#pragma unroll
+  for (int s = 0; s < TV_KC * V; ++s) red[s] = 0.0;
+  if (p.active) {
+    Window<V, ND> wf, wg;
+    load_window<V, ND>(d, f, p.g, p.i, p.j, p.k, wf);
+    load_window<V, ND>(d, gin, p.g, p.i, p.j, p.k, wg);
+    const int cz = (ND == 3) ? 1 : 0;
+    const size_t e = (size_t)p.g * d.npix + ((size_t)p.k * d.ny + p.j) * d.nx + p.i;
+    const size_t plane = (size_t)d.G * d.npix * V;
+    const float eps2 = tp.eps * tp.eps;
+    float vv[V], wA[ND][V];
+    Pack<V>::ldcg(v, e, vv);
+#pragma unroll
+    for (int A = 0; A < ND; ++A) Pack<V>::ldcg(w + A * plane, e, wA[A]);
+#pragma unroll
+    for (int c = 0; c < TV_KC; ++c) {
+      if (k0 + c >= tp.kmax) break;
+      const float t = tp.t[k0 + c];
+      Window<V, ND> wt;
+#pragma unroll
+      for (int a = 0; a < (ND == 3 ? 3 : 1); ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b)
+#pragma unroll
+          for (int x = 0; x < 3; ++x)
+#pragma unroll
+            for (int s = 0; s < V; ++s) wt.c[a][b][x][s] = fmaf(-t, wg.c[a][b][x][s], wf.c[a][b][x][s]);
+#pragma unroll
+      for (int s = 0; s < V; ++s) {
+        if (!todo[s]) continue;
+        float etv = 0.0f;
+#pragma unroll
+        for (int A = 0; A < ND; ++A)
+          if (wA[A][s] != 0.0f) etv = fmaf(wA[A][s], sqrtf(face_n0sq<V, ND>(wt, A, cz, 1, 1, s) + eps2) - tp.eps, etv);
+        const float df = wt.c[cz][1][1][s] - vv[s];
+        red[c * V + s] = 0.5 * (double)tp.lambda * (double)df * (double)df + (double)etv / (double)ND;
+      }
+    }
+  }
+  grid_reduce<TV_KC * V>(red, part + (size_t)p.g * p.nblk * TV_KC * V, counter + p.g, p.nblk, p.blk, p.tid, 128,
+                         [&](double(&sum)[TV_KC * V]) {
+#pragma unroll
+                           for (int s = 0; s < V; ++s) {
+                             const int sl = p.g * V + s;
+                             if (sc.kacc[sl] >= 0) continue;
+                             const double e0 = sc.e0[sl], g2 = sc.g2[sl];
+                             for (int c = 0; c < TV_KC && k0 + c < tp.kmax; ++c) {
+                               const double t = (double)tp.t[k0 + c];
+                               if (sum[c * V + s] <= e0 - (double)tp.c_armijo * t * g2) {
+                                 sc.kacc[sl] = k0 + c;
+                                 sc.tacc[sl] = tp.t[k0 + c];
+                                 break;
+                               }
+                             }
+                           }
+                         });
+}
+
+// a6.2 + a7  f <- f - t g for slices that accepted a step; optional positivity clamp; sweep record.
+template <int V>
+__global__ void __launch_bounds__(256) k_tv_apply(Dims d, float* __restrict__ f, const float* __restrict__ gin, Scal sc,
+                                                  int clamp, ctr_sweep_stat* stats) {
+  const int g = blockIdx.y;
+  const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
+  if (idx == 0 && stats) {
+#pragma unroll
+    for (int s = 0; s < V; ++s) {
+      const int sl = g * V + s;
+      stats[sl].e0 = sc.e0[sl];
+      stats[sl].g2 = sc.g2[sl];
+      stats[sl].k = sc.kacc[sl];
+    }
+  }
+  if (idx >= (size_t)d.npix) return;
+  const size_t e = (size_t)g * d.npix + idx;
+  float fv[V], gv[V];
+  Pack<V>::ldcg(f, e, fv);
+  Pack<V>::ldcg(gin, e, gv);
+#pragma unroll
+  for (int s = 0; s < V; ++s) {
+    const float t = sc.tacc[g * V + s];  // 0 when nothing was accepted
+    float nf = sc.kacc[g * V + s] >= 0 ? fmaf(-t, gv[s], fv[s]) : fv[s];
+    if (clamp) nf = fmaxf(nf, 0.0f);
+    fv[s] = nf;
+  }
+  Pack<V>::st(f, e, fv);
+}
+
+template <int V>
+__global__ void __launch_bounds__(256) k_clamp(Dims d, float* __restrict__ f) {
+  const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
+  if (idx >= (size_t)d.npix) return;
+  const size_t e = (size_t)blockIdx.y * d.npix + idx;
+  float fv[V];
+  Pack<V>::ldcg(f, e, fv);
+#pragma unroll
+  for (int s = 0; s < V; ++s) fv[s] = fmaxf(fv[s], 0.0f);
+  Pack<V>::st(f, e, fv);
+}
+
+// ---------------------------------------------------------------------------------------------
+// host drivers
+// ---------------------------------------------------------------------------------------------
+static ctr_sweep_stat* stat_slot(ctr_handle* h) {
+  const int Bp = h->d.G * h->d.V;
+  return h->stats + (size_t)(h->sweep_count % CTR_STAT_SWEEPS) * Bp;
+}
+
+template <int V, int ND>
+static int tv_update_weights_t(ctr_handle* h, const float* f, float* w, cudaStream_t st) {
+  const Dims& d = h->d;
+  const dim3 grid = vox_grid(d), block(32, 4);
+  const int Bp = d.G * d.V;
+  const float eps2 = h->p.eps * h->p.eps;
+  ctr_sweep_stat* rec = stat_slot(h);
+  ProfScope prof(h, CTR_PROF_TV, st);
+  if (h->p.weights_mode == 1) {
+    // plain TV: weights are 1; sigma is not needed (reported as 0)
+    k_tv_faces<V, ND><<<grid, block, 0, st>>>(d, f, h->n0, h->hist);
+    CTR_LAUNCHED(h);
+    CTR_CUDA(h, cudaMemsetAsync(h->hist, 0, sizeof(unsigned) * 2048 * Bp, st));
+  } else {
+    k_tv_faces<V, ND><<<grid, block, 0, st>>>(d, f, h->n0, h->hist);
+    CTR_LAUNCHED(h);
+    k_tv_select<<<Bp, 256, 0, st>>>(h->sc, h->hist, 2048, 20, 1, 0, h->sel_k, eps2, rec, Bp);
+    CTR_LAUNCHED(h);
+    k_tv_hist<V, ND><<<grid, block, 0, st>>>(d, h->n0, h->hist, h->sc, 10, 1023u, 20);
+    CTR_LAUNCHED(h);
+    k_tv_select<<<Bp, 256, 0, st>>>(h->sc, h->hist, 1024, 10, 0, 0, 0, eps2, rec, Bp);
+    CTR_LAUNCHED(h);
+    k_tv_hist<V, ND><<<grid, block, 0, st>>>(d, h->n0, h->hist, h->sc, 0, 1023u, 10);
+    CTR_LAUNCHED(h);
+    k_tv_select<<<Bp, 256, 0, st>>>(h->sc, h->hist, 1024, 0, 0, 1, 0, eps2, rec, Bp);
+    CTR_LAUNCHED(h);
+  }
+  k_tv_weights<V, ND><<<grid, block, 0, st>>>(d, h->n0, w, h->sc, h->p.weights_mode);
+  CTR_LAUNCHED(h);
+  return CTR_OK;
+}
+
+int tv_update_weights(ctr_handle* h, const float* f, float* w, cudaStream_t st) {
+  if (h->d.ndim == 3) return tv_update_weights_t<1, 3>(h, f, w, st);
+  return h->d.V == 1 ? tv_update_weights_t<1, 2>(h, f, w, st) : tv_update_weights_t<4, 2>(h, f, w, st);
+}
+
+static TvParams make_tv_params(const ctr_handle* h, float lambda) {
+  TvParams tp;
+  tp.lambda = lambda;
+  tp.eps = h->p.eps;
+  tp.c_armijo = h->p.armijo_c;
+  tp.kmax = h->p.armijo_max;
+  tp.weights_mode = h->p.weights_mode;
+  double t = (double)h->p.armijo_t0;
+  for (int k = 0; k < CTR_MAX_ARMIJO; ++k) {
+    tp.t[k] = (float)t;
+    t *= (double)h->p.armijo_rho;
+  }
+  return tp;
+}
+
+template <int V, int ND>
+static int tv_sweep_t(ctr_handle* h, float* f, const float* v, const float* w, float lambda, int clamp,
+                      cudaStream_t st) {
+  const Dims& d = h->d;
+  const dim3 grid = vox_grid(d), block(32, 4);
+  const TvParams tp = make_tv_params(h, lambda);
+  float* g = h->gimg;
+  ProfScope prof(h, CTR_PROF_TV, st);
+  k_tv_gradient<V, ND><<<grid, block, 0, st>>>(d, f, v, w, g, tp, h->sc, h->part, h->counters + 2 * d.G);
+  CTR_LAUNCHED(h);
+  for (int k0 = 0; k0 < tp.kmax; k0 += TV_KC) {
+    k_tv_trial<V, ND><<<grid, block, 0, st>>>(d, f, g, v, w, tp, k0, h->sc, h->part, h->counters + 3 * d.G);
+    CTR_LAUNCHED(h);
+  }
+  k_tv_apply<V><<<dim3((d.npix + 255) / 256, d.G), 256, 0, st>>>(d, f, g, h->sc, clamp, stat_slot(h));
+  CTR_LAUNCHED(h);
+  h->sweep_count++;
+  return CTR_OK;
+}
+
+int tv_sweep(ctr_handle* h, float* f, const float* v, const float* w, float lambda, int clamp, cudaStream_t st) {
+  if (h->d.ndim == 3) return tv_sweep_t<1, 3>(h, f, v, w, lambda, clamp, st);
+  return h->d.V == 1 ? tv_sweep_t<1, 2>(h, f, v, w, lambda, clamp, st) : tv_sweep_t<4, 2>(h, f, v, w, lambda, clamp, st);
+}
+
+int tv_clamp(ctr_handle* h, float* f, cudaStream_t st) {
+  const Dims& d = h->d;
+  dim3 grid((d.npix + 255) / 256, d.G);
+  if (d.V == 1) k_clamp<1><<<grid, 256, 0, st>>>(d, f);
+  else k_clamp<4><<<grid, 256, 0, st>>>(d, f);
+  CTR_LAUNCHED(h);
+  return CTR_OK;
+}
+
+}  // namespace ctr

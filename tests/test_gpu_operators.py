@@ -1,0 +1,177 @@
+"""GPU parity of the projector pair through the C ABI (ctr_forward / ctr_back) against the fp64
+oracle, element by element on the same seeded inputs. Tolerance (north_star): relative L2 <= 1e-5
+for one P or P^T application; adjoint identity <= 1e-5; the two kernels' matrices bit-identical."""
+import numpy as np
+import pytest
+
+from ctr_inputs import get_config, make_case, scaled_config
+from ctr_inputs.configs import Config
+
+pytestmark = pytest.mark.gpu
+
+TOL_OP = 1e-5
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+@pytest.fixture(scope="module")
+def ctr():
+    import paper_1009_2288_b200 as m
+    m.load_library()
+    return m
+
+
+def rel(a, b):
+    return float(np.linalg.norm(np.asarray(a, np.float64) - b) / np.linalg.norm(b))
+
+
+def gpu_forward(ctr, torch, cfg, img):
+    h = ctr.ctr_create(cfg)
+    x = torch.from_numpy(np.ascontiguousarray(img, dtype=np.float32)).cuda()
+    y = torch.full(h.sino_shape, float("nan"), dtype=torch.float32, device="cuda")
+    h.ctr_forward(x, y)
+    torch.cuda.synchronize()
+    h.close()
+    return y.cpu().numpy()
+
+
+def gpu_back(ctr, torch, cfg, sino):
+    h = ctr.ctr_create(cfg)
+    y = torch.from_numpy(np.ascontiguousarray(sino, dtype=np.float32)).cuda()
+    x = torch.full(h.img_shape, float("nan"), dtype=torch.float32, device="cuda")
+    h.ctr_back(y, x)
+    torch.cuda.synchronize()
+    h.close()
+    return x.cpu().numpy()
+
+
+def odd2d(**kw):
+    base = dict(name="odd", index=92, ndim=2, nx=37, ny=29, nz=1, dx=1.3, dy=0.9, dz=1.0, nviews=17, nu=53,
+                nv=1, du=1.7, dv=1.0, dso=300.0, dsd=520.0, cx=1.1, cy=-2.3, u_off=0.4, theta0=0.1)
+    base.update(kw)
+    return Config(**base)
+
+
+@pytest.mark.parametrize("name", ["c1", "c2", "c3"])
+def test_forward_and_back_match_oracle(ctr, torch_cuda, orc, name):
+    cfg = get_config(name)
+    case = make_case(cfg)
+    truth, sino = case["truth"][0], case["sino"][0]
+    got = gpu_forward(ctr, torch_cuda, cfg, truth[None])[0]
+    want = orc.forward(cfg, truth.astype(np.float64))
+    assert rel(got, want) <= TOL_OP
+    got = gpu_back(ctr, torch_cuda, cfg, sino[None])[0]
+    want = orc.back(cfg, sino.astype(np.float64))
+    assert rel(got, want) <= TOL_OP
+
+
+@pytest.mark.parametrize("cfg", [odd2d(), odd2d(det_type=1, du=1.0), odd2d(nx=1, ny=1, dx=5.0, dy=5.0),
+                                 odd2d(nviews=8, nu=11, theta0=0.0, cx=0.0, cy=0.0, u_off=0.0)],
+                         ids=["ragged", "arc", "single-pixel", "axis-parallel"])
+def test_odd_geometries_random_inputs(ctr, torch_cuda, orc, cfg):
+    """Ragged sizes (not multiples of any tile), off-centre grid, detector shift, arc detector,
+    rays exactly parallel to an axis (odd nu, theta = 0/90/...). Random (rough) inputs."""
+    rng = np.random.default_rng(21)
+    x = rng.random((1, cfg.ny, cfg.nx)).astype(np.float32)
+    y = rng.random((1, cfg.nviews, cfg.nu)).astype(np.float32)
+    assert rel(gpu_forward(ctr, torch_cuda, cfg, x)[0], orc.forward(cfg, x[0].astype(np.float64))) <= 2e-5
+    assert rel(gpu_back(ctr, torch_cuda, cfg, y)[0], orc.back(cfg, y[0].astype(np.float64))) <= 2e-5
+
+
+def test_batched_slices_match_oracle_per_slice(ctr, torch_cuda, orc):
+    """V = 4 internal layout with a ragged batch (6 = 4 + 2) on the c2 geometry."""
+    cfg = scaled_config("c2", batch=6)
+    case = make_case(cfg)
+    got_s = gpu_forward(ctr, torch_cuda, cfg, case["truth"])
+    got_i = gpu_back(ctr, torch_cuda, cfg, case["sino"])
+    assert got_s.shape == (6, cfg.nviews, cfg.nu) and got_i.shape == (6, cfg.ny, cfg.nx)
+    for sl in (0, 3, 5):
+        assert rel(got_s[sl], orc.forward(cfg, case["truth"][sl].astype(np.float64))) <= TOL_OP
+        assert rel(got_i[sl], orc.back(cfg, case["sino"][sl].astype(np.float64))) <= TOL_OP
+    # batched result == single-slice result, bit for bit (same arithmetic per slice)
+    one = scaled_config("c2", batch=1)
+    assert np.array_equal(gpu_forward(ctr, torch_cuda, one, case["truth"][4:5])[0], got_s[4])
+    assert np.array_equal(gpu_back(ctr, torch_cuda, one, case["sino"][4:5])[0], got_i[4])
+
+
+@pytest.mark.parametrize("name,batch", [("c1", 1), ("c3", 1), ("c2", 5)])
+def test_adjoint_identity_on_gpu(ctr, torch_cuda, name, batch):
+    """PAPER.md:471 (A3'): <Px,y> = <x,P^T y> to fp32 rounding (dots accumulated in fp64)."""
+    cfg = scaled_config(name, batch=batch)
+    rng = np.random.default_rng(22)
+    x = rng.random((batch, cfg.ny, cfg.nx)).astype(np.float32)
+    y = rng.random((batch, cfg.nviews, cfg.nu)).astype(np.float32)
+    px = gpu_forward(ctr, torch_cuda, cfg, x).astype(np.float64)
+    pty = gpu_back(ctr, torch_cuda, cfg, y).astype(np.float64)
+    for sl in range(batch):
+        lhs, rhs = (px[sl] * y[sl]).sum(), (x[sl] * pty[sl]).sum()
+        assert abs(lhs - rhs) <= TOL_OP * np.linalg.norm(px[sl]) * np.linalg.norm(y[sl])
+        assert abs(lhs - rhs) <= 2e-6 * abs(lhs)
+
+
+def test_forward_and_back_use_bit_identical_matrices(ctr, torch_cuda, orc):
+    """Exact transpose: probing P with unit images and P^T with unit sinograms gives the same
+    matrix bit for bit, and it equals the oracle's dense matrix to fp32 accuracy."""
+    cfg = odd2d(nx=9, ny=7, nviews=6, nu=14, dx=2.0, dy=1.5)
+    npix, nray = cfg.nx * cfg.ny, cfg.nviews * cfg.nu
+    torch = torch_cuda
+    h = ctr.ctr_create(cfg)
+    A_f = np.zeros((nray, npix), np.float32)
+    A_b = np.zeros((nray, npix), np.float32)
+    x = torch.zeros(h.img_shape, device="cuda")
+    y = torch.zeros(h.sino_shape, device="cuda")
+    for j in range(npix):
+        x.zero_()
+        x.view(-1)[j] = 1.0
+        h.ctr_forward(x, y)
+        A_f[:, j] = y.view(-1).cpu().numpy()
+    for r in range(nray):
+        y.zero_()
+        y.view(-1)[r] = 1.0
+        h.ctr_back(y, x)
+        A_b[r, :] = x.view(-1).cpu().numpy()
+    h.close()
+    assert np.array_equal(A_f, A_b)
+    A = orc.matrix(cfg)
+    assert np.max(np.abs(A_f - A)) <= 2e-5 * A.max()
+    assert ((A_f > 0) == (A > 1e-4)).mean() > 0.98
+
+
+def test_zero_and_linearity(ctr, torch_cuda):
+    cfg = get_config("c1")
+    z = gpu_forward(ctr, torch_cuda, cfg, np.zeros((1, cfg.ny, cfg.nx), np.float32))
+    assert np.all(z == 0)
+    zb = gpu_back(ctr, torch_cuda, cfg, np.zeros((1, cfg.nviews, cfg.nu), np.float32))
+    assert np.all(zb == 0)
+
+
+def test_invalid_arguments(ctr, torch_cuda):
+    torch = torch_cuda
+    with pytest.raises(ctr.CtrError) as e:
+        ctr.ctr_create(scaled_config("c1", dsd=100.0))      # dsd <= dso
+    assert e.value.status == -1
+    with pytest.raises(ctr.CtrError) as e:
+        ctr.ctr_create(scaled_config("c1", dso=40.0, dsd=949.0))  # source inside the image circle
+    assert e.value.status == -2
+    h = ctr.ctr_create(get_config("c1"))
+    x = torch.zeros(h.img_shape, device="cuda")
+    b = torch.zeros(h.sino_shape, device="cuda")
+    with pytest.raises(ctr.CtrError):
+        h.ctr_cgls(b, x, -1)
+    with pytest.raises(ctr.CtrError):
+        h.ctr_update_weights(x, torch.zeros(h.w_shape, device="cuda"), quantile=0.0)
+    with pytest.raises(ValueError):
+        h.ctr_forward(x, torch.zeros(3, device="cuda"))
+    mis = torch.zeros(h.n_img + 1, device="cuda")[1:]        # 4-byte aligned only
+    rc = h._L.ctr_forward(h._h, mis.data_ptr(), b.data_ptr(), None)
+    assert rc == -1
+    x0 = x.clone()
+    h.ctr_cgls(b, x, 0)                                      # n_iter = 0: no-op
+    torch.cuda.synchronize()
+    assert torch.equal(x, x0)
+    h.close()

@@ -210,9 +210,12 @@ def test_cgls_converges_to_dense_least_squares(orc):
     rng = np.random.default_rng(11)
     b = A @ rng.random(cfg.nx * cfg.ny) + 0.01 * rng.standard_normal(A.shape[0])
     x_ls = np.linalg.lstsq(A, b, rcond=None)[0]
-    x = orc.cgls(cfg, b.reshape(cfg.nviews, cfg.nu), np.zeros((cfg.ny, cfg.nx)), 400).ravel()
+    x = orc.cgls(cfg, b.reshape(cfg.nviews, cfg.nu), np.zeros((cfg.ny, cfg.nx)), 400, reorth=False).ravel()
     assert np.linalg.norm(A @ x - A @ x_ls) <= 1e-8 * np.linalg.norm(b)
     assert np.linalg.norm(x - x_ls) <= 1e-6 * np.linalg.norm(x_ls)
+    # re-orthogonalised: finite termination after at most rank(A) = 64 steps
+    x = orc.cgls(cfg, b.reshape(cfg.nviews, cfg.nu), np.zeros((cfg.ny, cfg.nx)), 64, reorth=True).ravel()
+    assert np.linalg.norm(A @ x - A @ x_ls) <= 1e-8 * np.linalg.norm(b)
 
 
 def test_cgls_first_iterate_and_monotone_residual(orc):
@@ -239,6 +242,66 @@ def test_cgls_first_iterate_and_monotone_residual(orc):
     assert all(res[m + 1] <= res[m] * (1 + 1e-12) for m in range(11))
     # n_iter = 0 is the identity
     assert np.array_equal(orc.cgls(cfg, b.reshape(cfg.nviews, cfg.nu), x0.reshape(cfg.ny, cfg.nx), 0).ravel(), x0)
+
+
+def krylov_minimiser(A, b, x0, n):
+    """The DEFINITION of the n-th CGLS iterate (Hestenes & Stiefel): argmin ||A x - b|| over
+    x0 + span{(A^T A)^i A^T r0, i < n}. Built without any CG recurrence: an orthonormal Krylov
+    basis by Arnoldi with doubly applied Gram-Schmidt in extended precision, then a small dense
+    least-squares solve."""
+    L = np.longdouble
+    A_, r0 = A.astype(L), (b - A @ x0).astype(L)
+    v = A_.T @ r0
+    Q = []
+    for i in range(n):
+        for _ in range(2):
+            for q in Q:
+                v = v - (q @ v) * q
+        nv = np.sqrt(v @ v)
+        if nv == 0:
+            break
+        Q.append(v / nv)
+        v = A_.T @ (A_ @ Q[-1])
+    Qm = np.stack(Q, axis=1)
+    AQ = (A_ @ Qm).astype(np.float64)
+    c = np.linalg.lstsq(AQ, r0.astype(np.float64), rcond=None)[0]
+    return x0 + Qm.astype(np.float64) @ c
+
+
+@pytest.mark.parametrize("n", [1, 3, 6, 10, 15])
+def test_cgls_iterate_is_the_krylov_subspace_minimiser(orc, n):
+    """Pins the re-orthogonalised CGLS (reading S24) to the textbook definition of the iterate,
+    and shows the recurrence as printed agrees with it while it is still numerically orthogonal."""
+    cfg = tiny2d()
+    A = brute_matrix(cfg)
+    rng = np.random.default_rng(16)
+    b = A @ rng.random(A.shape[1]) + 0.05 * rng.standard_normal(A.shape[0])
+    x0 = 0.1 * rng.random(A.shape[1])
+    want = krylov_minimiser(A, b, x0, n)
+    got = orc.cgls(cfg, b.reshape(cfg.nviews, cfg.nu), x0.reshape(cfg.ny, cfg.nx), n, reorth=True).ravel()
+    assert np.linalg.norm(got - want) <= 1e-9 * np.linalg.norm(want)
+    plain = orc.cgls(cfg, b.reshape(cfg.nviews, cfg.nu), x0.reshape(cfg.ny, cfg.nx), n, reorth=False).ravel()
+    if n <= 6:
+        assert np.linalg.norm(plain - want) <= 1e-9 * np.linalg.norm(want)
+
+
+def test_cgls_reorthogonalised_is_reproducible_where_the_printed_recurrence_is_not(orc):
+    """Reading S24, measured on the seeded c1 workload with 15 iterations: a 1e-13 relative
+    perturbation of y moves the printed recurrence's result by orders of magnitude more than the
+    re-orthogonalised one (loss of orthogonality once the dominant singular direction converged)."""
+    cfg = get_config("c1")
+    y = make_case(cfg)["sino"][0].astype(np.float64)
+    yp = y * (1 + 1e-13 * np.random.default_rng(17).standard_normal(y.shape))
+    z = np.zeros((cfg.ny, cfg.nx))
+    d = {}
+    for re in (False, True):
+        a, b = orc.cgls(cfg, y, z, 15, reorth=re), orc.cgls(cfg, yp, z, 15, reorth=re)
+        d[re] = np.linalg.norm(a - b) / np.linalg.norm(a)
+    assert d[True] <= 1e-10
+    assert d[False] >= 1e3 * d[True]
+    # early iterations: both variants are the same iterate
+    a, b = orc.cgls(cfg, y, z, 5, reorth=False), orc.cgls(cfg, y, z, 5, reorth=True)
+    assert np.linalg.norm(a - b) <= 1e-9 * np.linalg.norm(a)
 
 
 # ---------------------------------------------------------------- O5-O8: A2 / A3
