@@ -121,34 +121,41 @@ __global__ void __launch_bounds__(256) k_img_uupdate(size_t n, float* __restrict
 // Gram-Schmidt against the stored unit gradients b_i restores it:
 //   pass 1 (k_reorth_dots): c_i = <b_i, g> for NB basis vectors per launch, fp64 accumulation
 //   pass 2 (k_reorth_sub) : g <- g - sum_i c_i b_i, gamma' = ||g||^2, beta = gamma'/gamma (:432)
-#define REORTH_NB 4
+#define REORTH_NB 8   /* basis vectors per k_reorth_dots launch */
+#define REORTH_E 8    /* elements per thread (block covers 256 * REORTH_E elements) */
 template <int V>
 __global__ void __launch_bounds__(256) k_reorth_dots(size_t n, size_t nimg, const float* __restrict__ gi,
                                                      const float* __restrict__ basis, int i0, int nb, int Bp, Scal sc,
                                                      double* part, unsigned* counter) {
-  const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
   const int g = blockIdx.y;
   double red[REORTH_NB * V];
 #pragma unroll
   for (int q = 0; q < REORTH_NB * V; ++q) red[q] = 0.0;
-  if (idx < n) {
-    float gv[V];
-    Pack<V>::ldcg(gi, (size_t)g * n + idx, gv);
+  const size_t base = (size_t)blockIdx.x * 256 * REORTH_E + threadIdx.x;
+#pragma unroll 2
+  for (int e = 0; e < REORTH_E; ++e) {
+    const size_t idx = base + (size_t)e * 256;
+    if (idx < n) {
+      float gv[V];
+      Pack<V>::ldcg(gi, (size_t)g * n + idx, gv);
 #pragma unroll
-    for (int q = 0; q < REORTH_NB; ++q) {
-      if (q < nb) {
-        float bv[V];
-        Pack<V>::ldcg(basis + (size_t)(i0 + q) * nimg, (size_t)g * n + idx, bv);
+      for (int q = 0; q < REORTH_NB; ++q) {
+        if (q < nb) {
+          float bv[V];
+          Pack<V>::ldcg(basis + (size_t)(i0 + q) * nimg, (size_t)g * n + idx, bv);
 #pragma unroll
-        for (int c = 0; c < V; ++c) red[q * V + c] = (double)bv[c] * (double)gv[c];
+          for (int c = 0; c < V; ++c) red[q * V + c] = fma((double)bv[c], (double)gv[c], red[q * V + c]);
+        }
       }
     }
   }
   grid_reduce<REORTH_NB * V>(red, part + (size_t)g * gridDim.x * REORTH_NB * V, counter + g, gridDim.x, blockIdx.x,
                              threadIdx.x, 256, [&](double(&sum)[REORTH_NB * V]) {
-                               for (int q = 0; q < nb; ++q)
 #pragma unroll
-                                 for (int c = 0; c < V; ++c) sc.coef[(size_t)(i0 + q) * Bp + g * V + c] = (float)sum[q * V + c];
+                               for (int q = 0; q < REORTH_NB; ++q)
+#pragma unroll
+                                 for (int c = 0; c < V; ++c)
+                                   if (q < nb) sc.coef[(size_t)(i0 + q) * Bp + g * V + c] = (float)sum[q * V + c];
                              });
 }
 
@@ -222,12 +229,13 @@ static int vec_reorth(ctr_handle* h, float* g, int nb, int first, cudaStream_t s
   const size_t n = d.npix;
   const int Bp = d.G * d.V;
   dim3 grid((unsigned)((n + 255) / 256), d.G);
+  dim3 dgrid((unsigned)((n + 256 * REORTH_E - 1) / (256 * REORTH_E)), d.G);
   ProfScope prof(h, CTR_PROF_VECTOR, st);
   if (nb > CTR_MAX_BASIS) nb = CTR_MAX_BASIS;
   for (int i0 = 0; i0 < nb; i0 += REORTH_NB) {
     const int cnt = nb - i0 < REORTH_NB ? nb - i0 : REORTH_NB;
-    if (d.V == 1) k_reorth_dots<1><<<grid, 256, 0, st>>>(n, h->nimg, g, h->basis, i0, cnt, Bp, h->sc, h->part, h->counters + 4 * d.G);
-    else k_reorth_dots<4><<<grid, 256, 0, st>>>(n, h->nimg, g, h->basis, i0, cnt, Bp, h->sc, h->part, h->counters + 4 * d.G);
+    if (d.V == 1) k_reorth_dots<1><<<dgrid, 256, 0, st>>>(n, h->nimg, g, h->basis, i0, cnt, Bp, h->sc, h->part, h->counters + 4 * d.G);
+    else k_reorth_dots<4><<<dgrid, 256, 0, st>>>(n, h->nimg, g, h->basis, i0, cnt, Bp, h->sc, h->part, h->counters + 4 * d.G);
     CTR_LAUNCHED(h);
   }
   if (d.V == 1) k_reorth_sub<1><<<grid, 256, 0, st>>>(n, h->nimg, g, h->basis, nb, Bp, first, h->sc, h->part, h->counters + 5 * d.G);
@@ -347,7 +355,7 @@ void ctr_destroy(ctr_handle* h) {
   if (!h) return;
   cudaDeviceSynchronize();
   void* bufs[] = {h->rays, h->rays2, h->views, h->ximg, h->bsino, h->r, h->q, h->s, h->gimg, h->v, h->w, h->n0,
-                  h->part, h->counters, h->hist, h->scal_block, h->stats, h->basis};
+                  h->part, h->counters, h->hist, h->scal_block, h->stats, h->basis, h->win, h->imgT};
   for (void* b : bufs)
     if (b) cudaFree(b);
   if (h->prof_ev) {
@@ -430,6 +438,8 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
   A((void**)&h->rays, sizeof(float4) * d.nray);
   if (d.ndim == 3) A((void**)&h->rays2, sizeof(float4) * d.nray);
   A((void**)&h->views, sizeof(float2) * d.nviews);
+  if (d.ndim == 2) A((void**)&h->win, sizeof(unsigned short) * (size_t)d.nviews * d.npix);
+  if (d.ndim == 2) A((void**)&h->imgT, h->nimg * fb);
   A((void**)&h->ximg, h->nimg * fb);
   A((void**)&h->bsino, h->nsino * fb);
   A((void**)&h->r, h->nsino * fb);
@@ -444,7 +454,7 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
     size_t nblk_tv = (size_t)((d.nx + 31) / 32) * ((d.ny + 3) / 4) * d.nz;
     size_t nblk_p = (size_t)(d.nray + 127) / 128;
     size_t nblk = nblk_tv > nblk_p ? nblk_tv : nblk_p;
-    h->part_len = (size_t)d.G * nblk * 4 * d.V;
+    h->part_len = (size_t)d.G * nblk * 8 * d.V;
     A((void**)&h->part, h->part_len * sizeof(double));
   }
   A((void**)&h->counters, sizeof(unsigned) * CTR_NCOUNTERS * d.G);

@@ -58,6 +58,8 @@ __global__ void k_fan_build(FanGeomD g, const float* __restrict__ angles, float4
   rays[r] = make_float4((float)x0, mf, xdrv ? -(float)L : (float)L, K);
 }
 
+int fan_build_window(ctr_handle* h);
+
 int fan_build_tables(ctr_handle* h) {
   const ctr_geometry& g = h->g;
   FanGeomD gd;
@@ -77,26 +79,118 @@ int fan_build_tables(ctr_handle* h) {
   CTR_LAUNCHED(h);
   CTR_CUDA(h, cudaDeviceSynchronize());
   if (d_angles) cudaFree(d_angles);
-  return CTR_OK;
+  return fan_build_window(h);
 }
 
 // ------------------------------------------------------------------------------------------------
-// a1  P: one thread per (ray, slice group). The thread walks the slabs of the ray's driving axis;
-// per slab it touches at most two cells (|m| <= 1). Lanes of a warp are adjacent bins of one view,
-// so their cells are adjacent in memory when the driving axis is y.
+// Candidate bins of a pixel in one view: rays that can cross the pixel project into a short window
+// around the projection of its centre. The half width is a strict bound (half diagonal of the pixel
+// times the largest magnification over the pixel) plus a guard, so approximate reciprocals are fine.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void fan_window(const Dims& d, float2 cs, float px, float py, int& b_lo, int& b_hi) {
+  const float rp = d.rvox, sdu = d.dsd * d.inv_du;
+  const float den = fmaf(px, cs.x, fmaf(py, cs.y, d.dso));  // distance along the central ray
+  const float aa = fmaf(py, cs.x, -px * cs.y);              // lateral offset
+  const float ell = aa * aa + den * den;
+  float bc, hb;
+  if (d.det_type == 0) {
+    const float inv = __frcp_rn(den - rp);
+    bc = fmaf(sdu * aa, __frcp_rn(den), d.boff_u);
+    hb = rp * sdu * (ell * rsqrtf(ell) + rp) * inv * inv;
+  } else {
+    bc = fmaf(atan2f(aa, den), sdu, d.boff_u);
+    hb = rp * sdu * __frcp_rn(ell * rsqrtf(ell) - rp);
+  }
+  b_lo = max(0, (int)ceilf(bc - hb - 0.02f));
+  b_hi = min(d.nu - 1, (int)floorf(bc + hb + 0.02f));
+}
+
+// weight of ray R in pixel (cell coordinates fi,fj / biased bi,bj): the gather side of slab_weights()
+__device__ __forceinline__ float fan_pixel_weight(const float4 R, float fi, float fj, float bi, float bj) {
+  const bool xdrv = R.z < 0.0f;
+  const float sc_ = xdrv ? fi : fj, tgt = xdrv ? bj : bi;
+  const float oa = fmaf(R.y, sc_, R.x);
+  const float ob = fmaf(R.y, sc_ + 1.0f, R.x);
+  const SlabW w = slab_weights(oa, ob, fabsf(R.z), R.w);
+  return (w.ra == tgt ? w.wa : 0.0f) + (w.rb == tgt ? w.wb : 0.0f);
+}
+
+// Window table: win[view][pixel] = first_bin << 4 | count, the EXACT range of
+// bins whose rays have a non-zero weight in the pixel, found once per handle by evaluating the
+// weight function over the conservative window. overflow[0] is raised if a count exceeds 15.
+__global__ void __launch_bounds__(128) k_fan_window(Dims d, const float4* __restrict__ rays,
+                                                    const float2* __restrict__ views, unsigned short* __restrict__ win,
+                                                    int* __restrict__ overflow) {
+  const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 4 + threadIdx.y, k = blockIdx.z;
+  if (i >= d.nx || j >= d.ny) return;
+  const float fi = (float)(i - d.c0x), fj = (float)(j - d.c0y);
+  const float bi = bias_of(i - d.c0x), bj = bias_of(j - d.c0y);
+  const float px = fmaf((float)i + 0.5f, d.dx, d.xlo), py = fmaf((float)j + 0.5f, d.dy, d.ylo);
+  int b_lo, b_hi, first = -1, last = -2;
+  fan_window(d, __ldg(&views[k]), px, py, b_lo, b_hi);
+  for (int b = b_lo; b <= b_hi; ++b) {
+    if (fan_pixel_weight(__ldg(&rays[k * d.nu + b]), fi, fj, bi, bj) != 0.0f) {
+      if (first < 0) first = b;
+      last = b;
+    }
+  }
+  int cnt = last - first + 1;
+  if (first < 0) { first = 0; cnt = 0; }
+  if (cnt > 15 || first > 4095) { atomicExch(overflow, 1); cnt = 0; }
+  win[(size_t)k * d.npix + (size_t)j * d.nx + i] = (unsigned short)((first << 4) | cnt);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Transposed copy imgT[g][i][j] = img[g][j][i] (32x32 tiles through shared memory). Rays whose driving
+// axis is x walk columns of the image; reading them from the transposed copy makes their accesses as
+// contiguous as those of y-driving rays (ncu, round 1: the forward projector was L1-wavefront bound).
+// ------------------------------------------------------------------------------------------------
+template <int V>
+__global__ void __launch_bounds__(256) k_transpose(int nx, int ny, const float* __restrict__ img, float* __restrict__ imgT) {
+  __shared__ float tile[32][33][V];
+  const int g = blockIdx.z, i0 = blockIdx.x * 32, j0 = blockIdx.y * 32;
+  const size_t np = (size_t)nx * ny;
+  for (int r = threadIdx.y; r < 32; r += 8) {
+    const int i = i0 + threadIdx.x, j = j0 + r;
+    if (i < nx && j < ny) {
+      float v[V];
+      Pack<V>::ldcg(img, (size_t)g * np + (size_t)j * nx + i, v);
+#pragma unroll
+      for (int c = 0; c < V; ++c) tile[r][threadIdx.x][c] = v[c];
+    }
+  }
+  __syncthreads();
+  for (int r = threadIdx.y; r < 32; r += 8) {
+    const int j = j0 + threadIdx.x, i = i0 + r;
+    if (i < nx && j < ny) {
+      float v[V];
+#pragma unroll
+      for (int c = 0; c < V; ++c) v[c] = tile[threadIdx.x][r][c];
+      Pack<V>::st(imgT, (size_t)g * np + (size_t)i * ny + j, v);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1  P: one thread per ray and VG slice groups (V slices each). The thread walks the slabs of the
+// ray's driving axis; per slab it touches at most two cells (|m| <= 1) and the geometry is shared by
+// all V*VG slices. Lanes of a warp are adjacent bins of one view, so their cells are adjacent in
+// memory (y-driving rays read img, x-driving rays read the transposed copy imgT).
 // MODE 0: out = P x        MODE 1: out = bs - P x   (CGLS r0)
 // MODE 2: out = P x and delta = ||out||^2 per slice -> a = gamma/delta (App. I step 1, :423)
 // ------------------------------------------------------------------------------------------------
-template <int V, int MODE>
+template <int V, int VG, int MODE>
 __global__ void __launch_bounds__(128) k_fan_forward(Dims d, const float4* __restrict__ rays,
-                                                     const float* __restrict__ img, float* __restrict__ out,
-                                                     const float* __restrict__ bs, Scal sc, double* part,
-                                                     unsigned* counter) {
+                                                     const float* __restrict__ img, const float* __restrict__ imgT,
+                                                     float* __restrict__ out, const float* __restrict__ bs, Scal sc,
+                                                     double* part, unsigned* counter) {
   const int r = blockIdx.x * 128 + threadIdx.x;
-  const int g = blockIdx.y;
-  float acc[V];
+  const int g0 = blockIdx.y * VG;
+  float acc[VG][V];
 #pragma unroll
-  for (int c = 0; c < V; ++c) acc[c] = 0.0f;
+  for (int q = 0; q < VG; ++q)
+#pragma unroll
+    for (int c = 0; c < V; ++c) acc[q][c] = 0.0f;
 
   if (r < d.nray) {
     const float4 R = __ldg(&rays[r]);
@@ -104,7 +198,6 @@ __global__ void __launch_bounds__(128) k_fan_forward(Dims d, const float4* __res
     const bool xdrv = R.z < 0.0f;
     const int n_drv = xdrv ? d.nx : d.ny, n_oth = xdrv ? d.ny : d.nx;
     const int c_drv = xdrv ? d.c0x : d.c0y, c_oth = xdrv ? d.c0y : d.c0x;
-    const int st_drv = xdrv ? 1 : d.nx, st_oth = xdrv ? d.nx : 1;
     // slabs in which the ray can be inside [-c_oth, n_oth - c_oth) (two cells of margin)
     int s0 = 0, s1 = n_drv;
     const float lo = (float)(-c_oth) - 1.0f, hi = (float)(n_oth - c_oth) + 1.0f;
@@ -118,158 +211,211 @@ __global__ void __launch_bounds__(128) k_fan_forward(Dims d, const float4* __res
     } else if (x0 < lo || x0 > hi) {
       s1 = 0;
     }
-    const float* base = img + (size_t)g * d.npix * V;
+    const float* base[VG];
+#pragma unroll
+    for (int q = 0; q < VG; ++q)
+      base[q] = (xdrv ? imgT : img) + (size_t)min(g0 + q, d.G - 1) * d.npix * V;
     float y = (float)(s0 - c_drv);
     float oa = fmaf(m, y, x0);
+    size_t row = (size_t)s0 * n_oth;
     for (int s = s0; s < s1; ++s) {
       const float ob = fmaf(m, y + 1.0f, x0);
       const SlabW w = slab_weights(oa, ob, L, K);
       const int ia = cell_of(w.ra) + c_oth, ib = cell_of(w.rb) + c_oth;
-      const size_t row = (size_t)s * st_drv;
       if ((unsigned)ia < (unsigned)n_oth) {
-        float f[V];
-        Pack<V>::ld(base, row + (size_t)ia * st_oth, f);
 #pragma unroll
-        for (int c = 0; c < V; ++c) acc[c] = fmaf(w.wa, f[c], acc[c]);
+        for (int q = 0; q < VG; ++q) {
+          float f[V];
+          Pack<V>::ld(base[q], row + ia, f);
+#pragma unroll
+          for (int c = 0; c < V; ++c) acc[q][c] = fmaf(w.wa, f[c], acc[q][c]);
+        }
       }
       if (w.wb != 0.0f && (unsigned)ib < (unsigned)n_oth) {
-        float f[V];
-        Pack<V>::ld(base, row + (size_t)ib * st_oth, f);
 #pragma unroll
-        for (int c = 0; c < V; ++c) acc[c] = fmaf(w.wb, f[c], acc[c]);
+        for (int q = 0; q < VG; ++q) {
+          float f[V];
+          Pack<V>::ld(base[q], row + ib, f);
+#pragma unroll
+          for (int c = 0; c < V; ++c) acc[q][c] = fmaf(w.wb, f[c], acc[q][c]);
+        }
       }
       oa = ob;
       y += 1.0f;
+      row += n_oth;
     }
-    const size_t e = (size_t)g * d.nray + r;
-    if (MODE == 1) {
-      float b[V];
-      Pack<V>::ld(bs, e, b);
 #pragma unroll
-      for (int c = 0; c < V; ++c) acc[c] = b[c] - acc[c];
+    for (int q = 0; q < VG; ++q) {
+      if (g0 + q < d.G) {
+        const size_t e = (size_t)(g0 + q) * d.nray + r;
+        if (MODE == 1) {
+          float b[V];
+          Pack<V>::ld(bs, e, b);
+#pragma unroll
+          for (int c = 0; c < V; ++c) acc[q][c] = b[c] - acc[q][c];
+        }
+        Pack<V>::st(out, e, acc[q]);
+      }
     }
-    Pack<V>::st(out, e, acc);
   }
   if (MODE == 2) {
-    double v[V];
+    double v[VG * V];
 #pragma unroll
-    for (int c = 0; c < V; ++c) v[c] = (double)acc[c] * (double)acc[c];
-    grid_reduce<V>(v, part + (size_t)g * gridDim.x * V, counter + g, gridDim.x, blockIdx.x, threadIdx.x, 128,
-                   [&](double(&sum)[V]) {
+    for (int q = 0; q < VG; ++q)
 #pragma unroll
-                     for (int c = 0; c < V; ++c) {
-                       const int sl = g * V + c;
-                       const double gamma = sc.gamma[sl];
-                       sc.a[sl] = (sum[c] > 0.0 && gamma > 0.0) ? (float)(gamma / sum[c]) : 0.0f;  // S4
-                     }
-                   });
+      for (int c = 0; c < V; ++c) v[q * V + c] = (double)acc[q][c] * (double)acc[q][c];
+    grid_reduce<VG * V>(v, part + (size_t)blockIdx.y * gridDim.x * VG * V, counter + blockIdx.y, gridDim.x,
+                        blockIdx.x, threadIdx.x, 128, [&](double(&sum)[VG * V]) {
+#pragma unroll
+                          for (int q = 0; q < VG; ++q)
+#pragma unroll
+                            for (int c = 0; c < V; ++c) {
+                              if (g0 + q >= d.G) continue;
+                              const int sl = (g0 + q) * V + c;
+                              const double gamma = sc.gamma[sl];
+                              sc.a[sl] = (sum[q * V + c] > 0.0 && gamma > 0.0) ? (float)(gamma / sum[q * V + c]) : 0.0f;  // S4
+                            }
+                        });
   }
 }
 
 // ------------------------------------------------------------------------------------------------
-// a2  P^T (gather): one thread per (pixel, slice group). For every view the bins whose rays can
-// cross the pixel form a short window around the projection of the pixel centre; the window is a
-// strict superset (half diagonal of the pixel, projected, plus a guard), and slab_weights() gives
-// exactly 0 for rays that miss. Accumulation order is fixed (views ascending, bins ascending).
+// a2  P^T (gather): one thread per pixel and VG slice groups. For every view the bins whose rays have
+// a non-zero weight in the pixel come from the window table (TABLE = 1) or, if the table does not fit
+// its 12+4-bit encoding, from fan_window(); slab_weights() gives exactly 0 for rays that miss.
+// Accumulation order is fixed (views ascending, bins ascending); no atomics.
 // MODE 0: out = P^T y
 // MODE 2: out = g = P^T r and, fused, u += a s (App. I step 2) for the pixel it owns.
 // (gamma, beta come from the re-orthogonalisation pass that follows, ctr_api.cu.)
 // ------------------------------------------------------------------------------------------------
-template <int V, int MODE>
+template <int V, int VG, int MODE, int TABLE>
 __global__ void __launch_bounds__(128) k_fan_back(Dims d, const float4* __restrict__ rays,
                                                   const float2* __restrict__ views,
+                                                  const unsigned short* __restrict__ win,
                                                   const float* __restrict__ sino, float* __restrict__ out,
                                                   const float* __restrict__ s_img, float* __restrict__ u_img, Scal sc) {
   const int i = blockIdx.x * 32 + threadIdx.x;
   const int j = blockIdx.y * 4 + threadIdx.y;
-  const int g = blockIdx.z;
-  const bool active = (i < d.nx) && (j < d.ny);
-  float acc[V];
+  const int g0 = blockIdx.z * VG;
+  if (i >= d.nx || j >= d.ny) return;
+  float acc[VG][V];
 #pragma unroll
-  for (int c = 0; c < V; ++c) acc[c] = 0.0f;
-
-  if (active) {
-    const float fi = (float)(i - d.c0x), fj = (float)(j - d.c0y);
-    const float bi = bias_of(i - d.c0x), bj = bias_of(j - d.c0y);
-    const float px = fmaf((float)i + 0.5f, d.dx, d.xlo), py = fmaf((float)j + 0.5f, d.dy, d.ylo);
-    const float* sg = sino + (size_t)g * d.nray * V;
-    const float rp = d.rvox, sdu = d.dsd * d.inv_du;
-    for (int k = 0; k < d.nviews; ++k) {
-      const float2 cs = __ldg(&views[k]);
-      const float den = fmaf(px, cs.x, fmaf(py, cs.y, d.dso));  // distance along the central ray
-      const float aa = fmaf(py, cs.x, -px * cs.y);              // lateral offset
-      const float ell = sqrtf(fmaf(aa, aa, den * den));
-      float bc, hb;
-      if (d.det_type == 0) {
-        const float inv = 1.0f / (den - rp);
-        bc = fmaf(sdu * aa, 1.0f / den, d.boff_u);
-        hb = rp * sdu * (ell + rp) * inv * inv;
-      } else {
-        bc = fmaf(atan2f(aa, den), sdu, d.boff_u);
-        hb = rp * sdu / (ell - rp);
-      }
-      const int b_lo = max(0, (int)ceilf(bc - hb - 0.02f));
-      const int b_hi = min(d.nu - 1, (int)floorf(bc + hb + 0.02f));
-      const int rbase = k * d.nu;
-      for (int b = b_lo; b <= b_hi; ++b) {
-        const float4 R = __ldg(&rays[rbase + b]);
-        const bool xdrv = R.z < 0.0f;
-        const float sc_ = xdrv ? fi : fj, tgt = xdrv ? bj : bi;
-        const float oa = fmaf(R.y, sc_, R.x);
-        const float ob = fmaf(R.y, sc_ + 1.0f, R.x);
-        const SlabW w = slab_weights(oa, ob, fabsf(R.z), R.w);
-        const float wt = (w.ra == tgt ? w.wa : 0.0f) + (w.rb == tgt ? w.wb : 0.0f);
-        if (wt != 0.0f) {
+  for (int q = 0; q < VG; ++q)
+#pragma unroll
+    for (int c = 0; c < V; ++c) acc[q][c] = 0.0f;
+  const float fi = (float)(i - d.c0x), fj = (float)(j - d.c0y);
+  const float bi = bias_of(i - d.c0x), bj = bias_of(j - d.c0y);
+  const float px = fmaf((float)i + 0.5f, d.dx, d.xlo), py = fmaf((float)j + 0.5f, d.dy, d.ylo);
+  const size_t pix = (size_t)j * d.nx + i;
+  const float* sg[VG];
+#pragma unroll
+  for (int q = 0; q < VG; ++q) sg[q] = sino + (size_t)min(g0 + q, d.G - 1) * d.nray * V;
+  for (int k = 0; k < d.nviews; ++k) {
+    int b_lo, b_hi;
+    if (TABLE) {
+      const unsigned w = __ldg(&win[(size_t)k * d.npix + pix]);
+      b_lo = (int)(w >> 4);
+      b_hi = b_lo + (int)(w & 15u) - 1;
+    } else {
+      fan_window(d, __ldg(&views[k]), px, py, b_lo, b_hi);
+    }
+    const int rbase = k * d.nu;
+    for (int b = b_lo; b <= b_hi; ++b) {
+      const float wt = fan_pixel_weight(__ldg(&rays[rbase + b]), fi, fj, bi, bj);
+      if (wt != 0.0f) {
+#pragma unroll
+        for (int q = 0; q < VG; ++q) {
           float y[V];
-          Pack<V>::ld(sg, (size_t)(rbase + b), y);
+          Pack<V>::ld(sg[q], (size_t)(rbase + b), y);
 #pragma unroll
-          for (int c = 0; c < V; ++c) acc[c] = fmaf(wt, y[c], acc[c]);
+          for (int c = 0; c < V; ++c) acc[q][c] = fmaf(wt, y[c], acc[q][c]);
         }
       }
     }
-    const size_t e = (size_t)g * d.npix + (size_t)j * d.nx + i;
-    Pack<V>::st(out, e, acc);
+  }
+#pragma unroll
+  for (int q = 0; q < VG; ++q) {
+    if (g0 + q >= d.G) continue;
+    const size_t e = (size_t)(g0 + q) * d.npix + pix;
+    Pack<V>::st(out, e, acc[q]);
     if (MODE == 2) {
       float sv[V], uv[V];
       Pack<V>::ldcg(s_img, e, sv);
       Pack<V>::ldcg(u_img, e, uv);
 #pragma unroll
-      for (int c = 0; c < V; ++c) uv[c] = fmaf(sc.a[g * V + c], sv[c], uv[c]);
+      for (int c = 0; c < V; ++c) uv[c] = fmaf(sc.a[(g0 + q) * V + c], sv[c], uv[c]);
       Pack<V>::st(u_img, e, uv);
     }
   }
 }
 
-template <int V>
+// ------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------
+int fan_build_window(ctr_handle* h) {
+  const Dims& d = h->d;
+  h->win_ok = 0;
+  if (d.nu > 4095) return CTR_OK;
+  int* d_flag = nullptr;
+  CTR_CUDA(h, cudaMalloc(&d_flag, sizeof(int)));
+  CTR_CUDA(h, cudaMemset(d_flag, 0, sizeof(int)));
+  dim3 grid((d.nx + 31) / 32, (d.ny + 3) / 4, d.nviews), block(32, 4);
+  k_fan_window<<<grid, block>>>(d, h->rays, h->views, h->win, d_flag);
+  CTR_LAUNCHED(h);
+  int flag = 1;
+  CTR_CUDA(h, cudaMemcpy(&flag, d_flag, sizeof(int), cudaMemcpyDeviceToHost));
+  cudaFree(d_flag);
+  h->win_ok = flag ? 0 : 1;
+  return CTR_OK;
+}
+
+template <int V, int VG>
 static int fan_forward_v(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st) {
   const Dims& d = h->d;
-  dim3 grid((d.nray + 127) / 128, d.G);
-  unsigned* cnt = h->counters + 0 * d.G;
   ProfScope prof(h, CTR_PROF_FORWARD, st);
-  if (mode == 0) k_fan_forward<V, 0><<<grid, 128, 0, st>>>(d, h->rays, img, out, bs, h->sc, h->part, cnt);
-  else if (mode == 1) k_fan_forward<V, 1><<<grid, 128, 0, st>>>(d, h->rays, img, out, bs, h->sc, h->part, cnt);
-  else k_fan_forward<V, 2><<<grid, 128, 0, st>>>(d, h->rays, img, out, bs, h->sc, h->part, cnt);
+  {
+    dim3 tg((d.nx + 31) / 32, (d.ny + 31) / 32, d.G), tb(32, 8);
+    k_transpose<V><<<tg, tb, 0, st>>>(d.nx, d.ny, img, h->imgT);
+    CTR_LAUNCHED(h);
+  }
+  dim3 grid((d.nray + 127) / 128, (d.G + VG - 1) / VG);
+  unsigned* cnt = h->counters + 0 * d.G;
+  if (mode == 0) k_fan_forward<V, VG, 0><<<grid, 128, 0, st>>>(d, h->rays, img, h->imgT, out, bs, h->sc, h->part, cnt);
+  else if (mode == 1) k_fan_forward<V, VG, 1><<<grid, 128, 0, st>>>(d, h->rays, img, h->imgT, out, bs, h->sc, h->part, cnt);
+  else k_fan_forward<V, VG, 2><<<grid, 128, 0, st>>>(d, h->rays, img, h->imgT, out, bs, h->sc, h->part, cnt);
   CTR_LAUNCHED(h);
   return CTR_OK;
 }
 
 int fan_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st) {
-  return h->d.V == 1 ? fan_forward_v<1>(h, img, out, mode, bs, st) : fan_forward_v<4>(h, img, out, mode, bs, st);
+  if (h->d.V == 1) return fan_forward_v<1, 1>(h, img, out, mode, bs, st);
+  if (h->d.G >= 3) return fan_forward_v<4, 4>(h, img, out, mode, bs, st);
+  if (h->d.G == 2) return fan_forward_v<4, 2>(h, img, out, mode, bs, st);
+  return fan_forward_v<4, 1>(h, img, out, mode, bs, st);
 }
 
-template <int V>
+template <int V, int VG>
 static int fan_back_v(ctr_handle* h, const float* sino, float* out, int mode, const float* s, float* u, cudaStream_t st) {
   const Dims& d = h->d;
-  dim3 grid((d.nx + 31) / 32, (d.ny + 3) / 4, d.G), block(32, 4);
+  dim3 grid((d.nx + 31) / 32, (d.ny + 3) / 4, (d.G + VG - 1) / VG), block(32, 4);
   ProfScope prof(h, CTR_PROF_BACK, st);
-  if (mode == 0) k_fan_back<V, 0><<<grid, block, 0, st>>>(d, h->rays, h->views, sino, out, s, u, h->sc);
-  else k_fan_back<V, 2><<<grid, block, 0, st>>>(d, h->rays, h->views, sino, out, s, u, h->sc);
+#define CTR_BACK_LAUNCH(M, T) \
+  k_fan_back<V, VG, M, T><<<grid, block, 0, st>>>(d, h->rays, h->views, h->win, sino, out, s, u, h->sc)
+  if (h->win_ok) {
+    if (mode == 0) CTR_BACK_LAUNCH(0, 1); else CTR_BACK_LAUNCH(2, 1);
+  } else {
+    if (mode == 0) CTR_BACK_LAUNCH(0, 0); else CTR_BACK_LAUNCH(2, 0);
+  }
+#undef CTR_BACK_LAUNCH
   CTR_LAUNCHED(h);
   return CTR_OK;
 }
 
 int fan_back(ctr_handle* h, const float* sino, float* out, int mode, const float* s, float* u, cudaStream_t st) {
-  return h->d.V == 1 ? fan_back_v<1>(h, sino, out, mode, s, u, st) : fan_back_v<4>(h, sino, out, mode, s, u, st);
+  if (h->d.V == 1) return fan_back_v<1, 1>(h, sino, out, mode, s, u, st);
+  if (h->d.G >= 3) return fan_back_v<4, 4>(h, sino, out, mode, s, u, st);
+  if (h->d.G == 2) return fan_back_v<4, 2>(h, sino, out, mode, s, u, st);
+  return fan_back_v<4, 1>(h, sino, out, mode, s, u, st);
 }
 
 }  // namespace ctr

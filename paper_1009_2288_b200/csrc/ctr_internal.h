@@ -67,6 +67,9 @@ struct ctr_handle {
   float4* rays;    // [nviews*nv*nu]  (2D: {x0, m, +-L, K}); 3D: see ctr_cone.cu
   float4* rays2;   // 3D second half of the ray record
   float2* views;   // [nviews] (cos, sin)
+  unsigned short* win;  // [nviews][npix] first_bin << 4 | count (2D gather window table)
+  int win_ok;           // table usable (nu <= 4095 and every count <= 15)
+  float* imgT;          // transposed copy of the image being projected, [G][nx][ny]
   // scratch, internal layout [G][n][V]
   size_t nimg, nsino;  // floats per internal image / sinogram (all groups)
   float *ximg, *bsino, *r, *q, *s, *gimg, *v, *w, *n0;
