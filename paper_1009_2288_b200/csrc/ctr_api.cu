@@ -422,6 +422,7 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
   d.dso = g->dso; d.dsd = g->dsd;
   d.inv_du = 1.0f / g->du;
   d.inv_dv = g->ndim == 3 ? 1.0f / g->dv : 1.0f;
+  d.dvz = g->ndim == 3 ? g->dv / g->dz : 1.0f;
   d.boff_u = (float)((g->nu - 1) / 2.0 - (double)g->u_off);
   d.boff_v = (float)((g->nv - 1) / 2.0 - (double)g->v_off);
   d.rvox = 0.5f * sqrtf(d.dx * d.dx + d.dy * d.dy + (g->ndim == 3 ? d.dz * d.dz : 0.0f));
@@ -435,11 +436,11 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
   auto A = [&](void** p, size_t bytes) {
     if (e == cudaSuccess) e = cudaMalloc(p, bytes ? bytes : 16);
   };
-  A((void**)&h->rays, sizeof(float4) * d.nray);
-  if (d.ndim == 3) A((void**)&h->rays2, sizeof(float4) * d.nray);
+  A((void**)&h->rays, sizeof(float4) * (size_t)d.nviews * d.nu);
+  if (d.ndim == 3) A((void**)&h->rays2, sizeof(float4) * (size_t)d.nviews * d.nu);
   A((void**)&h->views, sizeof(float2) * d.nviews);
-  if (d.ndim == 2) A((void**)&h->win, sizeof(unsigned short) * (size_t)d.nviews * d.npix);
-  if (d.ndim == 2) A((void**)&h->imgT, h->nimg * fb);
+  A((void**)&h->win, sizeof(unsigned short) * (size_t)d.nviews * d.nx * d.ny);
+  A((void**)&h->imgT, h->nimg * fb);
   A((void**)&h->ximg, h->nimg * fb);
   A((void**)&h->bsino, h->nsino * fb);
   A((void**)&h->r, h->nsino * fb);

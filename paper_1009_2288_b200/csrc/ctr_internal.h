@@ -28,6 +28,7 @@ struct Dims {
   float dx, dy, dz;       // mm
   float dso, dsd;
   float inv_du, inv_dv;   // 1/pitch
+  float dvz;              // dv/dz (3D: detector row pitch in voxel heights)
   float boff_u, boff_v;   // (n-1)/2 - off : bin = coord/pitch + boff
   float rvox;             // half diagonal of a voxel, mm
   int det_type;

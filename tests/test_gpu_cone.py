@@ -1,0 +1,172 @@
+"""GPU parity of the 3D cone-beam path (config c5's geometry family) through the C ABI against the
+fp64 oracle: projector pair, bit-identical matrices, adjoint, CGLS, 3D EP-TV weights / sweep and
+a short reconstruction. Tolerances as in 2D (north_star): 1e-5 per operator, 1e-3 final image."""
+import numpy as np
+import pytest
+
+from ctr_inputs import get_config, make_case, scaled_config
+from ctr_inputs.configs import Config
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+@pytest.fixture(scope="module")
+def ctr():
+    import paper_1009_2288_b200 as m
+    m.load_library()
+    return m
+
+
+def rel(a, b):
+    return float(np.linalg.norm(np.asarray(a, np.float64) - b) / np.linalg.norm(b))
+
+
+def to_gpu(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+
+def small3d(**kw):
+    """c5's scanner scaled down: ragged sizes, off-centre grid, shifted detector."""
+    base = dict(name="s3", index=93, ndim=3, nx=45, ny=38, nz=21, dx=2.0, dy=2.2, dz=2.5, nviews=11, nu=70, nv=40,
+                du=2.9, dv=3.1, dso=1000.0, dsd=1500.0, cx=1.5, cy=-2.0, cz=0.8, u_off=0.3, v_off=-0.4,
+                theta0=0.2, n_outer=2, n_cgls=5, n_gd=3, lam=0.02)
+    base.update(kw)
+    return Config(**base)
+
+
+def mini_c5():
+    """c5 at 1/4 linear size (same distances, 4x larger voxels and bins)."""
+    return scaled_config("c5", nx=128, ny=128, nz=32, dx=3.2, dy=3.2, dz=3.2, nu=128, nv=96, du=3.12, dv=3.12,
+                         nviews=20, n_outer=2, n_cgls=6)
+
+
+def test_forward_back_match_oracle_small(ctr, torch_cuda, orc):
+    torch = torch_cuda
+    for cfg in (small3d(), small3d(nviews=8, theta0=0.0, cx=0.0, cy=0.0, cz=0.0, u_off=0.0, v_off=0.0, nu=71, nv=41)):
+        rng = np.random.default_rng(41)
+        x = rng.random((cfg.nz, cfg.ny, cfg.nx)).astype(np.float32)
+        y = rng.random((cfg.nviews, cfg.nv, cfg.nu)).astype(np.float32)
+        h = ctr.ctr_create(cfg)
+        sino = torch.full(h.sino_shape, float("nan"), device="cuda")
+        img = torch.full(h.img_shape, float("nan"), device="cuda")
+        h.ctr_forward(to_gpu(torch, x), sino)
+        h.ctr_back(to_gpu(torch, y), img)
+        torch.cuda.synchronize()
+        px, pty = sino.cpu().numpy(), img.cpu().numpy()
+        h.close()
+        assert rel(px, orc.forward(cfg, x.astype(np.float64))) <= 2e-5
+        assert rel(pty, orc.back(cfg, y.astype(np.float64))) <= 2e-5
+        lhs, rhs = (px.astype(np.float64) * y).sum(), (x * pty.astype(np.float64)).sum()
+        assert abs(lhs - rhs) <= 2e-6 * abs(lhs)
+
+
+def test_matrices_bit_identical_3d(ctr, torch_cuda, orc):
+    cfg = small3d(nx=6, ny=5, nz=4, nviews=5, nu=9, nv=7, dx=8.0, dy=9.0, dz=10.0, du=11.0, dv=12.0)
+    torch = torch_cuda
+    nvox, nray = cfg.nx * cfg.ny * cfg.nz, cfg.nviews * cfg.nu * cfg.nv
+    h = ctr.ctr_create(cfg)
+    x = torch.zeros(h.img_shape, device="cuda")
+    y = torch.zeros(h.sino_shape, device="cuda")
+    A_f = np.zeros((nray, nvox), np.float32)
+    A_b = np.zeros((nray, nvox), np.float32)
+    for j in range(nvox):
+        x.zero_()
+        x.view(-1)[j] = 1.0
+        h.ctr_forward(x, y)
+        A_f[:, j] = y.view(-1).cpu().numpy()
+    for r in range(nray):
+        y.zero_()
+        y.view(-1)[r] = 1.0
+        h.ctr_back(y, x)
+        A_b[r, :] = x.view(-1).cpu().numpy()
+    h.close()
+    assert np.array_equal(A_f, A_b)
+    A = orc.matrix(cfg)
+    assert np.max(np.abs(A_f - A)) <= 2e-5 * A.max()
+
+
+def test_mini_c5_operators_and_reconstruction(ctr, torch_cuda, orc):
+    torch = torch_cuda
+    cfg = mini_c5()
+    case = make_case(cfg)
+    h = ctr.ctr_create(cfg)
+    sino = torch.zeros(h.sino_shape, device="cuda")
+    img = torch.zeros(h.img_shape, device="cuda")
+    h.ctr_forward(to_gpu(torch, case["truth"]), sino)
+    h.ctr_back(to_gpu(torch, case["sino"]), img)
+    torch.cuda.synchronize()
+    assert rel(sino.cpu().numpy(), orc.forward(cfg, case["truth"].astype(np.float64))) <= 1e-5
+    assert rel(img.cpu().numpy(), orc.back(cfg, case["sino"].astype(np.float64))) <= 1e-5
+    # CGLS
+    x = torch.zeros(h.img_shape, device="cuda")
+    h.ctr_cgls(to_gpu(torch, case["sino"]), x, 6)
+    torch.cuda.synchronize()
+    want = orc.cgls(cfg, case["sino"].astype(np.float64), np.zeros(cfg.img_shape), 6)
+    assert rel(x.cpu().numpy(), want.reshape(cfg.img_shape)) <= 1e-4
+    # full (short) schedule
+    h.ctr_reconstruct(to_gpu(torch, case["sino"]), img, ctr.make_params(cfg))
+    torch.cuda.synchronize()
+    stats = h.ctr_get_stats()
+    got = img.cpu().numpy()
+    h.close()
+    want, w_ref, log = orc.reconstruct(cfg, case["sino"].astype(np.float64), cfg)
+    ks = [r["k"] for r in stats]
+    print(f"[parity] mini-c5 {cfg.n_outer}x({cfg.n_cgls}+{cfg.n_gd}): image rel-L2 {rel(got, want):.3e}, ks {ks}")
+    assert ks == list(log[:, 1].astype(int))
+    assert max(abs(r["sigma"] - l[0]) / l[0] for r, l in zip(stats, log)) <= 2e-3
+    assert got.min() >= 0.0
+    assert rel(got, want) <= 1e-3
+
+
+def test_tv_3d_matches_oracle(ctr, torch_cuda, orc):
+    torch = torch_cuda
+    cfg = small3d()
+    rng = np.random.default_rng(42)
+    j, i = np.mgrid[0:cfg.ny, 0:cfg.nx]
+    base = 0.02 * ((i - 20) ** 2 + (j - 18) ** 2 < 150)[None].repeat(cfg.nz, 0)
+    v = (base + 0.002 * rng.standard_normal(base.shape)).astype(np.float32)
+    h = ctr.ctr_create(cfg)
+    h.ctr_set_params(ctr.make_params(cfg))
+    f = to_gpu(torch, v)
+    vg = to_gpu(torch, v)
+    w = torch.full(h.w_shape, float("nan"), device="cuda")
+    f_ref = v.astype(np.float64)
+    for sweep in range(2):
+        h.ctr_update_weights(f, w, quantile=cfg.sigma_quantile)
+        torch.cuda.synchronize()
+        w_ref, s_ref = orc.update_weights(f_ref, cfg.sigma_quantile, cfg.eps, 0, ndim=3)
+        assert np.max(np.abs(w.cpu().numpy() - w_ref)) <= 2e-5
+        h.ctr_eptv_step(f, vg, w, cfg.lam)
+        torch.cuda.synchronize()
+        st = h.ctr_get_stats()[-1]
+        f_new, k, E0, G, t = orc.eptv_step(f_ref, v.astype(np.float64), w_ref, cfg.lam, cfg, ndim=3)
+        assert st["k"] == k and abs(st["sigma"] - s_ref) <= 1e-5 * s_ref
+        assert abs(st["e0"] - E0) <= 1e-5 * abs(E0) and abs(st["g2"] - G) <= 1e-4 * G
+        assert rel(f.cpu().numpy(), f_new) <= 1e-5
+        f_ref = f_new
+    h.close()
+
+
+@pytest.mark.slow
+def test_c5_full_size_operators(ctr, torch_cuda, orc):
+    """configs[4] at full size (512x512x128, 60 x 384 x 512): P and P^T against the oracle."""
+    torch = torch_cuda
+    cfg = get_config("c5")
+    case = make_case(cfg, supersample=1)
+    h = ctr.ctr_create(cfg)
+    sino = torch.zeros(h.sino_shape, device="cuda")
+    img = torch.zeros(h.img_shape, device="cuda")
+    h.ctr_forward(to_gpu(torch, case["truth"]), sino)
+    h.ctr_back(to_gpu(torch, case["sino"]), img)
+    torch.cuda.synchronize()
+    px, pty = sino.cpu().numpy(), img.cpu().numpy()
+    h.close()
+    assert rel(px, orc.forward(cfg, case["truth"].astype(np.float64))) <= 1e-5
+    assert rel(pty, orc.back(cfg, case["sino"].astype(np.float64))) <= 1e-5
