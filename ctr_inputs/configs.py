@@ -52,10 +52,10 @@ class Config:
     n_gd: int = 5
     lam: float = 0.02
     sigma_quantile: float = 0.90
-    eps: float = 1e-6
+    eps: float = 1e-4
     armijo_t0: float = 1e-3
     armijo_rho: float = 0.5
-    armijo_c: float = 1e-4
+    armijo_c: float = 0.5
     armijo_max: int = 16
     weights_mode: int = 0
     positivity: int = 1

@@ -91,7 +91,7 @@ typedef struct {
   int32_t pad;
 } ctr_sweep_stat;
 
-/* Defaults: n_outer 1, n_cgls 10, n_gd 5, lambda 0.01, q 0.90, eps 1e-6, t0 1e-3, rho 0.5, c 1e-4,
+/* Defaults: n_outer 1, n_cgls 10, n_gd 5, lambda 0.01, q 0.90, eps 1e-4, t0 1e-3, rho 0.5, c 0.5 (S25),
  * armijo_max 16, EP-TV, positivity on, warm_start off. */
 void ctr_default_params(ctr_params* p);
 

@@ -112,8 +112,8 @@ def make_geom(g) -> OrcGeom:
 def make_params(p) -> OrcParams:
     d = p.params_dict() if hasattr(p, "params_dict") else dict(p)
     op = OrcParams()
-    defaults = dict(n_outer=1, n_cgls=1, n_gd=5, lam=0.01, sigma_quantile=0.90, eps=1e-6,
-                    armijo_t0=1e-3, armijo_rho=0.5, armijo_c=1e-4, armijo_max=16,
+    defaults = dict(n_outer=1, n_cgls=1, n_gd=5, lam=0.01, sigma_quantile=0.90, eps=1e-4,
+                    armijo_t0=1e-3, armijo_rho=0.5, armijo_c=0.5, armijo_max=16,
                     weights_mode=0, positivity=1, reorth=1)
     defaults.update(d)
     for k in ("n_outer", "n_cgls", "n_gd", "armijo_max", "weights_mode", "positivity", "reorth"):

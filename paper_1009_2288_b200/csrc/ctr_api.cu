@@ -62,184 +62,200 @@ static int unpack(ctr_handle* h, const float* src, float* dst, size_t n, int pla
 
 // ---------------------------------------------------------------------------------------------
 // a3  CGLS vector updates (App. I steps 2, 3, 5), per-slice scalars from device.
+// The arrays are [GS][nl] V-packs with nl = n * LQ: pack idx of super-group gs belongs to slice group
+// gs * LQ + idx % LQ (slice-interleaved layout; LQ = 1, V = 1 for a single slice).
 // ---------------------------------------------------------------------------------------------
 template <int V>
-__global__ void __launch_bounds__(256) k_sino_axpy(size_t n, float* __restrict__ r, const float* __restrict__ q, Scal sc) {
+__global__ void __launch_bounds__(256) k_sino_axpy(size_t nl, int LQ, float* __restrict__ r, const float* __restrict__ q,
+                                                   Scal sc) {
   const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
-  const int g = blockIdx.y;
-  if (idx >= n) return;
+  const int gs = blockIdx.y;
+  if (idx >= nl) return;
+  const int sl0 = (gs * LQ + (int)(idx % LQ)) * V;
   float rv[V], qv[V];
-  Pack<V>::ldcg(r, (size_t)g * n + idx, rv);
-  Pack<V>::ldcg(q, (size_t)g * n + idx, qv);
+  Pack<V>::ldcg(r, (size_t)gs * nl + idx, rv);
+  Pack<V>::ldcg(q, (size_t)gs * nl + idx, qv);
 #pragma unroll
-  for (int c = 0; c < V; ++c) rv[c] = fmaf(-sc.a[g * V + c], qv[c], rv[c]);  // r <- r - a P s
-  Pack<V>::st(r, (size_t)g * n + idx, rv);
+  for (int c = 0; c < V; ++c) rv[c] = fmaf(-sc.a[sl0 + c], qv[c], rv[c]);  // r <- r - a P s
+  Pack<V>::st(r, (size_t)gs * nl + idx, rv);
 }
 
 // s <- g + beta s (App. I step 5, :435; first = 1: s <- g) and store the unit gradient g/||g||
 // as the next basis vector of the re-orthogonalisation (S24).
 template <int V>
-__global__ void __launch_bounds__(256) k_img_supdate(size_t n, float* __restrict__ s, const float* __restrict__ gi,
+__global__ void __launch_bounds__(256) k_img_supdate(size_t nl, int LQ, float* __restrict__ s, const float* __restrict__ gi,
                                                      float* __restrict__ bnew, Scal sc, int first) {
   const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
-  const int g = blockIdx.y;
-  if (idx >= n) return;
+  const int gs = blockIdx.y;
+  if (idx >= nl) return;
+  const int sl0 = (gs * LQ + (int)(idx % LQ)) * V;
   float sv[V], gv[V], bv[V];
-  Pack<V>::ldcg(gi, (size_t)g * n + idx, gv);
+  Pack<V>::ldcg(gi, (size_t)gs * nl + idx, gv);
   if (first) {
 #pragma unroll
     for (int c = 0; c < V; ++c) sv[c] = gv[c];
   } else {
-    Pack<V>::ldcg(s, (size_t)g * n + idx, sv);
+    Pack<V>::ldcg(s, (size_t)gs * nl + idx, sv);
 #pragma unroll
-    for (int c = 0; c < V; ++c) sv[c] = fmaf(sc.beta[g * V + c], sv[c], gv[c]);
+    for (int c = 0; c < V; ++c) sv[c] = fmaf(sc.beta[sl0 + c], sv[c], gv[c]);
   }
-  Pack<V>::st(s, (size_t)g * n + idx, sv);
+  Pack<V>::st(s, (size_t)gs * nl + idx, sv);
   if (bnew) {
 #pragma unroll
-    for (int c = 0; c < V; ++c) bv[c] = gv[c] * sc.ginv[g * V + c];
-    Pack<V>::st(bnew, (size_t)g * n + idx, bv);
+    for (int c = 0; c < V; ++c) bv[c] = gv[c] * sc.ginv[sl0 + c];
+    Pack<V>::st(bnew, (size_t)gs * nl + idx, bv);
   }
 }
 
 template <int V>
-__global__ void __launch_bounds__(256) k_img_uupdate(size_t n, float* __restrict__ u, const float* __restrict__ s, Scal sc) {
+__global__ void __launch_bounds__(256) k_img_uupdate(size_t nl, int LQ, float* __restrict__ u, const float* __restrict__ s,
+                                                     Scal sc) {
   const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
-  const int g = blockIdx.y;
-  if (idx >= n) return;
+  const int gs = blockIdx.y;
+  if (idx >= nl) return;
+  const int sl0 = (gs * LQ + (int)(idx % LQ)) * V;
   float uv[V], sv[V];
-  Pack<V>::ldcg(u, (size_t)g * n + idx, uv);
-  Pack<V>::ldcg(s, (size_t)g * n + idx, sv);
+  Pack<V>::ldcg(u, (size_t)gs * nl + idx, uv);
+  Pack<V>::ldcg(s, (size_t)gs * nl + idx, sv);
 #pragma unroll
-  for (int c = 0; c < V; ++c) uv[c] = fmaf(sc.a[g * V + c], sv[c], uv[c]);  // u <- u + a s
-  Pack<V>::st(u, (size_t)g * n + idx, uv);
+  for (int c = 0; c < V; ++c) uv[c] = fmaf(sc.a[sl0 + c], sv[c], uv[c]);  // u <- u + a s
+  Pack<V>::st(u, (size_t)gs * nl + idx, uv);
 }
 
 // Re-orthogonalisation of the CGLS gradients (S24). In exact arithmetic P^T r^(m+1) is
 // orthogonal to every earlier P^T r^(i) (Hestenes & Stiefel); in fp32 that is lost
 // after ~6 iterations and the iterate then lags the exact one by a whole step. Classical
 // Gram-Schmidt against the stored unit gradients b_i restores it:
-//   pass 1 (k_reorth_dots): c_i = <b_i, g> for NB basis vectors per launch, fp64 accumulation
+//   pass 1 (k_reorth_dots): c_i = <b_i, g> for NB basis vectors per launch (per-thread fp32 partial
+//                           sums over a thread's elements, everything above that in fp64)
 //   pass 2 (k_reorth_sub) : g <- g - sum_i c_i b_i, gamma' = ||g||^2, beta = gamma'/gamma (:432)
 #define REORTH_NB 8   /* basis vectors per k_reorth_dots launch */
-#define REORTH_E 8    /* elements per thread (block covers 256 * REORTH_E elements) */
 template <int V>
-__global__ void __launch_bounds__(256) k_reorth_dots(size_t n, size_t nimg, const float* __restrict__ gi,
+__global__ void __launch_bounds__(256) k_reorth_dots(size_t nl, int LQ, size_t nimg, const float* __restrict__ gi,
                                                      const float* __restrict__ basis, int i0, int nb, int Bp, Scal sc,
                                                      double* part, unsigned* counter) {
-  const int g = blockIdx.y;
-  double red[REORTH_NB * V];
+  const int gs = blockIdx.y;
+  float acc[REORTH_NB * V];
 #pragma unroll
-  for (int q = 0; q < REORTH_NB * V; ++q) red[q] = 0.0;
-  const size_t base = (size_t)blockIdx.x * 256 * REORTH_E + threadIdx.x;
+  for (int q = 0; q < REORTH_NB * V; ++q) acc[q] = 0.0f;
+  // grid-stride loop (the stride is a multiple of 256, hence of LQ: a thread stays in its segment)
 #pragma unroll 2
-  for (int e = 0; e < REORTH_E; ++e) {
-    const size_t idx = base + (size_t)e * 256;
-    if (idx < n) {
+  for (size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x; idx < nl; idx += (size_t)gridDim.x * 256) {
+    {
       float gv[V];
-      Pack<V>::ldcg(gi, (size_t)g * n + idx, gv);
+      Pack<V>::ldcg(gi, (size_t)gs * nl + idx, gv);
 #pragma unroll
       for (int q = 0; q < REORTH_NB; ++q) {
         if (q < nb) {
           float bv[V];
-          Pack<V>::ldcg(basis + (size_t)(i0 + q) * nimg, (size_t)g * n + idx, bv);
+          Pack<V>::ldcg(basis + (size_t)(i0 + q) * nimg, (size_t)gs * nl + idx, bv);
 #pragma unroll
-          for (int c = 0; c < V; ++c) red[q * V + c] = fma((double)bv[c], (double)gv[c], red[q * V + c]);
+          for (int c = 0; c < V; ++c) acc[q * V + c] = fmaf(bv[c], gv[c], acc[q * V + c]);
         }
       }
     }
   }
-  grid_reduce<REORTH_NB * V>(red, part + (size_t)g * gridDim.x * REORTH_NB * V, counter + g, gridDim.x, blockIdx.x,
-                             threadIdx.x, 256, [&](double(&sum)[REORTH_NB * V]) {
+  double red[REORTH_NB * V];
 #pragma unroll
-                               for (int q = 0; q < REORTH_NB; ++q)
+  for (int q = 0; q < REORTH_NB * V; ++q) red[q] = (double)acc[q];
+  grid_reduce_q<REORTH_NB * V, 8>(red, LQ, part + (size_t)gs * gridDim.x * LQ * REORTH_NB * V, counter + gs, gridDim.x,
+                                  blockIdx.x, threadIdx.x, [&](int qq, double(&sum)[REORTH_NB * V]) {
 #pragma unroll
-                                 for (int c = 0; c < V; ++c)
-                                   if (q < nb) sc.coef[(size_t)(i0 + q) * Bp + g * V + c] = (float)sum[q * V + c];
-                             });
+                                    for (int q = 0; q < REORTH_NB; ++q)
+#pragma unroll
+                                      for (int c = 0; c < V; ++c)
+                                        if (q < nb)
+                                          sc.coef[(size_t)(i0 + q) * Bp + (gs * LQ + qq) * V + c] = (float)sum[q * V + c];
+                                  });
 }
 
 template <int V>
-__global__ void __launch_bounds__(256) k_reorth_sub(size_t n, size_t nimg, float* __restrict__ gi,
+__global__ void __launch_bounds__(256) k_reorth_sub(size_t nl, int LQ, size_t nimg, float* __restrict__ gi,
                                                     const float* __restrict__ basis, int nb, int Bp, int first, Scal sc,
                                                     double* part, unsigned* counter) {
-  const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
-  const int g = blockIdx.y;
+  const int gs = blockIdx.y;
+  const int sl0 = (gs * LQ + (int)(threadIdx.x % LQ)) * V;
   double red[V];
 #pragma unroll
   for (int c = 0; c < V; ++c) red[c] = 0.0;
-  if (idx < n) {
+  for (size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x; idx < nl; idx += (size_t)gridDim.x * 256) {
     float gv[V];
-    Pack<V>::ldcg(gi, (size_t)g * n + idx, gv);
+    Pack<V>::ldcg(gi, (size_t)gs * nl + idx, gv);
+#pragma unroll 4
     for (int q = 0; q < nb; ++q) {
       float bv[V];
-      Pack<V>::ldcg(basis + (size_t)q * nimg, (size_t)g * n + idx, bv);
+      Pack<V>::ldcg(basis + (size_t)q * nimg, (size_t)gs * nl + idx, bv);
 #pragma unroll
-      for (int c = 0; c < V; ++c) gv[c] = fmaf(-sc.coef[(size_t)q * Bp + g * V + c], bv[c], gv[c]);
+      for (int c = 0; c < V; ++c) gv[c] = fmaf(-sc.coef[(size_t)q * Bp + sl0 + c], bv[c], gv[c]);
     }
-    if (nb > 0) Pack<V>::st(gi, (size_t)g * n + idx, gv);
+    if (nb > 0) Pack<V>::st(gi, (size_t)gs * nl + idx, gv);
 #pragma unroll
-    for (int c = 0; c < V; ++c) red[c] = (double)gv[c] * (double)gv[c];
+    for (int c = 0; c < V; ++c) red[c] = fma((double)gv[c], (double)gv[c], red[c]);
   }
-  grid_reduce<V>(red, part + (size_t)g * gridDim.x * V, counter + g, gridDim.x, blockIdx.x, threadIdx.x, 256,
-                 [&](double(&sum)[V]) {
+  grid_reduce_q<V, 8>(red, LQ, part + (size_t)gs * gridDim.x * LQ * V, counter + gs, gridDim.x, blockIdx.x, threadIdx.x,
+                      [&](int qq, double(&sum)[V]) {
 #pragma unroll
-                   for (int c = 0; c < V; ++c) {
-                     const int sl = g * V + c;
-                     if (!first) {
-                       const double gamma = sc.gamma[sl];
-                       sc.beta[sl] = gamma > 0.0 ? (float)(sum[c] / gamma) : 0.0f;  // S4
-                     }
-                     sc.gamma[sl] = sum[c];
-                     sc.ginv[sl] = sum[c] > 0.0 ? (float)(1.0 / sqrt(sum[c])) : 0.0f;
-                   }
-                 });
+                        for (int c = 0; c < V; ++c) {
+                          const int sl = (gs * LQ + qq) * V + c;
+                          if (!first) {
+                            const double gamma = sc.gamma[sl];
+                            sc.beta[sl] = gamma > 0.0 ? (float)(sum[c] / gamma) : 0.0f;  // S4
+                          }
+                          sc.gamma[sl] = sum[c];
+                          sc.ginv[sl] = sum[c] > 0.0 ? (float)(1.0 / sqrt(sum[c])) : 0.0f;
+                        }
+                      });
 }
 
 static int vec_sino_axpy(ctr_handle* h, float* r, const float* q, cudaStream_t st) {
-  const size_t n = h->d.nray;
-  dim3 grid((unsigned)((n + 255) / 256), h->d.G);
+  const Dims& d = h->d;
+  const size_t nl = (size_t)d.nray * d.LQ;
+  dim3 grid((unsigned)((nl + 255) / 256), d.GS);
   ProfScope prof(h, CTR_PROF_VECTOR, st);
-  if (h->d.V == 1) k_sino_axpy<1><<<grid, 256, 0, st>>>(n, r, q, h->sc);
-  else k_sino_axpy<4><<<grid, 256, 0, st>>>(n, r, q, h->sc);
+  if (d.V == 1) k_sino_axpy<1><<<grid, 256, 0, st>>>(nl, d.LQ, r, q, h->sc);
+  else k_sino_axpy<4><<<grid, 256, 0, st>>>(nl, d.LQ, r, q, h->sc);
   CTR_LAUNCHED(h);
   return CTR_OK;
 }
 static int vec_img_supdate(ctr_handle* h, float* s, const float* g, float* bnew, int first, cudaStream_t st) {
-  const size_t n = h->d.npix;
-  dim3 grid((unsigned)((n + 255) / 256), h->d.G);
+  const Dims& d = h->d;
+  const size_t nl = (size_t)d.npix * d.LQ;
+  dim3 grid((unsigned)((nl + 255) / 256), d.GS);
   ProfScope prof(h, CTR_PROF_VECTOR, st);
-  if (h->d.V == 1) k_img_supdate<1><<<grid, 256, 0, st>>>(n, s, g, bnew, h->sc, first);
-  else k_img_supdate<4><<<grid, 256, 0, st>>>(n, s, g, bnew, h->sc, first);
+  if (d.V == 1) k_img_supdate<1><<<grid, 256, 0, st>>>(nl, d.LQ, s, g, bnew, h->sc, first);
+  else k_img_supdate<4><<<grid, 256, 0, st>>>(nl, d.LQ, s, g, bnew, h->sc, first);
   CTR_LAUNCHED(h);
   return CTR_OK;
 }
 static int vec_img_uupdate(ctr_handle* h, float* u, const float* s, cudaStream_t st) {
-  const size_t n = h->d.npix;
-  dim3 grid((unsigned)((n + 255) / 256), h->d.G);
+  const Dims& d = h->d;
+  const size_t nl = (size_t)d.npix * d.LQ;
+  dim3 grid((unsigned)((nl + 255) / 256), d.GS);
   ProfScope prof(h, CTR_PROF_VECTOR, st);
-  if (h->d.V == 1) k_img_uupdate<1><<<grid, 256, 0, st>>>(n, u, s, h->sc);
-  else k_img_uupdate<4><<<grid, 256, 0, st>>>(n, u, s, h->sc);
+  if (d.V == 1) k_img_uupdate<1><<<grid, 256, 0, st>>>(nl, d.LQ, u, s, h->sc);
+  else k_img_uupdate<4><<<grid, 256, 0, st>>>(nl, d.LQ, u, s, h->sc);
   CTR_LAUNCHED(h);
   return CTR_OK;
 }
 // g <- g minus its components along basis[0..nb), then gamma / beta / 1/||g||
 static int vec_reorth(ctr_handle* h, float* g, int nb, int first, cudaStream_t st) {
   const Dims& d = h->d;
-  const size_t n = d.npix;
+  const size_t nl = (size_t)d.npix * d.LQ;
   const int Bp = d.G * d.V;
-  dim3 grid((unsigned)((n + 255) / 256), d.G);
-  dim3 dgrid((unsigned)((n + 256 * REORTH_E - 1) / (256 * REORTH_E)), d.G);
+  // persistent-size grids: few partial sums for the finishing block of the reductions
+  const unsigned want = (unsigned)((nl + 255) / 256), cap = (unsigned)(CTR_REDUCE_BLOCKS / d.GS > 0 ? CTR_REDUCE_BLOCKS / d.GS : 1);
+  dim3 grid(want < cap ? want : cap, d.GS);
+  dim3 dgrid = grid;
   ProfScope prof(h, CTR_PROF_VECTOR, st);
   if (nb > CTR_MAX_BASIS) nb = CTR_MAX_BASIS;
   for (int i0 = 0; i0 < nb; i0 += REORTH_NB) {
     const int cnt = nb - i0 < REORTH_NB ? nb - i0 : REORTH_NB;
-    if (d.V == 1) k_reorth_dots<1><<<dgrid, 256, 0, st>>>(n, h->nimg, g, h->basis, i0, cnt, Bp, h->sc, h->part, h->counters + 4 * d.G);
-    else k_reorth_dots<4><<<dgrid, 256, 0, st>>>(n, h->nimg, g, h->basis, i0, cnt, Bp, h->sc, h->part, h->counters + 4 * d.G);
+    if (d.V == 1) k_reorth_dots<1><<<dgrid, 256, 0, st>>>(nl, d.LQ, h->nimg, g, h->basis, i0, cnt, Bp, h->sc, h->part, h->counters + 4 * d.G);
+    else k_reorth_dots<4><<<dgrid, 256, 0, st>>>(nl, d.LQ, h->nimg, g, h->basis, i0, cnt, Bp, h->sc, h->part, h->counters + 4 * d.G);
     CTR_LAUNCHED(h);
   }
-  if (d.V == 1) k_reorth_sub<1><<<grid, 256, 0, st>>>(n, h->nimg, g, h->basis, nb, Bp, first, h->sc, h->part, h->counters + 5 * d.G);
-  else k_reorth_sub<4><<<grid, 256, 0, st>>>(n, h->nimg, g, h->basis, nb, Bp, first, h->sc, h->part, h->counters + 5 * d.G);
+  if (d.V == 1) k_reorth_sub<1><<<grid, 256, 0, st>>>(nl, d.LQ, h->nimg, g, h->basis, nb, Bp, first, h->sc, h->part, h->counters + 5 * d.G);
+  else k_reorth_sub<4><<<grid, 256, 0, st>>>(nl, d.LQ, h->nimg, g, h->basis, nb, Bp, first, h->sc, h->part, h->counters + 5 * d.G);
   CTR_LAUNCHED(h);
   return CTR_OK;
 }
@@ -331,8 +347,8 @@ extern "C" {
 void ctr_default_params(ctr_params* p) {
   if (!p) return;
   p->n_outer = 1; p->n_cgls = 10; p->n_gd = 5;
-  p->lambda = 0.01f; p->sigma_quantile = 0.90f; p->eps = 1e-6f;
-  p->armijo_t0 = 1e-3f; p->armijo_rho = 0.5f; p->armijo_c = 1e-4f; p->armijo_max = 16;
+  p->lambda = 0.01f; p->sigma_quantile = 0.90f; p->eps = 1e-4f;
+  p->armijo_t0 = 1e-3f; p->armijo_rho = 0.5f; p->armijo_c = 0.5f; p->armijo_max = 16;
   p->weights_mode = 0; p->positivity = 1; p->warm_start = 0;
 }
 
@@ -355,7 +371,7 @@ void ctr_destroy(ctr_handle* h) {
   if (!h) return;
   cudaDeviceSynchronize();
   void* bufs[] = {h->rays, h->rays2, h->views, h->ximg, h->bsino, h->r, h->q, h->s, h->gimg, h->v, h->w, h->n0,
-                  h->part, h->counters, h->hist, h->scal_block, h->stats, h->basis, h->win, h->imgT};
+                  h->part, h->counters, h->hist, h->scal_block, h->stats, h->basis, h->win, h->imgT, h->win2, h->usi};
   for (void* b : bufs)
     if (b) cudaFree(b);
   if (h->prof_ev) {
@@ -414,7 +430,16 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
   d.nray = g->nviews * g->nu * g->nv;
   d.B = g->batch;
   d.V = g->batch > 1 ? 4 : 1;
-  d.G = (g->batch + d.V - 1) / d.V;
+  {
+    // groups of V slices; batched: LQ groups (a power of two <= 16) form a super-group of the
+    // slice-interleaved layout, and the group count is padded to a whole number of super-groups
+    const int g0 = (g->batch + d.V - 1) / d.V;
+    d.LQ = 1;
+    if (d.V == 4) while (d.LQ < 16 && d.LQ < g0) d.LQ *= 2;
+    d.GS = (g0 + d.LQ - 1) / d.LQ;
+    d.G = d.GS * d.LQ;
+  }
+  d.nvp = (g->nviews + 15) / 16 * 16;
   d.dx = g->dx; d.dy = g->dy; d.dz = g->ndim == 3 ? g->dz : 1.0f;
   d.xlo = (float)((double)g->cx - g->nx * (double)g->dx / 2.0);
   d.ylo = (float)((double)g->cy - g->ny * (double)g->dy / 2.0);
@@ -440,7 +465,11 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
   if (d.ndim == 3) A((void**)&h->rays2, sizeof(float4) * (size_t)d.nviews * d.nu);
   A((void**)&h->views, sizeof(float2) * d.nviews);
   A((void**)&h->win, sizeof(unsigned short) * (size_t)d.nviews * d.nx * d.ny);
-  A((void**)&h->imgT, h->nimg * fb);
+  if (d.V == 1) A((void**)&h->imgT, h->nimg * fb);
+  else {
+    A((void**)&h->win2, sizeof(unsigned short) * (size_t)d.npix * d.nvp);
+    A((void**)&h->usi, h->nimg * fb);
+  }
   A((void**)&h->ximg, h->nimg * fb);
   A((void**)&h->bsino, h->nsino * fb);
   A((void**)&h->r, h->nsino * fb);
@@ -456,6 +485,11 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
     size_t nblk_p = (size_t)(d.nray + 127) / 128;
     size_t nblk = nblk_tv > nblk_p ? nblk_tv : nblk_p;
     h->part_len = (size_t)d.G * nblk * 8 * d.V;
+    // segmented reductions of the CGLS kernels: [GS][blocks][LQ][N] with N <= 8 * V
+    size_t nblk_f = ((size_t)d.nray + 8 * (32 / d.LQ) - 1) / (8 * (32 / d.LQ));
+    size_t nblk_q = nblk_f > CTR_REDUCE_BLOCKS ? nblk_f : CTR_REDUCE_BLOCKS;
+    size_t need_q = (size_t)d.GS * nblk_q * d.LQ * 8 * d.V;
+    if (need_q > h->part_len) h->part_len = need_q;
     A((void**)&h->part, h->part_len * sizeof(double));
   }
   A((void**)&h->counters, sizeof(unsigned) * CTR_NCOUNTERS * d.G);
@@ -511,9 +545,9 @@ int ctr_forward(ctr_handle* h, const float* d_img, float* d_sino, void* stream) 
   h->last_stream = st;
   if (h->d.V == 1) return op_forward(h, d_img, d_sino, 0, nullptr, st);
   int rc;
-  if ((rc = pack(h, d_img, h->ximg, h->d.npix, 1, st))) return rc;
-  if ((rc = op_forward(h, h->ximg, h->q, 0, nullptr, st))) return rc;
-  return unpack(h, h->q, d_sino, h->d.nray, 1, st);
+  if ((rc = si_from_abi(h, d_img, h->usi, h->d.npix, st))) return rc;
+  if ((rc = op_forward(h, h->usi, h->q, 0, nullptr, st))) return rc;
+  return si_to_abi(h, h->q, d_sino, h->d.nray, st);
 }
 
 int ctr_back(ctr_handle* h, const float* d_sino, float* d_img, void* stream) {
@@ -523,9 +557,9 @@ int ctr_back(ctr_handle* h, const float* d_sino, float* d_img, void* stream) {
   h->last_stream = st;
   if (h->d.V == 1) return op_back(h, d_sino, d_img, 0, nullptr, nullptr, st);
   int rc;
-  if ((rc = pack(h, d_sino, h->bsino, h->d.nray, 1, st))) return rc;
+  if ((rc = si_from_abi(h, d_sino, h->bsino, h->d.nray, st))) return rc;
   if ((rc = op_back(h, h->bsino, h->gimg, 0, nullptr, nullptr, st))) return rc;
-  return unpack(h, h->gimg, d_img, h->d.npix, 1, st);
+  return si_to_abi(h, h->gimg, d_img, h->d.npix, st);
 }
 
 int ctr_cgls(ctr_handle* h, const float* d_b, float* d_x, int n_iter, void* stream) {
@@ -537,10 +571,10 @@ int ctr_cgls(ctr_handle* h, const float* d_b, float* d_x, int n_iter, void* stre
   h->last_stream = st;
   if (h->d.V == 1) return cgls_internal(h, d_b, d_x, n_iter, false, st);
   int rc;
-  if ((rc = pack(h, d_b, h->bsino, h->d.nray, 1, st))) return rc;
-  if ((rc = pack(h, d_x, h->ximg, h->d.npix, 1, st))) return rc;
-  if ((rc = cgls_internal(h, h->bsino, h->ximg, n_iter, false, st))) return rc;
-  return unpack(h, h->ximg, d_x, h->d.npix, 1, st);
+  if ((rc = si_from_abi(h, d_b, h->bsino, h->d.nray, st))) return rc;
+  if ((rc = si_from_abi(h, d_x, h->usi, h->d.npix, st))) return rc;
+  if ((rc = cgls_internal(h, h->bsino, h->usi, n_iter, false, st))) return rc;
+  return si_to_abi(h, h->usi, d_x, h->d.npix, st);
 }
 
 int ctr_update_weights(ctr_handle* h, const float* d_x, float* d_w, float quantile, float* d_sigma, void* stream) {
@@ -604,14 +638,23 @@ int ctr_reconstruct_w(ctr_handle* h, const float* d_sino, float* d_img, float* d
   float* f = direct ? d_img : h->ximg;
   const float* b = d_sino;
   if (!direct) {
-    if ((rc = pack(h, d_sino, h->bsino, h->d.nray, 1, st))) return rc;
+    if ((rc = si_from_abi(h, d_sino, h->bsino, h->d.nray, st))) return rc;  // slice-interleaved
     b = h->bsino;
   }
   if ((rc = ensure_basis(h, P.n_cgls))) return rc;
   if (!P.warm_start) CTR_CUDA(h, cudaMemsetAsync(f, 0, h->nimg * sizeof(float), st));            // f^(0) = 0 (:171)
   else if (!direct && (rc = pack(h, d_img, h->ximg, h->d.npix, 1, st))) return rc;
   for (int it = 0; it < P.n_outer; ++it) {
-    if ((rc = cgls_internal(h, b, f, P.n_cgls, it == 0 && !P.warm_start, st))) return rc;        // Step 1 (:171)
+    const bool x0_zero = it == 0 && !P.warm_start;
+    if (direct) {
+      if ((rc = cgls_internal(h, b, f, P.n_cgls, x0_zero, st))) return rc;                        // Step 1 (:171)
+    } else if (P.n_cgls > 0) {
+      // batched: CGLS runs in the slice-interleaved layout, the TV sweeps in the group-planar one
+      if (x0_zero) CTR_CUDA(h, cudaMemsetAsync(h->usi, 0, h->nimg * sizeof(float), st));
+      else if ((rc = si_from_planar(h, f, h->usi, h->d.npix, st))) return rc;
+      if ((rc = cgls_internal(h, b, h->usi, P.n_cgls, x0_zero, st))) return rc;                   // Step 1 (:171)
+      if ((rc = si_to_planar(h, h->usi, f, h->d.npix, st))) return rc;
+    }
     if (P.n_gd > 0)
       CTR_CUDA(h, cudaMemcpyAsync(h->v, f, h->nimg * sizeof(float), cudaMemcpyDeviceToDevice, st));  // v = CGLS result
     for (int s = 0; s < P.n_gd; ++s) {                                                            // Step 2 (:172)

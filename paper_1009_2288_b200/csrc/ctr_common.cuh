@@ -86,6 +86,64 @@ __device__ __forceinline__ void grid_reduce(double (&v)[N], double* part, unsign
 }
 
 // ---------------------------------------------------------------------------------------------
+// Segmented variant for the slice-interleaved layout: thread tid holds N partial
+// sums that belong to segment tid % LQ (LQ a power of two <= 16, block size NW * 32); the
+// sums are kept apart per segment. fin(q, sums) is called by thread q < LQ of the last block with the
+// totals of segment q. Partials: part[(blk * LQ + q) * N + n]. Order of additions is fixed.
+// ---------------------------------------------------------------------------------------------
+template <int N, int NW>
+__device__ __forceinline__ void block_sum_q(double (&v)[N], double (*sm)[NW][16], int LQ, int tid) {
+  const int lane = tid & 31, wid = tid >> 5;
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    double w = v[n];
+    for (int o = 16; o >= LQ; o >>= 1) w += __shfl_down_sync(0xffffffffu, w, o);
+    if (lane < LQ) sm[n][wid][lane] = w;
+  }
+  __syncthreads();
+  if (tid < LQ) {
+#pragma unroll
+    for (int n = 0; n < N; ++n) {
+      double w = 0.0;
+      for (int k = 0; k < NW; ++k) w += sm[n][k][tid];
+      v[n] = w;
+    }
+  }
+  __syncthreads();
+}
+
+template <int N, int NW, class Fin>
+__device__ __forceinline__ void grid_reduce_q(double (&v)[N], int LQ, double* part, unsigned* counter, unsigned nblk,
+                                              unsigned blk, int tid, Fin fin) {
+  __shared__ double sm[N][NW][16];  // LQ <= 16
+  __shared__ bool last;
+  block_sum_q<N, NW>(v, sm, LQ, tid);
+  if (tid < LQ) {
+#pragma unroll
+    for (int n = 0; n < N; ++n) part[((size_t)blk * LQ + tid) * N + n] = v[n];
+    __threadfence();
+  }
+  __syncthreads();
+  if (tid == 0) {
+    unsigned t = atomicInc(counter, nblk - 1);
+    last = (t == nblk - 1);
+  }
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
+  double acc[N];
+#pragma unroll
+  for (int n = 0; n < N; ++n) acc[n] = 0.0;
+  const int q = tid & (LQ - 1);
+  for (unsigned b = tid / LQ; b < nblk; b += (NW * 32) / LQ) {
+#pragma unroll
+    for (int n = 0; n < N; ++n) acc[n] += __ldcg(&part[((size_t)b * LQ + q) * N + n]);
+  }
+  block_sum_q<N, NW>(acc, sm, LQ, tid);
+  if (tid < LQ) fin(tid, acc);
+}
+
+// ---------------------------------------------------------------------------------------------
 // The ONE definition of the system-matrix entry, used by both P (ctr_forward) and P^T (ctr_back).
 //
 // A ray is stored in grid-index coordinates with its driving axis d (the axis along which it

@@ -6,6 +6,7 @@
 //   P^T : PAPER.md:193 (why not scatter), :471 (adjoint condition A3'); north_star: exact transpose
 #include "ctr_common.cuh"
 #include "ctr_internal.h"
+#include "ctr_fan_geom.cuh"
 
 namespace ctr {
 
@@ -82,39 +83,6 @@ int fan_build_tables(ctr_handle* h) {
   return fan_build_window(h);
 }
 
-// ------------------------------------------------------------------------------------------------
-// Candidate bins of a pixel in one view: rays that can cross the pixel project into a short window
-// around the projection of its centre. The half width is a strict bound (half diagonal of the pixel
-// times the largest magnification over the pixel) plus a guard, so approximate reciprocals are fine.
-// ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void fan_window(const Dims& d, float2 cs, float px, float py, int& b_lo, int& b_hi) {
-  const float rp = d.rvox, sdu = d.dsd * d.inv_du;
-  const float den = fmaf(px, cs.x, fmaf(py, cs.y, d.dso));  // distance along the central ray
-  const float aa = fmaf(py, cs.x, -px * cs.y);              // lateral offset
-  const float ell = aa * aa + den * den;
-  float bc, hb;
-  if (d.det_type == 0) {
-    const float inv = __frcp_rn(den - rp);
-    bc = fmaf(sdu * aa, __frcp_rn(den), d.boff_u);
-    hb = rp * sdu * (ell * rsqrtf(ell) + rp) * inv * inv;
-  } else {
-    bc = fmaf(atan2f(aa, den), sdu, d.boff_u);
-    hb = rp * sdu * __frcp_rn(ell * rsqrtf(ell) - rp);
-  }
-  b_lo = max(0, (int)ceilf(bc - hb - 0.02f));
-  b_hi = min(d.nu - 1, (int)floorf(bc + hb + 0.02f));
-}
-
-// weight of ray R in pixel (cell coordinates fi,fj / biased bi,bj): the gather side of slab_weights()
-__device__ __forceinline__ float fan_pixel_weight(const float4 R, float fi, float fj, float bi, float bj) {
-  const bool xdrv = R.z < 0.0f;
-  const float sc_ = xdrv ? fi : fj, tgt = xdrv ? bj : bi;
-  const float oa = fmaf(R.y, sc_, R.x);
-  const float ob = fmaf(R.y, sc_ + 1.0f, R.x);
-  const SlabW w = slab_weights(oa, ob, fabsf(R.z), R.w);
-  return (w.ra == tgt ? w.wa : 0.0f) + (w.rb == tgt ? w.wb : 0.0f);
-}
-
 // Window table: win[view][pixel] = first_bin << 4 | count, the EXACT range of
 // bins whose rays have a non-zero weight in the pixel, found once per handle by evaluating the
 // weight function over the conservative window. overflow[0] is raised if a count exceeds 15.
@@ -138,6 +106,13 @@ __global__ void __launch_bounds__(128) k_fan_window(Dims d, const float4* __rest
   if (first < 0) { first = 0; cnt = 0; }
   if (cnt > 15 || first > 4095) { atomicExch(overflow, 1); cnt = 0; }
   win[(size_t)k * d.npix + (size_t)j * d.nx + i] = (unsigned short)((first << 4) | cnt);
+}
+
+// win2[pixel][view] = win[view][pixel] (views contiguous: the batched gather takes LQ views per step)
+__global__ void __launch_bounds__(256) k_win_transpose(const unsigned short* __restrict__ win,
+                                                       unsigned short* __restrict__ win2, int npix, int nvp) {
+  const int p = blockIdx.x * 256 + threadIdx.x, k = blockIdx.y;
+  if (p < npix) win2[(size_t)p * nvp + k] = win[(size_t)k * npix + p];
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -366,6 +341,11 @@ int fan_build_window(ctr_handle* h) {
   CTR_CUDA(h, cudaMemcpy(&flag, d_flag, sizeof(int), cudaMemcpyDeviceToHost));
   cudaFree(d_flag);
   h->win_ok = flag ? 0 : 1;
+  if (h->win_ok && h->win2) {
+    k_win_transpose<<<dim3((d.npix + 255) / 256, d.nviews), 256>>>(h->win, h->win2, d.npix, d.nvp);
+    CTR_LAUNCHED(h);
+    CTR_CUDA(h, cudaDeviceSynchronize());
+  }
   return CTR_OK;
 }
 
@@ -387,11 +367,10 @@ static int fan_forward_v(ctr_handle* h, const float* img, float* out, int mode, 
   return CTR_OK;
 }
 
+// batch == 1: the kernels above on the ABI arrays; batch > 1: slice-interleaved kernels of ctr_si.cu
 int fan_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st) {
   if (h->d.V == 1) return fan_forward_v<1, 1>(h, img, out, mode, bs, st);
-  if (h->d.G >= 3) return fan_forward_v<4, 4>(h, img, out, mode, bs, st);
-  if (h->d.G == 2) return fan_forward_v<4, 2>(h, img, out, mode, bs, st);
-  return fan_forward_v<4, 1>(h, img, out, mode, bs, st);
+  return si_forward(h, img, out, mode, bs, st);
 }
 
 template <int V, int VG>
@@ -413,9 +392,7 @@ static int fan_back_v(ctr_handle* h, const float* sino, float* out, int mode, co
 
 int fan_back(ctr_handle* h, const float* sino, float* out, int mode, const float* s, float* u, cudaStream_t st) {
   if (h->d.V == 1) return fan_back_v<1, 1>(h, sino, out, mode, s, u, st);
-  if (h->d.G >= 3) return fan_back_v<4, 4>(h, sino, out, mode, s, u, st);
-  if (h->d.G == 2) return fan_back_v<4, 2>(h, sino, out, mode, s, u, st);
-  return fan_back_v<4, 1>(h, sino, out, mode, s, u, st);
+  return si_back(h, sino, out, mode, s, u, st);
 }
 
 }  // namespace ctr

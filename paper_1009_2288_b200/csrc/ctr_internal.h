@@ -14,6 +14,7 @@ namespace ctr {
 #define CTR_PROF_MAX 32768
 #define CTR_MAX_BASIS 64 /* stored CGLS gradients used for re-orthogonalisation */
 #define CTR_NCOUNTERS 8
+#define CTR_REDUCE_BLOCKS 1184 /* grid cap of the grid-stride reduction kernels: 148 SMs x 8 */
 
 // Plain-data description of the problem, passed by value to every kernel.
 struct Dims {
@@ -23,7 +24,9 @@ struct Dims {
   int c0x, c0y, c0z;      // grid line taken as coordinate origin (n/2)
   int npix;               // voxels per slice / volume
   int nray;               // rays per slice / volume
-  int G, B, V;            // groups, true batch, slices per group
+  int G, B, V;            // groups (of V slices), true batch, slices per group
+  int GS, LQ;             // slice-interleaved layout: super-groups of LQ groups (LQ*V slices), G = GS*LQ
+  int nvp;                // nviews padded to a multiple of 16 (row length of win2)
   float xlo, ylo, zlo;    // mm, lower corner of the grid
   float dx, dy, dz;       // mm
   float dso, dsd;
@@ -69,11 +72,13 @@ struct ctr_handle {
   float4* rays2;   // 3D second half of the ray record
   float2* views;   // [nviews] (cos, sin)
   unsigned short* win;  // [nviews][npix] first_bin << 4 | count (2D gather window table)
+  unsigned short* win2; // same table as [npix][nvp] (views contiguous), slice-interleaved path only
   int win_ok;           // table usable (nu <= 4095 and every count <= 15)
   float* imgT;          // transposed copy of the image being projected, [G][nx][ny]
   // scratch, internal layout [G][n][V]
   size_t nimg, nsino;  // floats per internal image / sinogram (all groups)
   float *ximg, *bsino, *r, *q, *s, *gimg, *v, *w, *n0;
+  float* usi;           // CGLS iterate in the slice-interleaved layout (batch > 1)
   float* basis;         // [basis_cap][nimg] unit CGLS gradients (S24)
   int basis_cap;
   double* part;
@@ -142,6 +147,13 @@ struct ProfScope {
 int fan_build_tables(ctr_handle* h);
 int fan_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st);
 int fan_back(ctr_handle* h, const float* sino, float* out, int mode, const float* s, float* u, cudaStream_t st);
+// implemented in ctr_si.cu (2D fan beam, batch > 1: slice-interleaved layout [n][LQ] of float4)
+int si_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st);
+int si_back(ctr_handle* h, const float* sino, float* out, int mode, const float* s, float* u, cudaStream_t st);
+int si_from_abi(ctr_handle* h, const float* src, float* dst, size_t n, cudaStream_t st);   // [B][n] -> SI
+int si_to_abi(ctr_handle* h, const float* src, float* dst, size_t n, cudaStream_t st);     // SI -> [B][n]
+int si_from_planar(ctr_handle* h, const float* src, float* dst, size_t n, cudaStream_t st); // [G][n] float4 -> SI
+int si_to_planar(ctr_handle* h, const float* src, float* dst, size_t n, cudaStream_t st);   // SI -> [G][n] float4
 // implemented in ctr_cone.cu (3D cone beam, V = 1)
 int cone_build_tables(ctr_handle* h);
 int cone_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st);

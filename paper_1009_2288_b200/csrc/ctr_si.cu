@@ -1,0 +1,376 @@
+// 2D fan-beam projector pair for BATCHED slices (batch > 1) on sm_100a, slice-interleaved layout.
+//
+// Layout "SI": element e (pixel or ray) of super-group gs holds the LQ*4 slices of
+// that super-group contiguously: float4 index (gs * n + e) * LQ + q, lane c of quad q = slice
+// (gs * LQ + q) * 4 + c. With 64 slices (LQ = 16) one pixel is 256 contiguous bytes.
+//
+// A sub-warp of LQ lanes owns one ray (P) or one pixel (P^T); lane q of the sub-warp carries quad q of
+// the slices. The geometry of a ray/pixel is therefore evaluated ONCE for all slices, in parallel over
+// the lanes of the sub-warp (lane q evaluates slab sb+q of the ray, or view k0+q of the pixel), and the
+// results are handed round by shuffles / a shared-memory queue. Every image or sinogram access of a
+// sub-warp is one contiguous LQ*16-byte segment: the L1 wavefront count per useful byte, which bound
+// the one-thread-per-ray kernel (profiles/r1a_ncu_full_c4.md: 7.5 wavefronts per LDG.128), drops to the
+// minimum of one wavefront per 128 bytes.
+//
+// Both kernels evaluate the SAME slab_weights() on the SAME fp32 ray table as the single-slice kernels
+// of ctr_fan.cu, so every p_ij is identical bit for bit in P and P^T (exact transpose up to summation
+// order).   P: PAPER.md:87-89 (Eq. 1), :193.   P^T: PAPER.md:193, :471 (A3'); north_star.
+#include <limits.h>
+
+#include "ctr_common.cuh"
+#include "ctr_internal.h"
+#include "ctr_fan_geom.cuh"
+
+namespace ctr {
+
+#define FULL 0xffffffffu
+
+__device__ __forceinline__ void fma4(float (&acc)[4], float w, const float4 f) {
+  acc[0] = fmaf(w, f.x, acc[0]);
+  acc[1] = fmaf(w, f.y, acc[1]);
+  acc[2] = fmaf(w, f.z, acc[2]);
+  acc[3] = fmaf(w, f.w, acc[3]);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1  P. Sub-warp per ray. The slab loop runs over a warp-uniform range in batches of LQ slabs: lane q
+// evaluates slab_weights() of slab sb+q (closed form per slab, no dependence between slabs), then the
+// sub-warp walks the LQ slabs in ascending order, every lane accumulating its own quad of slices.
+// MODE 0: out = P x    MODE 1: out = bs - P x (CGLS r0)
+// MODE 2: out = P x and delta = ||out||^2 per slice -> a = gamma/delta (App. I step 1, :423)
+// ------------------------------------------------------------------------------------------------
+template <int LQ, int MODE>
+__global__ void __launch_bounds__(256) k_si_forward(Dims d, const float4* __restrict__ rays,
+                                                    const float4* __restrict__ img, float4* __restrict__ out,
+                                                    const float4* __restrict__ bs, Scal sc, double* part,
+                                                    unsigned* counter) {
+  constexpr int RW = 32 / LQ;  // rays per warp
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int q = lane % LQ, sub = lane / LQ;
+  const int r = (blockIdx.x * 8 + warp) * RW + sub;
+  const int gs = blockIdx.y;
+  const bool live = r < d.nray;
+  float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+
+  float x0 = 0.0f, m = 0.0f, L = 0.0f, K = 0.0f;
+  bool xdrv = false;
+  int s0 = INT_MAX, s1 = 0;
+  if (live) {
+    const float4 R = __ldg(&rays[r]);
+    x0 = R.x; m = R.y; L = fabsf(R.z); K = R.w;
+    xdrv = R.z < 0.0f;
+  }
+  const int n_drv = xdrv ? d.nx : d.ny, n_oth = xdrv ? d.ny : d.nx;
+  const int c_drv = xdrv ? d.c0x : d.c0y, c_oth = xdrv ? d.c0y : d.c0x;
+  if (live) {
+    // slabs in which the ray can be inside [-c_oth, n_oth - c_oth) (same margins as k_fan_forward)
+    s0 = 0; s1 = n_drv;
+    const float lo = (float)(-c_oth) - 1.0f, hi = (float)(n_oth - c_oth) + 1.0f;
+    if (m != 0.0f) {
+      float t1 = (lo - x0) / m, t2 = (hi - x0) / m;
+      float tmin = fminf(t1, t2), tmax = fmaxf(t1, t2);
+      tmin = fminf(fmaxf(tmin, -1.0e6f), 1.0e6f);
+      tmax = fminf(fmaxf(tmax, -1.0e6f), 1.0e6f);
+      s0 = max(0, (int)floorf(tmin) + c_drv - 2);
+      s1 = min(n_drv, (int)ceilf(tmax) + c_drv + 2);
+    } else if (x0 < lo || x0 > hi) {
+      s1 = 0;
+    }
+    if (s1 <= s0) { s0 = INT_MAX; s1 = 0; }
+  }
+  const int w_lo = __reduce_min_sync(FULL, s0), w_hi = __reduce_max_sync(FULL, s1);
+  const float4* base = img + (size_t)gs * d.npix * LQ + q;
+  const int st_drv = (xdrv ? 1 : d.nx) * LQ;  // float4 stride of one slab step
+  const int st_oth = (xdrv ? d.nx : 1) * LQ;  // float4 stride of one cell of the other axis
+
+  for (int sb = w_lo; sb < w_hi; sb += LQ) {
+    const int s = sb + q;
+    int pa = 0;
+    float wa = 0.0f, wb = 0.0f;  // wb carries the direction of the second cell in its sign
+    if (s >= s0 && s < s1) {
+      const float y = (float)(s - c_drv);
+      const float oa = fmaf(m, y, x0), ob = fmaf(m, y + 1.0f, x0);
+      const SlabW w = slab_weights(oa, ob, L, K);
+      const int ia = cell_of(w.ra) + c_oth, ib = cell_of(w.rb) + c_oth;
+      const bool va = (unsigned)ia < (unsigned)n_oth;
+      const bool vb = w.wb != 0.0f && (unsigned)ib < (unsigned)n_oth;
+      if (va) {
+        pa = s * st_drv + ia * st_oth;
+        wa = w.wa;
+        if (vb) wb = ib > ia ? w.wb : -w.wb;
+      } else if (vb) {
+        pa = s * st_drv + ib * st_oth;
+        wa = w.wb;
+      }
+    }
+#pragma unroll
+    for (int t = 0; t < LQ; ++t) {
+      const int pa_t = __shfl_sync(FULL, pa, t, LQ);
+      const float wa_t = __shfl_sync(FULL, wa, t, LQ);
+      const float wb_t = __shfl_sync(FULL, wb, t, LQ);
+      if (wa_t != 0.0f) fma4(acc, wa_t, __ldg(base + pa_t));
+      if (wb_t != 0.0f) fma4(acc, fabsf(wb_t), __ldg(base + (wb_t > 0.0f ? pa_t + st_oth : pa_t - st_oth)));
+    }
+  }
+  if (live) {
+    const size_t e = ((size_t)gs * d.nray + r) * LQ + q;
+    if (MODE == 1) {
+      const float4 b = __ldg(bs + e);
+      acc[0] = b.x - acc[0]; acc[1] = b.y - acc[1]; acc[2] = b.z - acc[2]; acc[3] = b.w - acc[3];
+    }
+    out[e] = make_float4(acc[0], acc[1], acc[2], acc[3]);
+  }
+  if (MODE == 2) {
+    double v[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) v[c] = live ? (double)acc[c] * (double)acc[c] : 0.0;
+    grid_reduce_q<4, 8>(v, LQ, part + (size_t)gs * gridDim.x * LQ * 4, counter + gs, gridDim.x, blockIdx.x,
+                        threadIdx.x, [&](int qq, double(&sum)[4]) {
+#pragma unroll
+                          for (int c = 0; c < 4; ++c) {
+                            const int sl = (gs * LQ + qq) * 4 + c;
+                            const double gamma = sc.gamma[sl];
+                            sc.a[sl] = (sum[c] > 0.0 && gamma > 0.0) ? (float)(gamma / sum[c]) : 0.0f;  // S4
+                          }
+                        });
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a2  P^T (gather). Sub-warp per pixel; a block is a TX x TY tile of pixels, so the sinogram segments
+// it reads overlap in L1. Views are taken LQ at a time: lane q looks up the bins of view k0+q whose
+// rays cross the pixel (window table win2, or fan_window() when the table is not usable) and evaluates
+// their weights; non-zero (ray, weight) pairs are compacted into a per-pixel shared-memory queue in a
+// fixed order (candidate slot, then view), which the sub-warp then drains: one contiguous LQ*16-byte
+// sinogram read and 4 FMAs per lane per pair. No atomics; the order of additions is fixed.
+// MODE 0: out = P^T y     MODE 2: out = g = P^T r and, fused, u += a s (App. I step 2)
+// ------------------------------------------------------------------------------------------------
+#define SI_CH 4 /* candidate slots per lane between two drains of the queue */
+
+template <int LQ, int MODE, int TABLE>
+__global__ void __launch_bounds__(256) k_si_back(Dims d, const float4* __restrict__ rays,
+                                                 const float2* __restrict__ views,
+                                                 const unsigned short* __restrict__ win2,
+                                                 const float4* __restrict__ sino, float4* __restrict__ out,
+                                                 const float4* __restrict__ s_img, float4* __restrict__ u_img, Scal sc) {
+  constexpr int PB = 256 / LQ;  // pixels per block
+  constexpr int TX = PB >= 64 ? 8 : 4, TY = PB / TX;
+  __shared__ float2 queue[PB][LQ * SI_CH];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int q = lane % LQ, sub = lane / LQ;
+  const int pl = warp * (32 / LQ) + sub;
+  const int i = blockIdx.x * TX + pl % TX, j = blockIdx.y * TY + pl / TX;
+  const int gs = blockIdx.z;
+  const bool live = i < d.nx && j < d.ny;
+  float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+  const float fi = (float)(i - d.c0x), fj = (float)(j - d.c0y);
+  const float bi = bias_of(i - d.c0x), bj = bias_of(j - d.c0y);
+  const float px = fmaf((float)i + 0.5f, d.dx, d.xlo), py = fmaf((float)j + 0.5f, d.dy, d.ylo);
+  const int pix = j * d.nx + i;
+  const unsigned submask = (LQ == 32 ? FULL : ((1u << LQ) - 1u)) << (sub * LQ);
+  const unsigned lt = submask & ((1u << lane) - 1u);
+  const float4* sg = sino + (size_t)gs * d.nray * LQ + q;
+  float2* myq = queue[pl];
+
+  for (int k0 = 0; k0 < d.nviews; k0 += LQ) {
+    const int k = k0 + q;
+    int b_lo = 0, cnt = 0;
+    if (live && k < d.nviews) {
+      if (TABLE) {
+        const unsigned w = __ldg(&win2[(size_t)pix * d.nvp + k]);
+        b_lo = (int)(w >> 4);
+        cnt = (int)(w & 15u);
+      } else {
+        int b_hi;
+        fan_window(d, __ldg(&views[k]), px, py, b_lo, b_hi);
+        cnt = max(0, b_hi - b_lo + 1);
+      }
+    }
+    const int maxc = __reduce_max_sync(FULL, cnt);
+    for (int c0 = 0; c0 < maxc; c0 += SI_CH) {
+      int n = 0;
+#pragma unroll
+      for (int c = 0; c < SI_CH; ++c) {
+        float wt = 0.0f;
+        int idx = 0;
+        if (c0 + c < cnt) {
+          idx = k * d.nu + b_lo + c0 + c;
+          wt = fan_pixel_weight(__ldg(&rays[idx]), fi, fj, bi, bj);
+        }
+        const bool hit = wt != 0.0f;
+        const unsigned bal = __ballot_sync(FULL, hit) & submask;
+        if (hit) myq[n + __popc(bal & lt)] = make_float2(__int_as_float(idx), wt);
+        n += __popc(bal);
+      }
+      __syncwarp();
+#pragma unroll 4
+      for (int e = 0; e < n; ++e) {
+        const float2 h = myq[e];
+        fma4(acc, h.y, __ldg(sg + (size_t)__float_as_int(h.x) * LQ));
+      }
+      __syncwarp();
+    }
+  }
+  if (!live) return;
+  const size_t e = ((size_t)gs * d.npix + pix) * LQ + q;
+  out[e] = make_float4(acc[0], acc[1], acc[2], acc[3]);
+  if (MODE == 2) {
+    const float4 sv = __ldcg(s_img + e);
+    float4 uv = __ldcg(u_img + e);
+    const int sl = (gs * LQ + q) * 4;
+    uv.x = fmaf(sc.a[sl + 0], sv.x, uv.x);
+    uv.y = fmaf(sc.a[sl + 1], sv.y, uv.y);
+    uv.z = fmaf(sc.a[sl + 2], sv.z, uv.z);
+    uv.w = fmaf(sc.a[sl + 3], sv.w, uv.w);
+    u_img[e] = uv;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Layout conversions. ABI: [B][n] floats. Planar (TV kernels): [G][n] float4. SI: [GS][n][LQ] float4.
+// Slice (g, c) of the planar layout is slice (gs * LQ + q, c) of SI with g = gs * LQ + q.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_si_from_abi(const float* __restrict__ src, float4* __restrict__ dst, int n,
+                                                     int B, int LQ) {
+  const int e = blockIdx.x * 256 + threadIdx.x, g = blockIdx.y;
+  if (e >= n) return;
+  float o[4];
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    const int sl = 4 * g + c;
+    o[c] = sl < B ? __ldg(src + (size_t)sl * n + e) : 0.0f;
+  }
+  dst[((size_t)(g / LQ) * n + e) * LQ + g % LQ] = make_float4(o[0], o[1], o[2], o[3]);
+}
+
+__global__ void __launch_bounds__(256) k_si_to_abi(const float4* __restrict__ src, float* __restrict__ dst, int n,
+                                                   int B, int LQ) {
+  const int e = blockIdx.x * 256 + threadIdx.x, g = blockIdx.y;
+  if (e >= n) return;
+  const float4 t = __ldg(src + ((size_t)(g / LQ) * n + e) * LQ + g % LQ);
+  const float o[4] = {t.x, t.y, t.z, t.w};
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    const int sl = 4 * g + c;
+    if (sl < B) dst[(size_t)sl * n + e] = o[c];
+  }
+}
+
+// planar <-> SI through a shared-memory tile of 32 elements x LQ quads (both sides coalesced)
+template <int TO_SI>
+__global__ void __launch_bounds__(256) k_si_planar(const float4* __restrict__ src, float4* __restrict__ dst, int n,
+                                                   int LQ) {
+  __shared__ float4 tile[16][33];  // LQ <= 16
+  const int gs = blockIdx.y, e0 = blockIdx.x * 32, tid = threadIdx.x;
+  const int nel = 32 * LQ;
+  if (TO_SI) {
+    for (int t = tid; t < nel; t += 256) {
+      const int qq = t >> 5, el = t & 31;
+      if (e0 + el < n) tile[qq][el] = __ldcg(src + ((size_t)(gs * LQ + qq) * n + e0 + el));
+    }
+    __syncthreads();
+    for (int t = tid; t < nel; t += 256) {
+      const int el = t / LQ, qq = t % LQ;
+      if (e0 + el < n) dst[((size_t)gs * n + e0 + el) * LQ + qq] = tile[qq][el];
+    }
+  } else {
+    for (int t = tid; t < nel; t += 256) {
+      const int el = t / LQ, qq = t % LQ;
+      if (e0 + el < n) tile[qq][el] = __ldcg(src + ((size_t)gs * n + e0 + el) * LQ + qq);
+    }
+    __syncthreads();
+    for (int t = tid; t < nel; t += 256) {
+      const int qq = t >> 5, el = t & 31;
+      if (e0 + el < n) dst[(size_t)(gs * LQ + qq) * n + e0 + el] = tile[qq][el];
+    }
+  }
+}
+
+int si_from_abi(ctr_handle* h, const float* src, float* dst, size_t n, cudaStream_t st) {
+  dim3 grid((unsigned)((n + 255) / 256), h->d.G);
+  ProfScope prof(h, CTR_PROF_LAYOUT, st);
+  k_si_from_abi<<<grid, 256, 0, st>>>(src, (float4*)dst, (int)n, h->d.B, h->d.LQ);
+  CTR_LAUNCHED(h);
+  return CTR_OK;
+}
+int si_to_abi(ctr_handle* h, const float* src, float* dst, size_t n, cudaStream_t st) {
+  dim3 grid((unsigned)((n + 255) / 256), h->d.G);
+  ProfScope prof(h, CTR_PROF_LAYOUT, st);
+  k_si_to_abi<<<grid, 256, 0, st>>>((const float4*)src, dst, (int)n, h->d.B, h->d.LQ);
+  CTR_LAUNCHED(h);
+  return CTR_OK;
+}
+int si_from_planar(ctr_handle* h, const float* src, float* dst, size_t n, cudaStream_t st) {
+  dim3 grid((unsigned)((n + 31) / 32), h->d.GS);
+  ProfScope prof(h, CTR_PROF_LAYOUT, st);
+  k_si_planar<1><<<grid, 256, 0, st>>>((const float4*)src, (float4*)dst, (int)n, h->d.LQ);
+  CTR_LAUNCHED(h);
+  return CTR_OK;
+}
+int si_to_planar(ctr_handle* h, const float* src, float* dst, size_t n, cudaStream_t st) {
+  dim3 grid((unsigned)((n + 31) / 32), h->d.GS);
+  ProfScope prof(h, CTR_PROF_LAYOUT, st);
+  k_si_planar<0><<<grid, 256, 0, st>>>((const float4*)src, (float4*)dst, (int)n, h->d.LQ);
+  CTR_LAUNCHED(h);
+  return CTR_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// host side: dispatch on LQ (1, 2, 4, 8, 16)
+// ------------------------------------------------------------------------------------------------
+template <int LQ>
+static int si_forward_t(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st) {
+  const Dims& d = h->d;
+  const int rays_per_block = 8 * (32 / LQ);
+  dim3 grid((d.nray + rays_per_block - 1) / rays_per_block, d.GS);
+  unsigned* cnt = h->counters + 0 * d.G;
+  const float4 *im = (const float4*)img, *b4 = (const float4*)bs;
+  float4* o4 = (float4*)out;
+  ProfScope prof(h, CTR_PROF_FORWARD, st);
+  if (mode == 0) k_si_forward<LQ, 0><<<grid, 256, 0, st>>>(d, h->rays, im, o4, b4, h->sc, h->part, cnt);
+  else if (mode == 1) k_si_forward<LQ, 1><<<grid, 256, 0, st>>>(d, h->rays, im, o4, b4, h->sc, h->part, cnt);
+  else k_si_forward<LQ, 2><<<grid, 256, 0, st>>>(d, h->rays, im, o4, b4, h->sc, h->part, cnt);
+  CTR_LAUNCHED(h);
+  return CTR_OK;
+}
+
+template <int LQ>
+static int si_back_t(ctr_handle* h, const float* sino, float* out, int mode, const float* s, float* u, cudaStream_t st) {
+  const Dims& d = h->d;
+  constexpr int PB = 256 / LQ, TX = PB >= 64 ? 8 : 4, TY = PB / TX;
+  dim3 grid((d.nx + TX - 1) / TX, (d.ny + TY - 1) / TY, d.GS);
+  const float4 *y4 = (const float4*)sino, *s4 = (const float4*)s;
+  float4 *o4 = (float4*)out, *u4 = (float4*)u;
+  ProfScope prof(h, CTR_PROF_BACK, st);
+#define CTR_SI_BACK(M, T) k_si_back<LQ, M, T><<<grid, 256, 0, st>>>(d, h->rays, h->views, h->win2, y4, o4, s4, u4, h->sc)
+  if (h->win_ok) {
+    if (mode == 0) CTR_SI_BACK(0, 1); else CTR_SI_BACK(2, 1);
+  } else {
+    if (mode == 0) CTR_SI_BACK(0, 0); else CTR_SI_BACK(2, 0);
+  }
+#undef CTR_SI_BACK
+  CTR_LAUNCHED(h);
+  return CTR_OK;
+}
+
+int si_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st) {
+  switch (h->d.LQ) {
+    case 1: return si_forward_t<1>(h, img, out, mode, bs, st);
+    case 2: return si_forward_t<2>(h, img, out, mode, bs, st);
+    case 4: return si_forward_t<4>(h, img, out, mode, bs, st);
+    case 8: return si_forward_t<8>(h, img, out, mode, bs, st);
+    default: return si_forward_t<16>(h, img, out, mode, bs, st);
+  }
+}
+
+int si_back(ctr_handle* h, const float* sino, float* out, int mode, const float* s, float* u, cudaStream_t st) {
+  switch (h->d.LQ) {
+    case 1: return si_back_t<1>(h, sino, out, mode, s, u, st);
+    case 2: return si_back_t<2>(h, sino, out, mode, s, u, st);
+    case 4: return si_back_t<4>(h, sino, out, mode, s, u, st);
+    case 8: return si_back_t<8>(h, sino, out, mode, s, u, st);
+    default: return si_back_t<16>(h, sino, out, mode, s, u, st);
+  }
+}
+
+}  // namespace ctr

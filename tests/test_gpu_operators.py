@@ -93,10 +93,11 @@ def test_batched_slices_match_oracle_per_slice(ctr, torch_cuda, orc):
     for sl in (0, 3, 5):
         assert rel(got_s[sl], orc.forward(cfg, case["truth"][sl].astype(np.float64))) <= TOL_OP
         assert rel(got_i[sl], orc.back(cfg, case["sino"][sl].astype(np.float64))) <= TOL_OP
-    # batched result == single-slice result, bit for bit (same arithmetic per slice)
+    # batched vs single-slice kernels: same p_ij bit for bit; P also adds them in the same order, the
+    # batched gather P^T in a different fixed order (ctr_si.cu), so that one agrees to fp32 rounding only
     one = scaled_config("c2", batch=1)
     assert np.array_equal(gpu_forward(ctr, torch_cuda, one, case["truth"][4:5])[0], got_s[4])
-    assert np.array_equal(gpu_back(ctr, torch_cuda, one, case["sino"][4:5])[0], got_i[4])
+    assert rel(gpu_back(ctr, torch_cuda, one, case["sino"][4:5])[0], got_i[4].astype(np.float64)) <= 1e-6
 
 
 @pytest.mark.parametrize("name,batch", [("c1", 1), ("c3", 1), ("c2", 5)])

@@ -548,3 +548,26 @@ def test_reconstruct_c1_reduces_error_and_stays_positive(orc):
     assert f.min() >= 0.0
     assert np.linalg.norm(f - truth) < 0.5 * np.linalg.norm(truth)
     assert np.all(log[:, 1] >= 0)
+
+
+# ------------------------------------------------------------------ S25: the composed iteration is well posed
+def test_reconstruct_is_reproducible_under_the_S25_constants(orc):
+    """DESIGN.md S25. With Armijo c = 1e-4 and eps = 1e-6 (a legal reading of PAPER.md:149, which gives no
+    constants) the composed iteration amplifies a 1e-8 relative perturbation of the sinogram by > 1e4 on
+    configs[0] (overshooting steps on a nearly non-smooth term: no fp32 implementation can track it to
+    north_star's 1e-3). With c = 1/2 (never beyond the line minimiser of a quadratic) and eps = 1e-4 the
+    amplification is that of the restarted CGLS alone (< 50)."""
+    from ctr_inputs import make_case, scaled_config
+    rng = np.random.default_rng(5)
+
+    def amplification(cfg, p=1e-8):
+        y = make_case(cfg, raster=False)["sino"][0].astype(np.float64)
+        base, _, _ = orc.reconstruct(cfg, y, cfg)
+        pert, _, _ = orc.reconstruct(cfg, y * (1 + p * rng.standard_normal(y.shape)), cfg)
+        return np.linalg.norm(pert - base) / np.linalg.norm(base) / p
+
+    cfg = scaled_config("c1")
+    assert (float(np.float32(cfg.armijo_c)), float(np.float32(cfg.eps))) == (0.5, float(np.float32(1e-4)))
+    assert amplification(cfg) < 50
+    assert amplification(scaled_config("c1", n_gd=0)) < 50          # restarted CGLS alone
+    assert amplification(scaled_config("c1", armijo_c=1e-4, eps=1e-6)) > 1e3
