@@ -158,15 +158,7 @@ __global__ void __launch_bounds__(256) k_reorth_dots(size_t nl, int LQ, size_t n
   double red[REORTH_NB * V];
 #pragma unroll
   for (int q = 0; q < REORTH_NB * V; ++q) red[q] = (double)acc[q];
-  grid_reduce_q<REORTH_NB * V, 8>(red, LQ, part + (size_t)gs * gridDim.x * LQ * REORTH_NB * V, counter + gs, gridDim.x,
-                                  blockIdx.x, threadIdx.x, [&](int qq, double(&sum)[REORTH_NB * V]) {
-#pragma unroll
-                                    for (int q = 0; q < REORTH_NB; ++q)
-#pragma unroll
-                                      for (int c = 0; c < V; ++c)
-                                        if (q < nb)
-                                          sc.coef[(size_t)(i0 + q) * Bp + (gs * LQ + qq) * V + c] = (float)sum[q * V + c];
-                                  });
+  block_partials_q<REORTH_NB * V, 8>(red, LQ, part + (size_t)gs * gridDim.x * LQ * REORTH_NB * V, blockIdx.x, threadIdx.x);
 }
 
 template <int V>
@@ -192,19 +184,59 @@ __global__ void __launch_bounds__(256) k_reorth_sub(size_t nl, int LQ, size_t ni
 #pragma unroll
     for (int c = 0; c < V; ++c) red[c] = fma((double)gv[c], (double)gv[c], red[c]);
   }
-  grid_reduce_q<V, 8>(red, LQ, part + (size_t)gs * gridDim.x * LQ * V, counter + gs, gridDim.x, blockIdx.x, threadIdx.x,
-                      [&](int qq, double(&sum)[V]) {
-#pragma unroll
-                        for (int c = 0; c < V; ++c) {
-                          const int sl = (gs * LQ + qq) * V + c;
-                          if (!first) {
-                            const double gamma = sc.gamma[sl];
-                            sc.beta[sl] = gamma > 0.0 ? (float)(sum[c] / gamma) : 0.0f;  // S4
-                          }
-                          sc.gamma[sl] = sum[c];
-                          sc.ginv[sl] = sum[c] > 0.0 ? (float)(1.0 / sqrt(sum[c])) : 0.0f;
-                        }
-                      });
+  block_partials_q<V, 8>(red, LQ, part + (size_t)gs * gridDim.x * LQ * V, blockIdx.x, threadIdx.x);
+}
+
+// Finishing pass of the segmented reductions: block (q, gs) adds the partials part[gs][b][q][0..N) over the
+// blocks b in a fixed order and applies the scalar update of the producing kernel:
+//   FIN_ALPHA  N = V:       delta = ||P s||^2 -> a = gamma/delta            (App. I step 1)
+//   FIN_COEF   N = NB * V:  c_i = <b_i, g>                                   (S24)
+//   FIN_GAMMA  N = V:       gamma' = ||g||^2, beta = gamma'/gamma, 1/||g||   (App. I step 4, :432)
+template <int N>
+__global__ void __launch_bounds__(256) k_finish(int mode, const double* __restrict__ part, int nblk, int LQ, int V,
+                                                int i0, int nb, int Bp, int first, Scal sc) {
+  __shared__ double sm[256];
+  const int q = blockIdx.x, gs = blockIdx.y, t = threadIdx.x;
+  const int n = t % N, b0 = t / N;
+  constexpr int NB0 = 256 / N;
+  double acc = 0.0;
+  const double* p = part + ((size_t)gs * nblk * LQ + q) * N + n;
+#pragma unroll 4
+  for (int b = b0; b < nblk; b += NB0) acc += __ldcg(p + (size_t)b * LQ * N);
+  sm[t] = acc;
+  __syncthreads();
+  if (t >= N) return;
+  double sum = 0.0;
+  for (int j = 0; j < NB0; ++j) sum += sm[j * N + n];
+  const int c = n % V, sl = (gs * LQ + q) * V + c;
+  if (mode == CTR_FIN_ALPHA) {
+    const double gamma = sc.gamma[sl];
+    sc.a[sl] = (sum > 0.0 && gamma > 0.0) ? (float)(gamma / sum) : 0.0f;  // S4
+  } else if (mode == CTR_FIN_COEF) {
+    const int qb = n / V;
+    if (qb < nb) sc.coef[(size_t)(i0 + qb) * Bp + sl] = (float)sum;
+  } else {
+    if (!first) {
+      const double gamma = sc.gamma[sl];
+      sc.beta[sl] = gamma > 0.0 ? (float)(sum / gamma) : 0.0f;  // S4
+    }
+    sc.gamma[sl] = sum;
+    sc.ginv[sl] = sum > 0.0 ? (float)(1.0 / sqrt(sum)) : 0.0f;
+  }
+}
+
+int reduce_finish(ctr_handle* h, int mode, int N, int nblk, int i0, int nb, int first, cudaStream_t st) {
+  const Dims& d = h->d;
+  dim3 grid(d.LQ, d.GS);
+  const int Bp = d.G * d.V;
+  switch (N) {
+    case 1: k_finish<1><<<grid, 256, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
+    case 4: k_finish<4><<<grid, 256, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
+    case 8: k_finish<8><<<grid, 256, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
+    default: k_finish<32><<<grid, 256, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
+  }
+  CTR_LAUNCHED(h);
+  return CTR_OK;
 }
 
 static int vec_sino_axpy(ctr_handle* h, float* r, const float* q, cudaStream_t st) {
@@ -253,11 +285,13 @@ static int vec_reorth(ctr_handle* h, float* g, int nb, int first, cudaStream_t s
     if (d.V == 1) k_reorth_dots<1><<<dgrid, 256, 0, st>>>(nl, d.LQ, h->nimg, g, h->basis, i0, cnt, Bp, h->sc, h->part, h->counters + 4 * d.G);
     else k_reorth_dots<4><<<dgrid, 256, 0, st>>>(nl, d.LQ, h->nimg, g, h->basis, i0, cnt, Bp, h->sc, h->part, h->counters + 4 * d.G);
     CTR_LAUNCHED(h);
+    int rc = reduce_finish(h, CTR_FIN_COEF, REORTH_NB * d.V, (int)dgrid.x, i0, cnt, 0, st);
+    if (rc) return rc;
   }
   if (d.V == 1) k_reorth_sub<1><<<grid, 256, 0, st>>>(nl, d.LQ, h->nimg, g, h->basis, nb, Bp, first, h->sc, h->part, h->counters + 5 * d.G);
   else k_reorth_sub<4><<<grid, 256, 0, st>>>(nl, d.LQ, h->nimg, g, h->basis, nb, Bp, first, h->sc, h->part, h->counters + 5 * d.G);
   CTR_LAUNCHED(h);
-  return CTR_OK;
+  return reduce_finish(h, CTR_FIN_GAMMA, d.V, (int)grid.x, 0, 0, first, st);
 }
 
 static int op_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st) {
@@ -371,7 +405,7 @@ void ctr_destroy(ctr_handle* h) {
   if (!h) return;
   cudaDeviceSynchronize();
   void* bufs[] = {h->rays, h->rays2, h->views, h->ximg, h->bsino, h->r, h->q, h->s, h->gimg, h->v, h->w, h->n0,
-                  h->part, h->counters, h->hist, h->scal_block, h->stats, h->basis, h->win, h->imgT, h->win2, h->usi};
+                  h->part, h->counters, h->hist, h->scal_block, h->stats, h->basis, h->win, h->imgT, h->win2, h->usi, h->hits, h->hcnt};
   for (void* b : bufs)
     if (b) cudaFree(b);
   if (h->prof_ev) {
@@ -524,6 +558,7 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
   }
   set_quantile(h, h->p.sigma_quantile);
   int rc = d.ndim == 3 ? cone_build_tables(h) : fan_build_tables(h);
+  if (rc == CTR_OK && d.ndim == 2 && d.V == 4) rc = si_build_hits(h);
   if (rc != CTR_OK) { ctr_destroy(h); return rc; }
   *out = h;
   return CTR_OK;

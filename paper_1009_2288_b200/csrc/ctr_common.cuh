@@ -88,8 +88,7 @@ __device__ __forceinline__ void grid_reduce(double (&v)[N], double* part, unsign
 // ---------------------------------------------------------------------------------------------
 // Segmented variant for the slice-interleaved layout: thread tid holds N partial
 // sums that belong to segment tid % LQ (LQ a power of two <= 16, block size NW * 32); the
-// sums are kept apart per segment. fin(q, sums) is called by thread q < LQ of the last block with the
-// totals of segment q. Partials: part[(blk * LQ + q) * N + n]. Order of additions is fixed.
+// sums are kept apart per segment. Order of additions is fixed.
 // ---------------------------------------------------------------------------------------------
 template <int N, int NW>
 __device__ __forceinline__ void block_sum_q(double (&v)[N], double (*sm)[NW][16], int LQ, int tid) {
@@ -112,35 +111,17 @@ __device__ __forceinline__ void block_sum_q(double (&v)[N], double (*sm)[NW][16]
   __syncthreads();
 }
 
-template <int N, int NW, class Fin>
-__device__ __forceinline__ void grid_reduce_q(double (&v)[N], int LQ, double* part, unsigned* counter, unsigned nblk,
-                                              unsigned blk, int tid, Fin fin) {
+// block partials of a segmented reduction: part[(blk * LQ + q) * N + n]; a finishing kernel
+// (k_finish, ctr_api.cu) adds them over the blocks in a fixed order. A single finishing BLOCK inside the
+// producing kernel cost 120-350 us per launch at 64 slices (profiles/r1b): hence the extra tiny launch.
+template <int N, int NW>
+__device__ __forceinline__ void block_partials_q(double (&v)[N], int LQ, double* part, unsigned blk, int tid) {
   __shared__ double sm[N][NW][16];  // LQ <= 16
-  __shared__ bool last;
   block_sum_q<N, NW>(v, sm, LQ, tid);
   if (tid < LQ) {
 #pragma unroll
     for (int n = 0; n < N; ++n) part[((size_t)blk * LQ + tid) * N + n] = v[n];
-    __threadfence();
   }
-  __syncthreads();
-  if (tid == 0) {
-    unsigned t = atomicInc(counter, nblk - 1);
-    last = (t == nblk - 1);
-  }
-  __syncthreads();
-  if (!last) return;
-  __threadfence();
-  double acc[N];
-#pragma unroll
-  for (int n = 0; n < N; ++n) acc[n] = 0.0;
-  const int q = tid & (LQ - 1);
-  for (unsigned b = tid / LQ; b < nblk; b += (NW * 32) / LQ) {
-#pragma unroll
-    for (int n = 0; n < N; ++n) acc[n] += __ldcg(&part[((size_t)b * LQ + q) * N + n]);
-  }
-  block_sum_q<N, NW>(acc, sm, LQ, tid);
-  if (tid < LQ) fin(tid, acc);
 }
 
 // ---------------------------------------------------------------------------------------------

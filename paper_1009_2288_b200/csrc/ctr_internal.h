@@ -78,6 +78,9 @@ struct ctr_handle {
   // scratch, internal layout [G][n][V]
   size_t nimg, nsino;  // floats per internal image / sinogram (all groups)
   float *ximg, *bsino, *r, *q, *s, *gimg, *v, *w, *n0;
+  float2* hits;         // [npix][hits_cap] (ray index * LQ, p_ij): pixel hit table of the batched gather P^T
+  int* hcnt;            // [npix] entries used per pixel
+  int hits_cap;
   float* usi;           // CGLS iterate in the slice-interleaved layout (batch > 1)
   float* basis;         // [basis_cap][nimg] unit CGLS gradients (S24)
   int basis_cap;
@@ -150,6 +153,7 @@ int fan_back(ctr_handle* h, const float* sino, float* out, int mode, const float
 // implemented in ctr_si.cu (2D fan beam, batch > 1: slice-interleaved layout [n][LQ] of float4)
 int si_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st);
 int si_back(ctr_handle* h, const float* sino, float* out, int mode, const float* s, float* u, cudaStream_t st);
+int si_build_hits(ctr_handle* h);
 int si_from_abi(ctr_handle* h, const float* src, float* dst, size_t n, cudaStream_t st);   // [B][n] -> SI
 int si_to_abi(ctr_handle* h, const float* src, float* dst, size_t n, cudaStream_t st);     // SI -> [B][n]
 int si_from_planar(ctr_handle* h, const float* src, float* dst, size_t n, cudaStream_t st); // [G][n] float4 -> SI
@@ -162,6 +166,8 @@ int cone_back(ctr_handle* h, const float* sino, float* out, int mode, const floa
 int tv_update_weights(ctr_handle* h, const float* f, float* w, cudaStream_t st);
 int tv_sweep(ctr_handle* h, float* f, const float* v, const float* w, float lambda, int clamp, cudaStream_t st);
 int tv_clamp(ctr_handle* h, float* f, cudaStream_t st);
-// implemented in ctr_api.cu
+// implemented in ctr_api.cu: finishing pass of a segmented reduction (block partials in h->part)
+enum { CTR_FIN_ALPHA = 0, CTR_FIN_COEF = 1, CTR_FIN_GAMMA = 2 };
+int reduce_finish(ctr_handle* h, int mode, int N, int nblk, int i0, int nb, int first, cudaStream_t st);
 
 }  // namespace ctr

@@ -80,13 +80,14 @@ __global__ void __launch_bounds__(256) k_si_forward(Dims d, const float4* __rest
   }
   const int w_lo = __reduce_min_sync(FULL, s0), w_hi = __reduce_max_sync(FULL, s1);
   const float4* base = img + (size_t)gs * d.npix * LQ + q;
+  asm volatile("" : "+l"(base));  // keep the pointer in a register pair: one IMAD.WIDE per address
   const int st_drv = (xdrv ? 1 : d.nx) * LQ;  // float4 stride of one slab step
   const int st_oth = (xdrv ? d.nx : 1) * LQ;  // float4 stride of one cell of the other axis
 
   for (int sb = w_lo; sb < w_hi; sb += LQ) {
     const int s = sb + q;
-    int pa = 0;
-    float wa = 0.0f, wb = 0.0f;  // wb carries the direction of the second cell in its sign
+    int pa = 0, pb = 0;
+    float wa = 0.0f, wb = 0.0f;
     if (s >= s0 && s < s1) {
       const float y = (float)(s - c_drv);
       const float oa = fmaf(m, y, x0), ob = fmaf(m, y + 1.0f, x0);
@@ -97,7 +98,7 @@ __global__ void __launch_bounds__(256) k_si_forward(Dims d, const float4* __rest
       if (va) {
         pa = s * st_drv + ia * st_oth;
         wa = w.wa;
-        if (vb) wb = ib > ia ? w.wb : -w.wb;
+        if (vb) { pb = s * st_drv + ib * st_oth; wb = w.wb; }
       } else if (vb) {
         pa = s * st_drv + ib * st_oth;
         wa = w.wb;
@@ -108,8 +109,9 @@ __global__ void __launch_bounds__(256) k_si_forward(Dims d, const float4* __rest
       const int pa_t = __shfl_sync(FULL, pa, t, LQ);
       const float wa_t = __shfl_sync(FULL, wa, t, LQ);
       const float wb_t = __shfl_sync(FULL, wb, t, LQ);
+      const int pb_t = __shfl_sync(FULL, pb, t, LQ);
       if (wa_t != 0.0f) fma4(acc, wa_t, __ldg(base + pa_t));
-      if (wb_t != 0.0f) fma4(acc, fabsf(wb_t), __ldg(base + (wb_t > 0.0f ? pa_t + st_oth : pa_t - st_oth)));
+      if (wb_t != 0.0f) fma4(acc, wb_t, __ldg(base + pb_t));
     }
   }
   if (live) {
@@ -124,15 +126,7 @@ __global__ void __launch_bounds__(256) k_si_forward(Dims d, const float4* __rest
     double v[4];
 #pragma unroll
     for (int c = 0; c < 4; ++c) v[c] = live ? (double)acc[c] * (double)acc[c] : 0.0;
-    grid_reduce_q<4, 8>(v, LQ, part + (size_t)gs * gridDim.x * LQ * 4, counter + gs, gridDim.x, blockIdx.x,
-                        threadIdx.x, [&](int qq, double(&sum)[4]) {
-#pragma unroll
-                          for (int c = 0; c < 4; ++c) {
-                            const int sl = (gs * LQ + qq) * 4 + c;
-                            const double gamma = sc.gamma[sl];
-                            sc.a[sl] = (sum[c] > 0.0 && gamma > 0.0) ? (float)(gamma / sum[c]) : 0.0f;  // S4
-                          }
-                        });
+    block_partials_q<4, 8>(v, LQ, part + (size_t)gs * gridDim.x * LQ * 4, blockIdx.x, threadIdx.x);
   }
 }
 
@@ -224,6 +218,124 @@ __global__ void __launch_bounds__(256) k_si_back(Dims d, const float4* __restric
     uv.w = fmaf(sc.a[sl + 3], sv.w, uv.w);
     u_img[e] = uv;
   }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a2 with the pixel hit table ("store P^T as a lookup table" - the strategy the paper uses
+// when the matrix fits; here 8 bytes per non-zero, ~300 MB at 512^2 x 60 x 888, against 180 GB of HBM).
+// hits[pix][0..hcnt[pix]) = (ray index * LQ, p_ij) for every ray with a non-zero weight in the pixel,
+// views ascending, bins ascending; the weights are the values fan_pixel_weight() returns, so P^T stays
+// the bit-exact transpose of P. The table is shared by all slices: its 300 MB are read once per
+// application (coalesced, ~45 us of HBM time) instead of evaluating ~180 candidate rays per pixel.
+// ------------------------------------------------------------------------------------------------
+template <int TABLE>
+__global__ void __launch_bounds__(128) k_hits_build(Dims d, const float4* __restrict__ rays,
+                                                    const float2* __restrict__ views,
+                                                    const unsigned short* __restrict__ win, int* __restrict__ hcnt,
+                                                    float2* __restrict__ hits, int HC, int scale) {
+  const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 4 + threadIdx.y;
+  if (i >= d.nx || j >= d.ny) return;
+  const float fi = (float)(i - d.c0x), fj = (float)(j - d.c0y);
+  const float bi = bias_of(i - d.c0x), bj = bias_of(j - d.c0y);
+  const float px = fmaf((float)i + 0.5f, d.dx, d.xlo), py = fmaf((float)j + 0.5f, d.dy, d.ylo);
+  const int pix = j * d.nx + i;
+  int n = 0;
+  for (int k = 0; k < d.nviews; ++k) {
+    int b_lo, b_hi;
+    if (TABLE) {
+      const unsigned w = __ldg(&win[(size_t)k * d.npix + pix]);
+      b_lo = (int)(w >> 4);
+      b_hi = b_lo + (int)(w & 15u) - 1;
+    } else {
+      fan_window(d, __ldg(&views[k]), px, py, b_lo, b_hi);
+    }
+    for (int b = b_lo; b <= b_hi; ++b) {
+      const float wt = fan_pixel_weight(__ldg(&rays[k * d.nu + b]), fi, fj, bi, bj);
+      if (wt != 0.0f) {
+        if (hits) hits[(size_t)pix * HC + n] = make_float2(__int_as_float((k * d.nu + b) * scale), wt);
+        ++n;
+      }
+    }
+  }
+  if (hits) {
+    for (int e = n; e < HC; ++e) hits[(size_t)pix * HC + e] = make_float2(0.0f, 0.0f);
+  } else {
+    hcnt[pix] = n;
+  }
+}
+
+template <int LQ, int MODE>
+__global__ void __launch_bounds__(256) k_si_back_tab(Dims d, const int* __restrict__ hcnt,
+                                                     const float2* __restrict__ hits, int HC,
+                                                     const float4* __restrict__ sino, float4* __restrict__ out,
+                                                     const float4* __restrict__ s_img, float4* __restrict__ u_img,
+                                                     Scal sc) {
+  constexpr int PB = 256 / LQ;  // pixels per block
+  constexpr int TX = PB >= 64 ? 8 : 4, TY = PB / TX;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int q = lane % LQ, sub = lane / LQ;
+  const int pl = warp * (32 / LQ) + sub;
+  const int i = blockIdx.x * TX + pl % TX, j = blockIdx.y * TY + pl / TX;
+  const int gs = blockIdx.z;
+  const bool live = i < d.nx && j < d.ny;
+  const int pix = j * d.nx + i;
+  float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+  const int cnt = live ? __ldg(&hcnt[pix]) : 0;
+  const int wmax = __reduce_max_sync(FULL, cnt);
+  const float4* sg = sino + (size_t)gs * d.nray * LQ + q;
+  asm volatile("" : "+l"(sg));
+  const float2* hp = hits + (size_t)(live ? pix : 0) * HC + q;
+  for (int e0 = 0; e0 < wmax; e0 += LQ) {
+    float2 h = make_float2(0.0f, 0.0f);
+    if (e0 + q < cnt) h = __ldcs(hp + e0);  // streamed once per application: do not keep in L1
+#pragma unroll
+    for (int t = 0; t < LQ; ++t) {
+      const float w_t = __shfl_sync(FULL, h.y, t, LQ);
+      const int i_t = __float_as_int(__shfl_sync(FULL, h.x, t, LQ));
+      if (w_t != 0.0f) fma4(acc, w_t, __ldg(sg + i_t));
+    }
+  }
+  if (!live) return;
+  const size_t e = ((size_t)gs * d.npix + pix) * LQ + q;
+  out[e] = make_float4(acc[0], acc[1], acc[2], acc[3]);
+  if (MODE == 2) {
+    const float4 sv = __ldcg(s_img + e);
+    float4 uv = __ldcg(u_img + e);
+    const int sl = (gs * LQ + q) * 4;
+    uv.x = fmaf(sc.a[sl + 0], sv.x, uv.x);
+    uv.y = fmaf(sc.a[sl + 1], sv.y, uv.y);
+    uv.z = fmaf(sc.a[sl + 2], sv.z, uv.z);
+    uv.w = fmaf(sc.a[sl + 3], sv.w, uv.w);
+    u_img[e] = uv;
+  }
+}
+
+// built once per handle (ctr_create); on allocation failure the on-the-fly kernel k_si_back is used
+int si_build_hits(ctr_handle* h) {
+  const Dims& d = h->d;
+  h->hits = nullptr;
+  h->hits_cap = 0;
+  if (cudaMalloc((void**)&h->hcnt, sizeof(int) * (size_t)d.npix) != cudaSuccess) { cudaGetLastError(); h->hcnt = nullptr; return CTR_OK; }
+  dim3 grid((d.nx + 31) / 32, (d.ny + 3) / 4), block(32, 4);
+  if (h->win_ok) k_hits_build<1><<<grid, block>>>(d, h->rays, h->views, h->win, h->hcnt, nullptr, 0, d.LQ);
+  else k_hits_build<0><<<grid, block>>>(d, h->rays, h->views, h->win, h->hcnt, nullptr, 0, d.LQ);
+  CTR_LAUNCHED(h);
+  // capacity = largest count, rounded up to a whole number of LQ-entry chunks
+  int* host = (int*)malloc(sizeof(int) * (size_t)d.npix);
+  if (!host) return CTR_ENOMEM;
+  CTR_CUDA(h, cudaMemcpy(host, h->hcnt, sizeof(int) * (size_t)d.npix, cudaMemcpyDeviceToHost));
+  int mx = 0;
+  for (int p = 0; p < d.npix; ++p) mx = host[p] > mx ? host[p] : mx;
+  free(host);
+  const int HC = (mx + 15) / 16 * 16;
+  if (HC == 0 || (size_t)d.nray * d.LQ >= (1u << 31)) return CTR_OK;
+  if (cudaMalloc((void**)&h->hits, sizeof(float2) * (size_t)d.npix * HC) != cudaSuccess) { cudaGetLastError(); h->hits = nullptr; return CTR_OK; }
+  h->hits_cap = HC;
+  if (h->win_ok) k_hits_build<1><<<grid, block>>>(d, h->rays, h->views, h->win, h->hcnt, h->hits, HC, d.LQ);
+  else k_hits_build<0><<<grid, block>>>(d, h->rays, h->views, h->win, h->hcnt, h->hits, HC, d.LQ);
+  CTR_LAUNCHED(h);
+  CTR_CUDA(h, cudaDeviceSynchronize());
+  return CTR_OK;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -331,6 +443,7 @@ static int si_forward_t(ctr_handle* h, const float* img, float* out, int mode, c
   else if (mode == 1) k_si_forward<LQ, 1><<<grid, 256, 0, st>>>(d, h->rays, im, o4, b4, h->sc, h->part, cnt);
   else k_si_forward<LQ, 2><<<grid, 256, 0, st>>>(d, h->rays, im, o4, b4, h->sc, h->part, cnt);
   CTR_LAUNCHED(h);
+  if (mode == 2) return reduce_finish(h, CTR_FIN_ALPHA, 4, (int)grid.x, 0, 0, 0, st);  // a = gamma/||P s||^2
   return CTR_OK;
 }
 
@@ -342,6 +455,12 @@ static int si_back_t(ctr_handle* h, const float* sino, float* out, int mode, con
   const float4 *y4 = (const float4*)sino, *s4 = (const float4*)s;
   float4 *o4 = (float4*)out, *u4 = (float4*)u;
   ProfScope prof(h, CTR_PROF_BACK, st);
+  if (h->hits) {
+    if (mode == 0) k_si_back_tab<LQ, 0><<<grid, 256, 0, st>>>(d, h->hcnt, h->hits, h->hits_cap, y4, o4, s4, u4, h->sc);
+    else k_si_back_tab<LQ, 2><<<grid, 256, 0, st>>>(d, h->hcnt, h->hits, h->hits_cap, y4, o4, s4, u4, h->sc);
+    CTR_LAUNCHED(h);
+    return CTR_OK;
+  }
 #define CTR_SI_BACK(M, T) k_si_back<LQ, M, T><<<grid, 256, 0, st>>>(d, h->rays, h->views, h->win2, y4, o4, s4, u4, h->sc)
   if (h->win_ok) {
     if (mode == 0) CTR_SI_BACK(0, 1); else CTR_SI_BACK(2, 1);
