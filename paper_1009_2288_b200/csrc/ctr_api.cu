@@ -275,9 +275,12 @@ static int vec_reorth(ctr_handle* h, float* g, int nb, int first, cudaStream_t s
   const size_t nl = (size_t)d.npix * d.LQ;
   const int Bp = d.G * d.V;
   // persistent-size grids: few partial sums for the finishing block of the reductions
-  const unsigned want = (unsigned)((nl + 255) / 256), cap = (unsigned)(CTR_REDUCE_BLOCKS / d.GS > 0 ? CTR_REDUCE_BLOCKS / d.GS : 1);
+  const unsigned want = (unsigned)((nl + 255) / 256);
+  unsigned cap = (unsigned)(CTR_REDUCE_BLOCKS / d.GS), dcap = (unsigned)(h->dots_blocks / d.GS);
+  if (cap < 1) cap = 1;
+  if (dcap < 1) dcap = 1;
   dim3 grid(want < cap ? want : cap, d.GS);
-  dim3 dgrid = grid;
+  dim3 dgrid(want < dcap ? want : dcap, d.GS);  // exactly one resident wave of the register-heavy kernel
   ProfScope prof(h, CTR_PROF_VECTOR, st);
   if (nb > CTR_MAX_BASIS) nb = CTR_MAX_BASIS;
   for (int i0 = 0; i0 < nb; i0 += REORTH_NB) {
@@ -557,6 +560,14 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
     h->sc.coef = (float*)p;
   }
   set_quantile(h, h->p.sigma_quantile);
+  {
+    int per_sm = 0;
+    cudaError_t oe = d.V == 1 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_reorth_dots<1>, 256, 0)
+                              : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_reorth_dots<4>, 256, 0);
+    if (oe != cudaSuccess || per_sm < 1) { cudaGetLastError(); per_sm = 2; }
+    h->dots_blocks = per_sm * prop.multiProcessorCount;
+    if (h->dots_blocks > CTR_REDUCE_BLOCKS) h->dots_blocks = CTR_REDUCE_BLOCKS;
+  }
   int rc = d.ndim == 3 ? cone_build_tables(h) : fan_build_tables(h);
   if (rc == CTR_OK && d.ndim == 2 && d.V == 4) rc = si_build_hits(h);
   if (rc != CTR_OK) { ctr_destroy(h); return rc; }

@@ -84,6 +84,7 @@ struct ctr_handle {
   float* usi;           // CGLS iterate in the slice-interleaved layout (batch > 1)
   float* basis;         // [basis_cap][nimg] unit CGLS gradients (S24)
   int basis_cap;
+  int dots_blocks;      // resident blocks of k_reorth_dots on this device (its grid size)
   double* part;
   size_t part_len;
   unsigned* counters;   // [CTR_NCOUNTERS][G]

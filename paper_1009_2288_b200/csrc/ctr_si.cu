@@ -51,6 +51,12 @@ __global__ void __launch_bounds__(256) k_si_forward(Dims d, const float4* __rest
   const int gs = blockIdx.y;
   const bool live = r < d.nray;
   float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+  // per-slab records {pa, wa, pb, wb} of the sub-warp's ray, written by the lane that evaluated the slab
+  // and read back as one broadcast LDS.128 per slab (a shuffle costs an L1 data-pipe wavefront each; four
+  // of them per slab were 40 % of the pipe, profiles/r1c). Rows are padded by one entry so that the
+  // sub-warps of a warp hit different banks.
+  __shared__ float4 slab[8][RW][LQ + 1];
+  float4* myslab = slab[warp][sub];
 
   float x0 = 0.0f, m = 0.0f, L = 0.0f, K = 0.0f;
   bool xdrv = false;
@@ -104,14 +110,14 @@ __global__ void __launch_bounds__(256) k_si_forward(Dims d, const float4* __rest
         wa = w.wb;
       }
     }
+    __syncwarp();
+    myslab[q] = make_float4(__int_as_float(pa), wa, __int_as_float(pb), wb);
+    __syncwarp();
 #pragma unroll
     for (int t = 0; t < LQ; ++t) {
-      const int pa_t = __shfl_sync(FULL, pa, t, LQ);
-      const float wa_t = __shfl_sync(FULL, wa, t, LQ);
-      const float wb_t = __shfl_sync(FULL, wb, t, LQ);
-      const int pb_t = __shfl_sync(FULL, pb, t, LQ);
-      if (wa_t != 0.0f) fma4(acc, wa_t, __ldg(base + pa_t));
-      if (wb_t != 0.0f) fma4(acc, wb_t, __ldg(base + pb_t));
+      const float4 rec = myslab[t];
+      if (rec.y != 0.0f) fma4(acc, rec.y, __ldg(base + __float_as_int(rec.x)));
+      if (rec.w != 0.0f) fma4(acc, rec.w, __ldg(base + __float_as_int(rec.z)));
     }
   }
   if (live) {
@@ -285,14 +291,20 @@ __global__ void __launch_bounds__(256) k_si_back_tab(Dims d, const int* __restri
   const float4* sg = sino + (size_t)gs * d.nray * LQ + q;
   asm volatile("" : "+l"(sg));
   const float2* hp = hits + (size_t)(live ? pix : 0) * HC + q;
+  // chunk of LQ table entries per pixel, handed round through shared memory (one broadcast LDS.64 per
+  // entry instead of two shuffles; rows padded so the sub-warps of a warp use different banks)
+  __shared__ float2 chunk[PB][LQ + 1];
+  float2* mych = chunk[pl];
   for (int e0 = 0; e0 < wmax; e0 += LQ) {
     float2 h = make_float2(0.0f, 0.0f);
     if (e0 + q < cnt) h = __ldcs(hp + e0);  // streamed once per application: do not keep in L1
+    __syncwarp();
+    mych[q] = h;
+    __syncwarp();
 #pragma unroll
     for (int t = 0; t < LQ; ++t) {
-      const float w_t = __shfl_sync(FULL, h.y, t, LQ);
-      const int i_t = __float_as_int(__shfl_sync(FULL, h.x, t, LQ));
-      if (w_t != 0.0f) fma4(acc, w_t, __ldg(sg + i_t));
+      const float2 rec = mych[t];
+      if (rec.y != 0.0f) fma4(acc, rec.y, __ldg(sg + __float_as_int(rec.x)));
     }
   }
   if (!live) return;
