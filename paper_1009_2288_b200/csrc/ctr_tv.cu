@@ -11,7 +11,6 @@
 
 namespace ctr {
 
-#define TV_KC 4 /* Armijo candidates evaluated per pass */
 
 // ---------------------------------------------------------------------------------------------
 // Neighbourhood access. The stencil of A2/A3 around voxel p needs f at p + {-1,0,1}^ndim minus
@@ -312,75 +311,202 @@ __global__ void __launch_bounds__(128) k_tv_gradient(Dims d, const float* __rest
 }
 
 // ---------------------------------------------------------------------------------------------
-// a6.1  Armijo trials k0 .. k0+TV_KC-1 in one pass: E(f - t_k g) with w frozen (O9). Slices that
-// already accepted a step contribute nothing; a group whose slices are all done exits at once.
+// a6.1  Armijo trials, TV_KA candidates per pass.
+// Along the search line every term of A3 is linear in t: the face magnitude of f - t g is
+//   N0^2(t) = a - 2 t b + t^2 c,   a = N0^2(f), c = N0^2(g), b = the mixed form (same stencil),
+// so (a, b, c) are formed once per face from differences of the f and g windows and each candidate
+// costs two FMAs and a square root per face. The fidelity term is a quadratic in t with three
+// candidate-independent sums: lambda/2 (D0 - 2 t D1 + t^2 D2), D0 = |f-v|^2, D1 = <f-v,g>, D2 = |g|^2.
+// E(f - t_k g) with w frozen (O9) is assembled in fp64 by k_tv_trial_finish, which takes the first k with
+// E <= E0 - c t_k |g|^2. Slices that accepted a step in an earlier pass are skipped.
 // ---------------------------------------------------------------------------------------------
+#define TV_KA 8 /* the square roots make the pass MUFU-bound: 8 covers the accepted k of every sweep seen */
+
+// the linear forms of A3 on the face between the centre cell and its +A neighbour,
+// evaluated on windows wf and wg: returns a = sum c_i Lf_i^2, b = sum c_i Lf_i Lg_i, c = sum c_i Lg_i^2
 template <int V, int ND>
-__global__ void __launch_bounds__(128) k_tv_trial(Dims d, const float* __restrict__ f, const float* __restrict__ gin,
+__device__ __forceinline__ void face_forms(const Window<V, ND>& wf, const Window<V, ND>& wg, int A, int s, float& a,
+                                           float& b, float& c) {
+  const int cz = (ND == 3) ? 1 : 0;
+  const int ez = (A == 2), ey = (A == 1), ex = (A == 0);
+  const float df = wf.c[cz + ez][1 + ey][1 + ex][s] - wf.c[cz][1][1][s];
+  const float dg = wg.c[cz + ez][1 + ey][1 + ex][s] - wg.c[cz][1][1][s];
+  a = df * df; b = df * dg; c = dg * dg;
+#pragma unroll
+  for (int T = 0; T < ND; ++T) {
+    if (T == A) continue;
+    const int tz = (T == 2), ty = (T == 1), tx = (T == 0);
+#pragma unroll
+    for (int sg = -1; sg <= 1; sg += 2) {
+      // m(+T) - m0 (sg = +1) or m0 - m(-T) (sg = -1), as half the sum of two differences
+      const float lf = 0.5f * ((wf.c[cz + ez + sg * tz][1 + ey + sg * ty][1 + ex + sg * tx][s] - wf.c[cz + ez][1 + ey][1 + ex][s]) +
+                               (wf.c[cz + sg * tz][1 + sg * ty][1 + sg * tx][s] - wf.c[cz][1][1][s]));
+      const float lg = 0.5f * ((wg.c[cz + ez + sg * tz][1 + ey + sg * ty][1 + ex + sg * tx][s] - wg.c[cz + ez][1 + ey][1 + ex][s]) +
+                               (wg.c[cz + sg * tz][1 + sg * ty][1 + sg * tx][s] - wg.c[cz][1][1][s]));
+      a = fmaf(0.5f * lf, lf, a);
+      b = fmaf(0.5f * lf, lg, b);
+      c = fmaf(0.5f * lg, lg, c);
+    }
+  }
+}
+
+// block (32, 8); partials part[g][blk][NV], NV = TV_KA * V (TV energies, fp32 sums of one block's voxels
+// widened to fp64) + 3 * V (D0, D1, D2 in fp64)
+template <int V, int ND>
+__global__ void __launch_bounds__(256, 2) k_tv_trial(Dims d, const float* __restrict__ f, const float* __restrict__ gin,
                                                   const float* __restrict__ v, const float* __restrict__ w, TvParams tp,
-                                                  int k0, Scal sc, double* part, unsigned* counter) {
-  const Vox p = vox_of_thread(d);
+                                                  int k0, Scal sc, double* part) {
+  constexpr int NE = TV_KA * V, NV = NE + 3 * V;
+  __shared__ float colsum[8][32][33];
+  __shared__ double wsum[8][NV];
+  const int nby = (d.ny + 7) / 8;
+  const int i = blockIdx.x * 32 + threadIdx.x;
+  const int k = blockIdx.y / nby;
+  const int j = (blockIdx.y - k * nby) * 8 + threadIdx.y;
+  const int g = blockIdx.z;
+  const int lane = threadIdx.x, wid = threadIdx.y, tid = wid * 32 + lane;
+  const bool active = i < d.nx && j < d.ny;
+  const unsigned blk = blockIdx.y * gridDim.x + blockIdx.x, nblk = gridDim.x * gridDim.y;
   bool todo[V], any = false;
 #pragma unroll
-  for (int s = 0; s < V; ++s) { todo[s] = sc.kacc[p.g * V + s] < 0; any |= todo[s]; }
+  for (int s = 0; s < V; ++s) { todo[s] = sc.kacc[g * V + s] < 0; any |= todo[s]; }
   if (!any) return;
-  double red[TV_KC * V];
+  float et[NE];
+  double dd[3 * V];
 #pragma unroll
-  for (int s = 0; s < TV_KC * V; ++s) red[s] = 0.0;
-  if (p.active) {
+  for (int q = 0; q < NE; ++q) et[q] = 0.0f;
+#pragma unroll
+  for (int q = 0; q < 3 * V; ++q) dd[q] = 0.0;
+  if (active) {
     Window<V, ND> wf, wg;
-    load_window<V, ND>(d, f, p.g, p.i, p.j, p.k, wf);
-    load_window<V, ND>(d, gin, p.g, p.i, p.j, p.k, wg);
+    load_window<V, ND>(d, f, g, i, j, k, wf);
+    load_window<V, ND>(d, gin, g, i, j, k, wg);
     const int cz = (ND == 3) ? 1 : 0;
-    const size_t e = (size_t)p.g * d.npix + ((size_t)p.k * d.ny + p.j) * d.nx + p.i;
+    const size_t e = (size_t)g * d.npix + ((size_t)k * d.ny + j) * d.nx + i;
     const size_t plane = (size_t)d.G * d.npix * V;
-    const float eps2 = tp.eps * tp.eps;
-    float vv[V], wA[ND][V];
+    const float eps = tp.eps, eps2 = tp.eps * tp.eps;
+    float vv[V];
     Pack<V>::ldcg(v, e, vv);
 #pragma unroll
-    for (int A = 0; A < ND; ++A) Pack<V>::ldcg(w + A * plane, e, wA[A]);
+    for (int s = 0; s < V; ++s) {
+      const float df = wf.c[cz][1][1][s] - vv[s], gg = wg.c[cz][1][1][s];
+      dd[s] = (double)df * (double)df;
+      dd[V + s] = (double)df * (double)gg;
+      dd[2 * V + s] = (double)gg * (double)gg;
+    }
+    // phase 1: the three forms of every face (the windows die here), eps^2 folded into a
+    float fa[ND][V], fb[ND][V], fc[ND][V], wA[ND][V];
 #pragma unroll
-    for (int c = 0; c < TV_KC; ++c) {
-      if (k0 + c >= tp.kmax) break;
-      const float t = tp.t[k0 + c];
-      Window<V, ND> wt;
-#pragma unroll
-      for (int a = 0; a < (ND == 3 ? 3 : 1); ++a)
-#pragma unroll
-        for (int b = 0; b < 3; ++b)
-#pragma unroll
-          for (int x = 0; x < 3; ++x)
-#pragma unroll
-            for (int s = 0; s < V; ++s) wt.c[a][b][x][s] = fmaf(-t, wg.c[a][b][x][s], wf.c[a][b][x][s]);
+    for (int A = 0; A < ND; ++A) {
+      Pack<V>::ldcg(w + A * plane, e, wA[A]);  // border faces store 0
 #pragma unroll
       for (int s = 0; s < V; ++s) {
-        if (!todo[s]) continue;
-        float etv = 0.0f;
+        float a, b, c;
+        face_forms<V, ND>(wf, wg, A, s, a, b, c);
+        fa[A][s] = a + eps2;
+        fb[A][s] = -2.0f * b;
+        fc[A][s] = c;
+        if (!todo[s]) wA[A][s] = 0.0f;
+      }
+    }
+    // phase 2: sum_A w_A sqrt(N0^2(t_q) + eps^2) per candidate; the "- eps sum w" part does not depend on t
 #pragma unroll
-        for (int A = 0; A < ND; ++A)
-          if (wA[A][s] != 0.0f) etv = fmaf(wA[A][s], sqrtf(face_n0sq<V, ND>(wt, A, cz, 1, 1, s) + eps2) - tp.eps, etv);
-        const float df = wt.c[cz][1][1][s] - vv[s];
-        red[c * V + s] = 0.5 * (double)tp.lambda * (double)df * (double)df + (double)etv / (double)ND;
+    for (int q = 0; q < TV_KA; ++q) {
+      const float t = tp.t[min(k0 + q, CTR_MAX_ARMIJO - 1)];
+#pragma unroll
+      for (int A = 0; A < ND; ++A)
+#pragma unroll
+        for (int s = 0; s < V; ++s) {
+          const float rad = fmaxf(fmaf(t, fmaf(t, fc[A][s], fb[A][s]), fa[A][s]), 1e-30f);
+          et[q * V + s] = fmaf(wA[A][s] * rad, rsqrtf(rad), et[q * V + s]);
+        }
+    }
+    {
+      float wsumv[V];
+#pragma unroll
+      for (int s = 0; s < V; ++s) {
+        wsumv[s] = 0.0f;
+#pragma unroll
+        for (int A = 0; A < ND; ++A) wsumv[s] += wA[A][s];
+#pragma unroll
+        for (int q = 0; q < TV_KA; ++q) et[q * V + s] = fmaf(-eps, wsumv[s], et[q * V + s]);
       }
     }
   }
-  grid_reduce<TV_KC * V>(red, part + (size_t)p.g * p.nblk * TV_KC * V, counter + p.g, p.nblk, p.blk, p.tid, 128,
-                         [&](double(&sum)[TV_KC * V]) {
+  // block reduction. TV energies: fp32 column sums over the 32 lanes of a warp through shared memory (32
+  // values per round, transposed so that lane q adds value q of all lanes in lane order), then fp64.
 #pragma unroll
-                           for (int s = 0; s < V; ++s) {
-                             const int sl = p.g * V + s;
-                             if (sc.kacc[sl] >= 0) continue;
-                             const double e0 = sc.e0[sl], g2 = sc.g2[sl];
-                             for (int c = 0; c < TV_KC && k0 + c < tp.kmax; ++c) {
-                               const double t = (double)tp.t[k0 + c];
-                               if (sum[c * V + s] <= e0 - (double)tp.c_armijo * t * g2) {
-                                 sc.kacc[sl] = k0 + c;
-                                 sc.tacc[sl] = tp.t[k0 + c];
-                                 break;
-                               }
-                             }
-                           }
-                         });
+  for (int r0 = 0; r0 < NE; r0 += 32) {
+#pragma unroll
+    for (int q = 0; q < 32; ++q)
+      if (r0 + q < NE) colsum[wid][q][lane] = et[r0 + q];
+    __syncwarp();
+    if (r0 + lane < NE) {
+      float sum = 0.0f;
+#pragma unroll 8
+      for (int l = 0; l < 32; ++l) sum += colsum[wid][lane][l];
+      wsum[wid][r0 + lane] = (double)sum;
+    }
+    __syncwarp();
+  }
+#pragma unroll
+  for (int q = 0; q < 3 * V; ++q) {
+    const double t = warp_sum(dd[q]);
+    if (lane == 0) wsum[wid][NE + q] = t;
+  }
+  __syncthreads();
+  if (tid < NV) {
+    double t = 0.0;
+#pragma unroll
+    for (int ww = 0; ww < 8; ++ww) t += wsum[ww][tid];
+    part[((size_t)g * nblk + blk) * NV + tid] = t;
+  }
+}
+
+// one block per slice group: adds the block partials in a fixed order, assembles E(t_k) in fp64 and takes
+// the Armijo decision (reading S14/S25) for each slice of the group
+template <int V>
+__global__ void __launch_bounds__(1024) k_tv_trial_finish(const double* __restrict__ part, int nblk, TvParams tp, int k0,
+                                                          int ndim, Scal sc) {
+  constexpr int NE = TV_KA * V, NV = NE + 3 * V, ROWS = 1024 / NV;
+  __shared__ double sm[ROWS][NV];
+  __shared__ double tot[NV];
+  const int g = blockIdx.x, t = threadIdx.x;
+  const int n = t % NV, row = t / NV;
+  bool any = false;
+#pragma unroll
+  for (int s = 0; s < V; ++s) any |= sc.kacc[g * V + s] < 0;
+  if (!any) return;  // k_tv_trial wrote nothing for this group
+  if (row < ROWS) {
+    double acc = 0.0;
+    const double* p = part + (size_t)g * nblk * NV + n;
+#pragma unroll 4
+    for (int b = row; b < nblk; b += ROWS) acc += __ldcg(p + (size_t)b * NV);
+    sm[row][n] = acc;
+  }
+  __syncthreads();
+  if (t < NV) {
+    double acc = 0.0;
+    for (int r = 0; r < ROWS; ++r) acc += sm[r][t];
+    tot[t] = acc;
+  }
+  __syncthreads();
+  if (t < V) {
+    const int sl = g * V + t;
+    if (sc.kacc[sl] < 0) {
+      const double e0 = sc.e0[sl], g2 = sc.g2[sl];
+      const double D0 = tot[NE + t], D1 = tot[NE + V + t], D2 = tot[NE + 2 * V + t];
+      for (int q = 0; q < TV_KA && k0 + q < tp.kmax; ++q) {
+        const double tk = (double)tp.t[k0 + q];
+        const double E = 0.5 * (double)tp.lambda * (D0 - 2.0 * tk * D1 + tk * tk * D2) + tot[q * V + t] / (double)ndim;
+        if (E <= e0 - (double)tp.c_armijo * tk * g2) {
+          sc.kacc[sl] = k0 + q;
+          sc.tacc[sl] = tp.t[k0 + q];
+          break;
+        }
+      }
+    }
+  }
 }
 
 // a6.2 + a7  f <- f - t g for slices that accepted a step; optional positivity clamp; sweep record.
@@ -495,8 +621,11 @@ static int tv_sweep_t(ctr_handle* h, float* f, const float* v, const float* w, f
   ProfScope prof(h, CTR_PROF_TV, st);
   k_tv_gradient<V, ND><<<grid, block, 0, st>>>(d, f, v, w, g, tp, h->sc, h->part, h->counters + 2 * d.G);
   CTR_LAUNCHED(h);
-  for (int k0 = 0; k0 < tp.kmax; k0 += TV_KC) {
-    k_tv_trial<V, ND><<<grid, block, 0, st>>>(d, f, g, v, w, tp, k0, h->sc, h->part, h->counters + 3 * d.G);
+  const dim3 tgrid((d.nx + 31) / 32, ((d.ny + 7) / 8) * d.nz, d.G), tblock(32, 8);
+  for (int k0 = 0; k0 < tp.kmax; k0 += TV_KA) {
+    k_tv_trial<V, ND><<<tgrid, tblock, 0, st>>>(d, f, g, v, w, tp, k0, h->sc, h->part);
+    CTR_LAUNCHED(h);
+    k_tv_trial_finish<V><<<d.G, 1024, 0, st>>>(h->part, (int)(tgrid.x * tgrid.y), tp, k0, d.ndim, h->sc);
     CTR_LAUNCHED(h);
   }
   k_tv_apply<V><<<dim3((d.npix + 255) / 256, d.G), 256, 0, st>>>(d, f, g, h->sc, clamp, stat_slot(h));
