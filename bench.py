@@ -135,6 +135,7 @@ def main():
     import torch
     import torch.distributed as dist
     import paper_1009_2288_b200 as ctr
+    from paper_1009_2288_b200 import shard
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -148,7 +149,7 @@ def main():
     K, W = args.steps, max(args.warmup, 0)
 
     # each rank reconstructs its own slices: slice seeds rank*batch .. rank*batch+batch-1
-    case = make_case(cfg, slices=range(rank * batch, rank * batch + batch), raster=False)
+    case = make_case(cfg, slices=shard.slice_range(rank, world, batch), raster=False)
     sino_host = torch.from_numpy(case["sino"]).pin_memory()
     sino = sino_host.cuda(non_blocking=True)
     h = ctr.ctr_create(cfg)
@@ -197,10 +198,7 @@ def main():
     barrier()
     ms_e2e = e0.elapsed_time(e1)
 
-    t = torch.tensor([ms, ms_e2e], device="cuda", dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms, ms_e2e = t.tolist()
+    ms, ms_e2e = shard.max_over_ranks([ms, ms_e2e], device="cuda")
     value = world * batch * K / (ms * 1e-3)
     e2e_value = world * batch * K / (ms_e2e * 1e-3)
 
@@ -232,25 +230,43 @@ def main():
         dist.destroy_process_group()
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the batched kernels at c4, from the committed
+# ncu --set full captures (profiles/r1e_ncu_full_c4.md); None for workloads that were not captured
+NCU_TRAFFIC_C4 = {"forward": 131.7e6, "back": 496.7e6}
+
+
 def roofline(cfg, batch, prof, peaks):
-    """Dominant kernel = the projector pair. Both are bound by plain ALU work:
-    algorithmic work per application = 2 flop (one FMA) per non-zero of P, i.e. per ray-pixel
-    intersection, x slices. nnz(P) per slice is counted from the geometry (2.95e7
-    for the 512^2 / 60 x 888 geometry). Peak = fp32 FMA peak, 148 SMs x 128 lanes x 2 flop x sm_max_mhz."""
+    """Dominant kernel = the slower of the projector pair (a1 / a2). Both are bound by on-chip work, not HBM
+    (DESIGN.md section 6): algorithmic work per application = one FMA (2 flop) per non-zero of P, i.e. per
+    ray-pixel intersection, per slice; nnz(P) per slice is counted from the geometry (2.95e7
+    for the 512^2 / 60 x 888 geometry). Peak = fp32 FMA peak of the chip, 148 SMs x 128 lanes x 2 flop x
+    sm_max_mhz (B200_PROFILING.md unit counts, MEASURED_PEAKS.json clock). The HBM view of the same launch
+    (compulsory image + sinogram bytes against the measured copy bandwidth) is reported beside it, as
+    BASELINE.json's metric asks, with the ncu-measured DRAM traffic."""
     nnz = {"c1": 2.32e5, "c2": 4.60e6, "c3": 2.95e7, "c4": 2.95e7, "c5": 4.37e9}[cfg.name]
     kind = max(("forward", "back"), key=lambda k: prof[k][0])
-    ms, n = prof[kind]
+    names = {"forward": "k_si_forward (P, a1)" if batch > 1 else "k_fan_forward (P, a1)",
+             "back": "k_si_back_tab (P^T gather, a2)" if batch > 1 else "k_fan_back (P^T gather, a2)"}
     sm_mhz = peaks.get("sm_max_mhz", 1965.0)
     peak = 148 * 128 * 2 * sm_mhz * 1e6 / 1e12
-    achieved = 2.0 * nnz * batch / (ms / max(n, 1) * 1e-3) / 1e12
-    bytes_alg = 4.0 * batch * (cfg.nx * cfg.ny * cfg.nz + cfg.nviews * cfg.nu * cfg.nv)
     hbm = peaks.get("hbm_gbs", 6650.0)
-    return {"bound": "alu", "kernel": "k_fan_back (P^T gather)" if kind == "back" else "k_fan_forward (P)",
-            "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
-            "peak_source": "derived: 148 SM x 128 FMA lanes x 2 x sm_max_mhz (MEASURED_PEAKS.json clock)",
-            "avg_launch_ms": ms / max(n, 1),
-            "compulsory_GBps": bytes_alg / (ms / max(n, 1) * 1e-3) / 1e9,
-            "compulsory_GBps_frac_of_measured_hbm": bytes_alg / (ms / max(n, 1) * 1e-3) / 1e9 / hbm}
+    bytes_alg = 4.0 * batch * (cfg.nx * cfg.ny * cfg.nz + cfg.nviews * cfg.nu * cfg.nv)
+
+    def one(k):
+        ms, n = prof[k]
+        sec = ms / max(n, 1) * 1e-3
+        ach = 2.0 * nnz * batch / sec / 1e12
+        return {"kernel": names[k], "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                "avg_launch_ms": sec * 1e3, "launches": n,
+                "traffic": NCU_TRAFFIC_C4.get(k) if (cfg.name == "c4" and batch == 64) else None,
+                "compulsory_GBps": bytes_alg / sec / 1e9,
+                "compulsory_GBps_frac_of_measured_hbm": bytes_alg / sec / 1e9 / hbm}
+
+    out = {"bound": "alu", **one(kind),
+           "peak_source": "derived: 148 SM x 128 fp32 FMA lanes x 2 flop x sm_max_mhz (MEASURED_PEAKS.json clock); "
+                          "hbm_gbs of measured" if "hbm_gbs" in peaks else "fallback 6650 GB/s",
+           "other": one("back" if kind == "forward" else "forward")}
+    return out
 
 
 if __name__ == "__main__":
