@@ -176,3 +176,54 @@ def test_invalid_arguments(ctr, torch_cuda):
     torch.cuda.synchronize()
     assert torch.equal(x, x0)
     h.close()
+
+
+# ------------------------------------------------------------------ the bench configuration itself
+def test_c4_full_batch_operators_and_cgls(ctr, torch_cuda, orc):
+    """configs[3] as bench.py launches it: 64 slices (LQ = 16, hit-table gather). P, P^T and three CGLS
+    iterations on all 64 slices in one call; slices 0, 21 and 63 are compared with the oracle one by one,
+    the adjoint identity is checked on every slice."""
+    torch = torch_cuda
+    cfg = get_config("c4")
+    assert cfg.batch == 64
+    rng = np.random.default_rng(404)
+    x = rng.random((64, cfg.ny, cfg.nx), dtype=np.float32)
+    y = rng.random((64, cfg.nviews, cfg.nu), dtype=np.float32)
+    # slice 21: a structured image (disc + ramp) rather than noise
+    jj, ii = np.mgrid[0:cfg.ny, 0:cfg.nx]
+    x[21] = (0.019 * (((ii - 260) ** 2 + (jj - 240) ** 2) < 200 ** 2) + 1e-5 * ii).astype(np.float32)
+    h = ctr.ctr_create(cfg)
+    xg, yg = torch.from_numpy(x).cuda(), torch.from_numpy(y).cuda()
+    Px = torch.full(h.sino_shape, float("nan"), device="cuda")
+    Pty = torch.full(h.img_shape, float("nan"), device="cuda")
+    h.ctr_forward(xg, Px)
+    h.ctr_back(yg, Pty)
+    u = torch.zeros(h.img_shape, device="cuda")
+    u[21] = 0.01
+    h.ctr_cgls(Px, u, 3)                      # consistent data: b = P x
+    torch.cuda.synchronize()
+    lhs = (Px.double() * yg.double()).sum(dim=(1, 2))
+    rhs = (xg.double() * Pty.double()).sum(dim=(1, 2))
+    nrm = Px.double().flatten(1).norm(dim=1) * yg.double().flatten(1).norm(dim=1)
+    assert float(((lhs - rhs).abs() / nrm).max()) <= 1e-5
+    Px, Pty, u = Px.cpu().numpy(), Pty.cpu().numpy(), u.cpu().numpy()
+    h.close()
+    for sl in (0, 21, 63):
+        want_s = orc.forward(cfg, x[sl].astype(np.float64))
+        assert rel(Px[sl], want_s) <= TOL_OP
+        assert rel(Pty[sl], orc.back(cfg, y[sl].astype(np.float64))) <= TOL_OP
+        x0 = np.full((cfg.ny, cfg.nx), 0.01 if sl == 21 else 0.0)
+        assert rel(u[sl], orc.cgls(cfg, Px[sl].astype(np.float64), x0, 3)) <= 1e-4
+
+
+def test_two_super_groups(ctr, torch_cuda, orc):
+    """batch 70 -> 18 quads -> LQ = 16, two super-groups, the second mostly padding."""
+    cfg = scaled_config("c1", batch=70)
+    rng = np.random.default_rng(405)
+    x = rng.random((70, cfg.ny, cfg.nx), dtype=np.float32)
+    y = rng.random((70, cfg.nviews, cfg.nu), dtype=np.float32)
+    got_s = gpu_forward(ctr, torch_cuda, cfg, x)
+    got_i = gpu_back(ctr, torch_cuda, cfg, y)
+    for sl in (0, 63, 64, 69):
+        assert rel(got_s[sl], orc.forward(cfg, x[sl].astype(np.float64))) <= TOL_OP
+        assert rel(got_i[sl], orc.back(cfg, y[sl].astype(np.float64))) <= TOL_OP

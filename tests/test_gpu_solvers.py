@@ -240,3 +240,14 @@ def test_reconstruct_variants(ctr, torch_cuda, orc):
         assert rel(img[0], want) <= 1e-3
         if cfg.n_gd:
             assert [r["k"] for r in stats] == list(log[:, 1].astype(int))
+
+
+def test_reconstruct_c4_full_batch_one_step(ctr, torch_cuda, orc):
+    """configs[3] in bench.py's launch configuration (64 slices per call), one outer iteration at the full
+    per-iteration schedule (15 CGLS + 5 GD); slices 7 and 50 against the oracle."""
+    cfg = scaled_config("c4", n_outer=1)
+    case = make_case(cfg, raster=False)
+    img, stats, _, _ = run_reconstruct(ctr, torch_cuda, cfg, case["sino"])
+    assert len(stats) == cfg.n_gd * 64
+    for sl in (7, 50):
+        compare_with_oracle(orc, cfg, case["sino"][sl], img[sl], stats[sl::64])
