@@ -124,12 +124,14 @@ __global__ void __launch_bounds__(256) k_img_uupdate(size_t nl, int LQ, float* _
 
 // Re-orthogonalisation of the CGLS gradients (S24). In exact arithmetic P^T r^(m+1) is
 // orthogonal to every earlier P^T r^(i) (Hestenes & Stiefel); in fp32 that is lost
-// after ~6 iterations and the iterate then lags the exact one by a whole step. Classical
-// Gram-Schmidt against the stored unit gradients b_i restores it:
+// after ~6 iterations and the iterate then lags the exact one by a whole step. What is lost is the
+// orthogonality to the FIRST gradients (the dominant singular directions converge first): projecting
+// g against b_0..b_3 only tracks the oracle's full re-orthogonalisation to 1e-6 on every config
+// (S24, table), at a constant cost per iteration. Classical Gram-Schmidt against them:
 //   pass 1 (k_reorth_dots): c_i = <b_i, g> for NB basis vectors per launch (per-thread fp32 partial
 //                           sums over a thread's elements, everything above that in fp64)
 //   pass 2 (k_reorth_sub) : g <- g - sum_i c_i b_i, gamma' = ||g||^2, beta = gamma'/gamma (:432)
-#define REORTH_NB 8   /* basis vectors per k_reorth_dots launch */
+#define REORTH_NB 4   /* basis vectors per k_reorth_dots launch (= CTR_MAX_BASIS: one launch) */
 template <int V>
 __global__ void __launch_bounds__(256) k_reorth_dots(size_t nl, int LQ, size_t nimg, const float* __restrict__ gi,
                                                      const float* __restrict__ basis, int i0, int nb, int Bp, Scal sc,
@@ -232,8 +234,7 @@ int reduce_finish(ctr_handle* h, int mode, int N, int nblk, int i0, int nb, int 
   switch (N) {
     case 1: k_finish<1><<<grid, 256, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
     case 4: k_finish<4><<<grid, 256, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
-    case 8: k_finish<8><<<grid, 256, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
-    default: k_finish<32><<<grid, 256, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
+    default: k_finish<16><<<grid, 256, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
   }
   CTR_LAUNCHED(h);
   return CTR_OK;
