@@ -39,15 +39,19 @@ __device__ __forceinline__ void fma4(float (&acc)[4], float w, const float4 f) {
 // MODE 0: out = P x    MODE 1: out = bs - P x (CGLS r0)
 // MODE 2: out = P x and delta = ||out||^2 per slice -> a = gamma/delta (App. I step 1, :423)
 // ------------------------------------------------------------------------------------------------
+#ifndef SI_FWD_WARPS
+#define SI_FWD_WARPS 8 /* warps per block (16 adjacent rays at LQ = 16); 4, 16 and 32 measured slower */
+#endif
+
 template <int LQ, int MODE>
-__global__ void __launch_bounds__(256) k_si_forward(Dims d, const float4* __restrict__ rays,
+__global__ void __launch_bounds__(SI_FWD_WARPS * 32) k_si_forward(Dims d, const float4* __restrict__ rays,
                                                     const float4* __restrict__ img, float4* __restrict__ out,
                                                     const float4* __restrict__ bs, Scal sc, double* part,
                                                     unsigned* counter) {
   constexpr int RW = 32 / LQ;  // rays per warp
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int q = lane % LQ, sub = lane / LQ;
-  const int r = (blockIdx.x * 8 + warp) * RW + sub;
+  const int r = (blockIdx.x * SI_FWD_WARPS + warp) * RW + sub;
   const int gs = blockIdx.y;
   const bool live = r < d.nray;
   float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
@@ -55,7 +59,7 @@ __global__ void __launch_bounds__(256) k_si_forward(Dims d, const float4* __rest
   // and read back as one broadcast LDS.128 per slab (a shuffle costs an L1 data-pipe wavefront each; four
   // of them per slab were 40 % of the pipe, profiles/r1c). Rows are padded by one entry so that the
   // sub-warps of a warp hit different banks.
-  __shared__ float4 slab[8][RW][LQ + 1];
+  __shared__ float4 slab[SI_FWD_WARPS][RW][LQ + 1];
   float4* myslab = slab[warp][sub];
 
   float x0 = 0.0f, m = 0.0f, L = 0.0f, K = 0.0f;
@@ -132,7 +136,7 @@ __global__ void __launch_bounds__(256) k_si_forward(Dims d, const float4* __rest
     double v[4];
 #pragma unroll
     for (int c = 0; c < 4; ++c) v[c] = live ? (double)acc[c] * (double)acc[c] : 0.0;
-    block_partials_q<4, 8>(v, LQ, part + (size_t)gs * gridDim.x * LQ * 4, blockIdx.x, threadIdx.x);
+    block_partials_q<4, SI_FWD_WARPS>(v, LQ, part + (size_t)gs * gridDim.x * LQ * 4, blockIdx.x, threadIdx.x);
   }
 }
 
@@ -445,15 +449,15 @@ int si_to_planar(ctr_handle* h, const float* src, float* dst, size_t n, cudaStre
 template <int LQ>
 static int si_forward_t(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st) {
   const Dims& d = h->d;
-  const int rays_per_block = 8 * (32 / LQ);
+  const int rays_per_block = SI_FWD_WARPS * (32 / LQ), nt = SI_FWD_WARPS * 32;
   dim3 grid((d.nray + rays_per_block - 1) / rays_per_block, d.GS);
   unsigned* cnt = h->counters + 0 * d.G;
   const float4 *im = (const float4*)img, *b4 = (const float4*)bs;
   float4* o4 = (float4*)out;
   ProfScope prof(h, CTR_PROF_FORWARD, st);
-  if (mode == 0) k_si_forward<LQ, 0><<<grid, 256, 0, st>>>(d, h->rays, im, o4, b4, h->sc, h->part, cnt);
-  else if (mode == 1) k_si_forward<LQ, 1><<<grid, 256, 0, st>>>(d, h->rays, im, o4, b4, h->sc, h->part, cnt);
-  else k_si_forward<LQ, 2><<<grid, 256, 0, st>>>(d, h->rays, im, o4, b4, h->sc, h->part, cnt);
+  if (mode == 0) k_si_forward<LQ, 0><<<grid, nt, 0, st>>>(d, h->rays, im, o4, b4, h->sc, h->part, cnt);
+  else if (mode == 1) k_si_forward<LQ, 1><<<grid, nt, 0, st>>>(d, h->rays, im, o4, b4, h->sc, h->part, cnt);
+  else k_si_forward<LQ, 2><<<grid, nt, 0, st>>>(d, h->rays, im, o4, b4, h->sc, h->part, cnt);
   CTR_LAUNCHED(h);
   if (mode == 2) return reduce_finish(h, CTR_FIN_ALPHA, 4, (int)grid.x, 0, 0, 0, st);  // a = gamma/||P s||^2
   return CTR_OK;
