@@ -246,7 +246,7 @@ def roofline(cfg, batch, prof, peaks):
     nnz = {"c1": 2.32e5, "c2": 4.60e6, "c3": 2.95e7, "c4": 2.95e7, "c5": 4.37e9}[cfg.name]
     kind = max(("forward", "back"), key=lambda k: prof[k][0])
     names = {"forward": "k_si_forward (P, a1)" if batch > 1 else "k_fan_forward (P, a1)",
-             "back": "k_si_back_tab (P^T gather, a2)" if batch > 1 else "k_fan_back (P^T gather, a2)"}
+             "back": "k_si_back_quad (P^T gather, a2)" if batch > 1 else "k_fan_back (P^T gather, a2)"}
     sm_mhz = peaks.get("sm_max_mhz", 1965.0)
     peak = 148 * 128 * 2 * sm_mhz * 1e6 / 1e12
     hbm = peaks.get("hbm_gbs", 6650.0)

@@ -78,8 +78,9 @@ struct ctr_handle {
   // scratch, internal layout [G][n][V]
   size_t nimg, nsino;  // floats per internal image / sinogram (all groups)
   float *ximg, *bsino, *r, *q, *s, *gimg, *v, *w, *n0;
-  float2* hits;         // [npix][hits_cap] (ray index * LQ, p_ij): pixel hit table of the batched gather P^T
-  int* hcnt;            // [npix] entries used per pixel
+  int* qidx;            // [nquad][hits_cap] ray index * LQ (-1: padding): quad hit table of the batched gather P^T
+  float4* qwts;         // [nquad][hits_cap] p_ij of that ray in the four pixels of the 2 x 2 quad
+  int* qcnt;            // [nquad] entries used per quad
   int hits_cap;
   float* usi;           // CGLS iterate in the slice-interleaved layout (batch > 1)
   float* basis;         // [basis_cap][nimg] unit CGLS gradients (S24)

@@ -231,124 +231,185 @@ __global__ void __launch_bounds__(256) k_si_back(Dims d, const float4* __restric
 }
 
 // ------------------------------------------------------------------------------------------------
-// a2 with the pixel hit table ("store P^T as a lookup table" - the strategy the paper uses
-// when the matrix fits; here 8 bytes per non-zero, ~300 MB at 512^2 x 60 x 888, against 180 GB of HBM).
-// hits[pix][0..hcnt[pix]) = (ray index * LQ, p_ij) for every ray with a non-zero weight in the pixel,
-// views ascending, bins ascending; the weights are the values fan_pixel_weight() returns, so P^T stays
-// the bit-exact transpose of P. The table is shared by all slices: its 300 MB are read once per
-// application (coalesced, ~45 us of HBM time) instead of evaluating ~180 candidate rays per pixel.
+// a2 with the quad hit table ("store P^T as a lookup table" - the strategy the paper uses
+// when the matrix fits; here ~380 MB at 512^2 x 60 x 888, shared by all slices, against 180 GB of HBM).
+// A sub-warp owns a 2 x 2 quad of pixels: neighbouring pixels are crossed by largely the same rays, so one
+// 256-byte sinogram read serves up to four pixels (x 4 slices per lane = 16 FMAs): ~250 reads per quad
+// instead of 4 x 113, which is what the L1 data pipe - the bound of this kernel - sees.
+// qidx[quad][e] = ray index * LQ (or -1: padding), qwts[quad][e] = p_ij of that ray in pixels
+// (i0,j0), (i0+1,j0), (i0,j0+1), (i0+1,j0+1); views ascending, bins ascending. The weights are the values
+// fan_pixel_weight() returns (0 where the ray misses the pixel), so P^T stays the bit-exact transpose of P
+// and every pixel adds its non-zero terms in the same order as the single-slice kernel.
 // ------------------------------------------------------------------------------------------------
 template <int TABLE>
-__global__ void __launch_bounds__(128) k_hits_build(Dims d, const float4* __restrict__ rays,
-                                                    const float2* __restrict__ views,
-                                                    const unsigned short* __restrict__ win, int* __restrict__ hcnt,
-                                                    float2* __restrict__ hits, int HC, int scale) {
-  const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 4 + threadIdx.y;
-  if (i >= d.nx || j >= d.ny) return;
-  const float fi = (float)(i - d.c0x), fj = (float)(j - d.c0y);
-  const float bi = bias_of(i - d.c0x), bj = bias_of(j - d.c0y);
-  const float px = fmaf((float)i + 0.5f, d.dx, d.xlo), py = fmaf((float)j + 0.5f, d.dy, d.ylo);
-  const int pix = j * d.nx + i;
+__global__ void __launch_bounds__(128) k_qhits_build(Dims d, const float4* __restrict__ rays,
+                                                     const float2* __restrict__ views,
+                                                     const unsigned short* __restrict__ win, int* __restrict__ qcnt,
+                                                     int* __restrict__ qidx, float4* __restrict__ qwts, int HC,
+                                                     int scale) {
+  const int nqx = (d.nx + 1) / 2, nqy = (d.ny + 1) / 2;
+  const int qx = blockIdx.x * 32 + threadIdx.x, qy = blockIdx.y * 4 + threadIdx.y;
+  if (qx >= nqx || qy >= nqy) return;
+  const int quad = qy * nqx + qx;
+  float fi[4], fj[4], bi[4], bj[4], px[4], py[4];
+  int pix[4];
+  bool ok[4];
+#pragma unroll
+  for (int p = 0; p < 4; ++p) {
+    const int i = 2 * qx + (p & 1), j = 2 * qy + (p >> 1);
+    ok[p] = i < d.nx && j < d.ny;
+    fi[p] = (float)(i - d.c0x); fj[p] = (float)(j - d.c0y);
+    bi[p] = bias_of(i - d.c0x); bj[p] = bias_of(j - d.c0y);
+    px[p] = fmaf((float)i + 0.5f, d.dx, d.xlo); py[p] = fmaf((float)j + 0.5f, d.dy, d.ylo);
+    pix[p] = j * d.nx + i;
+  }
   int n = 0;
   for (int k = 0; k < d.nviews; ++k) {
-    int b_lo, b_hi;
-    if (TABLE) {
-      const unsigned w = __ldg(&win[(size_t)k * d.npix + pix]);
-      b_lo = (int)(w >> 4);
-      b_hi = b_lo + (int)(w & 15u) - 1;
-    } else {
-      fan_window(d, __ldg(&views[k]), px, py, b_lo, b_hi);
+    int lo[4], hi[4], b_lo = INT_MAX, b_hi = -1;
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+      lo[p] = 0; hi[p] = -1;
+      if (!ok[p]) continue;
+      if (TABLE) {
+        const unsigned w = __ldg(&win[(size_t)k * d.npix + pix[p]]);
+        lo[p] = (int)(w >> 4);
+        hi[p] = lo[p] + (int)(w & 15u) - 1;
+      } else {
+        fan_window(d, __ldg(&views[k]), px[p], py[p], lo[p], hi[p]);
+      }
+      if (hi[p] >= lo[p]) { b_lo = min(b_lo, lo[p]); b_hi = max(b_hi, hi[p]); }
     }
     for (int b = b_lo; b <= b_hi; ++b) {
-      const float wt = fan_pixel_weight(__ldg(&rays[k * d.nu + b]), fi, fj, bi, bj);
-      if (wt != 0.0f) {
-        if (hits) hits[(size_t)pix * HC + n] = make_float2(__int_as_float((k * d.nu + b) * scale), wt);
+      const float4 R = __ldg(&rays[k * d.nu + b]);
+      float w[4];
+      bool any = false;
+#pragma unroll
+      for (int p = 0; p < 4; ++p) {
+        w[p] = (b >= lo[p] && b <= hi[p]) ? fan_pixel_weight(R, fi[p], fj[p], bi[p], bj[p]) : 0.0f;
+        any |= w[p] != 0.0f;
+      }
+      if (any) {
+        if (qidx) {
+          qidx[(size_t)quad * HC + n] = (k * d.nu + b) * scale;
+          qwts[(size_t)quad * HC + n] = make_float4(w[0], w[1], w[2], w[3]);
+        }
         ++n;
       }
     }
   }
-  if (hits) {
-    for (int e = n; e < HC; ++e) hits[(size_t)pix * HC + e] = make_float2(0.0f, 0.0f);
+  if (qidx) {
+    for (int e = n; e < HC; ++e) {
+      qidx[(size_t)quad * HC + e] = -1;
+      qwts[(size_t)quad * HC + e] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    }
   } else {
-    hcnt[pix] = n;
+    qcnt[quad] = n;
   }
 }
 
 template <int LQ, int MODE>
-__global__ void __launch_bounds__(256) k_si_back_tab(Dims d, const int* __restrict__ hcnt,
-                                                     const float2* __restrict__ hits, int HC,
-                                                     const float4* __restrict__ sino, float4* __restrict__ out,
-                                                     const float4* __restrict__ s_img, float4* __restrict__ u_img,
-                                                     Scal sc) {
-  constexpr int PB = 256 / LQ;  // pixels per block
+__global__ void __launch_bounds__(256) k_si_back_quad(Dims d, const int* __restrict__ qcnt,
+                                                      const int* __restrict__ qidx, const float4* __restrict__ qwts,
+                                                      int HC, const float4* __restrict__ sino, float4* __restrict__ out,
+                                                      const float4* __restrict__ s_img, float4* __restrict__ u_img,
+                                                      Scal sc) {
+  constexpr int PB = 256 / LQ;  // quads per block
   constexpr int TX = PB >= 64 ? 8 : 4, TY = PB / TX;
+  // chunk of LQ table entries per quad, handed round through shared memory (broadcast reads; rows padded
+  // so that the sub-warps of a warp use different banks)
+  __shared__ float4 chw[PB][LQ + 1];
+  __shared__ int chi[PB][LQ + 1];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int q = lane % LQ, sub = lane / LQ;
   const int pl = warp * (32 / LQ) + sub;
-  const int i = blockIdx.x * TX + pl % TX, j = blockIdx.y * TY + pl / TX;
+  const int nqx = (d.nx + 1) / 2, nqy = (d.ny + 1) / 2;
+  const int qx = blockIdx.x * TX + pl % TX, qy = blockIdx.y * TY + pl / TX;
   const int gs = blockIdx.z;
-  const bool live = i < d.nx && j < d.ny;
-  const int pix = j * d.nx + i;
-  float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
-  const int cnt = live ? __ldg(&hcnt[pix]) : 0;
+  const bool live = qx < nqx && qy < nqy;
+  const int quad = live ? qy * nqx + qx : 0;
+  float acc[4][4];
+#pragma unroll
+  for (int p = 0; p < 4; ++p)
+#pragma unroll
+    for (int c = 0; c < 4; ++c) acc[p][c] = 0.0f;
+  const int cnt = live ? __ldg(&qcnt[quad]) : 0;
   const int wmax = __reduce_max_sync(FULL, cnt);
   const float4* sg = sino + (size_t)gs * d.nray * LQ + q;
   asm volatile("" : "+l"(sg));
-  const float2* hp = hits + (size_t)(live ? pix : 0) * HC + q;
-  // chunk of LQ table entries per pixel, handed round through shared memory (one broadcast LDS.64 per
-  // entry instead of two shuffles; rows padded so the sub-warps of a warp use different banks)
-  __shared__ float2 chunk[PB][LQ + 1];
-  float2* mych = chunk[pl];
+  const int* ip = qidx + (size_t)quad * HC + q;
+  const float4* wp = qwts + (size_t)quad * HC + q;
   for (int e0 = 0; e0 < wmax; e0 += LQ) {
-    float2 h = make_float2(0.0f, 0.0f);
-    if (e0 + q < cnt) h = __ldcs(hp + e0);  // streamed once per application: do not keep in L1
+    int id = -1;
+    float4 w4 = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    if (e0 + q < cnt) { id = __ldcs(ip + e0); w4 = __ldcs(wp + e0); }  // streamed once per application
     __syncwarp();
-    mych[q] = h;
+    chi[pl][q] = id;
+    chw[pl][q] = w4;
     __syncwarp();
 #pragma unroll
     for (int t = 0; t < LQ; ++t) {
-      const float2 rec = mych[t];
-      if (rec.y != 0.0f) fma4(acc, rec.y, __ldg(sg + __float_as_int(rec.x)));
+      const int it = chi[pl][t];
+      if (it >= 0) {
+        const float4 w = chw[pl][t];
+        const float4 y = __ldg(sg + it);
+        fma4(acc[0], w.x, y);
+        fma4(acc[1], w.y, y);
+        fma4(acc[2], w.z, y);
+        fma4(acc[3], w.w, y);
+      }
     }
   }
   if (!live) return;
-  const size_t e = ((size_t)gs * d.npix + pix) * LQ + q;
-  out[e] = make_float4(acc[0], acc[1], acc[2], acc[3]);
-  if (MODE == 2) {
-    const float4 sv = __ldcg(s_img + e);
-    float4 uv = __ldcg(u_img + e);
-    const int sl = (gs * LQ + q) * 4;
-    uv.x = fmaf(sc.a[sl + 0], sv.x, uv.x);
-    uv.y = fmaf(sc.a[sl + 1], sv.y, uv.y);
-    uv.z = fmaf(sc.a[sl + 2], sv.z, uv.z);
-    uv.w = fmaf(sc.a[sl + 3], sv.w, uv.w);
-    u_img[e] = uv;
+#pragma unroll
+  for (int p = 0; p < 4; ++p) {
+    const int i = 2 * qx + (p & 1), j = 2 * qy + (p >> 1);
+    if (i >= d.nx || j >= d.ny) continue;
+    const size_t e = ((size_t)gs * d.npix + (size_t)j * d.nx + i) * LQ + q;
+    out[e] = make_float4(acc[p][0], acc[p][1], acc[p][2], acc[p][3]);
+    if (MODE == 2) {
+      const float4 sv = __ldcg(s_img + e);
+      float4 uv = __ldcg(u_img + e);
+      const int sl = (gs * LQ + q) * 4;
+      uv.x = fmaf(sc.a[sl + 0], sv.x, uv.x);
+      uv.y = fmaf(sc.a[sl + 1], sv.y, uv.y);
+      uv.z = fmaf(sc.a[sl + 2], sv.z, uv.z);
+      uv.w = fmaf(sc.a[sl + 3], sv.w, uv.w);
+      u_img[e] = uv;
+    }
   }
 }
 
 // built once per handle (ctr_create); on allocation failure the on-the-fly kernel k_si_back is used
 int si_build_hits(ctr_handle* h) {
   const Dims& d = h->d;
-  h->hits = nullptr;
+  h->qidx = nullptr;
+  h->qwts = nullptr;
   h->hits_cap = 0;
-  if (cudaMalloc((void**)&h->hcnt, sizeof(int) * (size_t)d.npix) != cudaSuccess) { cudaGetLastError(); h->hcnt = nullptr; return CTR_OK; }
-  dim3 grid((d.nx + 31) / 32, (d.ny + 3) / 4), block(32, 4);
-  if (h->win_ok) k_hits_build<1><<<grid, block>>>(d, h->rays, h->views, h->win, h->hcnt, nullptr, 0, d.LQ);
-  else k_hits_build<0><<<grid, block>>>(d, h->rays, h->views, h->win, h->hcnt, nullptr, 0, d.LQ);
+  const int nqx = (d.nx + 1) / 2, nqy = (d.ny + 1) / 2, nquad = nqx * nqy;
+  if (cudaMalloc((void**)&h->qcnt, sizeof(int) * (size_t)nquad) != cudaSuccess) { cudaGetLastError(); h->qcnt = nullptr; return CTR_OK; }
+  dim3 grid((nqx + 31) / 32, (nqy + 3) / 4), block(32, 4);
+  if (h->win_ok) k_qhits_build<1><<<grid, block>>>(d, h->rays, h->views, h->win, h->qcnt, nullptr, nullptr, 0, d.LQ);
+  else k_qhits_build<0><<<grid, block>>>(d, h->rays, h->views, h->win, h->qcnt, nullptr, nullptr, 0, d.LQ);
   CTR_LAUNCHED(h);
-  // capacity = largest count, rounded up to a whole number of LQ-entry chunks
-  int* host = (int*)malloc(sizeof(int) * (size_t)d.npix);
+  // capacity = largest count, rounded up to a whole number of 16-entry chunks
+  int* host = (int*)malloc(sizeof(int) * (size_t)nquad);
   if (!host) return CTR_ENOMEM;
-  CTR_CUDA(h, cudaMemcpy(host, h->hcnt, sizeof(int) * (size_t)d.npix, cudaMemcpyDeviceToHost));
+  CTR_CUDA(h, cudaMemcpy(host, h->qcnt, sizeof(int) * (size_t)nquad, cudaMemcpyDeviceToHost));
   int mx = 0;
-  for (int p = 0; p < d.npix; ++p) mx = host[p] > mx ? host[p] : mx;
+  for (int p = 0; p < nquad; ++p) mx = host[p] > mx ? host[p] : mx;
   free(host);
   const int HC = (mx + 15) / 16 * 16;
   if (HC == 0 || (size_t)d.nray * d.LQ >= (1u << 31)) return CTR_OK;
-  if (cudaMalloc((void**)&h->hits, sizeof(float2) * (size_t)d.npix * HC) != cudaSuccess) { cudaGetLastError(); h->hits = nullptr; return CTR_OK; }
+  if (cudaMalloc((void**)&h->qidx, sizeof(int) * (size_t)nquad * HC) != cudaSuccess) { cudaGetLastError(); h->qidx = nullptr; return CTR_OK; }
+  if (cudaMalloc((void**)&h->qwts, sizeof(float4) * (size_t)nquad * HC) != cudaSuccess) {
+    cudaGetLastError();
+    cudaFree(h->qidx);
+    h->qidx = nullptr; h->qwts = nullptr;
+    return CTR_OK;
+  }
   h->hits_cap = HC;
-  if (h->win_ok) k_hits_build<1><<<grid, block>>>(d, h->rays, h->views, h->win, h->hcnt, h->hits, HC, d.LQ);
-  else k_hits_build<0><<<grid, block>>>(d, h->rays, h->views, h->win, h->hcnt, h->hits, HC, d.LQ);
+  if (h->win_ok) k_qhits_build<1><<<grid, block>>>(d, h->rays, h->views, h->win, h->qcnt, h->qidx, h->qwts, HC, d.LQ);
+  else k_qhits_build<0><<<grid, block>>>(d, h->rays, h->views, h->win, h->qcnt, h->qidx, h->qwts, HC, d.LQ);
   CTR_LAUNCHED(h);
   CTR_CUDA(h, cudaDeviceSynchronize());
   return CTR_OK;
@@ -471,9 +532,10 @@ static int si_back_t(ctr_handle* h, const float* sino, float* out, int mode, con
   const float4 *y4 = (const float4*)sino, *s4 = (const float4*)s;
   float4 *o4 = (float4*)out, *u4 = (float4*)u;
   ProfScope prof(h, CTR_PROF_BACK, st);
-  if (h->hits) {
-    if (mode == 0) k_si_back_tab<LQ, 0><<<grid, 256, 0, st>>>(d, h->hcnt, h->hits, h->hits_cap, y4, o4, s4, u4, h->sc);
-    else k_si_back_tab<LQ, 2><<<grid, 256, 0, st>>>(d, h->hcnt, h->hits, h->hits_cap, y4, o4, s4, u4, h->sc);
+  if (h->qwts) {
+    dim3 qgrid(((d.nx + 1) / 2 + TX - 1) / TX, ((d.ny + 1) / 2 + TY - 1) / TY, d.GS);
+    if (mode == 0) k_si_back_quad<LQ, 0><<<qgrid, 256, 0, st>>>(d, h->qcnt, h->qidx, h->qwts, h->hits_cap, y4, o4, s4, u4, h->sc);
+    else k_si_back_quad<LQ, 2><<<qgrid, 256, 0, st>>>(d, h->qcnt, h->qidx, h->qwts, h->hits_cap, y4, o4, s4, u4, h->sc);
     CTR_LAUNCHED(h);
     return CTR_OK;
   }
