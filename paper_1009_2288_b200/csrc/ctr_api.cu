@@ -665,12 +665,12 @@ int ctr_eptv_step(ctr_handle* h, float* d_x, const float* d_v, const float* d_w,
   if (!(lambda >= 0.0f)) return set_err(h, CTR_EINVAL, "ctr_eptv_step: lambda < 0");
   cudaStream_t st = (cudaStream_t)stream;
   h->last_stream = st;
-  if (h->d.V == 1) return tv_sweep(h, d_x, d_v, d_w, lambda, 0, st);
+  if (h->d.V == 1) return tv_sweep(h, d_x, d_v, d_w, lambda, 0, 0, st);
   int rc;
   if ((rc = pack(h, d_x, h->ximg, h->d.npix, 1, st))) return rc;
   if ((rc = pack(h, d_v, h->v, h->d.npix, 1, st))) return rc;
   if ((rc = pack(h, d_w, h->w, h->d.npix, h->d.ndim, st))) return rc;
-  if ((rc = tv_sweep(h, h->ximg, h->v, h->w, lambda, 0, st))) return rc;
+  if ((rc = tv_sweep(h, h->ximg, h->v, h->w, lambda, 0, 0, st))) return rc;
   return unpack(h, h->ximg, d_x, h->d.npix, 1, st);
 }
 
@@ -709,7 +709,7 @@ int ctr_reconstruct_w(ctr_handle* h, const float* d_sino, float* d_img, float* d
       CTR_CUDA(h, cudaMemcpyAsync(h->v, f, h->nimg * sizeof(float), cudaMemcpyDeviceToDevice, st));  // v = CGLS result
     for (int s = 0; s < P.n_gd; ++s) {                                                            // Step 2 (:172)
       if ((rc = tv_update_weights(h, f, h->w, st))) return rc;
-      if ((rc = tv_sweep(h, f, h->v, h->w, P.lambda, (s == P.n_gd - 1) && P.positivity, st))) return rc;
+      if ((rc = tv_sweep(h, f, h->v, h->w, P.lambda, (s == P.n_gd - 1) && P.positivity, 1, st))) return rc;
     }
     if (P.n_gd == 0 && P.positivity && (rc = tv_clamp(h, f, st))) return rc;                     // Step 3 (:173)
   }

@@ -157,12 +157,18 @@ __global__ void __launch_bounds__(128) k_tv_hist(Dims d, const float* __restrict
     float val[V];
     const bool inside = p.active && pos[A] < lim[A];
     if (inside) Pack<V>::ldcg(n0 + (size_t)A * d.G * d.npix * V, e, val);
+    unsigned bits[V];
+    bool valid[V], anyv = false;
 #pragma unroll
     for (int s = 0; s < V; ++s) {
-      const unsigned bits = inside ? __float_as_uint(val[s]) : 0u;
-      const bool valid = inside && (bits >> prefix_shift) == pre[s];
-      hist_add(hs[s], bits, shift, mask, valid);
+      bits[s] = inside ? __float_as_uint(val[s]) : 0u;
+      valid[s] = inside && (bits[s] >> prefix_shift) == pre[s];
+      anyv |= valid[s];
     }
+    // only a small fraction of the values carries the prefix found so far: most warps have nothing to add
+    if (!__any_sync(0xffffffffu, anyv)) continue;
+#pragma unroll
+    for (int s = 0; s < V; ++s) hist_add(hs[s], bits[s], shift, mask, valid[s]);
   }
   __syncthreads();
   for (int t = p.tid; t < V * 1024; t += 128) {
@@ -242,10 +248,14 @@ __global__ void __launch_bounds__(128) k_tv_weights(Dims d, const float* __restr
 // a5  gradient g = lambda (f - v) - sum_A (flux_A(p) - flux_A(p - e_A)),
 //     flux_A = w_A d_A / sqrt(N0^2 + eps^2) (A2), plus G = ||g||^2 and E0 (O9).
 // ---------------------------------------------------------------------------------------------
-template <int V, int ND>
+// N0ST = 1: the N0^2 planes written by k_tv_faces for THIS f are read back (ctr_reconstruct: the weight
+// update of the same sweep has just produced them); N0ST = 0: recomputed from the window (ctr_eptv_step,
+// where the caller's x need not be the image of the last weight update).
+template <int V, int ND, int N0ST>
 __global__ void __launch_bounds__(128) k_tv_gradient(Dims d, const float* __restrict__ f, const float* __restrict__ v,
-                                                     const float* __restrict__ w, float* __restrict__ gout,
-                                                     TvParams tp, Scal sc, double* part, unsigned* counter) {
+                                                     const float* __restrict__ w, const float* __restrict__ n0st,
+                                                     float* __restrict__ gout, TvParams tp, Scal sc, double* part,
+                                                     unsigned* counter) {
   const Vox p = vox_of_thread(d);
   double red[2 * V];
 #pragma unroll
@@ -276,11 +286,20 @@ __global__ void __launch_bounds__(128) k_tv_gradient(Dims d, const float* __rest
         for (int s = 0; s < V; ++s) wm[s] = 0.0f;
       }
       const int ez = (A == 2), ey = (A == 1), ex = (A == 0);
+      float sp[V], sm_[V];
+      if (N0ST) {
+        Pack<V>::ldcg(n0st + A * plane, e, sp);
+        if (pos[A] > 0) Pack<V>::ldcg(n0st + A * plane, e - stride[A], sm_);
+        else {
+#pragma unroll
+          for (int s = 0; s < V; ++s) sm_[s] = 0.0f;
+        }
+      }
 #pragma unroll
       for (int s = 0; s < V; ++s) {
         // face towards +A (owned by this voxel) and face towards -A (owned by the neighbour)
-        const float n0p = face_n0sq<V, ND>(win, A, cz, 1, 1, s) + eps2;
-        const float n0m = face_n0sq<V, ND>(win, A, cz - ez, 1 - ey, 1 - ex, s) + eps2;
+        const float n0p = (N0ST ? sp[s] : face_n0sq<V, ND>(win, A, cz, 1, 1, s)) + eps2;
+        const float n0m = (N0ST ? sm_[s] : face_n0sq<V, ND>(win, A, cz - ez, 1 - ey, 1 - ex, s)) + eps2;
         const float dp = win.c[cz + ez][1 + ey][1 + ex][s] - win.c[cz][1][1][s];
         const float dm = win.c[cz][1][1][s] - win.c[cz - ez][1 - ey][1 - ex][s];
         const float fp = (wp[s] != 0.0f && n0p > 0.0f) ? wp[s] * dp * rsqrtf(n0p) : 0.0f;
@@ -613,13 +632,14 @@ static TvParams make_tv_params(const ctr_handle* h, float lambda) {
 
 template <int V, int ND>
 static int tv_sweep_t(ctr_handle* h, float* f, const float* v, const float* w, float lambda, int clamp,
-                      cudaStream_t st) {
+                      int n0_valid, cudaStream_t st) {
   const Dims& d = h->d;
   const dim3 grid = vox_grid(d), block(32, 4);
   const TvParams tp = make_tv_params(h, lambda);
   float* g = h->gimg;
   ProfScope prof(h, CTR_PROF_TV, st);
-  k_tv_gradient<V, ND><<<grid, block, 0, st>>>(d, f, v, w, g, tp, h->sc, h->part, h->counters + 2 * d.G);
+  if (n0_valid) k_tv_gradient<V, ND, 1><<<grid, block, 0, st>>>(d, f, v, w, h->n0, g, tp, h->sc, h->part, h->counters + 2 * d.G);
+  else k_tv_gradient<V, ND, 0><<<grid, block, 0, st>>>(d, f, v, w, h->n0, g, tp, h->sc, h->part, h->counters + 2 * d.G);
   CTR_LAUNCHED(h);
   const dim3 tgrid((d.nx + 31) / 32, ((d.ny + 7) / 8) * d.nz, d.G), tblock(32, 8);
   for (int k0 = 0; k0 < tp.kmax; k0 += TV_KA) {
@@ -634,9 +654,11 @@ static int tv_sweep_t(ctr_handle* h, float* f, const float* v, const float* w, f
   return CTR_OK;
 }
 
-int tv_sweep(ctr_handle* h, float* f, const float* v, const float* w, float lambda, int clamp, cudaStream_t st) {
-  if (h->d.ndim == 3) return tv_sweep_t<1, 3>(h, f, v, w, lambda, clamp, st);
-  return h->d.V == 1 ? tv_sweep_t<1, 2>(h, f, v, w, lambda, clamp, st) : tv_sweep_t<4, 2>(h, f, v, w, lambda, clamp, st);
+int tv_sweep(ctr_handle* h, float* f, const float* v, const float* w, float lambda, int clamp, int n0_valid,
+             cudaStream_t st) {
+  if (h->d.ndim == 3) return tv_sweep_t<1, 3>(h, f, v, w, lambda, clamp, n0_valid, st);
+  return h->d.V == 1 ? tv_sweep_t<1, 2>(h, f, v, w, lambda, clamp, n0_valid, st)
+                     : tv_sweep_t<4, 2>(h, f, v, w, lambda, clamp, n0_valid, st);
 }
 
 int tv_clamp(ctr_handle* h, float* f, cudaStream_t st) {
