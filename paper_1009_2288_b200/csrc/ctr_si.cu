@@ -39,12 +39,15 @@ __device__ __forceinline__ void fma4(float (&acc)[4], float w, const float4 f) {
 // MODE 0: out = P x    MODE 1: out = bs - P x (CGLS r0)
 // MODE 2: out = P x and delta = ||out||^2 per slice -> a = gamma/delta (App. I step 1, :423)
 // ------------------------------------------------------------------------------------------------
+#ifndef SI_FWD_MINB
+#define SI_FWD_MINB 4 /* 64 registers: more loads in flight than the 40 ptxas picks unprompted (6.76 vs 7.07 ms per step) */
+#endif
 #ifndef SI_FWD_WARPS
 #define SI_FWD_WARPS 8 /* warps per block (16 adjacent rays at LQ = 16); 4, 16 and 32 measured slower */
 #endif
 
 template <int LQ, int MODE>
-__global__ void __launch_bounds__(SI_FWD_WARPS * 32) k_si_forward(Dims d, const float4* __restrict__ rays,
+__global__ void __launch_bounds__(SI_FWD_WARPS * 32, SI_FWD_MINB) k_si_forward(Dims d, const float4* __restrict__ rays,
                                                     const float4* __restrict__ img, float4* __restrict__ out,
                                                     const float4* __restrict__ bs, Scal sc, double* part,
                                                     unsigned* counter) {
@@ -307,8 +310,11 @@ __global__ void __launch_bounds__(128) k_qhits_build(Dims d, const float4* __res
   }
 }
 
+#ifndef SI_BACK_MINB
+#define SI_BACK_MINB 4
+#endif
 template <int LQ, int MODE>
-__global__ void __launch_bounds__(256) k_si_back_quad(Dims d, const int* __restrict__ qcnt,
+__global__ void __launch_bounds__(256, SI_BACK_MINB) k_si_back_quad(Dims d, const int* __restrict__ qcnt,
                                                       const int* __restrict__ qidx, const float4* __restrict__ qwts,
                                                       int HC, const float4* __restrict__ sino, float4* __restrict__ out,
                                                       const float4* __restrict__ s_img, float4* __restrict__ u_img,
