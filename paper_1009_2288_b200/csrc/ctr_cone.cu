@@ -171,23 +171,18 @@ __global__ void __launch_bounds__(128) k_cone_forward(Dims d, const float4* __re
 // voxel's z-extent at the nearest / farthest in-plane distance. The in-plane part of the weight is
 // evaluated once per column and reused for every row. No atomics, fixed accumulation order.
 // ------------------------------------------------------------------------------------------------
-template <int MODE>
-__global__ void __launch_bounds__(128) k_cone_back(Dims d, const float4* __restrict__ TA, const float4* __restrict__ TB,
-                                                   const float2* __restrict__ views, const unsigned short* __restrict__ win,
-                                                   const float* __restrict__ sino, float* __restrict__ out,
-                                                   const float* __restrict__ s_img, float* __restrict__ u_img, Scal sc) {
-  const int i = blockIdx.x * 32 + threadIdx.x;
-  const int nby = (d.ny + 3) / 4;
-  const int k = blockIdx.y / nby;
-  const int j = (blockIdx.y - k * nby) * 4 + threadIdx.y;
-  if (i >= d.nx || j >= d.ny) return;
+// all rays with a non-zero weight in voxel (i, j, k), in a fixed order (views, columns, rows ascending):
+// visit(ray index, p_ij)
+template <class Visit>
+__device__ __forceinline__ void cone_voxel_hits(const Dims& d, const float4* __restrict__ TA, const float4* __restrict__ TB,
+                                                const float2* __restrict__ views, const unsigned short* __restrict__ win,
+                                                int i, int j, int k, Visit visit) {
   const float fi = (float)(i - d.c0x), fj = (float)(j - d.c0y);
   const float bi = bias_of(i - d.c0x), bj = bias_of(j - d.c0y), bk = bias_of(k - d.c0z);
   const float px = fmaf((float)i + 0.5f, d.dx, d.xlo), py = fmaf((float)j + 0.5f, d.dy, d.ylo);
   const float z_lo = fmaf((float)k, d.dz, d.zlo), z_hi = z_lo + d.dz;  // voxel z-extent, mm
   const float rxy = 0.5f * sqrtf(d.dx * d.dx + d.dy * d.dy);
   const size_t pix = (size_t)j * d.nx + i;
-  float acc = 0.0f;
   for (int kv = 0; kv < d.nviews; ++kv) {
     const unsigned w = __ldg(&win[(size_t)kv * d.nx * d.ny + pix]);
     const int a_lo = (int)(w >> 4), a_cnt = (int)(w & 15u);
@@ -214,10 +209,86 @@ __global__ void __launch_bounds__(128) k_cone_back(Dims d, const float4* __restr
         float wt = 0.0f;
 #pragma unroll
         for (int q = 0; q < 3; ++q) wt += (p.po[q] == tgt && p.pz[q] == bk) ? p.w[q] : 0.0f;
-        if (wt != 0.0f) acc = fmaf(wt, __ldg(sino + ((size_t)kv * d.nv + b) * d.nu + a), acc);
+        if (wt != 0.0f) visit((kv * d.nv + b) * d.nu + a, wt);
       }
     }
   }
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(128) k_cone_back(Dims d, const float4* __restrict__ TA, const float4* __restrict__ TB,
+                                                   const float2* __restrict__ views, const unsigned short* __restrict__ win,
+                                                   const float* __restrict__ sino, float* __restrict__ out,
+                                                   const float* __restrict__ s_img, float* __restrict__ u_img, Scal sc) {
+  const int i = blockIdx.x * 32 + threadIdx.x;
+  const int nby = (d.ny + 3) / 4;
+  const int k = blockIdx.y / nby;
+  const int j = (blockIdx.y - k * nby) * 4 + threadIdx.y;
+  if (i >= d.nx || j >= d.ny) return;
+  float acc = 0.0f;
+  cone_voxel_hits(d, TA, TB, views, win, i, j, k, [&](int ray, float wt) { acc = fmaf(wt, __ldg(sino + ray), acc); });
+  const size_t e = ((size_t)k * d.ny + j) * d.nx + i;
+  out[e] = acc;
+  if (MODE == 2) u_img[e] = fmaf(sc.a[0], __ldcg(s_img + e), __ldcg(u_img + e));
+}
+
+// ------------------------------------------------------------------------------------------------
+// a2 (3D) with the stored transpose (P^T "as a lookup table"): the hits of
+// every voxel, (ray index, p_ij) pairs exactly as cone_voxel_hits() produces them, in sliced-ELL form: a
+// warp = 32 consecutive voxels of an x-row owns cap[warp] rows of 32 pairs at tab[off[warp] + e * 32 + lane]
+// (cap = the largest count in the warp; missing entries have weight 0). ~8 bytes per non-zero of P (4.4e9
+// at c5: ~40 GB of the 180 GB of HBM), streamed once per application with 256-byte coalesced reads, in the
+// same order as the on-the-fly gather: the two kernels give identical bits.
+// PASS 0: count per voxel -> warp maximum; PASS 1: fill.
+// ------------------------------------------------------------------------------------------------
+template <int PASS>
+__global__ void __launch_bounds__(128) k_cone_table(Dims d, const float4* __restrict__ TA, const float4* __restrict__ TB,
+                                                    const float2* __restrict__ views, const unsigned short* __restrict__ win,
+                                                    int* __restrict__ cap, const size_t* __restrict__ off,
+                                                    float2* __restrict__ tab) {
+  const int i = blockIdx.x * 32 + threadIdx.x;
+  const int nby = (d.ny + 3) / 4, nxw = gridDim.x;
+  const int k = blockIdx.y / nby;
+  const int j = (blockIdx.y - k * nby) * 4 + threadIdx.y;
+  if (j >= d.ny) return;  // whole warp
+  const int warp = (k * d.ny + j) * nxw + blockIdx.x;
+  int n = 0;
+  if (PASS == 0) {
+    if (i < d.nx) cone_voxel_hits(d, TA, TB, views, win, i, j, k, [&](int, float) { ++n; });
+    const int m = __reduce_max_sync(0xffffffffu, n);
+    if (threadIdx.x == 0) cap[warp] = m;
+  } else {
+    float2* row = tab + off[warp] + threadIdx.x;
+    if (i < d.nx)
+      cone_voxel_hits(d, TA, TB, views, win, i, j, k, [&](int ray, float wt) {
+        row[(size_t)n * 32] = make_float2(__int_as_float(ray), wt);
+        ++n;
+      });
+    const int m = cap[warp];
+    for (int e = n; e < m; ++e) row[(size_t)e * 32] = make_float2(0.0f, 0.0f);
+  }
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(128) k_cone_back_tab(Dims d, const int* __restrict__ cap, const size_t* __restrict__ off,
+                                                       const float2* __restrict__ tab, const float* __restrict__ sino,
+                                                       float* __restrict__ out, const float* __restrict__ s_img,
+                                                       float* __restrict__ u_img, Scal sc) {
+  const int i = blockIdx.x * 32 + threadIdx.x;
+  const int nby = (d.ny + 3) / 4, nxw = gridDim.x;
+  const int k = blockIdx.y / nby;
+  const int j = (blockIdx.y - k * nby) * 4 + threadIdx.y;
+  if (j >= d.ny) return;
+  const int warp = (k * d.ny + j) * nxw + blockIdx.x;
+  const int m = __ldg(&cap[warp]);
+  const float2* row = tab + __ldg(&off[warp]) + threadIdx.x;
+  float acc = 0.0f;
+#pragma unroll 4
+  for (int e = 0; e < m; ++e) {
+    const float2 h = __ldcs(row + (size_t)e * 32);
+    if (h.y != 0.0f) acc = fmaf(h.y, __ldg(sino + __float_as_int(h.x)), acc);
+  }
+  if (i >= d.nx) return;
   const size_t e = ((size_t)k * d.ny + j) * d.nx + i;
   out[e] = acc;
   if (MODE == 2) u_img[e] = fmaf(sc.a[0], __ldcg(s_img + e), __ldcg(u_img + e));
@@ -278,6 +349,45 @@ __global__ void __launch_bounds__(128) k_cone_window(Dims d, const float4* __res
 // ------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------
+// stored transpose: best effort (skipped when the table does not fit in free device memory)
+static int cone_build_stored(ctr_handle* h) {
+  const Dims& d = h->d;
+  h->ctab = nullptr; h->ccap = nullptr; h->coff = nullptr;
+  const int nxw = (d.nx + 31) / 32;
+  const size_t nwarp = (size_t)d.nz * d.ny * nxw;
+  dim3 grid(nxw, ((d.ny + 3) / 4) * d.nz), block(32, 4);
+  if (cudaMalloc((void**)&h->ccap, sizeof(int) * nwarp) != cudaSuccess) { cudaGetLastError(); h->ccap = nullptr; return CTR_OK; }
+  k_cone_table<0><<<grid, block>>>(d, h->rays, h->rays2, h->views, h->win, h->ccap, nullptr, nullptr);
+  CTR_LAUNCHED(h);
+  int* cap = (int*)malloc(sizeof(int) * nwarp);
+  size_t* off = (size_t*)malloc(sizeof(size_t) * nwarp);
+  if (!cap || !off) { free(cap); free(off); return CTR_ENOMEM; }
+  CTR_CUDA(h, cudaMemcpy(cap, h->ccap, sizeof(int) * nwarp, cudaMemcpyDeviceToHost));
+  size_t total = 0;
+  for (size_t w = 0; w < nwarp; ++w) { off[w] = total; total += (size_t)cap[w] * 32; }
+  free(cap);
+  size_t free_b = 0, total_b = 0;
+  cudaMemGetInfo(&free_b, &total_b);
+  const size_t need = total * sizeof(float2) + nwarp * sizeof(size_t);
+  bool ok = total > 0 && need + (size_t(2) << 30) < free_b;  // leave 2 GiB of head room
+  if (ok && cudaMalloc((void**)&h->coff, sizeof(size_t) * nwarp) != cudaSuccess) { cudaGetLastError(); h->coff = nullptr; ok = false; }
+  if (ok && cudaMalloc((void**)&h->ctab, total * sizeof(float2)) != cudaSuccess) { cudaGetLastError(); h->ctab = nullptr; ok = false; }
+  if (!ok) {
+    free(off);
+    if (h->coff) cudaFree(h->coff);
+    cudaFree(h->ccap);
+    h->coff = nullptr; h->ccap = nullptr; h->ctab = nullptr;
+    return CTR_OK;
+  }
+  cudaError_t ce = cudaMemcpy(h->coff, off, sizeof(size_t) * nwarp, cudaMemcpyHostToDevice);
+  free(off);
+  if (ce != cudaSuccess) return cuda_fail(h, ce, "cone table offsets");
+  k_cone_table<1><<<grid, block>>>(d, h->rays, h->rays2, h->views, h->win, h->ccap, h->coff, h->ctab);
+  CTR_LAUNCHED(h);
+  CTR_CUDA(h, cudaDeviceSynchronize());
+  return CTR_OK;
+}
+
 int cone_build_tables(ctr_handle* h) {
   const ctr_geometry& g = h->g;
   const Dims& d = h->d;
@@ -310,7 +420,7 @@ int cone_build_tables(ctr_handle* h) {
   if (flags[0]) return set_err(h, CTR_EGEOM, "cone beam: a voxel sees more than 15 detector columns per view (or nu > 4095)");
   if (flags[1]) return set_err(h, CTR_EGEOM, "cone beam: a ray advances more than one voxel in z per in-plane voxel (|mz| > 1)");
   h->win_ok = 1;
-  return CTR_OK;
+  return cone_build_stored(h);
 }
 
 int cone_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st) {
@@ -333,6 +443,12 @@ int cone_back(ctr_handle* h, const float* sino, float* out, int mode, const floa
   const Dims& d = h->d;
   ProfScope prof(h, CTR_PROF_BACK, st);
   dim3 grid((d.nx + 31) / 32, ((d.ny + 3) / 4) * d.nz), block(32, 4);
+  if (h->ctab) {
+    if (mode == 0) k_cone_back_tab<0><<<grid, block, 0, st>>>(d, h->ccap, h->coff, h->ctab, sino, out, s, u, h->sc);
+    else k_cone_back_tab<2><<<grid, block, 0, st>>>(d, h->ccap, h->coff, h->ctab, sino, out, s, u, h->sc);
+    CTR_LAUNCHED(h);
+    return CTR_OK;
+  }
   if (mode == 0) k_cone_back<0><<<grid, block, 0, st>>>(d, h->rays, h->rays2, h->views, h->win, sino, out, s, u, h->sc);
   else k_cone_back<2><<<grid, block, 0, st>>>(d, h->rays, h->rays2, h->views, h->win, sino, out, s, u, h->sc);
   CTR_LAUNCHED(h);

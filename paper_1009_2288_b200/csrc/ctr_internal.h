@@ -82,6 +82,9 @@ struct ctr_handle {
   float4* qwts;         // [nquad][hits_cap] p_ij of that ray in the four pixels of the 2 x 2 quad
   int* qcnt;            // [nquad] entries used per quad
   int hits_cap;
+  float2* ctab;         // 3D stored transpose, sliced ELL (ctr_cone.cu): (ray index, p_ij) pairs
+  int* ccap;            // [warps] rows per warp of 32 voxels
+  size_t* coff;         // [warps] offset of the warp's rows in ctab
   float* usi;           // CGLS iterate in the slice-interleaved layout (batch > 1)
   float* basis;         // [basis_cap][nimg] unit CGLS gradients (S24)
   int basis_cap;
