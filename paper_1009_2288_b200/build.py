@@ -13,7 +13,7 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libctr.so"
 SOURCES = ["ctr_api.cu", "ctr_fan.cu", "ctr_si.cu", "ctr_tv.cu", "ctr_cone.cu"]
-HEADERS = ["ctr_common.cuh", "ctr_internal.h", "ctr_fan_geom.cuh", "../../include/ctr.h"]
+HEADERS = ["ctr_common.cuh", "ctr_internal.h", "ctr_fan_geom.cuh", "ctr_ell.cuh", "../../include/ctr.h"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared"]
 

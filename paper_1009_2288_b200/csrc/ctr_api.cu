@@ -409,7 +409,7 @@ void ctr_destroy(ctr_handle* h) {
   if (!h) return;
   cudaDeviceSynchronize();
   void* bufs[] = {h->rays, h->rays2, h->views, h->ximg, h->bsino, h->r, h->q, h->s, h->gimg, h->v, h->w, h->n0,
-                  h->part, h->counters, h->hist, h->scal_block, h->stats, h->basis, h->win, h->imgT, h->win2, h->usi, h->qidx, h->qwts, h->qcnt, h->ctab, h->ccap, h->coff};
+                  h->part, h->counters, h->hist, h->scal_block, h->stats, h->basis, h->win, h->imgT, h->win2, h->usi, h->qidx, h->qwts, h->qcnt, h->ell_p.tab, h->ell_p.cap, h->ell_p.off, h->ell_pt.tab, h->ell_pt.cap, h->ell_pt.off};
   for (void* b : bufs)
     if (b) cudaFree(b);
   if (h->prof_ev) {

@@ -12,6 +12,7 @@
 // at the two crossing parameters t_o, t_z in [0,1].
 #include "ctr_common.cuh"
 #include "ctr_internal.h"
+#include "ctr_ell.cuh"
 
 namespace ctr {
 
@@ -233,66 +234,62 @@ __global__ void __launch_bounds__(128) k_cone_back(Dims d, const float4* __restr
 }
 
 // ------------------------------------------------------------------------------------------------
-// a2 (3D) with the stored transpose (P^T "as a lookup table"): the hits of
-// every voxel, (ray index, p_ij) pairs exactly as cone_voxel_hits() produces them, in sliced-ELL form: a
-// warp = 32 consecutive voxels of an x-row owns cap[warp] rows of 32 pairs at tab[off[warp] + e * 32 + lane]
-// (cap = the largest count in the warp; missing entries have weight 0). ~8 bytes per non-zero of P (4.4e9
-// at c5: ~40 GB of the 180 GB of HBM), streamed once per application with 256-byte coalesced reads, in the
-// same order as the on-the-fly gather: the two kernels give identical bits.
-// PASS 0: count per voxel -> warp maximum; PASS 1: fill.
+// Row visitors for the stored matrices (ctr_ell.cuh): the same entries, in the same order, as the
+// on-the-fly kernels above add them.
 // ------------------------------------------------------------------------------------------------
-template <int PASS>
-__global__ void __launch_bounds__(128) k_cone_table(Dims d, const float4* __restrict__ TA, const float4* __restrict__ TB,
-                                                    const float2* __restrict__ views, const unsigned short* __restrict__ win,
-                                                    int* __restrict__ cap, const size_t* __restrict__ off,
-                                                    float2* __restrict__ tab) {
-  const int i = blockIdx.x * 32 + threadIdx.x;
-  const int nby = (d.ny + 3) / 4, nxw = gridDim.x;
-  const int k = blockIdx.y / nby;
-  const int j = (blockIdx.y - k * nby) * 4 + threadIdx.y;
-  if (j >= d.ny) return;  // whole warp
-  const int warp = (k * d.ny + j) * nxw + blockIdx.x;
-  int n = 0;
-  if (PASS == 0) {
-    if (i < d.nx) cone_voxel_hits(d, TA, TB, views, win, i, j, k, [&](int, float) { ++n; });
-    const int m = __reduce_max_sync(0xffffffffu, n);
-    if (threadIdx.x == 0) cap[warp] = m;
-  } else {
-    float2* row = tab + off[warp] + threadIdx.x;
-    if (i < d.nx)
-      cone_voxel_hits(d, TA, TB, views, win, i, j, k, [&](int ray, float wt) {
-        row[(size_t)n * 32] = make_float2(__int_as_float(ray), wt);
-        ++n;
-      });
-    const int m = cap[warp];
-    for (int e = n; e < m; ++e) row[(size_t)e * 32] = make_float2(0.0f, 0.0f);
+struct ConeVoxelHits {  // rows of P^T: voxel (i, j, k), row = (k ny + j) nx + i; index = ray (kv nv + b) nu + a
+  const float4 *TA, *TB;
+  const float2* views;
+  const unsigned short* win;
+  template <class Visit>
+  __device__ __forceinline__ void operator()(const Dims& d, size_t row, Visit visit) const {
+    const int i = (int)(row % d.nx), j = (int)((row / d.nx) % d.ny), k = (int)(row / ((size_t)d.nx * d.ny));
+    cone_voxel_hits(d, TA, TB, views, win, i, j, k, visit);
   }
-}
+};
 
-template <int MODE>
-__global__ void __launch_bounds__(128) k_cone_back_tab(Dims d, const int* __restrict__ cap, const size_t* __restrict__ off,
-                                                       const float2* __restrict__ tab, const float* __restrict__ sino,
-                                                       float* __restrict__ out, const float* __restrict__ s_img,
-                                                       float* __restrict__ u_img, Scal sc) {
-  const int i = blockIdx.x * 32 + threadIdx.x;
-  const int nby = (d.ny + 3) / 4, nxw = gridDim.x;
-  const int k = blockIdx.y / nby;
-  const int j = (blockIdx.y - k * nby) * 4 + threadIdx.y;
-  if (j >= d.ny) return;
-  const int warp = (k * d.ny + j) * nxw + blockIdx.x;
-  const int m = __ldg(&cap[warp]);
-  const float2* row = tab + __ldg(&off[warp]) + threadIdx.x;
-  float acc = 0.0f;
-#pragma unroll 4
-  for (int e = 0; e < m; ++e) {
-    const float2 h = __ldcs(row + (size_t)e * 32);
-    if (h.y != 0.0f) acc = fmaf(h.y, __ldg(sino + __float_as_int(h.x)), acc);
+struct ConeRayHits {  // rows of P: ray (k, b, a), row = (k nv + b) nu + a; index = voxel (iz ny + y) nx + x
+  const float4 *TA, *TB;
+  template <class Visit>
+  __device__ __forceinline__ void operator()(const Dims& d, size_t row, Visit visit) const {
+    const int a = (int)(row % d.nu), b = (int)((row / d.nu) % d.nv), k = (int)(row / ((size_t)d.nu * d.nv));
+    const int ka = k * d.nu + a;
+    const Ray3 R = cone_ray(__ldg(&TA[ka]), __ldg(&TB[ka]), b, d);
+    const int n_drv = R.xdrv ? d.nx : d.ny, n_oth = R.xdrv ? d.ny : d.nx;
+    const int c_drv = R.xdrv ? d.c0x : d.c0y, c_oth = R.xdrv ? d.c0y : d.c0x;
+    float tlo = -1.0e6f, thi = 1.0e6f;
+    {
+      const float lo = (float)(-c_oth) - 1.0f, hi = (float)(n_oth - c_oth) + 1.0f;
+      if (R.mo != 0.0f) {
+        const float t1 = (lo - R.o0) / R.mo, t2 = (hi - R.o0) / R.mo;
+        tlo = fmaxf(tlo, fminf(t1, t2)); thi = fminf(thi, fmaxf(t1, t2));
+      } else if (R.o0 < lo || R.o0 > hi) thi = -2.0e6f;
+      const float zl = (float)(-d.c0z) - 1.0f, zh = (float)(d.nz - d.c0z) + 1.0f;
+      if (R.mz != 0.0f) {
+        const float t1 = (zl - R.z0) / R.mz, t2 = (zh - R.z0) / R.mz;
+        tlo = fmaxf(tlo, fminf(t1, t2)); thi = fminf(thi, fmaxf(t1, t2));
+      } else if (R.z0 < zl || R.z0 > zh) thi = -2.0e6f;
+    }
+    int s0 = 0, s1 = 0;
+    if (thi >= tlo) {
+      s0 = max(0, (int)floorf(tlo) + c_drv - 2);
+      s1 = min(n_drv, (int)ceilf(thi) + c_drv + 2);
+    }
+    float y = (float)(s0 - c_drv);
+    float oa = fmaf(R.mo, y, R.o0), za = fmaf(R.mz, y, R.z0);
+    for (int s = s0; s < s1; ++s) {
+      const float ob = fmaf(R.mo, y + 1.0f, R.o0), zb = fmaf(R.mz, y + 1.0f, R.z0);
+      const Slab3 p = slab3_pieces(slab3_o(oa, ob, R.inv_mo), slab3_o(za, zb, R.inv_mz), R.L);
+#pragma unroll
+      for (int q = 0; q < 3; ++q) {
+        const int io = cell_of(p.po[q]) + c_oth, iz = cell_of(p.pz[q]) + d.c0z;
+        if (p.w[q] != 0.0f && (unsigned)io < (unsigned)n_oth && (unsigned)iz < (unsigned)d.nz)
+          visit(R.xdrv ? (iz * d.ny + io) * d.nx + s : (iz * d.ny + s) * d.nx + io, p.w[q]);
+      }
+      oa = ob; za = zb; y += 1.0f;
+    }
   }
-  if (i >= d.nx) return;
-  const size_t e = ((size_t)k * d.ny + j) * d.nx + i;
-  out[e] = acc;
-  if (MODE == 2) u_img[e] = fmaf(sc.a[0], __ldcg(s_img + e), __ldcg(u_img + e));
-}
+};
 
 // volT[z][x][y] = vol[z][y][x]
 __global__ void __launch_bounds__(256) k_transpose3(int nx, int ny, const float* __restrict__ vol, float* __restrict__ volT) {
@@ -349,45 +346,6 @@ __global__ void __launch_bounds__(128) k_cone_window(Dims d, const float4* __res
 // ------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------
-// stored transpose: best effort (skipped when the table does not fit in free device memory)
-static int cone_build_stored(ctr_handle* h) {
-  const Dims& d = h->d;
-  h->ctab = nullptr; h->ccap = nullptr; h->coff = nullptr;
-  const int nxw = (d.nx + 31) / 32;
-  const size_t nwarp = (size_t)d.nz * d.ny * nxw;
-  dim3 grid(nxw, ((d.ny + 3) / 4) * d.nz), block(32, 4);
-  if (cudaMalloc((void**)&h->ccap, sizeof(int) * nwarp) != cudaSuccess) { cudaGetLastError(); h->ccap = nullptr; return CTR_OK; }
-  k_cone_table<0><<<grid, block>>>(d, h->rays, h->rays2, h->views, h->win, h->ccap, nullptr, nullptr);
-  CTR_LAUNCHED(h);
-  int* cap = (int*)malloc(sizeof(int) * nwarp);
-  size_t* off = (size_t*)malloc(sizeof(size_t) * nwarp);
-  if (!cap || !off) { free(cap); free(off); return CTR_ENOMEM; }
-  CTR_CUDA(h, cudaMemcpy(cap, h->ccap, sizeof(int) * nwarp, cudaMemcpyDeviceToHost));
-  size_t total = 0;
-  for (size_t w = 0; w < nwarp; ++w) { off[w] = total; total += (size_t)cap[w] * 32; }
-  free(cap);
-  size_t free_b = 0, total_b = 0;
-  cudaMemGetInfo(&free_b, &total_b);
-  const size_t need = total * sizeof(float2) + nwarp * sizeof(size_t);
-  bool ok = total > 0 && need + (size_t(2) << 30) < free_b;  // leave 2 GiB of head room
-  if (ok && cudaMalloc((void**)&h->coff, sizeof(size_t) * nwarp) != cudaSuccess) { cudaGetLastError(); h->coff = nullptr; ok = false; }
-  if (ok && cudaMalloc((void**)&h->ctab, total * sizeof(float2)) != cudaSuccess) { cudaGetLastError(); h->ctab = nullptr; ok = false; }
-  if (!ok) {
-    free(off);
-    if (h->coff) cudaFree(h->coff);
-    cudaFree(h->ccap);
-    h->coff = nullptr; h->ccap = nullptr; h->ctab = nullptr;
-    return CTR_OK;
-  }
-  cudaError_t ce = cudaMemcpy(h->coff, off, sizeof(size_t) * nwarp, cudaMemcpyHostToDevice);
-  free(off);
-  if (ce != cudaSuccess) return cuda_fail(h, ce, "cone table offsets");
-  k_cone_table<1><<<grid, block>>>(d, h->rays, h->rays2, h->views, h->win, h->ccap, h->coff, h->ctab);
-  CTR_LAUNCHED(h);
-  CTR_CUDA(h, cudaDeviceSynchronize());
-  return CTR_OK;
-}
-
 int cone_build_tables(ctr_handle* h) {
   const ctr_geometry& g = h->g;
   const Dims& d = h->d;
@@ -420,12 +378,16 @@ int cone_build_tables(ctr_handle* h) {
   if (flags[0]) return set_err(h, CTR_EGEOM, "cone beam: a voxel sees more than 15 detector columns per view (or nu > 4095)");
   if (flags[1]) return set_err(h, CTR_EGEOM, "cone beam: a ray advances more than one voxel in z per in-plane voxel (|mz| > 1)");
   h->win_ok = 1;
-  return cone_build_stored(h);
+  // stored matrices (best effort; ~40 GB each at c5)
+  int rc = ell_build(h, ConeVoxelHits{h->rays, h->rays2, h->views, h->win}, (size_t)d.npix, h->ell_pt);
+  if (rc == CTR_OK) rc = ell_build(h, ConeRayHits{h->rays, h->rays2}, (size_t)d.nray, h->ell_p);
+  return rc;
 }
 
 int cone_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st) {
   const Dims& d = h->d;
   ProfScope prof(h, CTR_PROF_FORWARD, st);
+  if (h->ell_p.tab) return ell_forward(h, h->ell_p, img, out, mode, bs, st);
   {
     dim3 tg((d.nx + 31) / 32, (d.ny + 31) / 32, d.nz), tb(32, 8);
     k_transpose3<<<tg, tb, 0, st>>>(d.nx, d.ny, img, h->imgT);
@@ -443,12 +405,7 @@ int cone_back(ctr_handle* h, const float* sino, float* out, int mode, const floa
   const Dims& d = h->d;
   ProfScope prof(h, CTR_PROF_BACK, st);
   dim3 grid((d.nx + 31) / 32, ((d.ny + 3) / 4) * d.nz), block(32, 4);
-  if (h->ctab) {
-    if (mode == 0) k_cone_back_tab<0><<<grid, block, 0, st>>>(d, h->ccap, h->coff, h->ctab, sino, out, s, u, h->sc);
-    else k_cone_back_tab<2><<<grid, block, 0, st>>>(d, h->ccap, h->coff, h->ctab, sino, out, s, u, h->sc);
-    CTR_LAUNCHED(h);
-    return CTR_OK;
-  }
+  if (h->ell_pt.tab) return ell_back(h, h->ell_pt, sino, out, mode, s, u, st);
   if (mode == 0) k_cone_back<0><<<grid, block, 0, st>>>(d, h->rays, h->rays2, h->views, h->win, sino, out, s, u, h->sc);
   else k_cone_back<2><<<grid, block, 0, st>>>(d, h->rays, h->rays2, h->views, h->win, sino, out, s, u, h->sc);
   CTR_LAUNCHED(h);

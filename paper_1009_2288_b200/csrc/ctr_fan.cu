@@ -7,6 +7,7 @@
 #include "ctr_common.cuh"
 #include "ctr_internal.h"
 #include "ctr_fan_geom.cuh"
+#include "ctr_ell.cuh"
 
 namespace ctr {
 
@@ -325,6 +326,73 @@ __global__ void __launch_bounds__(128) k_fan_back(Dims d, const float4* __restri
 }
 
 // ------------------------------------------------------------------------------------------------
+// Row visitors for the stored matrices of a single slice (ctr_ell.cuh; the paper's lookup-table strategy,
+// PAPER.md:193): the same entries, in the same order, as k_fan_forward<1,1,*> / k_fan_back<1,1,*> add them.
+// ------------------------------------------------------------------------------------------------
+struct FanRayHits {  // rows of P: ray r = k nu + b; index = pixel j nx + i
+  const float4* rays;
+  template <class Visit>
+  __device__ __forceinline__ void operator()(const Dims& d, size_t row, Visit visit) const {
+    const float4 R = __ldg(&rays[row]);
+    const float x0 = R.x, m = R.y, L = fabsf(R.z), K = R.w;
+    const bool xdrv = R.z < 0.0f;
+    const int n_drv = xdrv ? d.nx : d.ny, n_oth = xdrv ? d.ny : d.nx;
+    const int c_drv = xdrv ? d.c0x : d.c0y, c_oth = xdrv ? d.c0y : d.c0x;
+    int s0 = 0, s1 = n_drv;
+    const float lo = (float)(-c_oth) - 1.0f, hi = (float)(n_oth - c_oth) + 1.0f;
+    if (m != 0.0f) {
+      float t1 = (lo - x0) / m, t2 = (hi - x0) / m;
+      float tmin = fminf(t1, t2), tmax = fmaxf(t1, t2);
+      tmin = fminf(fmaxf(tmin, -1.0e6f), 1.0e6f);
+      tmax = fminf(fmaxf(tmax, -1.0e6f), 1.0e6f);
+      s0 = max(0, (int)floorf(tmin) + c_drv - 2);
+      s1 = min(n_drv, (int)ceilf(tmax) + c_drv + 2);
+    } else if (x0 < lo || x0 > hi) {
+      s1 = 0;
+    }
+    float y = (float)(s0 - c_drv);
+    float oa = fmaf(m, y, x0);
+    for (int s = s0; s < s1; ++s) {
+      const float ob = fmaf(m, y + 1.0f, x0);
+      const SlabW w = slab_weights(oa, ob, L, K);
+      const int ia = cell_of(w.ra) + c_oth, ib = cell_of(w.rb) + c_oth;
+      if (w.wa != 0.0f && (unsigned)ia < (unsigned)n_oth) visit(xdrv ? ia * d.nx + s : s * d.nx + ia, w.wa);
+      if (w.wb != 0.0f && (unsigned)ib < (unsigned)n_oth) visit(xdrv ? ib * d.nx + s : s * d.nx + ib, w.wb);
+      oa = ob;
+      y += 1.0f;
+    }
+  }
+};
+
+struct FanPixelHits {  // rows of P^T: pixel j nx + i; index = ray k nu + b
+  const float4* rays;
+  const float2* views;
+  const unsigned short* win;
+  int table;
+  template <class Visit>
+  __device__ __forceinline__ void operator()(const Dims& d, size_t row, Visit visit) const {
+    const int i = (int)(row % d.nx), j = (int)(row / d.nx);
+    const float fi = (float)(i - d.c0x), fj = (float)(j - d.c0y);
+    const float bi = bias_of(i - d.c0x), bj = bias_of(j - d.c0y);
+    const float px = fmaf((float)i + 0.5f, d.dx, d.xlo), py = fmaf((float)j + 0.5f, d.dy, d.ylo);
+    for (int k = 0; k < d.nviews; ++k) {
+      int b_lo, b_hi;
+      if (table) {
+        const unsigned w = __ldg(&win[(size_t)k * d.npix + row]);
+        b_lo = (int)(w >> 4);
+        b_hi = b_lo + (int)(w & 15u) - 1;
+      } else {
+        fan_window(d, __ldg(&views[k]), px, py, b_lo, b_hi);
+      }
+      for (int b = b_lo; b <= b_hi; ++b) {
+        const float wt = fan_pixel_weight(__ldg(&rays[k * d.nu + b]), fi, fj, bi, bj);
+        if (wt != 0.0f) visit(k * d.nu + b, wt);
+      }
+    }
+  }
+};
+
+// ------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------
 int fan_build_window(ctr_handle* h) {
@@ -345,6 +413,15 @@ int fan_build_window(ctr_handle* h) {
     k_win_transpose<<<dim3((d.npix + 255) / 256, d.nviews), 256>>>(h->win, h->win2, d.npix, d.nvp);
     CTR_LAUNCHED(h);
     CTR_CUDA(h, cudaDeviceSynchronize());
+  }
+  if (d.V == 1) {
+    // single slice: stored P^T (best effort). P stays on the fly unless CTR_STORED_P is set: a ray's row has
+    // ~n entries read one after the other and a slice has too few rays to hide that latency (c3: 198 us
+    // stored against 76 us on the fly), whereas P^T has many short rows (46 us against 119 us).
+    int rc = CTR_OK;
+    if (getenv("CTR_STORED_P")) rc = ell_build(h, FanRayHits{h->rays}, (size_t)d.nray, h->ell_p);
+    if (rc == CTR_OK) rc = ell_build(h, FanPixelHits{h->rays, h->views, h->win, h->win_ok}, (size_t)d.npix, h->ell_pt);
+    return rc;
   }
   return CTR_OK;
 }
@@ -369,6 +446,10 @@ static int fan_forward_v(ctr_handle* h, const float* img, float* out, int mode, 
 
 // batch == 1: the kernels above on the ABI arrays; batch > 1: slice-interleaved kernels of ctr_si.cu
 int fan_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st) {
+  if (h->d.V == 1 && h->ell_p.tab) {
+    ProfScope prof(h, CTR_PROF_FORWARD, st);
+    return ell_forward(h, h->ell_p, img, out, mode, bs, st);
+  }
   if (h->d.V == 1) return fan_forward_v<1, 1>(h, img, out, mode, bs, st);
   return si_forward(h, img, out, mode, bs, st);
 }
@@ -391,6 +472,10 @@ static int fan_back_v(ctr_handle* h, const float* sino, float* out, int mode, co
 }
 
 int fan_back(ctr_handle* h, const float* sino, float* out, int mode, const float* s, float* u, cudaStream_t st) {
+  if (h->d.V == 1 && h->ell_pt.tab) {
+    ProfScope prof(h, CTR_PROF_BACK, st);
+    return ell_back(h, h->ell_pt, sino, out, mode, s, u, st);
+  }
   if (h->d.V == 1) return fan_back_v<1, 1>(h, sino, out, mode, s, u, st);
   return si_back(h, sino, out, mode, s, u, st);
 }

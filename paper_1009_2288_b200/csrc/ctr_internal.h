@@ -53,6 +53,14 @@ struct Scal {
   float* coef;     // [CTR_MAX_BASIS][Bp] projections of g on the stored unit gradients
 };
 
+// stored system matrix, sliced ELL (ctr_ell.cuh)
+struct EllTable {
+  float2* tab;    // (index, weight) pairs
+  int* cap;       // [warps] slabs per warp of 32 rows
+  size_t* off;    // [warps] offset of the warp's slabs in tab
+  size_t nrows, bytes;
+};
+
 struct TvParams {
   float lambda, eps, c_armijo;
   int kmax;
@@ -82,9 +90,7 @@ struct ctr_handle {
   float4* qwts;         // [nquad][hits_cap] p_ij of that ray in the four pixels of the 2 x 2 quad
   int* qcnt;            // [nquad] entries used per quad
   int hits_cap;
-  float2* ctab;         // 3D stored transpose, sliced ELL (ctr_cone.cu): (ray index, p_ij) pairs
-  int* ccap;            // [warps] rows per warp of 32 voxels
-  size_t* coff;         // [warps] offset of the warp's rows in ctab
+  ctr::EllTable ell_p, ell_pt;  // stored P (rows = rays) and P^T (rows = voxels), batch = 1 only; tab == NULL: on the fly
   float* usi;           // CGLS iterate in the slice-interleaved layout (batch > 1)
   float* basis;         // [basis_cap][nimg] unit CGLS gradients (S24)
   int basis_cap;

@@ -227,3 +227,30 @@ def test_two_super_groups(ctr, torch_cuda, orc):
     for sl in (0, 63, 64, 69):
         assert rel(got_s[sl], orc.forward(cfg, x[sl].astype(np.float64))) <= TOL_OP
         assert rel(got_i[sl], orc.back(cfg, y[sl].astype(np.float64))) <= TOL_OP
+
+
+# ------------------------------------------------------------------ stored matrices (single slice)
+def _both_ways(ctr, torch, cfg, x, y):
+    """(P x, P^T y) with the stored sliced-ELL matrices and with the on-the-fly kernels."""
+    import os
+    out = []
+    for no_tables in (False, True):
+        os.environ["CTR_NO_TABLES" if no_tables else "CTR_STORED_P"] = "1"   # stored P is opt-in in 2D
+        try:
+            out.append((gpu_forward(ctr, torch, cfg, x), gpu_back(ctr, torch, cfg, y)))
+        finally:
+            os.environ.pop("CTR_NO_TABLES", None)
+            os.environ.pop("CTR_STORED_P", None)
+    return out
+
+
+@pytest.mark.parametrize("cfg", [get_config("c2"), odd2d(), odd2d(det_type=1, du=1.0)], ids=["c2", "odd", "arc"])
+def test_stored_matrices_equal_on_the_fly_kernels(ctr, torch_cuda, cfg):
+    """The lookup-table operators hold the very values the on-the-fly kernels compute and add
+    them in the same order: identical bits."""
+    rng = np.random.default_rng(406)
+    x = rng.random((1, cfg.ny, cfg.nx), dtype=np.float32)
+    y = rng.random((1, cfg.nviews, cfg.nu), dtype=np.float32)
+    (s_tab, i_tab), (s_fly, i_fly) = _both_ways(ctr, torch_cuda, cfg, x, y)
+    assert np.array_equal(s_tab, s_fly)
+    assert np.array_equal(i_tab, i_fly)
