@@ -387,7 +387,7 @@ int cone_build_tables(ctr_handle* h) {
 int cone_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st) {
   const Dims& d = h->d;
   ProfScope prof(h, CTR_PROF_FORWARD, st);
-  if (h->ell_p.tab) return ell_forward(h, h->ell_p, img, out, mode, bs, st);
+  if (h->ell_p.tab) return ell_forward<1>(h, h->ell_p, img, out, mode, bs, st);
   {
     dim3 tg((d.nx + 31) / 32, (d.ny + 31) / 32, d.nz), tb(32, 8);
     k_transpose3<<<tg, tb, 0, st>>>(d.nx, d.ny, img, h->imgT);

@@ -47,7 +47,24 @@ __global__ void __launch_bounds__(128) k_ell_build(Dims d, Hits hits, size_t nro
 // out[row] = sum_e w_e in[idx_e]  (+ the CGLS epilogues of the on-the-fly kernels, V = 1)
 //   ROLE 0 (P):   MODE 0 plain, MODE 1 out = bs - P x, MODE 2 also delta = ||out||^2 -> a = gamma/delta
 //   ROLE 1 (P^T): MODE 0 plain, MODE 2 also u += a s for the voxel
-template <int ROLE, int MODE>
+// SPLIT > 1 (P of a single 2D slice): a ray's entries are dealt round-robin to SPLIT consecutive table rows
+// (threads) and the partial sums are added by a fixed shuffle tree - a slice has too few rays to hide the
+// latency of ~n dependent gathers per ray otherwise.
+template <int SPLIT, class Hits>
+struct SplitHits {
+  Hits hits;
+  template <class Visit>
+  __device__ __forceinline__ void operator()(const Dims& d, size_t row, Visit visit) const {
+    const int part = (int)(row % SPLIT);
+    int e = 0;
+    hits(d, row / SPLIT, [&](int idx, float wt) {
+      if (e % SPLIT == part) visit(idx, wt);
+      ++e;
+    });
+  }
+};
+
+template <int ROLE, int MODE, int SPLIT>
 __global__ void __launch_bounds__(128) k_ell_apply(size_t nrows, const int* __restrict__ cap, const size_t* __restrict__ off,
                                                    const float2* __restrict__ tab, const float* __restrict__ in,
                                                    float* __restrict__ out, const float* __restrict__ aux,
@@ -64,10 +81,15 @@ __global__ void __launch_bounds__(128) k_ell_apply(size_t nrows, const int* __re
       if (h.y != 0.0f) acc = fmaf(h.y, __ldg(in + __float_as_int(h.x)), acc);
     }
   }
-  if (row < nrows) {
-    if (ROLE == 0 && MODE == 1) acc = __ldg(aux + row) - acc;
-    out[row] = acc;
-    if (ROLE == 1 && MODE == 2) u_img[row] = fmaf(sc.a[0], __ldcg(aux + row), __ldcg(u_img + row));
+  if (SPLIT > 1) {
+#pragma unroll
+    for (int o = 1; o < SPLIT; o <<= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  }
+  if (row < nrows && row % SPLIT == 0) {
+    const size_t orow = row / SPLIT;
+    if (ROLE == 0 && MODE == 1) acc = __ldg(aux + orow) - acc;
+    out[orow] = acc;
+    if (ROLE == 1 && MODE == 2) u_img[orow] = fmaf(sc.a[0], __ldcg(aux + orow), __ldcg(u_img + orow));
   } else {
     acc = 0.0f;
   }
@@ -121,13 +143,14 @@ static int ell_build(ctr_handle* h, Hits hits, size_t nrows, EllTable& t) {
   return CTR_OK;
 }
 
+template <int SPLIT>
 static int ell_forward(ctr_handle* h, const EllTable& t, const float* img, float* out, int mode, const float* bs,
                        cudaStream_t st) {
   const unsigned nblk = (unsigned)((t.nrows + 127) / 128);
   unsigned* cnt = h->counters;
-  if (mode == 0) k_ell_apply<0, 0><<<nblk, 128, 0, st>>>(t.nrows, t.cap, t.off, t.tab, img, out, bs, nullptr, h->sc, h->part, cnt);
-  else if (mode == 1) k_ell_apply<0, 1><<<nblk, 128, 0, st>>>(t.nrows, t.cap, t.off, t.tab, img, out, bs, nullptr, h->sc, h->part, cnt);
-  else k_ell_apply<0, 2><<<nblk, 128, 0, st>>>(t.nrows, t.cap, t.off, t.tab, img, out, bs, nullptr, h->sc, h->part, cnt);
+  if (mode == 0) k_ell_apply<0, 0, SPLIT><<<nblk, 128, 0, st>>>(t.nrows, t.cap, t.off, t.tab, img, out, bs, nullptr, h->sc, h->part, cnt);
+  else if (mode == 1) k_ell_apply<0, 1, SPLIT><<<nblk, 128, 0, st>>>(t.nrows, t.cap, t.off, t.tab, img, out, bs, nullptr, h->sc, h->part, cnt);
+  else k_ell_apply<0, 2, SPLIT><<<nblk, 128, 0, st>>>(t.nrows, t.cap, t.off, t.tab, img, out, bs, nullptr, h->sc, h->part, cnt);
   CTR_LAUNCHED(h);
   return CTR_OK;
 }
@@ -135,8 +158,8 @@ static int ell_forward(ctr_handle* h, const EllTable& t, const float* img, float
 static int ell_back(ctr_handle* h, const EllTable& t, const float* sino, float* out, int mode, const float* s, float* u,
                     cudaStream_t st) {
   const unsigned nblk = (unsigned)((t.nrows + 127) / 128);
-  if (mode == 0) k_ell_apply<1, 0><<<nblk, 128, 0, st>>>(t.nrows, t.cap, t.off, t.tab, sino, out, s, u, h->sc, h->part, h->counters);
-  else k_ell_apply<1, 2><<<nblk, 128, 0, st>>>(t.nrows, t.cap, t.off, t.tab, sino, out, s, u, h->sc, h->part, h->counters);
+  if (mode == 0) k_ell_apply<1, 0, 1><<<nblk, 128, 0, st>>>(t.nrows, t.cap, t.off, t.tab, sino, out, s, u, h->sc, h->part, h->counters);
+  else k_ell_apply<1, 2, 1><<<nblk, 128, 0, st>>>(t.nrows, t.cap, t.off, t.tab, sino, out, s, u, h->sc, h->part, h->counters);
   CTR_LAUNCHED(h);
   return CTR_OK;
 }

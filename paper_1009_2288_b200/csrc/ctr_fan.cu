@@ -329,6 +329,10 @@ __global__ void __launch_bounds__(128) k_fan_back(Dims d, const float4* __restri
 // Row visitors for the stored matrices of a single slice (ctr_ell.cuh; the paper's lookup-table strategy,
 // PAPER.md:193): the same entries, in the same order, as k_fan_forward<1,1,*> / k_fan_back<1,1,*> add them.
 // ------------------------------------------------------------------------------------------------
+#ifndef FAN_SPLIT
+#define FAN_SPLIT 8
+#endif
+
 struct FanRayHits {  // rows of P: ray r = k nu + b; index = pixel j nx + i
   const float4* rays;
   template <class Visit>
@@ -415,11 +419,9 @@ int fan_build_window(ctr_handle* h) {
     CTR_CUDA(h, cudaDeviceSynchronize());
   }
   if (d.V == 1) {
-    // single slice: stored P^T (best effort). P stays on the fly unless CTR_STORED_P is set: a ray's row has
-    // ~n entries read one after the other and a slice has too few rays to hide that latency (c3: 198 us
-    // stored against 76 us on the fly), whereas P^T has many short rows (46 us against 119 us).
-    int rc = CTR_OK;
-    if (getenv("CTR_STORED_P")) rc = ell_build(h, FanRayHits{h->rays}, (size_t)d.nray, h->ell_p);
+    // single slice: stored P and P^T (best effort). A ray's row has ~n entries and a slice has few rays:
+    // each ray is dealt to FAN_SPLIT table rows (one thread each; c3: 198 us unsplit, 76 us on the fly).
+    int rc = ell_build(h, SplitHits<FAN_SPLIT, FanRayHits>{FanRayHits{h->rays}}, (size_t)d.nray * FAN_SPLIT, h->ell_p);
     if (rc == CTR_OK) rc = ell_build(h, FanPixelHits{h->rays, h->views, h->win, h->win_ok}, (size_t)d.npix, h->ell_pt);
     return rc;
   }
@@ -448,7 +450,7 @@ static int fan_forward_v(ctr_handle* h, const float* img, float* out, int mode, 
 int fan_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st) {
   if (h->d.V == 1 && h->ell_p.tab) {
     ProfScope prof(h, CTR_PROF_FORWARD, st);
-    return ell_forward(h, h->ell_p, img, out, mode, bs, st);
+    return ell_forward<FAN_SPLIT>(h, h->ell_p, img, out, mode, bs, st);
   }
   if (h->d.V == 1) return fan_forward_v<1, 1>(h, img, out, mode, bs, st);
   return si_forward(h, img, out, mode, bs, st);

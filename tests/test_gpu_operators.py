@@ -93,10 +93,10 @@ def test_batched_slices_match_oracle_per_slice(ctr, torch_cuda, orc):
     for sl in (0, 3, 5):
         assert rel(got_s[sl], orc.forward(cfg, case["truth"][sl].astype(np.float64))) <= TOL_OP
         assert rel(got_i[sl], orc.back(cfg, case["sino"][sl].astype(np.float64))) <= TOL_OP
-    # batched vs single-slice kernels: same p_ij bit for bit; P also adds them in the same order, the
-    # batched gather P^T in a different fixed order (ctr_si.cu), so that one agrees to fp32 rounding only
+    # batched vs single-slice operators: same p_ij bit for bit, added in different fixed orders (ctr_si.cu,
+    # ctr_ell.cuh), so they agree to fp32 rounding
     one = scaled_config("c2", batch=1)
-    assert np.array_equal(gpu_forward(ctr, torch_cuda, one, case["truth"][4:5])[0], got_s[4])
+    assert rel(gpu_forward(ctr, torch_cuda, one, case["truth"][4:5])[0], got_s[4].astype(np.float64)) <= 1e-6
     assert rel(gpu_back(ctr, torch_cuda, one, case["sino"][4:5])[0], got_i[4].astype(np.float64)) <= 1e-6
 
 
@@ -235,22 +235,23 @@ def _both_ways(ctr, torch, cfg, x, y):
     import os
     out = []
     for no_tables in (False, True):
-        os.environ["CTR_NO_TABLES" if no_tables else "CTR_STORED_P"] = "1"   # stored P is opt-in in 2D
+        if no_tables:
+            os.environ["CTR_NO_TABLES"] = "1"
         try:
             out.append((gpu_forward(ctr, torch, cfg, x), gpu_back(ctr, torch, cfg, y)))
         finally:
             os.environ.pop("CTR_NO_TABLES", None)
-            os.environ.pop("CTR_STORED_P", None)
     return out
 
 
 @pytest.mark.parametrize("cfg", [get_config("c2"), odd2d(), odd2d(det_type=1, du=1.0)], ids=["c2", "odd", "arc"])
 def test_stored_matrices_equal_on_the_fly_kernels(ctr, torch_cuda, cfg):
-    """The lookup-table operators hold the very values the on-the-fly kernels compute and add
-    them in the same order: identical bits."""
+    """The lookup-table operators hold the very values the on-the-fly kernels compute. P^T adds
+    them in the same order (identical bits); the stored P of a 2D slice splits every ray over 8 threads, so its
+    sums agree with the on-the-fly kernel to fp32 rounding."""
     rng = np.random.default_rng(406)
     x = rng.random((1, cfg.ny, cfg.nx), dtype=np.float32)
     y = rng.random((1, cfg.nviews, cfg.nu), dtype=np.float32)
     (s_tab, i_tab), (s_fly, i_fly) = _both_ways(ctr, torch_cuda, cfg, x, y)
-    assert np.array_equal(s_tab, s_fly)
+    assert rel(s_tab, s_fly.astype(np.float64)) <= 1e-6
     assert np.array_equal(i_tab, i_fly)
