@@ -231,8 +231,8 @@ def main():
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the batched kernels at c4, from the committed
-# ncu --set full captures (profiles/r1e_ncu_full_c4.md); None for workloads that were not captured
-NCU_TRAFFIC_C4 = {"forward": 123.2e6, "back": 491.4e6}
+# ncu --set full captures (profiles/r1f_ncu_full_c4.md); None for workloads that were not captured
+NCU_TRAFFIC_C4 = {"forward": 169.5e6, "back": 558.7e6}
 
 
 def roofline(cfg, batch, prof, peaks):
