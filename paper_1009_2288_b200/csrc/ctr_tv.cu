@@ -339,7 +339,7 @@ __global__ void __launch_bounds__(128) k_tv_gradient(Dims d, const float* __rest
 // E(f - t_k g) with w frozen (O9) is assembled in fp64 by k_tv_trial_finish, which takes the first k with
 // E <= E0 - c t_k |g|^2. Slices that accepted a step in an earlier pass are skipped.
 // ---------------------------------------------------------------------------------------------
-#define TV_KA 8 /* the square roots make the pass MUFU-bound: 8 covers the accepted k of every sweep seen */
+#define TV_KA 8 /* candidates per pass; k <= 5 in every sweep seen, a later pass covers the rest (6 measured no faster) */
 
 // the linear forms of A3 on the face between the centre cell and its +A neighbour,
 // evaluated on windows wf and wg: returns a = sum c_i Lf_i^2, b = sum c_i Lf_i Lg_i, c = sum c_i Lg_i^2
