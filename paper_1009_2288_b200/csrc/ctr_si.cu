@@ -16,6 +16,7 @@
 // of ctr_fan.cu, so every p_ij is identical bit for bit in P and P^T (exact transpose up to summation
 // order).   P: PAPER.md:87-89 (Eq. 1), :193.   P^T: PAPER.md:193, :471 (A3'); north_star.
 #include <limits.h>
+#include <stdlib.h>
 
 #include "ctr_common.cuh"
 #include "ctr_internal.h"
@@ -42,6 +43,8 @@ __device__ __forceinline__ void fma4(float (&acc)[4], float w, const float4 f) {
 #ifndef SI_FWD_MINB
 #define SI_FWD_MINB 4 /* 64 registers: more loads in flight than the 40 ptxas picks unprompted (6.76 vs 7.07 ms per step) */
 #endif
+// (A ray-quad table for P, the mirror image of the quad gather below, was built and measured in round 1:
+// 7.2-7.5 ms per step against 6.75 ms for this kernel - adjacent rays share pixels along one axis only.)
 #ifndef SI_FWD_WARPS
 #define SI_FWD_WARPS 8 /* warps per block (16 adjacent rays at LQ = 16); 4, 16 and 32 measured slower */
 #endif
@@ -391,6 +394,7 @@ int si_build_hits(ctr_handle* h) {
   h->qidx = nullptr;
   h->qwts = nullptr;
   h->hits_cap = 0;
+  if (getenv("CTR_NO_TABLES")) return CTR_OK;
   const int nqx = (d.nx + 1) / 2, nqy = (d.ny + 1) / 2, nquad = nqx * nqy;
   if (cudaMalloc((void**)&h->qcnt, sizeof(int) * (size_t)nquad) != cudaSuccess) { cudaGetLastError(); h->qcnt = nullptr; return CTR_OK; }
   dim3 grid((nqx + 31) / 32, (nqy + 3) / 4), block(32, 4);
