@@ -255,3 +255,12 @@ def test_stored_matrices_equal_on_the_fly_kernels(ctr, torch_cuda, cfg):
     (s_tab, i_tab), (s_fly, i_fly) = _both_ways(ctr, torch_cuda, cfg, x, y)
     assert rel(s_tab, s_fly.astype(np.float64)) <= 1e-6
     assert np.array_equal(i_tab, i_fly)
+
+
+def test_batched_gather_fallback_matches_quad_table(ctr, torch_cuda):
+    """batch > 1: the on-the-fly gather k_si_back (used when the quad hit table cannot be allocated) against
+    the table-driven k_si_back_quad: same p_ij, different fixed summation orders."""
+    cfg = scaled_config("c2", batch=9)
+    y = np.random.default_rng(407).random((9, cfg.nviews, cfg.nu), dtype=np.float32)
+    (_, i_tab), (_, i_fly) = _both_ways(ctr, torch_cuda, cfg, np.zeros((9, cfg.ny, cfg.nx), np.float32), y)
+    assert rel(i_tab, i_fly.astype(np.float64)) <= 1e-6
