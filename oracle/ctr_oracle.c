@@ -529,6 +529,52 @@ void orc_reconstruct(const orc_geom* g, const double* sino, const orc_params* p,
   free(v); free(w);
 }
 
+/* ------------------------------------------------------------------------------------------------
+ * NEXT-1: the paper's own "GPU-friendly" backprojector, Eq. (11) (derivation App. III
+ * :467-493), 2D only:
+ *     [P^T y](u*,v*) = (du_pix dv_pix / dbeta) * sum_theta y^theta(beta*) / l(u*,v*)
+ * (u*,v*) = pixel CENTRE, l = distance source -> pixel, beta* = fan angle of the line source -> pixel
+ * measured from the central ray, y^theta(beta*) by LINEAR interpolation between the two nearest detector
+ * units (:197, last sentence); a pixel whose beta* falls outside the outermost unit centres gets 0 from
+ * that view (reading S26). ARC detector (the paper's, :217): units equally spaced in beta,
+ * dbeta = du/dsd. FLAT detector (BASELINE.json's configs; not in the paper): the same formula after the
+ * change of variable t = dsd tan(beta): the unit at t* subtends dbeta(beta*) = du cos^2(beta*) / dsd.
+ * An approximate adjoint only: the paper reports |<f,P^T y> - <Pf,y>| below 1 % (:493).
+ * ------------------------------------------------------------------------------------------------ */
+void orc_back_eq11(const orc_geom* g, const double* sino /* [nviews][nu] */, double* img /* [ny][nx] */) {
+  const double xlo = g->cx - g->nx * g->dx / 2.0, ylo = g->cy - g->ny * g->dy / 2.0;
+  for (int j = 0; j < g->ny; ++j) {
+    for (int i = 0; i < g->nx; ++i) {
+      const double px = xlo + (i + 0.5) * g->dx, py = ylo + (j + 0.5) * g->dy;
+      double sum = 0.0;
+      for (int k = 0; k < g->nviews; ++k) {
+        const double th = view_angle(g, k), c = cos(th), s = sin(th);
+        const double rx = px + g->dso * c, ry = py + g->dso * s; /* pixel - source, source = -dso (c, s) */
+        const double along = rx * c + ry * s, lateral = -rx * s + ry * c;
+        const double l = sqrt(rx * rx + ry * ry);
+        const double beta = atan2(lateral, along);
+        double bstar, dbeta;
+        if (g->det_type == 1) {
+          bstar = beta * g->dsd / g->du + (g->nu - 1) / 2.0 - g->u_off;
+          dbeta = g->du / g->dsd;
+        } else {
+          bstar = g->dsd * tan(beta) / g->du + (g->nu - 1) / 2.0 - g->u_off;
+          dbeta = g->du * cos(beta) * cos(beta) / g->dsd;
+        }
+        if (!(bstar >= 0.0) || !(bstar <= (double)(g->nu - 1))) continue;
+        int b0 = (int)floor(bstar);
+        if (b0 > g->nu - 2) b0 = g->nu - 2;
+        if (b0 < 0) b0 = 0;
+        const double fr = bstar - b0;
+        const double y = g->nu > 1 ? (1.0 - fr) * sino[(long)k * g->nu + b0] + fr * sino[(long)k * g->nu + b0 + 1]
+                                   : sino[(long)k * g->nu];
+        sum += y / (l * dbeta);
+      }
+      img[(long)j * g->nx + i] = g->dx * g->dy * sum;
+    }
+  }
+}
+
 int orc_num_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

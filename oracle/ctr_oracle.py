@@ -64,6 +64,7 @@ def lib():
         L.orc_forward.argtypes = [G, _DP, _DP]
         L.orc_back.argtypes = [G, _DP, _DP]
         L.orc_matrix_row.argtypes = [G, i, i, i, _DP]
+        L.orc_back_eq11.argtypes = [G, _DP, _DP]
         L.orc_cgls.argtypes = [G, _DP, _DP, i, i]
         L.orc_face_mag2.argtypes = [i, i, i, i, _DP, _DP]
         L.orc_sigma.argtypes = [i, i, i, i, _DP, d, d]
@@ -158,6 +159,17 @@ def back(g, sino):
     img = np.zeros((og.nz, og.ny, og.nx))
     lib().orc_back(C.byref(og), _p(sino), _p(img))
     return img[0] if og.ndim == 2 else img
+
+
+def back_eq11(g, sino):
+    """NEXT-1: the paper's pixel-driven, interpolating backprojector Eq. (11), 2D."""
+    og = make_geom(g)
+    assert og.ndim == 2
+    sino = _c64(sino)
+    assert sino.size == og.nviews * og.nu
+    img = np.zeros((og.ny, og.nx))
+    lib().orc_back_eq11(C.byref(og), _p(sino), _p(img))
+    return img
 
 
 def matrix(g):
