@@ -106,6 +106,12 @@ int ctr_forward(ctr_handle* h, const float* d_img, float* d_sino, void* stream);
 /* a2: d_img = P^T d_sino, the exact transpose of ctr_forward's matrix (same p_ij, bit for bit), gather
  * form, no atomics (PAPER.md:193 explains why not scatter). d_img is overwritten. */
 int ctr_back(ctr_handle* h, const float* d_sino, float* d_img, void* stream);
+/* NEXT-1 (not on the hot path, not used by ctr_cgls): the paper's own pixel-driven backprojector, Eq. (11)
+ * (PAPER.md:195-197): d_img(u*,v*) = (dx dy / dbeta) sum_views y(beta*) / l, with y(beta*) linearly interpolated
+ * between the two nearest detector units (0 outside the outermost unit centres) and l the source-pixel
+ * distance; dbeta = du/dsd (ARC) or du cos^2(beta*)/dsd (FLAT). An APPROXIMATE adjoint of ctr_forward (the paper
+ * reports < 1 % mismatch, :493). 2D only (CTR_EINVAL otherwise). Same layouts as ctr_back; d_img is overwritten. */
+int ctr_back_pixel(ctr_handle* h, const float* d_sino, float* d_img, void* stream);
 /* a3: n_iter CGLS iterations on min ||P x - b||^2 from the start value in d_x;
  * d_x is updated in place to u^(n_iter). n_iter = 0 is a no-op. Zero denominators stop the update (S4). */
 int ctr_cgls(ctr_handle* h, const float* d_b, float* d_x, int n_iter, void* stream);

@@ -50,7 +50,7 @@ class ctr_sweep_stat(C.Structure):
                 ("k", C.c_int32), ("pad", C.c_int32)]
 
 
-EXPORTS = ["ctr_default_params", "ctr_create", "ctr_destroy", "ctr_forward", "ctr_back", "ctr_cgls",
+EXPORTS = ["ctr_default_params", "ctr_create", "ctr_destroy", "ctr_forward", "ctr_back", "ctr_back_pixel", "ctr_cgls",
            "ctr_update_weights", "ctr_eptv_step", "ctr_reconstruct", "ctr_reconstruct_w",
            "ctr_set_params", "ctr_get_stats", "ctr_launch_count", "ctr_strerror", "ctr_last_error",
            "ctr_profile_enable", "ctr_profile_read"]
@@ -73,6 +73,7 @@ def load_library():
     L.ctr_destroy.restype = None
     L.ctr_forward.argtypes = [H, fp, fp, vp]
     L.ctr_back.argtypes = [H, fp, fp, vp]
+    L.ctr_back_pixel.argtypes = [H, fp, fp, vp]
     L.ctr_cgls.argtypes = [H, fp, fp, C.c_int, vp]
     L.ctr_update_weights.argtypes = [H, fp, fp, C.c_float, fp, vp]
     L.ctr_eptv_step.argtypes = [H, fp, fp, fp, C.c_float, vp]
@@ -182,6 +183,10 @@ class Handle:
 
     def ctr_back(self, sino, img):
         self._check(self._L.ctr_back(self._h, _ptr(sino, self.n_sino, "sino"), _ptr(img, self.n_img, "img"), _stream()), "ctr_back")
+        return img
+
+    def ctr_back_pixel(self, sino, img):
+        self._check(self._L.ctr_back_pixel(self._h, _ptr(sino, self.n_sino, "sino"), _ptr(img, self.n_img, "img"), _stream()), "ctr_back_pixel")
         return img
 
     def ctr_cgls(self, b, x, n_iter):

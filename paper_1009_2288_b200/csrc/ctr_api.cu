@@ -408,7 +408,7 @@ long long ctr_launch_count(const ctr_handle* h) { return h ? h->launches : 0; }
 void ctr_destroy(ctr_handle* h) {
   if (!h) return;
   cudaDeviceSynchronize();
-  void* bufs[] = {h->rays, h->rays2, h->views, h->ximg, h->bsino, h->r, h->q, h->s, h->gimg, h->v, h->w, h->n0,
+  void* bufs[] = {h->rays, h->rays2, h->views, h->viewsd, h->ximg, h->bsino, h->r, h->q, h->s, h->gimg, h->v, h->w, h->n0,
                   h->part, h->counters, h->hist, h->scal_block, h->stats, h->basis, h->win, h->imgT, h->win2, h->usi, h->qidx, h->qwts, h->qcnt, h->ell_p.tab, h->ell_p.cap, h->ell_p.off, h->ell_pt.tab, h->ell_pt.cap, h->ell_pt.off};
   for (void* b : bufs)
     if (b) cudaFree(b);
@@ -502,6 +502,7 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
   A((void**)&h->rays, sizeof(float4) * (size_t)d.nviews * d.nu);
   if (d.ndim == 3) A((void**)&h->rays2, sizeof(float4) * (size_t)d.nviews * d.nu);
   A((void**)&h->views, sizeof(float2) * d.nviews);
+  A((void**)&h->viewsd, sizeof(double2) * d.nviews);
   A((void**)&h->win, sizeof(unsigned short) * (size_t)d.nviews * d.nx * d.ny);
   if (d.V == 1) A((void**)&h->imgT, h->nimg * fb);
   else {
@@ -610,6 +611,15 @@ int ctr_back(ctr_handle* h, const float* d_sino, float* d_img, void* stream) {
   if ((rc = si_from_abi(h, d_sino, h->bsino, h->d.nray, st))) return rc;
   if ((rc = op_back(h, h->bsino, h->gimg, 0, nullptr, nullptr, st))) return rc;
   return si_to_abi(h, h->gimg, d_img, h->d.npix, st);
+}
+
+int ctr_back_pixel(ctr_handle* h, const float* d_sino, float* d_img, void* stream) {
+  if (!h) return CTR_EINVAL;
+  if (!aligned16(d_img) || !aligned16(d_sino)) return set_err(h, CTR_EINVAL, "ctr_back_pixel: NULL or misaligned pointer");
+  if (h->d.ndim != 2) return set_err(h, CTR_EINVAL, "ctr_back_pixel: Eq. (11) is defined for 2D fan beams only");
+  cudaStream_t st = (cudaStream_t)stream;
+  h->last_stream = st;
+  return fan_back_eq11(h, d_sino, d_img, st);
 }
 
 int ctr_cgls(ctr_handle* h, const float* d_b, float* d_x, int n_iter, void* stream) {

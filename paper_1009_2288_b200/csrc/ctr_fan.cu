@@ -24,13 +24,16 @@ struct FanGeomD {
 };
 
 __global__ void k_fan_build(FanGeomD g, const float* __restrict__ angles, float4* __restrict__ rays,
-                            float2* __restrict__ views) {
+                            float2* __restrict__ views, double2* __restrict__ viewsd) {
   int r = blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= g.nviews * g.nu) return;
   int k = r / g.nu, b = r - k * g.nu;
   double th = angles ? (double)angles[k] : g.theta0 + g.dtheta * (double)k;
   double c = cos(th), s = sin(th);
-  if (b == 0) views[k] = make_float2((float)c, (float)s);
+  if (b == 0) {
+    views[k] = make_float2((float)c, (float)s);
+    viewsd[k] = make_double2(c, s);
+  }
   double Sx = -g.dso * c, Sy = -g.dso * s;
   double t = ((double)b - (g.nu - 1) / 2.0 + g.u_off) * g.du;
   double Dx, Dy;
@@ -77,7 +80,7 @@ int fan_build_tables(ctr_handle* h) {
     CTR_CUDA(h, cudaMemcpy(d_angles, g.angles, sizeof(float) * g.nviews, cudaMemcpyHostToDevice));
   }
   int n = g.nviews * g.nu;
-  k_fan_build<<<(n + 127) / 128, 128>>>(gd, d_angles, h->rays, h->views);
+  k_fan_build<<<(n + 127) / 128, 128>>>(gd, d_angles, h->rays, h->views, h->viewsd);
   CTR_LAUNCHED(h);
   CTR_CUDA(h, cudaDeviceSynchronize());
   if (d_angles) cudaFree(d_angles);
@@ -395,6 +398,74 @@ struct FanPixelHits {  // rows of P^T: pixel j nx + i; index = ray k nu + b
     }
   }
 };
+
+// ------------------------------------------------------------------------------------------------
+// NEXT-1: the paper's own backprojector, Eq. (11) (App. III :467-493):
+//   [P^T y](u*,v*) = (dx dy / dbeta) sum_theta y^theta(beta*) / l(u*,v*),  y^theta(beta*) by linear interpolation.
+// One thread per pixel (as in the paper, :197) serving up to SC slices; the geometry of a (pixel, view) pair
+// - fan angle, interpolation position, 1/(l dbeta) - is evaluated once in fp64 and shared by the slices;
+// interpolation and accumulation in fp32. ARC: dbeta = du/dsd; FLAT: dbeta(beta*) = du cos^2(beta*)/dsd
+// (reading S26). Works on the ABI arrays ([batch][nviews][nu] -> [batch][ny][nx]).
+// ------------------------------------------------------------------------------------------------
+template <int SC>
+__global__ void __launch_bounds__(128) k_back_eq11(Dims d, double du, double u_off, const double2* __restrict__ viewsd,
+                                                   const float* __restrict__ sino, float* __restrict__ img) {
+  const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 4 + threadIdx.y;
+  const int sl0 = blockIdx.z * SC;
+  if (i >= d.nx || j >= d.ny) return;
+  const double px = (double)d.xlo + ((double)i + 0.5) * (double)d.dx, py = (double)d.ylo + ((double)j + 0.5) * (double)d.dy;
+  const double dso = (double)d.dso, dsd = (double)d.dsd, boff = (d.nu - 1) / 2.0 - u_off;
+  float acc[SC];
+#pragma unroll
+  for (int c = 0; c < SC; ++c) acc[c] = 0.0f;
+  const size_t sstride = (size_t)d.nviews * d.nu;
+  for (int k = 0; k < d.nviews; ++k) {
+    const double2 cs = viewsd[k];
+    const double rx = px + dso * cs.x, ry = py + dso * cs.y;
+    const double along = rx * cs.x + ry * cs.y, lateral = -rx * cs.y + ry * cs.x;
+    const double l = sqrt(rx * rx + ry * ry);
+    double bstar, dbeta;
+    if (d.det_type == 1) {
+      bstar = atan2(lateral, along) * dsd / du + boff;
+      dbeta = du / dsd;
+    } else {
+      const double tb = lateral / along;  // tan(beta*)
+      bstar = dsd * tb / du + boff;
+      dbeta = du / (dsd * (1.0 + tb * tb));
+    }
+    if (!(along > 0.0) || !(bstar >= 0.0) || !(bstar <= (double)(d.nu - 1))) continue;
+    int b0 = (int)floor(bstar);
+    b0 = max(0, min(b0, d.nu - 2));
+    const float fr = (float)(bstar - (double)b0), wgt = (float)(1.0 / (l * dbeta));
+    const float* row = sino + (size_t)sl0 * sstride + (size_t)k * d.nu + b0;
+#pragma unroll
+    for (int c = 0; c < SC; ++c) {
+      if (sl0 + c < d.B) {
+        const float y0 = __ldg(row + c * sstride), y1 = d.nu > 1 ? __ldg(row + c * sstride + 1) : y0;
+        acc[c] = fmaf(wgt, fmaf(fr, y1 - y0, y0), acc[c]);
+      }
+    }
+  }
+  const float scale = d.dx * d.dy;
+#pragma unroll
+  for (int c = 0; c < SC; ++c)
+    if (sl0 + c < d.B) img[(size_t)(sl0 + c) * d.npix + (size_t)j * d.nx + i] = scale * acc[c];
+}
+
+int fan_back_eq11(ctr_handle* h, const float* sino, float* img, cudaStream_t st) {
+  const Dims& d = h->d;
+  ProfScope prof(h, CTR_PROF_BACK, st);
+  dim3 block(32, 4);
+  if (d.B == 1) {
+    dim3 grid((d.nx + 31) / 32, (d.ny + 3) / 4, 1);
+    k_back_eq11<1><<<grid, block, 0, st>>>(d, (double)h->g.du, (double)h->g.u_off, h->viewsd, sino, img);
+  } else {
+    dim3 grid((d.nx + 31) / 32, (d.ny + 3) / 4, (d.B + 7) / 8);
+    k_back_eq11<8><<<grid, block, 0, st>>>(d, (double)h->g.du, (double)h->g.u_off, h->viewsd, sino, img);
+  }
+  CTR_LAUNCHED(h);
+  return CTR_OK;
+}
 
 // ------------------------------------------------------------------------------------------------
 // host side

@@ -79,6 +79,7 @@ struct ctr_handle {
   float4* rays;    // [nviews*nv*nu]  (2D: {x0, m, +-L, K}); 3D: see ctr_cone.cu
   float4* rays2;   // 3D second half of the ray record
   float2* views;   // [nviews] (cos, sin)
+  double2* viewsd; // [nviews] (cos, sin) in fp64 (2D; Eq. (11) backprojector)
   unsigned short* win;  // [nviews][npix] first_bin << 4 | count (2D gather window table)
   unsigned short* win2; // same table as [npix][nvp] (views contiguous), slice-interleaved path only
   int win_ok;           // table usable (nu <= 4095 and every count <= 15)
@@ -161,6 +162,7 @@ struct ProfScope {
 int fan_build_tables(ctr_handle* h);
 int fan_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st);
 int fan_back(ctr_handle* h, const float* sino, float* out, int mode, const float* s, float* u, cudaStream_t st);
+int fan_back_eq11(ctr_handle* h, const float* sino, float* img, cudaStream_t st);  // ABI layouts, any batch
 // implemented in ctr_si.cu (2D fan beam, batch > 1: slice-interleaved layout [n][LQ] of float4)
 int si_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st);
 int si_back(ctr_handle* h, const float* sino, float* out, int mode, const float* s, float* u, cudaStream_t st);

@@ -264,3 +264,42 @@ def test_batched_gather_fallback_matches_quad_table(ctr, torch_cuda):
     y = np.random.default_rng(407).random((9, cfg.nviews, cfg.nu), dtype=np.float32)
     (_, i_tab), (_, i_fly) = _both_ways(ctr, torch_cuda, cfg, np.zeros((9, cfg.ny, cfg.nx), np.float32), y)
     assert rel(i_tab, i_fly.astype(np.float64)) <= 1e-6
+
+
+# ------------------------------------------------------------------ NEXT-1: the paper's backprojector Eq. (11)
+def gpu_back_pixel(ctr, torch, cfg, sino):
+    h = ctr.ctr_create(cfg)
+    y = torch.from_numpy(np.ascontiguousarray(sino, dtype=np.float32)).cuda()
+    x = torch.full(h.img_shape, float("nan"), dtype=torch.float32, device="cuda")
+    h.ctr_back_pixel(y, x)
+    torch.cuda.synchronize()
+    h.close()
+    return x.cpu().numpy()
+
+
+@pytest.mark.parametrize("cfg,batch", [(get_config("c2"), 1), (odd2d(), 1), (odd2d(det_type=1, du=1.0), 3),
+                                       (scaled_config("c1", batch=11), 11)], ids=["c2", "odd", "arc3", "c1x11"])
+def test_back_pixel_eq11_matches_oracle(ctr, torch_cuda, orc, cfg, batch):
+    """ctr_back_pixel (Eq. 11) against orc.back_eq11 on random sinograms (the hardest input
+    for an interpolating operator), relative L2 <= 1e-5 as for the other operators."""
+    if cfg.batch != batch:
+        cfg = Config(**{**cfg.__dict__, "batch": batch})
+    y = np.random.default_rng(408).random((batch, cfg.nviews, cfg.nu), dtype=np.float32)
+    got = gpu_back_pixel(ctr, torch_cuda, cfg, y)
+    for sl in sorted({0, batch // 2, batch - 1}):
+        assert rel(got[sl], orc.back_eq11(cfg, y[sl].astype(np.float64))) <= TOL_OP
+
+
+def test_back_pixel_adjoint_mismatch_below_one_percent_on_gpu(ctr, torch_cuda):
+    """The paper's printed number on the CUDA path: <f, Eq11(y)> vs <ctr_forward(f), y> on the
+    paper's scanner geometry (arc detector, :217) with smooth f and y."""
+    cfg = Config(name="paper", index=91, ndim=2, nx=512, ny=512, nz=1, dx=500.0 / 512, dy=500.0 / 512, dz=1.0,
+                 nviews=40, nu=888, nv=1, du=1.0239, dv=1.0, dso=541.0, dsd=949.075, det_type=1)
+    jj, ii = np.mgrid[0:512, 0:512]
+    f = np.exp(-(((ii - 300) * 0.9766) ** 2 + ((jj - 230) * 0.9766) ** 2) / (2 * 40.0 ** 2)).astype(np.float32)[None]
+    kk, bb = np.mgrid[0:cfg.nviews, 0:cfg.nu]
+    y = (1.0 + 0.5 * np.cos(2 * np.pi * kk / cfg.nviews) * np.cos(3.0 * (bb / cfg.nu - 0.5))).astype(np.float32)[None]
+    Pf = gpu_forward(ctr, torch_cuda, cfg, f).astype(np.float64)
+    Bty = gpu_back_pixel(ctr, torch_cuda, cfg, y).astype(np.float64)
+    lhs, rhs = float((f * Bty).sum()), float((Pf * y).sum())
+    assert 1e-9 * abs(rhs) < abs(lhs - rhs) <= 0.01 * abs(rhs)
