@@ -170,7 +170,6 @@ def main():
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
-    h.ctr_profile_enable(True)
     l0 = h.ctr_launch_count()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
@@ -180,20 +179,49 @@ def main():
     barrier()
     ms = ev0.elapsed_time(ev1)
     launches = h.ctr_launch_count() - l0
-    prof = h.ctr_profile_read()
-    h.ctr_profile_enable(False)
     clocks = sampler.stop()
 
-    # ---- end to end through the C ABI with HOST buffers: per step H2D(sino) + step + D2H(image)
+    # ---- per-kernel breakdown: the same K steps again with the library's event profiler on (an event pair
+    # around every launch group costs ~0.5 ms per step, so it stays out of the timed region above)
+    h.ctr_profile_enable(True)
+    steps(K, True)
+    barrier()
+    prof = h.ctr_profile_read()
+    h.ctr_profile_enable(False)
+
+    # ---- end to end through the C ABI with HOST buffers: per step H2D(sino) + step + D2H(image), all inside the
+    # timed region. The copies run on a second stream, double-buffered, so that the upload of step n+1 and the
+    # download of step n overlap the kernels of the neighbouring step (what a pipeline of batches would do).
     img.zero_()
     steps(1, False)
     barrier()
+    main, side = torch.cuda.current_stream(), torch.cuda.Stream()
+    sino_buf = [sino, torch.empty_like(sino)]
+    stage = torch.empty_like(img)
+    ev_in = [torch.cuda.Event(), torch.cuda.Event()]
+    ev_step, ev_out = torch.cuda.Event(), torch.cuda.Event()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
-    for _ in range(K):
-        sino.copy_(sino_host, non_blocking=True)
-        steps(1, True)
-        img_host.copy_(img, non_blocking=True)
+    side.wait_stream(main)
+    with torch.cuda.stream(side):
+        sino_buf[0].copy_(sino_host, non_blocking=True)
+        ev_in[0].record(side)
+    for n in range(K):
+        main.wait_event(ev_in[n % 2])
+        h.ctr_reconstruct(sino_buf[n % 2], img, ctr.make_params(cfg, n_outer=1, warm_start=1))
+        if n + 1 < K:
+            with torch.cuda.stream(side):          # this step's kernels have been enqueued on `main` already
+                sino_buf[(n + 1) % 2].copy_(sino_host, non_blocking=True)
+                ev_in[(n + 1) % 2].record(side)
+        if n > 0:
+            main.wait_event(ev_out)                # the previous download has left `stage`
+        stage.copy_(img, non_blocking=True)
+        ev_step.record(main)
+        with torch.cuda.stream(side):
+            side.wait_event(ev_step)
+            img_host.copy_(stage, non_blocking=True)
+            ev_out.record(side)
+    main.wait_event(ev_out)
     e1.record()
     barrier()
     ms_e2e = e0.elapsed_time(e1)
