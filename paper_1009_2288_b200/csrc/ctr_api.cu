@@ -137,15 +137,17 @@ __global__ void __launch_bounds__(256) k_reorth_dots(size_t nl, int LQ, size_t n
                                                      const float* __restrict__ basis, int i0, int nb, int Bp, Scal sc,
                                                      double* part, unsigned* counter) {
   const int gs = blockIdx.y;
-  float acc[REORTH_NB * V];
+  float acc[(REORTH_NB + 1) * V];  // slots [q][c]: <b_q, g> for q < NB, ||g||^2 for q = NB
 #pragma unroll
-  for (int q = 0; q < REORTH_NB * V; ++q) acc[q] = 0.0f;
+  for (int q = 0; q < (REORTH_NB + 1) * V; ++q) acc[q] = 0.0f;
   // grid-stride loop (the stride is a multiple of 256, hence of LQ: a thread stays in its segment)
 #pragma unroll 2
   for (size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x; idx < nl; idx += (size_t)gridDim.x * 256) {
     {
       float gv[V];
       Pack<V>::ldcg(gi, (size_t)gs * nl + idx, gv);
+#pragma unroll
+      for (int c = 0; c < V; ++c) acc[REORTH_NB * V + c] = fmaf(gv[c], gv[c], acc[REORTH_NB * V + c]);
 #pragma unroll
       for (int q = 0; q < REORTH_NB; ++q) {
         if (q < nb) {
@@ -157,73 +159,96 @@ __global__ void __launch_bounds__(256) k_reorth_dots(size_t nl, int LQ, size_t n
       }
     }
   }
-  double red[REORTH_NB * V];
+  double red[(REORTH_NB + 1) * V];
 #pragma unroll
-  for (int q = 0; q < REORTH_NB * V; ++q) red[q] = (double)acc[q];
-  block_partials_q<REORTH_NB * V, 8>(red, LQ, part + (size_t)gs * gridDim.x * LQ * REORTH_NB * V, blockIdx.x, threadIdx.x);
+  for (int q = 0; q < (REORTH_NB + 1) * V; ++q) red[q] = (double)acc[q];
+  block_partials_q<(REORTH_NB + 1) * V, 8>(red, LQ, part + (size_t)gs * gridDim.x * LQ * (REORTH_NB + 1) * V, blockIdx.x, threadIdx.x);
 }
 
+// g' = g - sum_i c_i b_i (never stored), s <- g' + beta s (App. I step 5, :435; first = 1: s <- g') and the
+// next unit gradient b_new = g'/||g'||, in one pass. gamma' = ||g'||^2 comes from Pythagoras in k_finish
+// (||g||^2 - sum c_i^2: the b_i are orthonormal), so no separate subtraction pass is needed.
 template <int V>
-__global__ void __launch_bounds__(256) k_reorth_sub(size_t nl, int LQ, size_t nimg, float* __restrict__ gi,
-                                                    const float* __restrict__ basis, int nb, int Bp, int first, Scal sc,
-                                                    double* part, unsigned* counter) {
+__global__ void __launch_bounds__(256) k_img_update(size_t nl, int LQ, size_t nimg, const float* __restrict__ gi,
+                                                    const float* __restrict__ basis, int nb, int Bp, float* __restrict__ s,
+                                                    float* __restrict__ bnew, int first, Scal sc) {
+  const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
   const int gs = blockIdx.y;
-  const int sl0 = (gs * LQ + (int)(threadIdx.x % LQ)) * V;
-  double red[V];
-#pragma unroll
-  for (int c = 0; c < V; ++c) red[c] = 0.0;
-  for (size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x; idx < nl; idx += (size_t)gridDim.x * 256) {
-    float gv[V];
-    Pack<V>::ldcg(gi, (size_t)gs * nl + idx, gv);
+  if (idx >= nl) return;
+  const int sl0 = (gs * LQ + (int)(idx % LQ)) * V;
+  const size_t e = (size_t)gs * nl + idx;
+  float gv[V], sv[V];
+  Pack<V>::ldcg(gi, e, gv);
 #pragma unroll 4
-    for (int q = 0; q < nb; ++q) {
-      float bv[V];
-      Pack<V>::ldcg(basis + (size_t)q * nimg, (size_t)gs * nl + idx, bv);
+  for (int q = 0; q < nb; ++q) {
+    float bv[V];
+    Pack<V>::ldcg(basis + (size_t)q * nimg, e, bv);
 #pragma unroll
-      for (int c = 0; c < V; ++c) gv[c] = fmaf(-sc.coef[(size_t)q * Bp + sl0 + c], bv[c], gv[c]);
-    }
-    if (nb > 0) Pack<V>::st(gi, (size_t)gs * nl + idx, gv);
-#pragma unroll
-    for (int c = 0; c < V; ++c) red[c] = fma((double)gv[c], (double)gv[c], red[c]);
+    for (int c = 0; c < V; ++c) gv[c] = fmaf(-sc.coef[(size_t)q * Bp + sl0 + c], bv[c], gv[c]);
   }
-  block_partials_q<V, 8>(red, LQ, part + (size_t)gs * gridDim.x * LQ * V, blockIdx.x, threadIdx.x);
+  if (first) {
+#pragma unroll
+    for (int c = 0; c < V; ++c) sv[c] = gv[c];
+  } else {
+    Pack<V>::ldcg(s, e, sv);
+#pragma unroll
+    for (int c = 0; c < V; ++c) sv[c] = fmaf(sc.beta[sl0 + c], sv[c], gv[c]);
+  }
+  Pack<V>::st(s, e, sv);
+  if (bnew) {
+#pragma unroll
+    for (int c = 0; c < V; ++c) gv[c] *= sc.ginv[sl0 + c];
+    Pack<V>::st(bnew, e, gv);
+  }
 }
 
 // Finishing pass of the segmented reductions: block (q, gs) adds the partials part[gs][b][q][0..N) over the
 // blocks b in a fixed order and applies the scalar update of the producing kernel:
 //   FIN_ALPHA  N = V:       delta = ||P s||^2 -> a = gamma/delta            (App. I step 1)
-//   FIN_COEF   N = NB * V:  c_i = <b_i, g>                                   (S24)
-//   FIN_GAMMA  N = V:       gamma' = ||g||^2, beta = gamma'/gamma, 1/||g||   (App. I step 4, :432)
+//   FIN_COEF   N = (NB+1) V: c_i = <b_i, g> (S24) and gamma' = ||g||^2 - sum_i c_i^2 = ||g - sum c_i b_i||^2,
+//                            beta = gamma'/gamma, 1/sqrt(gamma')               (App. I step 4, :432)
 template <int N>
 __global__ void __launch_bounds__(256) k_finish(int mode, const double* __restrict__ part, int nblk, int LQ, int V,
                                                 int i0, int nb, int Bp, int first, Scal sc) {
   __shared__ double sm[256];
+  __shared__ double tot[N];
   const int q = blockIdx.x, gs = blockIdx.y, t = threadIdx.x;
   const int n = t % N, b0 = t / N;
   constexpr int NB0 = 256 / N;
   double acc = 0.0;
   const double* p = part + ((size_t)gs * nblk * LQ + q) * N + n;
+  if (b0 < NB0) {
 #pragma unroll 4
-  for (int b = b0; b < nblk; b += NB0) acc += __ldcg(p + (size_t)b * LQ * N);
+    for (int b = b0; b < nblk; b += NB0) acc += __ldcg(p + (size_t)b * LQ * N);
+  }
   sm[t] = acc;
   __syncthreads();
-  if (t >= N) return;
   double sum = 0.0;
-  for (int j = 0; j < NB0; ++j) sum += sm[j * N + n];
+  if (t < N) {
+    for (int j = 0; j < NB0; ++j) sum += sm[j * N + n];
+    tot[t] = sum;
+  }
+  __syncthreads();
+  if (t >= N) return;
   const int c = n % V, sl = (gs * LQ + q) * V + c;
   if (mode == CTR_FIN_ALPHA) {
     const double gamma = sc.gamma[sl];
     sc.a[sl] = (sum > 0.0 && gamma > 0.0) ? (float)(gamma / sum) : 0.0f;  // S4
-  } else if (mode == CTR_FIN_COEF) {
-    const int qb = n / V;
-    if (qb < nb) sc.coef[(size_t)(i0 + qb) * Bp + sl] = (float)sum;
   } else {
-    if (!first) {
-      const double gamma = sc.gamma[sl];
-      sc.beta[sl] = gamma > 0.0 ? (float)(sum / gamma) : 0.0f;  // S4
+    const int qb = n / V, NBV = N / V - 1;
+    if (qb < nb) sc.coef[(size_t)(i0 + qb) * Bp + sl] = (float)sum;
+    if (qb == NBV) {
+      // the coefficients are applied in fp32: use their rounded values in Pythagoras too
+      double g2 = sum;
+      for (int i = 0; i < nb; ++i) { const double ci = (double)(float)tot[i * V + c]; g2 -= ci * ci; }
+      if (g2 < 0.0) g2 = 0.0;
+      if (!first) {
+        const double gamma = sc.gamma[sl];
+        sc.beta[sl] = gamma > 0.0 ? (float)(g2 / gamma) : 0.0f;  // S4
+      }
+      sc.gamma[sl] = g2;
+      sc.ginv[sl] = g2 > 0.0 ? (float)(1.0 / sqrt(g2)) : 0.0f;
     }
-    sc.gamma[sl] = sum;
-    sc.ginv[sl] = sum > 0.0 ? (float)(1.0 / sqrt(sum)) : 0.0f;
   }
 }
 
@@ -234,7 +259,8 @@ int reduce_finish(ctr_handle* h, int mode, int N, int nblk, int i0, int nb, int 
   switch (N) {
     case 1: k_finish<1><<<grid, 256, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
     case 4: k_finish<4><<<grid, 256, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
-    default: k_finish<16><<<grid, 256, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
+    case 5: k_finish<5><<<grid, 256, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
+    default: k_finish<20><<<grid, 256, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
   }
   CTR_LAUNCHED(h);
   return CTR_OK;
@@ -250,16 +276,6 @@ static int vec_sino_axpy(ctr_handle* h, float* r, const float* q, cudaStream_t s
   CTR_LAUNCHED(h);
   return CTR_OK;
 }
-static int vec_img_supdate(ctr_handle* h, float* s, const float* g, float* bnew, int first, cudaStream_t st) {
-  const Dims& d = h->d;
-  const size_t nl = (size_t)d.npix * d.LQ;
-  dim3 grid((unsigned)((nl + 255) / 256), d.GS);
-  ProfScope prof(h, CTR_PROF_VECTOR, st);
-  if (d.V == 1) k_img_supdate<1><<<grid, 256, 0, st>>>(nl, d.LQ, s, g, bnew, h->sc, first);
-  else k_img_supdate<4><<<grid, 256, 0, st>>>(nl, d.LQ, s, g, bnew, h->sc, first);
-  CTR_LAUNCHED(h);
-  return CTR_OK;
-}
 static int vec_img_uupdate(ctr_handle* h, float* u, const float* s, cudaStream_t st) {
   const Dims& d = h->d;
   const size_t nl = (size_t)d.npix * d.LQ;
@@ -270,32 +286,28 @@ static int vec_img_uupdate(ctr_handle* h, float* u, const float* s, cudaStream_t
   CTR_LAUNCHED(h);
   return CTR_OK;
 }
-// g <- g minus its components along basis[0..nb), then gamma / beta / 1/||g||
-static int vec_reorth(ctr_handle* h, float* g, int nb, int first, cudaStream_t st) {
+// App. I steps 4-5 with the re-orthogonalisation of S24: c_i = <b_i, g>, gamma' = ||g - sum c_i b_i||^2,
+// beta = gamma'/gamma; then s <- g' + beta s and the next unit gradient, without ever storing g'
+static int vec_direction(ctr_handle* h, const float* g, int nb, int first, float* bnew, cudaStream_t st) {
   const Dims& d = h->d;
   const size_t nl = (size_t)d.npix * d.LQ;
   const int Bp = d.G * d.V;
-  // persistent-size grids: few partial sums for the finishing block of the reductions
   const unsigned want = (unsigned)((nl + 255) / 256);
-  unsigned cap = (unsigned)(CTR_REDUCE_BLOCKS / d.GS), dcap = (unsigned)(h->dots_blocks / d.GS);
-  if (cap < 1) cap = 1;
+  unsigned dcap = (unsigned)(h->dots_blocks / d.GS);
   if (dcap < 1) dcap = 1;
-  dim3 grid(want < cap ? want : cap, d.GS);
+  dim3 grid(want, d.GS);
   dim3 dgrid(want < dcap ? want : dcap, d.GS);  // exactly one resident wave of the register-heavy kernel
   ProfScope prof(h, CTR_PROF_VECTOR, st);
   if (nb > CTR_MAX_BASIS) nb = CTR_MAX_BASIS;
-  for (int i0 = 0; i0 < nb; i0 += REORTH_NB) {
-    const int cnt = nb - i0 < REORTH_NB ? nb - i0 : REORTH_NB;
-    if (d.V == 1) k_reorth_dots<1><<<dgrid, 256, 0, st>>>(nl, d.LQ, h->nimg, g, h->basis, i0, cnt, Bp, h->sc, h->part, h->counters + 4 * d.G);
-    else k_reorth_dots<4><<<dgrid, 256, 0, st>>>(nl, d.LQ, h->nimg, g, h->basis, i0, cnt, Bp, h->sc, h->part, h->counters + 4 * d.G);
-    CTR_LAUNCHED(h);
-    int rc = reduce_finish(h, CTR_FIN_COEF, REORTH_NB * d.V, (int)dgrid.x, i0, cnt, 0, st);
-    if (rc) return rc;
-  }
-  if (d.V == 1) k_reorth_sub<1><<<grid, 256, 0, st>>>(nl, d.LQ, h->nimg, g, h->basis, nb, Bp, first, h->sc, h->part, h->counters + 5 * d.G);
-  else k_reorth_sub<4><<<grid, 256, 0, st>>>(nl, d.LQ, h->nimg, g, h->basis, nb, Bp, first, h->sc, h->part, h->counters + 5 * d.G);
+  if (d.V == 1) k_reorth_dots<1><<<dgrid, 256, 0, st>>>(nl, d.LQ, h->nimg, g, h->basis, 0, nb, Bp, h->sc, h->part, h->counters + 4 * d.G);
+  else k_reorth_dots<4><<<dgrid, 256, 0, st>>>(nl, d.LQ, h->nimg, g, h->basis, 0, nb, Bp, h->sc, h->part, h->counters + 4 * d.G);
   CTR_LAUNCHED(h);
-  return reduce_finish(h, CTR_FIN_GAMMA, d.V, (int)grid.x, 0, 0, first, st);
+  int rc = reduce_finish(h, CTR_FIN_COEF, (REORTH_NB + 1) * d.V, (int)dgrid.x, 0, nb, first, st);
+  if (rc) return rc;
+  if (d.V == 1) k_img_update<1><<<grid, 256, 0, st>>>(nl, d.LQ, h->nimg, g, h->basis, nb, Bp, h->s, bnew, first, h->sc);
+  else k_img_update<4><<<grid, 256, 0, st>>>(nl, d.LQ, h->nimg, g, h->basis, nb, Bp, h->s, bnew, first, h->sc);
+  CTR_LAUNCHED(h);
+  return CTR_OK;
 }
 
 static int op_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st) {
@@ -330,16 +342,14 @@ static int cgls_internal(ctr_handle* h, const float* b, float* u, int n_iter, bo
     CTR_CUDA(h, cudaMemcpyAsync(h->r, b, h->nsino * sizeof(float), cudaMemcpyDeviceToDevice, st));  // r0 = y
   } else if ((rc = op_forward(h, u, h->r, 1, b, st))) return rc;                                    // r0 = y - P u0
   if ((rc = op_back(h, h->r, h->gimg, 0, nullptr, nullptr, st))) return rc;                         // g0 = P^T r0
-  if ((rc = vec_reorth(h, h->gimg, 0, 1, st))) return rc;                                           // gamma0
-  if ((rc = vec_img_supdate(h, h->s, h->gimg, h->basis, 1, st))) return rc;                         // s0 = g0, b_0
+  if ((rc = vec_direction(h, h->gimg, 0, 1, h->basis, st))) return rc;                              // gamma0, s0 = g0, b_0
   for (int m = 0; m < n_iter; ++m) {
     if ((rc = op_forward(h, h->s, h->q, 2, nullptr, st))) return rc;     // q = P s, a = gamma/||q||^2
     if (m == n_iter - 1) return vec_img_uupdate(h, u, h->s, st);         // u += a s
     if ((rc = vec_sino_axpy(h, h->r, h->q, st))) return rc;              // r -= a q
     if ((rc = op_back(h, h->r, h->gimg, 2, h->s, u, st))) return rc;     // g = P^T r, u += a s
-    if ((rc = vec_reorth(h, h->gimg, m + 1, 0, st))) return rc;          // g _|_ b_0..b_m, gamma', beta
     float* bnew = (m + 1 < h->basis_cap) ? h->basis + (size_t)(m + 1) * h->nimg : nullptr;
-    if ((rc = vec_img_supdate(h, h->s, h->gimg, bnew, 0, st))) return rc;  // s = g + beta s, b_{m+1}
+    if ((rc = vec_direction(h, h->gimg, m + 1, 0, bnew, st))) return rc;  // g' _|_ b_0.., gamma', beta, s = g' + beta s, b_{m+1}
   }
   return CTR_OK;
 }

@@ -181,7 +181,7 @@ int tv_sweep(ctr_handle* h, float* f, const float* v, const float* w, float lamb
              cudaStream_t st);  // n0_valid: h->n0 holds the face magnitudes of THIS f (tv_update_weights just ran)
 int tv_clamp(ctr_handle* h, float* f, cudaStream_t st);
 // implemented in ctr_api.cu: finishing pass of a segmented reduction (block partials in h->part)
-enum { CTR_FIN_ALPHA = 0, CTR_FIN_COEF = 1, CTR_FIN_GAMMA = 2 };
+enum { CTR_FIN_ALPHA = 0, CTR_FIN_COEF = 1 };
 int reduce_finish(ctr_handle* h, int mode, int N, int nblk, int i0, int nb, int first, cudaStream_t st);
 
 }  // namespace ctr
