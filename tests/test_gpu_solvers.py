@@ -251,3 +251,21 @@ def test_reconstruct_c4_full_batch_one_step(ctr, torch_cuda, orc):
     assert len(stats) == cfg.n_gd * 64
     for sl in (7, 50):
         compare_with_oracle(orc, cfg, case["sino"][sl], img[sl], stats[sl::64])
+
+
+def test_reconstruct_c3_full_schedule(ctr, torch_cuda, orc):
+    """configs[2] at BASELINE.json's full schedule (30 outer x (15 CGLS + 5 GD)); the oracle needs about a minute."""
+    cfg = get_config("c3")
+    case = make_case(cfg)
+    img, stats, _, _ = run_reconstruct(ctr, torch_cuda, cfg, case["sino"])
+    compare_with_oracle(orc, cfg, case["sino"][0], img[0], stats)
+
+
+def test_reconstruct_c4_full_schedule_sampled_slice(ctr, torch_cuda, orc):
+    """configs[3] exactly as bench.py runs it - 64 slices per call, the full 30 x (15 + 5) schedule - with one
+    sampled slice checked against the oracle (the oracle needs about a minute per slice)."""
+    cfg = get_config("c4")
+    case = make_case(cfg, raster=False)
+    img, stats, _, _ = run_reconstruct(ctr, torch_cuda, cfg, case["sino"])
+    sl = 33
+    compare_with_oracle(orc, cfg, case["sino"][sl], img[sl], stats[sl::64])
