@@ -113,7 +113,7 @@ __device__ __forceinline__ void block_sum_q(double (&v)[N], double (*sm)[NW][16]
 
 // block partials of a segmented reduction: part[(blk * LQ + q) * N + n]; a finishing kernel
 // (k_finish, ctr_api.cu) adds them over the blocks in a fixed order. A single finishing BLOCK inside the
-// producing kernel cost 120-350 us per launch at 64 slices (profiles/r1b): hence the extra tiny launch.
+// producing kernel cost 120-350 us per launch at 64 slices (measured in round 1): hence the extra tiny launch.
 template <int N, int NW>
 __device__ __forceinline__ void block_partials_q(double (&v)[N], int LQ, double* part, unsigned blk, int tid) {
   __shared__ double sm[N][NW][16];  // LQ <= 16

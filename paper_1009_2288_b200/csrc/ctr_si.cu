@@ -63,7 +63,7 @@ __global__ void __launch_bounds__(SI_FWD_WARPS * 32, SI_FWD_MINB) k_si_forward(D
   float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
   // per-slab records {pa, wa, pb, wb} of the sub-warp's ray, written by the lane that evaluated the slab
   // and read back as one broadcast LDS.128 per slab (a shuffle costs an L1 data-pipe wavefront each; four
-  // of them per slab were 40 % of the pipe, profiles/r1c). Rows are padded by one entry so that the
+  // of them per slab were 40 % of the pipe, measured in round 1). Rows are padded by one entry so that the
   // sub-warps of a warp hit different banks.
   __shared__ float4 slab[SI_FWD_WARPS][RW][LQ + 1];
   float4* myslab = slab[warp][sub];
