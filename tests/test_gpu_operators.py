@@ -216,15 +216,17 @@ def test_c4_full_batch_operators_and_cgls(ctr, torch_cuda, orc):
         assert rel(u[sl], orc.cgls(cfg, Px[sl].astype(np.float64), x0, 3)) <= 1e-4
 
 
-def test_two_super_groups(ctr, torch_cuda, orc):
-    """batch 70 -> 18 quads -> LQ = 16, two super-groups, the second mostly padding."""
-    cfg = scaled_config("c1", batch=70)
+@pytest.mark.parametrize("batch", [2, 20, 70])
+def test_sub_warp_widths(ctr, torch_cuda, orc, batch):
+    """batch 2 -> LQ = 1 (32 rays per warp); 20 -> LQ = 8; 70 -> 18 quads -> LQ = 16, two super-groups, the
+    second mostly padding."""
+    cfg = scaled_config("c1", batch=batch)
     rng = np.random.default_rng(405)
-    x = rng.random((70, cfg.ny, cfg.nx), dtype=np.float32)
-    y = rng.random((70, cfg.nviews, cfg.nu), dtype=np.float32)
+    x = rng.random((batch, cfg.ny, cfg.nx), dtype=np.float32)
+    y = rng.random((batch, cfg.nviews, cfg.nu), dtype=np.float32)
     got_s = gpu_forward(ctr, torch_cuda, cfg, x)
     got_i = gpu_back(ctr, torch_cuda, cfg, y)
-    for sl in (0, 63, 64, 69):
+    for sl in sorted({0, min(63, batch - 1), min(64, batch - 1), batch - 1}):
         assert rel(got_s[sl], orc.forward(cfg, x[sl].astype(np.float64))) <= TOL_OP
         assert rel(got_i[sl], orc.back(cfg, y[sl].astype(np.float64))) <= TOL_OP
 
