@@ -290,7 +290,14 @@ def roofline(cfg, batch, prof, peaks):
                 "compulsory_GBps": bytes_alg / sec / 1e9,
                 "compulsory_GBps_frac_of_measured_hbm": bytes_alg / sec / 1e9 / hbm}
 
-    out = {"bound": "alu", **one(kind),
+    # the unit that actually binds both kernels (ncu: l1tex data pipe 78 % busy): every non-zero of P moves
+    # 4 bytes per slice through an L1; peak = 148 SMs x 128 B/clk x sm_max_mhz
+    sec_k = prof[kind][0] / max(prof[kind][1], 1) * 1e-3
+    l1_peak = 148 * 128 * sm_mhz * 1e6 / 1e12
+    l1 = {"bound": "l1 gather bandwidth", "achieved": 4.0 * nnz * batch / sec_k / 1e12, "peak": l1_peak, "unit": "TB/s",
+          "frac": 4.0 * nnz * batch / sec_k / 1e12 / l1_peak,
+          "note": "algorithmic gather bytes (4 B per non-zero of P per slice) over the L1 data-pipe peak"}
+    out = {"bound": "alu", **one(kind), "l1_view": l1,
            "peak_source": "derived: 148 SM x 128 fp32 FMA lanes x 2 flop x sm_max_mhz (MEASURED_PEAKS.json clock); "
                           "hbm_gbs of measured" if "hbm_gbs" in peaks else "fallback 6650 GB/s",
            "other": one("back" if kind == "forward" else "forward")}
