@@ -63,10 +63,11 @@ __global__ void __launch_bounds__(SI_FWD_WARPS * 32, SI_FWD_MINB) k_si_forward(D
   float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
   // per-slab records {pa, wa, pb, wb} of the sub-warp's ray, written by the lane that evaluated the slab
   // and read back as one broadcast LDS.128 per slab (a shuffle costs an L1 data-pipe wavefront each; four
-  // of them per slab were 40 % of the pipe, measured in round 1). The records of a warp's rays for the same
-  // slab are adjacent (one 32..512-byte segment, distinct banks), so that LDS is a single wavefront.
-  __shared__ float4 slab[SI_FWD_WARPS][LQ][RW];
-  float4* myslab = &slab[warp][0][sub];
+  // of them per slab were 40 % of the pipe, measured in round 1). Rows are padded by one entry so that the
+  // sub-warps of a warp hit different banks. (Interleaving the two rays' records per slab, and 8-byte
+  // records with the second length recomputed as L - wa, were measured: no gain / 50 % slower.)
+  __shared__ float4 slab[SI_FWD_WARPS][RW][LQ + 1];
+  float4* myslab = slab[warp][sub];
 
   float x0 = 0.0f, m = 0.0f, L = 0.0f, K = 0.0f;
   bool xdrv = false;
@@ -121,11 +122,11 @@ __global__ void __launch_bounds__(SI_FWD_WARPS * 32, SI_FWD_MINB) k_si_forward(D
       }
     }
     __syncwarp();
-    myslab[q * RW] = make_float4(__int_as_float(pa), wa, __int_as_float(pb), wb);
+    myslab[q] = make_float4(__int_as_float(pa), wa, __int_as_float(pb), wb);
     __syncwarp();
 #pragma unroll
     for (int t = 0; t < LQ; ++t) {
-      const float4 rec = myslab[t * RW];
+      const float4 rec = myslab[t];
       if (rec.y != 0.0f) fma4(acc, rec.y, __ldg(base + __float_as_int(rec.x)));
       if (rec.w != 0.0f) fma4(acc, rec.w, __ldg(base + __float_as_int(rec.z)));
     }
@@ -326,11 +327,10 @@ __global__ void __launch_bounds__(256, SI_BACK_MINB) k_si_back_quad(Dims d, cons
                                                       Scal sc) {
   constexpr int PB = 256 / LQ;  // quads per block
   constexpr int TX = PB >= 64 ? 8 : 4, TY = PB / TX;
-  // chunk of LQ table entries per quad, handed round through shared memory (broadcast reads; the entries
-  // of a warp's quads for the same slot are adjacent: one wavefront per read)
-  constexpr int QW = 32 / LQ;  // quads per warp
-  __shared__ float4 chw[8][LQ][QW];
-  __shared__ int chi[8][LQ][QW];
+  // chunk of LQ table entries per quad, handed round through shared memory (broadcast reads; rows padded
+  // so that the sub-warps of a warp use different banks)
+  __shared__ float4 chw[PB][LQ + 1];
+  __shared__ int chi[PB][LQ + 1];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int q = lane % LQ, sub = lane / LQ;
   const int pl = warp * (32 / LQ) + sub;
@@ -355,14 +355,14 @@ __global__ void __launch_bounds__(256, SI_BACK_MINB) k_si_back_quad(Dims d, cons
     float4 w4 = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
     if (e0 + q < cnt) { id = __ldcs(ip + e0); w4 = __ldcs(wp + e0); }  // streamed once per application
     __syncwarp();
-    chi[warp][q][sub] = id;
-    chw[warp][q][sub] = w4;
+    chi[pl][q] = id;
+    chw[pl][q] = w4;
     __syncwarp();
 #pragma unroll
     for (int t = 0; t < LQ; ++t) {
-      const int it = chi[warp][t][sub];
+      const int it = chi[pl][t];
       if (it >= 0) {
-        const float4 w = chw[warp][t][sub];
+        const float4 w = chw[pl][t];
         const float4 y = __ldg(sg + it);
         fma4(acc[0], w.x, y);
         fma4(acc[1], w.y, y);
