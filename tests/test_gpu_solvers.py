@@ -269,3 +269,22 @@ def test_reconstruct_c4_full_schedule_sampled_slice(ctr, torch_cuda, orc):
     img, stats, _, _ = run_reconstruct(ctr, torch_cuda, cfg, case["sino"])
     sl = 33
     compare_with_oracle(orc, cfg, case["sino"][sl], img[sl], stats[sl::64])
+
+
+@pytest.mark.parametrize("batch", [1, 5])
+def test_warm_start_continues_the_iteration(ctr, torch_cuda, batch):
+    """ctr_params.warm_start: two calls of one outer iteration each == one call of two (what bench.py's
+    end-to-end loop relies on)."""
+    torch = torch_cuda
+    cfg = scaled_config("c1", batch=batch, n_outer=2)
+    case = make_case(cfg, raster=False)
+    h = ctr.ctr_create(cfg)
+    sino = to_gpu(torch, case["sino"])
+    a = torch.zeros(h.img_shape, device="cuda")
+    b = torch.full(h.img_shape, float("nan"), device="cuda")
+    h.ctr_reconstruct(sino, a, ctr.make_params(cfg, n_outer=2))
+    h.ctr_reconstruct(sino, b, ctr.make_params(cfg, n_outer=1))
+    h.ctr_reconstruct(sino, b, ctr.make_params(cfg, n_outer=1, warm_start=1))
+    torch.cuda.synchronize()
+    assert torch.equal(a, b)
+    h.close()
