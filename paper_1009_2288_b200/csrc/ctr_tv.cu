@@ -68,6 +68,35 @@ __device__ __forceinline__ float face_n0sq(const Window<V, ND>& w, int A, int qz
   return n0;
 }
 
+// The same N0^2 for slice lanes (2h, 2h+1) at once with Blackwell's packed fp32x2 instructions (FFMA2 /
+// FADD2 / FMUL2, sm_100): the stencil kernels are bound by instruction issue, not by the FMA pipe, and a
+// packed instruction does two lanes' worth of arithmetic in one issue slot. Operation for operation the
+// same roundings as face_n0sq() (a - b is formed as fma(b, -1, a), which rounds identically).
+__device__ __forceinline__ float2 sub2(float2 a, float2 b) { return __ffma2_rn(b, make_float2(-1.0f, -1.0f), a); }
+
+template <int V, int ND>
+__device__ __forceinline__ float2 face_n0sq2(const Window<V, ND>& w, int A, int qz, int qy, int qx, int h) {
+  const int ez = (A == 2), ey = (A == 1), ex = (A == 0);
+  const float2 half = make_float2(0.5f, 0.5f);
+#define W2(z, y, x) make_float2(w.c[z][y][x][2 * h], w.c[z][y][x][2 * h + 1])
+  const float2 lo = W2(qz, qy, qx), hi = W2(qz + ez, qy + ey, qx + ex);
+  const float2 dd = sub2(hi, lo);
+  float2 n0 = __fmul2_rn(dd, dd);
+  const float2 m0 = __fmul2_rn(half, __fadd2_rn(hi, lo));
+#pragma unroll
+  for (int T = 0; T < ND; ++T) {
+    if (T == A) continue;
+    const int tz = (T == 2), ty = (T == 1), tx = (T == 0);
+    const float2 mp = __fmul2_rn(half, __fadd2_rn(W2(qz + ez + tz, qy + ey + ty, qx + ex + tx), W2(qz + tz, qy + ty, qx + tx)));
+    const float2 mm = __fmul2_rn(half, __fadd2_rn(W2(qz + ez - tz, qy + ey - ty, qx + ex - tx), W2(qz - tz, qy - ty, qx - tx)));
+    const float2 a = sub2(mp, m0), b = sub2(m0, mm);
+    n0 = __ffma2_rn(__fmul2_rn(half, a), a, n0);
+    n0 = __ffma2_rn(__fmul2_rn(half, b), b, n0);
+  }
+#undef W2
+  return n0;
+}
+
 // thread -> voxel mapping shared by all stencil kernels: block (32,4), grid (nx/32, ny/4 * nz, G)
 struct Vox {
   int i, j, k, g, tid;
@@ -117,9 +146,19 @@ __global__ void __launch_bounds__(128) k_tv_faces(Dims d, const float* __restric
     load_window<V, ND>(d, f, p.g, p.i, p.j, p.k, w);
     const int cz = (ND == 3) ? 1 : 0;
 #pragma unroll
-    for (int A = 0; A < ND; ++A)
+    for (int A = 0; A < ND; ++A) {
+      if (V % 2 == 0) {
 #pragma unroll
-      for (int s = 0; s < V; ++s) val[A][s] = pos[A] < lim[A] ? face_n0sq<V, ND>(w, A, cz, 1, 1, s) : 0.0f;
+        for (int hh = 0; hh < V / 2; ++hh) {
+          const float2 t = face_n0sq2<V, ND>(w, A, cz, 1, 1, hh);
+          val[A][2 * hh] = pos[A] < lim[A] ? t.x : 0.0f;
+          val[A][2 * hh + (V > 1)] = pos[A] < lim[A] ? t.y : 0.0f;
+        }
+      } else {
+#pragma unroll
+        for (int s = 0; s < V; ++s) val[A][s] = pos[A] < lim[A] ? face_n0sq<V, ND>(w, A, cz, 1, 1, s) : 0.0f;
+      }
+    }
     const size_t e = (size_t)p.g * d.npix + ((size_t)p.k * d.ny + p.j) * d.nx + p.i;
 #pragma unroll
     for (int A = 0; A < ND; ++A) Pack<V>::st(n0 + (size_t)A * d.G * d.npix * V, e, val[A]);
