@@ -408,6 +408,36 @@ __device__ __forceinline__ void face_forms(const Window<V, ND>& wf, const Window
   }
 }
 
+// face_forms() for slice lanes (2h, 2h+1) at once with packed fp32x2 instructions; same roundings per lane
+template <int V, int ND>
+__device__ __forceinline__ void face_forms2(const Window<V, ND>& wf, const Window<V, ND>& wg, int A, int h, float2& a,
+                                            float2& b, float2& c) {
+  const int cz = (ND == 3) ? 1 : 0;
+  const int ez = (A == 2), ey = (A == 1), ex = (A == 0);
+  const float2 half = make_float2(0.5f, 0.5f);
+#define F2(w, z, y, x) make_float2(w.c[z][y][x][2 * h], w.c[z][y][x][2 * h + 1])
+  const float2 df = sub2(F2(wf, cz + ez, 1 + ey, 1 + ex), F2(wf, cz, 1, 1));
+  const float2 dg = sub2(F2(wg, cz + ez, 1 + ey, 1 + ex), F2(wg, cz, 1, 1));
+  a = __fmul2_rn(df, df); b = __fmul2_rn(df, dg); c = __fmul2_rn(dg, dg);
+#pragma unroll
+  for (int T = 0; T < ND; ++T) {
+    if (T == A) continue;
+    const int tz = (T == 2), ty = (T == 1), tx = (T == 0);
+#pragma unroll
+    for (int sg = -1; sg <= 1; sg += 2) {
+      const float2 lf = __fmul2_rn(half, __fadd2_rn(sub2(F2(wf, cz + ez + sg * tz, 1 + ey + sg * ty, 1 + ex + sg * tx), F2(wf, cz + ez, 1 + ey, 1 + ex)),
+                                                   sub2(F2(wf, cz + sg * tz, 1 + sg * ty, 1 + sg * tx), F2(wf, cz, 1, 1))));
+      const float2 lg = __fmul2_rn(half, __fadd2_rn(sub2(F2(wg, cz + ez + sg * tz, 1 + ey + sg * ty, 1 + ex + sg * tx), F2(wg, cz + ez, 1 + ey, 1 + ex)),
+                                                   sub2(F2(wg, cz + sg * tz, 1 + sg * ty, 1 + sg * tx), F2(wg, cz, 1, 1))));
+      const float2 hlf = __fmul2_rn(half, lf), hlg = __fmul2_rn(half, lg);
+      a = __ffma2_rn(hlf, lf, a);
+      b = __ffma2_rn(hlf, lg, b);
+      c = __ffma2_rn(hlg, lg, c);
+    }
+  }
+#undef F2
+}
+
 // block (32, 8); partials part[g][blk][NV], NV = TV_KA * V (TV energies, fp32 sums of one block's voxels
 // widened to fp64) + 3 * V (D0, D1, D2 in fp64)
 template <int V, int ND>
@@ -452,45 +482,94 @@ __global__ void __launch_bounds__(256, 2) k_tv_trial(Dims d, const float* __rest
       dd[V + s] = (double)df * (double)gg;
       dd[2 * V + s] = (double)gg * (double)gg;
     }
-    // phase 1: the three forms of every face (the windows die here), eps^2 folded into a
-    float fa[ND][V], fb[ND][V], fc[ND][V], wA[ND][V];
+    if (V % 2 == 0) {
+      // packed path (V = 4): slice lanes in pairs, FFMA2 / FMUL2 throughout except max and rsqrt
+      constexpr int H = V / 2 > 0 ? V / 2 : 1;
+      float2 fa[ND][H], fb[ND][H], fc[ND][H], wA2[ND][H];
+      const float2 eps22 = make_float2(eps2, eps2), m2 = make_float2(-2.0f, -2.0f);
 #pragma unroll
-    for (int A = 0; A < ND; ++A) {
-      Pack<V>::ldcg(w + A * plane, e, wA[A]);  // border faces store 0
+      for (int A = 0; A < ND; ++A) {
+        float wv[V];
+        Pack<V>::ldcg(w + A * plane, e, wv);  // border faces store 0
 #pragma unroll
-      for (int s = 0; s < V; ++s) {
-        float a, b, c;
-        face_forms<V, ND>(wf, wg, A, s, a, b, c);
-        fa[A][s] = a + eps2;
-        fb[A][s] = -2.0f * b;
-        fc[A][s] = c;
-        if (!todo[s]) wA[A][s] = 0.0f;
-      }
-    }
-    // phase 2: sum_A w_A sqrt(N0^2(t_q) + eps^2) per candidate; the "- eps sum w" part does not depend on t
-#pragma unroll
-    for (int q = 0; q < TV_KA; ++q) {
-      const float t = tp.t[min(k0 + q, CTR_MAX_ARMIJO - 1)];
-#pragma unroll
-      for (int A = 0; A < ND; ++A)
-#pragma unroll
-        for (int s = 0; s < V; ++s) {
-          const float rad = fmaxf(fmaf(t, fmaf(t, fc[A][s], fb[A][s]), fa[A][s]), 1e-30f);
-          et[q * V + s] = fmaf(wA[A][s] * rad, rsqrtf(rad), et[q * V + s]);
+        for (int hh = 0; hh < H; ++hh) {
+          float2 a, b, c;
+          face_forms2<V, ND>(wf, wg, A, hh, a, b, c);
+          fa[A][hh] = __fadd2_rn(a, eps22);
+          fb[A][hh] = __fmul2_rn(m2, b);
+          fc[A][hh] = c;
+          wA2[A][hh] = make_float2(todo[2 * hh] ? wv[2 * hh] : 0.0f, todo[2 * hh + (V > 1)] ? wv[2 * hh + (V > 1)] : 0.0f);
         }
-    }
-    {
-      float wsumv[V];
+      }
 #pragma unroll
-      for (int s = 0; s < V; ++s) {
-        wsumv[s] = 0.0f;
+      for (int q = 0; q < TV_KA; ++q) {
+        const float t = tp.t[min(k0 + q, CTR_MAX_ARMIJO - 1)];
+        const float2 t2 = make_float2(t, t);
 #pragma unroll
-        for (int A = 0; A < ND; ++A) wsumv[s] += wA[A][s];
+        for (int hh = 0; hh < H; ++hh) {
+          float2 acc2 = make_float2(0.0f, 0.0f);
 #pragma unroll
-        for (int q = 0; q < TV_KA; ++q) et[q * V + s] = fmaf(-eps, wsumv[s], et[q * V + s]);
+          for (int A = 0; A < ND; ++A) {
+            float2 rad = __ffma2_rn(t2, __ffma2_rn(t2, fc[A][hh], fb[A][hh]), fa[A][hh]);
+            rad.x = fmaxf(rad.x, 1e-30f); rad.y = fmaxf(rad.y, 1e-30f);
+            acc2 = __ffma2_rn(__fmul2_rn(wA2[A][hh], rad), make_float2(rsqrtf(rad.x), rsqrtf(rad.y)), acc2);
+          }
+          et[q * V + 2 * hh] = acc2.x;
+          et[q * V + 2 * hh + (V > 1)] = acc2.y;
+        }
+      }
+#pragma unroll
+      for (int hh = 0; hh < H; ++hh) {
+        float2 ws = make_float2(0.0f, 0.0f);
+#pragma unroll
+        for (int A = 0; A < ND; ++A) ws = __fadd2_rn(ws, wA2[A][hh]);
+#pragma unroll
+        for (int q = 0; q < TV_KA; ++q) {
+          et[q * V + 2 * hh] = fmaf(-eps, ws.x, et[q * V + 2 * hh]);
+          et[q * V + 2 * hh + (V > 1)] = fmaf(-eps, ws.y, et[q * V + 2 * hh + (V > 1)]);
+        }
+      }
+    } else {
+    // phase 1: the three forms of every face (the windows die here), eps^2 folded into a
+      float fa[ND][V], fb[ND][V], fc[ND][V], wA[ND][V];
+  #pragma unroll
+      for (int A = 0; A < ND; ++A) {
+        Pack<V>::ldcg(w + A * plane, e, wA[A]);  // border faces store 0
+  #pragma unroll
+        for (int s = 0; s < V; ++s) {
+          float a, b, c;
+          face_forms<V, ND>(wf, wg, A, s, a, b, c);
+          fa[A][s] = a + eps2;
+          fb[A][s] = -2.0f * b;
+          fc[A][s] = c;
+          if (!todo[s]) wA[A][s] = 0.0f;
+        }
+      }
+      // phase 2: sum_A w_A sqrt(N0^2(t_q) + eps^2) per candidate; the "- eps sum w" part does not depend on t
+  #pragma unroll
+      for (int q = 0; q < TV_KA; ++q) {
+        const float t = tp.t[min(k0 + q, CTR_MAX_ARMIJO - 1)];
+  #pragma unroll
+        for (int A = 0; A < ND; ++A)
+  #pragma unroll
+          for (int s = 0; s < V; ++s) {
+            const float rad = fmaxf(fmaf(t, fmaf(t, fc[A][s], fb[A][s]), fa[A][s]), 1e-30f);
+            et[q * V + s] = fmaf(wA[A][s] * rad, rsqrtf(rad), et[q * V + s]);
+          }
+      }
+      {
+        float wsumv[V];
+  #pragma unroll
+        for (int s = 0; s < V; ++s) {
+          wsumv[s] = 0.0f;
+  #pragma unroll
+          for (int A = 0; A < ND; ++A) wsumv[s] += wA[A][s];
+  #pragma unroll
+          for (int q = 0; q < TV_KA; ++q) et[q * V + s] = fmaf(-eps, wsumv[s], et[q * V + s]);
+        }
       }
     }
-  }
+    }
   // block reduction. TV energies: fp32 column sums over the 32 lanes of a warp through shared memory (32
   // values per round, transposed so that lane q adds value q of all lanes in lane order), then fp64.
 #pragma unroll
