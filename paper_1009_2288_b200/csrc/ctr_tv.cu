@@ -97,18 +97,22 @@ __device__ __forceinline__ float2 face_n0sq2(const Window<V, ND>& w, int A, int 
   return n0;
 }
 
-// thread -> voxel mapping shared by all stencil kernels: block (32,4), grid (nx/32, ny/4 * nz, G)
+// thread -> voxel mapping shared by all stencil kernels: block (32,4), grid (nx/32, ny/(4 TV_ROWS) * nz, G);
+// a block sweeps TV_ROWS groups of 4 image rows (rr = 0..TV_ROWS-1), so that its fixed costs - zeroing and
+// flushing a shared histogram, a block-wide reduction of fp64 sums - are paid once per 32 x 4 TV_ROWS voxels
+// (they were most of the instructions of these kernels when a block handled 32 x 4 voxels only)
+#define TV_ROWS 4
 struct Vox {
   int i, j, k, g, tid;
   bool active;
   unsigned blk, nblk;
 };
-__device__ __forceinline__ Vox vox_of_thread(const Dims& d) {
+__device__ __forceinline__ Vox vox_of_thread(const Dims& d, int rr) {
   Vox v;
-  const int nby = (d.ny + 3) / 4;
+  const int nby = (d.ny + 4 * TV_ROWS - 1) / (4 * TV_ROWS);
   v.i = blockIdx.x * 32 + threadIdx.x;
   v.k = blockIdx.y / nby;
-  v.j = (blockIdx.y - v.k * nby) * 4 + threadIdx.y;
+  v.j = ((blockIdx.y - v.k * nby) * TV_ROWS + rr) * 4 + threadIdx.y;
   v.g = blockIdx.z;
   v.tid = threadIdx.y * 32 + threadIdx.x;
   v.active = v.i < d.nx && v.j < d.ny;
@@ -116,7 +120,9 @@ __device__ __forceinline__ Vox vox_of_thread(const Dims& d) {
   v.nblk = gridDim.x * gridDim.y;
   return v;
 }
-static dim3 vox_grid(const Dims& d) { return dim3((d.nx + 31) / 32, ((d.ny + 3) / 4) * d.nz, d.G); }
+static dim3 vox_grid(const Dims& d) {
+  return dim3((d.nx + 31) / 32, ((d.ny + 4 * TV_ROWS - 1) / (4 * TV_ROWS)) * d.nz, d.G);
+}
 
 // ---------------------------------------------------------------------------------------------
 // a4.1  faces: N0^2 of the ND faces owned by each voxel (towards +x, +y, +z) -> n0 planes, plus the
@@ -135,10 +141,12 @@ template <int V, int ND>
 __global__ void __launch_bounds__(128) k_tv_faces(Dims d, const float* __restrict__ f, float* __restrict__ n0,
                                                   unsigned* __restrict__ hist) {
   __shared__ unsigned hs[V][2048];
-  const Vox p = vox_of_thread(d);
-  for (int t = p.tid; t < V * 2048; t += 128) (&hs[0][0])[t] = 0;
+  const int tid0 = threadIdx.y * 32 + threadIdx.x;
+  for (int t = tid0; t < V * 2048; t += 128) (&hs[0][0])[t] = 0;
   __syncthreads();
   const int lim[3] = {d.nx - 1, d.ny - 1, d.nz - 1};
+  for (int rr = 0; rr < TV_ROWS; ++rr) {
+  const Vox p = vox_of_thread(d, rr);
   const int pos[3] = {p.i, p.j, p.k};
   float val[ND][V];
   if (p.active) {
@@ -169,10 +177,11 @@ __global__ void __launch_bounds__(128) k_tv_faces(Dims d, const float* __restric
 #pragma unroll
     for (int s = 0; s < V; ++s) hist_add(hs[s], valid ? __float_as_uint(val[A][s]) : 0u, 20, 2047u, valid);
   }
+  }  // rr
   __syncthreads();
-  for (int t = p.tid; t < V * 2048; t += 128) {
+  for (int t = tid0; t < V * 2048; t += 128) {
     const unsigned c = (&hs[0][0])[t];
-    if (c) atomicAdd(&hist[(size_t)(p.g * V + t / 2048) * 2048 + (t & 2047)], c);
+    if (c) atomicAdd(&hist[(size_t)(blockIdx.z * V + t / 2048) * 2048 + (t & 2047)], c);
   }
 }
 
@@ -182,14 +191,16 @@ template <int V, int ND>
 __global__ void __launch_bounds__(128) k_tv_hist(Dims d, const float* __restrict__ n0, unsigned* __restrict__ hist,
                                                  Scal sc, int shift, unsigned mask, int prefix_shift) {
   __shared__ unsigned hs[V][1024];
-  const Vox p = vox_of_thread(d);
-  for (int t = p.tid; t < V * 1024; t += 128) (&hs[0][0])[t] = 0;
+  const int tid0 = threadIdx.y * 32 + threadIdx.x;
+  for (int t = tid0; t < V * 1024; t += 128) (&hs[0][0])[t] = 0;
   __syncthreads();
   const int lim[3] = {d.nx - 1, d.ny - 1, d.nz - 1};
-  const int pos[3] = {p.i, p.j, p.k};
   unsigned pre[V];
 #pragma unroll
-  for (int s = 0; s < V; ++s) pre[s] = sc.sel_prefix[p.g * V + s] >> prefix_shift;
+  for (int s = 0; s < V; ++s) pre[s] = sc.sel_prefix[blockIdx.z * V + s] >> prefix_shift;
+  for (int rr = 0; rr < TV_ROWS; ++rr) {
+  const Vox p = vox_of_thread(d, rr);
+  const int pos[3] = {p.i, p.j, p.k};
   const size_t e = (size_t)p.g * d.npix + ((size_t)p.k * d.ny + p.j) * d.nx + p.i;
 #pragma unroll
   for (int A = 0; A < ND; ++A) {
@@ -209,10 +220,11 @@ __global__ void __launch_bounds__(128) k_tv_hist(Dims d, const float* __restrict
 #pragma unroll
     for (int s = 0; s < V; ++s) hist_add(hs[s], bits[s], shift, mask, valid[s]);
   }
+  }  // rr
   __syncthreads();
-  for (int t = p.tid; t < V * 1024; t += 128) {
+  for (int t = tid0; t < V * 1024; t += 128) {
     const unsigned c = (&hs[0][0])[t];
-    if (c) atomicAdd(&hist[(size_t)(p.g * V + t / 1024) * 2048 + (t & 1023)], c);
+    if (c) atomicAdd(&hist[(size_t)(blockIdx.z * V + t / 1024) * 2048 + (t & 1023)], c);
   }
 }
 
@@ -265,14 +277,15 @@ __global__ void __launch_bounds__(256) k_tv_select(Scal sc, unsigned* __restrict
 template <int V, int ND>
 __global__ void __launch_bounds__(128) k_tv_weights(Dims d, const float* __restrict__ n0, float* __restrict__ w,
                                                     Scal sc, int mode) {
-  const Vox p = vox_of_thread(d);
-  if (!p.active) return;
+  float inv[V];
+#pragma unroll
+  for (int s = 0; s < V; ++s) inv[s] = -1.0f / sc.sigma2[blockIdx.z * V + s];
+  for (int rr = 0; rr < TV_ROWS; ++rr) {
+  const Vox p = vox_of_thread(d, rr);
+  if (!p.active) continue;
   const int lim[3] = {d.nx - 1, d.ny - 1, d.nz - 1};
   const int pos[3] = {p.i, p.j, p.k};
   const size_t e = (size_t)p.g * d.npix + ((size_t)p.k * d.ny + p.j) * d.nx + p.i;
-  float inv[V];
-#pragma unroll
-  for (int s = 0; s < V; ++s) inv[s] = -1.0f / sc.sigma2[p.g * V + s];
 #pragma unroll
   for (int A = 0; A < ND; ++A) {
     float val[V], o[V];
@@ -281,6 +294,7 @@ __global__ void __launch_bounds__(128) k_tv_weights(Dims d, const float* __restr
     for (int s = 0; s < V; ++s) o[s] = pos[A] < lim[A] ? (mode == 1 ? 1.0f : expf(val[s] * inv[s])) : 0.0f;
     Pack<V>::st(w + (size_t)A * d.G * d.npix * V, e, o);
   }
+  }  // rr
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -295,10 +309,11 @@ __global__ void __launch_bounds__(128) k_tv_gradient(Dims d, const float* __rest
                                                      const float* __restrict__ w, const float* __restrict__ n0st,
                                                      float* __restrict__ gout, TvParams tp, Scal sc, double* part,
                                                      unsigned* counter) {
-  const Vox p = vox_of_thread(d);
   double red[2 * V];
 #pragma unroll
   for (int s = 0; s < 2 * V; ++s) red[s] = 0.0;
+  for (int rr = 0; rr < TV_ROWS; ++rr) {
+  const Vox p = vox_of_thread(d, rr);
   if (p.active) {
     Window<V, ND> win;
     load_window<V, ND>(d, f, p.g, p.i, p.j, p.k, win);
@@ -351,10 +366,12 @@ __global__ void __launch_bounds__(128) k_tv_gradient(Dims d, const float* __rest
 #pragma unroll
     for (int s = 0; s < V; ++s) {
       const float df = win.c[cz][1][1][s] - vv[s];
-      red[s] = (double)gv[s] * (double)gv[s];
-      red[V + s] = 0.5 * (double)tp.lambda * (double)df * (double)df + (double)etv[s] / (double)ND;
+      red[s] += (double)gv[s] * (double)gv[s];
+      red[V + s] += 0.5 * (double)tp.lambda * (double)df * (double)df + (double)etv[s] / (double)ND;
     }
   }
+  }  // rr
+  const Vox p = vox_of_thread(d, 0);
   grid_reduce<2 * V>(red, part + (size_t)p.g * p.nblk * 2 * V, counter + p.g, p.nblk, p.blk, p.tid, 128,
                      [&](double(&sum)[2 * V]) {
 #pragma unroll
@@ -378,6 +395,7 @@ __global__ void __launch_bounds__(128) k_tv_gradient(Dims d, const float* __rest
 // E(f - t_k g) with w frozen (O9) is assembled in fp64 by k_tv_trial_finish, which takes the first k with
 // E <= E0 - c t_k |g|^2. Slices that accepted a step in an earlier pass are skipped.
 // ---------------------------------------------------------------------------------------------
+#define TV_TROWS 2
 #define TV_KA 8 /* candidates per pass; k <= 5 in every sweep seen, a later pass covers the rest (6 measured no faster) */
 
 // the linear forms of A3 on the face between the centre cell and its +A neighbour,
@@ -447,13 +465,11 @@ __global__ void __launch_bounds__(256, 2) k_tv_trial(Dims d, const float* __rest
   constexpr int NE = TV_KA * V, NV = NE + 3 * V;
   __shared__ float colsum[8][32][33];
   __shared__ double wsum[8][NV];
-  const int nby = (d.ny + 7) / 8;
+  const int nby = (d.ny + 8 * TV_TROWS - 1) / (8 * TV_TROWS);
   const int i = blockIdx.x * 32 + threadIdx.x;
   const int k = blockIdx.y / nby;
-  const int j = (blockIdx.y - k * nby) * 8 + threadIdx.y;
   const int g = blockIdx.z;
   const int lane = threadIdx.x, wid = threadIdx.y, tid = wid * 32 + lane;
-  const bool active = i < d.nx && j < d.ny;
   const unsigned blk = blockIdx.y * gridDim.x + blockIdx.x, nblk = gridDim.x * gridDim.y;
   bool todo[V], any = false;
 #pragma unroll
@@ -465,6 +481,9 @@ __global__ void __launch_bounds__(256, 2) k_tv_trial(Dims d, const float* __rest
   for (int q = 0; q < NE; ++q) et[q] = 0.0f;
 #pragma unroll
   for (int q = 0; q < 3 * V; ++q) dd[q] = 0.0;
+  for (int rr = 0; rr < TV_TROWS; ++rr) {  // a block sweeps TV_TROWS groups of 8 rows: one reduction for all
+  const int j = ((blockIdx.y - k * nby) * TV_TROWS + rr) * 8 + threadIdx.y;
+  const bool active = i < d.nx && j < d.ny;
   if (active) {
     Window<V, ND> wf, wg;
     load_window<V, ND>(d, f, g, i, j, k, wf);
@@ -478,9 +497,9 @@ __global__ void __launch_bounds__(256, 2) k_tv_trial(Dims d, const float* __rest
 #pragma unroll
     for (int s = 0; s < V; ++s) {
       const float df = wf.c[cz][1][1][s] - vv[s], gg = wg.c[cz][1][1][s];
-      dd[s] = (double)df * (double)df;
-      dd[V + s] = (double)df * (double)gg;
-      dd[2 * V + s] = (double)gg * (double)gg;
+      dd[s] += (double)df * (double)df;
+      dd[V + s] += (double)df * (double)gg;
+      dd[2 * V + s] += (double)gg * (double)gg;
     }
     if (V % 2 == 0) {
       // packed path (V = 4): slice lanes in pairs, FFMA2 / FMUL2 throughout except max and rsqrt
@@ -514,8 +533,8 @@ __global__ void __launch_bounds__(256, 2) k_tv_trial(Dims d, const float* __rest
             rad.x = fmaxf(rad.x, 1e-30f); rad.y = fmaxf(rad.y, 1e-30f);
             acc2 = __ffma2_rn(__fmul2_rn(wA2[A][hh], rad), make_float2(rsqrtf(rad.x), rsqrtf(rad.y)), acc2);
           }
-          et[q * V + 2 * hh] = acc2.x;
-          et[q * V + 2 * hh + (V > 1)] = acc2.y;
+          et[q * V + 2 * hh] += acc2.x;
+          et[q * V + 2 * hh + (V > 1)] += acc2.y;
         }
       }
 #pragma unroll
@@ -570,6 +589,7 @@ __global__ void __launch_bounds__(256, 2) k_tv_trial(Dims d, const float* __rest
       }
     }
     }
+  }  // rr
   // block reduction. TV energies: fp32 column sums over the 32 lanes of a warp through shared memory (32
   // values per round, transposed so that lane q adds value q of all lanes in lane order), then fp64.
 #pragma unroll
@@ -759,7 +779,7 @@ static int tv_sweep_t(ctr_handle* h, float* f, const float* v, const float* w, f
   if (n0_valid) k_tv_gradient<V, ND, 1><<<grid, block, 0, st>>>(d, f, v, w, h->n0, g, tp, h->sc, h->part, h->counters + 2 * d.G);
   else k_tv_gradient<V, ND, 0><<<grid, block, 0, st>>>(d, f, v, w, h->n0, g, tp, h->sc, h->part, h->counters + 2 * d.G);
   CTR_LAUNCHED(h);
-  const dim3 tgrid((d.nx + 31) / 32, ((d.ny + 7) / 8) * d.nz, d.G), tblock(32, 8);
+  const dim3 tgrid((d.nx + 31) / 32, ((d.ny + 8 * TV_TROWS - 1) / (8 * TV_TROWS)) * d.nz, d.G), tblock(32, 8);
   for (int k0 = 0; k0 < tp.kmax; k0 += TV_KA) {
     k_tv_trial<V, ND><<<tgrid, tblock, 0, st>>>(d, f, g, v, w, tp, k0, h->sc, h->part);
     CTR_LAUNCHED(h);
