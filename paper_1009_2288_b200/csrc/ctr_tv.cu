@@ -97,22 +97,23 @@ __device__ __forceinline__ float2 face_n0sq2(const Window<V, ND>& w, int A, int 
   return n0;
 }
 
-// thread -> voxel mapping shared by all stencil kernels: block (32,4), grid (nx/32, ny/(4 TV_ROWS) * nz, G);
-// a block sweeps TV_ROWS groups of 4 image rows (rr = 0..TV_ROWS-1), so that its fixed costs - zeroing and
-// flushing a shared histogram, a block-wide reduction of fp64 sums - are paid once per 32 x 4 TV_ROWS voxels
-// (they were most of the instructions of these kernels when a block handled 32 x 4 voxels only)
-#define TV_ROWS 4
+// thread -> voxel mapping shared by all stencil kernels: block (32,4), grid (nx/32, ny/(4 rows) * nz, G);
+// a block sweeps `rows` groups of 4 image rows (rr = 0..rows-1; chosen by tv_rows() so that the grid still
+// fills the GPU), so that its fixed costs - zeroing and
+// flushing a shared histogram, a block-wide reduction of fp64 sums - are paid once per 32 x 4 rows voxels
+// (they were most of the instructions of these kernels when a block handled 32 x 4 voxels only: 4.1 -> 3.05 ms
+// of TV work per outer iteration at c4)
 struct Vox {
   int i, j, k, g, tid;
   bool active;
   unsigned blk, nblk;
 };
-__device__ __forceinline__ Vox vox_of_thread(const Dims& d, int rr) {
+__device__ __forceinline__ Vox vox_of_thread(const Dims& d, int rr, int rows) {
   Vox v;
-  const int nby = (d.ny + 4 * TV_ROWS - 1) / (4 * TV_ROWS);
+  const int nby = (d.ny + 4 * rows - 1) / (4 * rows);
   v.i = blockIdx.x * 32 + threadIdx.x;
   v.k = blockIdx.y / nby;
-  v.j = ((blockIdx.y - v.k * nby) * TV_ROWS + rr) * 4 + threadIdx.y;
+  v.j = ((blockIdx.y - v.k * nby) * rows + rr) * 4 + threadIdx.y;
   v.g = blockIdx.z;
   v.tid = threadIdx.y * 32 + threadIdx.x;
   v.active = v.i < d.nx && v.j < d.ny;
@@ -120,8 +121,16 @@ __device__ __forceinline__ Vox vox_of_thread(const Dims& d, int rr) {
   v.nblk = gridDim.x * gridDim.y;
   return v;
 }
-static dim3 vox_grid(const Dims& d) {
-  return dim3((d.nx + 31) / 32, ((d.ny + 4 * TV_ROWS - 1) / (4 * TV_ROWS)) * d.nz, d.G);
+static dim3 vox_grid(const Dims& d, int rows) {
+  return dim3((d.nx + 31) / 32, ((d.ny + 4 * rows - 1) / (4 * rows)) * d.nz, d.G);
+}
+// row groups per block: as many as leave at least ~16 blocks per SM (8 for the 256-thread trial kernel)
+static int tv_rows(const Dims& d, int rows_per_group, int max_rows, int min_blocks) {
+  const long long blocks = (long long)((d.nx + 31) / 32) * ((d.ny + rows_per_group - 1) / rows_per_group) * d.nz * d.G;
+  long long r = blocks / min_blocks;
+  if (r < 1) r = 1;
+  if (r > max_rows) r = max_rows;
+  return (int)r;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -138,15 +147,15 @@ __device__ __forceinline__ void hist_add(unsigned* hist_s, unsigned bits, int sh
 }
 
 template <int V, int ND>
-__global__ void __launch_bounds__(128) k_tv_faces(Dims d, const float* __restrict__ f, float* __restrict__ n0,
+__global__ void __launch_bounds__(128) k_tv_faces(Dims d, int rows, const float* __restrict__ f, float* __restrict__ n0,
                                                   unsigned* __restrict__ hist) {
   __shared__ unsigned hs[V][2048];
   const int tid0 = threadIdx.y * 32 + threadIdx.x;
   for (int t = tid0; t < V * 2048; t += 128) (&hs[0][0])[t] = 0;
   __syncthreads();
   const int lim[3] = {d.nx - 1, d.ny - 1, d.nz - 1};
-  for (int rr = 0; rr < TV_ROWS; ++rr) {
-  const Vox p = vox_of_thread(d, rr);
+  for (int rr = 0; rr < rows; ++rr) {
+  const Vox p = vox_of_thread(d, rr, rows);
   const int pos[3] = {p.i, p.j, p.k};
   float val[ND][V];
   if (p.active) {
@@ -188,7 +197,7 @@ __global__ void __launch_bounds__(128) k_tv_faces(Dims d, const float* __restric
 // a4.2  later radix passes over the stored N0^2 planes: only values whose higher bits equal the
 // prefix found so far are counted.
 template <int V, int ND>
-__global__ void __launch_bounds__(128) k_tv_hist(Dims d, const float* __restrict__ n0, unsigned* __restrict__ hist,
+__global__ void __launch_bounds__(128) k_tv_hist(Dims d, int rows, const float* __restrict__ n0, unsigned* __restrict__ hist,
                                                  Scal sc, int shift, unsigned mask, int prefix_shift) {
   __shared__ unsigned hs[V][1024];
   const int tid0 = threadIdx.y * 32 + threadIdx.x;
@@ -198,8 +207,8 @@ __global__ void __launch_bounds__(128) k_tv_hist(Dims d, const float* __restrict
   unsigned pre[V];
 #pragma unroll
   for (int s = 0; s < V; ++s) pre[s] = sc.sel_prefix[blockIdx.z * V + s] >> prefix_shift;
-  for (int rr = 0; rr < TV_ROWS; ++rr) {
-  const Vox p = vox_of_thread(d, rr);
+  for (int rr = 0; rr < rows; ++rr) {
+  const Vox p = vox_of_thread(d, rr, rows);
   const int pos[3] = {p.i, p.j, p.k};
   const size_t e = (size_t)p.g * d.npix + ((size_t)p.k * d.ny + p.j) * d.nx + p.i;
 #pragma unroll
@@ -275,13 +284,13 @@ __global__ void __launch_bounds__(256) k_tv_select(Scal sc, unsigned* __restrict
 
 // a4.4  w = exp(-N0^2/sigma^2) on interior faces, 0 on border faces; TV mode: 1
 template <int V, int ND>
-__global__ void __launch_bounds__(128) k_tv_weights(Dims d, const float* __restrict__ n0, float* __restrict__ w,
+__global__ void __launch_bounds__(128) k_tv_weights(Dims d, int rows, const float* __restrict__ n0, float* __restrict__ w,
                                                     Scal sc, int mode) {
   float inv[V];
 #pragma unroll
   for (int s = 0; s < V; ++s) inv[s] = -1.0f / sc.sigma2[blockIdx.z * V + s];
-  for (int rr = 0; rr < TV_ROWS; ++rr) {
-  const Vox p = vox_of_thread(d, rr);
+  for (int rr = 0; rr < rows; ++rr) {
+  const Vox p = vox_of_thread(d, rr, rows);
   if (!p.active) continue;
   const int lim[3] = {d.nx - 1, d.ny - 1, d.nz - 1};
   const int pos[3] = {p.i, p.j, p.k};
@@ -305,15 +314,15 @@ __global__ void __launch_bounds__(128) k_tv_weights(Dims d, const float* __restr
 // update of the same sweep has just produced them); N0ST = 0: recomputed from the window (ctr_eptv_step,
 // where the caller's x need not be the image of the last weight update).
 template <int V, int ND, int N0ST>
-__global__ void __launch_bounds__(128) k_tv_gradient(Dims d, const float* __restrict__ f, const float* __restrict__ v,
+__global__ void __launch_bounds__(128) k_tv_gradient(Dims d, int rows, const float* __restrict__ f, const float* __restrict__ v,
                                                      const float* __restrict__ w, const float* __restrict__ n0st,
                                                      float* __restrict__ gout, TvParams tp, Scal sc, double* part,
                                                      unsigned* counter) {
   double red[2 * V];
 #pragma unroll
   for (int s = 0; s < 2 * V; ++s) red[s] = 0.0;
-  for (int rr = 0; rr < TV_ROWS; ++rr) {
-  const Vox p = vox_of_thread(d, rr);
+  for (int rr = 0; rr < rows; ++rr) {
+  const Vox p = vox_of_thread(d, rr, rows);
   if (p.active) {
     Window<V, ND> win;
     load_window<V, ND>(d, f, p.g, p.i, p.j, p.k, win);
@@ -371,7 +380,7 @@ __global__ void __launch_bounds__(128) k_tv_gradient(Dims d, const float* __rest
     }
   }
   }  // rr
-  const Vox p = vox_of_thread(d, 0);
+  const Vox p = vox_of_thread(d, 0, rows);
   grid_reduce<2 * V>(red, part + (size_t)p.g * p.nblk * 2 * V, counter + p.g, p.nblk, p.blk, p.tid, 128,
                      [&](double(&sum)[2 * V]) {
 #pragma unroll
@@ -395,7 +404,6 @@ __global__ void __launch_bounds__(128) k_tv_gradient(Dims d, const float* __rest
 // E(f - t_k g) with w frozen (O9) is assembled in fp64 by k_tv_trial_finish, which takes the first k with
 // E <= E0 - c t_k |g|^2. Slices that accepted a step in an earlier pass are skipped.
 // ---------------------------------------------------------------------------------------------
-#define TV_TROWS 2
 #define TV_KA 8 /* candidates per pass; k <= 5 in every sweep seen, a later pass covers the rest (6 measured no faster) */
 
 // the linear forms of A3 on the face between the centre cell and its +A neighbour,
@@ -459,13 +467,13 @@ __device__ __forceinline__ void face_forms2(const Window<V, ND>& wf, const Windo
 // block (32, 8); partials part[g][blk][NV], NV = TV_KA * V (TV energies, fp32 sums of one block's voxels
 // widened to fp64) + 3 * V (D0, D1, D2 in fp64)
 template <int V, int ND>
-__global__ void __launch_bounds__(256, 2) k_tv_trial(Dims d, const float* __restrict__ f, const float* __restrict__ gin,
+__global__ void __launch_bounds__(256, 2) k_tv_trial(Dims d, int rows, const float* __restrict__ f, const float* __restrict__ gin,
                                                   const float* __restrict__ v, const float* __restrict__ w, TvParams tp,
                                                   int k0, Scal sc, double* part) {
   constexpr int NE = TV_KA * V, NV = NE + 3 * V;
   __shared__ float colsum[8][32][33];
   __shared__ double wsum[8][NV];
-  const int nby = (d.ny + 8 * TV_TROWS - 1) / (8 * TV_TROWS);
+  const int nby = (d.ny + 8 * rows - 1) / (8 * rows);
   const int i = blockIdx.x * 32 + threadIdx.x;
   const int k = blockIdx.y / nby;
   const int g = blockIdx.z;
@@ -481,8 +489,8 @@ __global__ void __launch_bounds__(256, 2) k_tv_trial(Dims d, const float* __rest
   for (int q = 0; q < NE; ++q) et[q] = 0.0f;
 #pragma unroll
   for (int q = 0; q < 3 * V; ++q) dd[q] = 0.0;
-  for (int rr = 0; rr < TV_TROWS; ++rr) {  // a block sweeps TV_TROWS groups of 8 rows: one reduction for all
-  const int j = ((blockIdx.y - k * nby) * TV_TROWS + rr) * 8 + threadIdx.y;
+  for (int rr = 0; rr < rows; ++rr) {  // a block sweeps `rows` groups of 8 rows: one reduction for all
+  const int j = ((blockIdx.y - k * nby) * rows + rr) * 8 + threadIdx.y;
   const bool active = i < d.nx && j < d.ny;
   if (active) {
     Window<V, ND> wf, wg;
@@ -719,31 +727,32 @@ static ctr_sweep_stat* stat_slot(ctr_handle* h) {
 template <int V, int ND>
 static int tv_update_weights_t(ctr_handle* h, const float* f, float* w, cudaStream_t st) {
   const Dims& d = h->d;
-  const dim3 grid = vox_grid(d), block(32, 4);
+  const int rows = tv_rows(d, 4, 8, 148 * 16);
+  const dim3 grid = vox_grid(d, rows), block(32, 4);
   const int Bp = d.G * d.V;
   const float eps2 = h->p.eps * h->p.eps;
   ctr_sweep_stat* rec = stat_slot(h);
   ProfScope prof(h, CTR_PROF_TV, st);
   if (h->p.weights_mode == 1) {
     // plain TV: weights are 1; sigma is not needed (reported as 0)
-    k_tv_faces<V, ND><<<grid, block, 0, st>>>(d, f, h->n0, h->hist);
+    k_tv_faces<V, ND><<<grid, block, 0, st>>>(d, rows, f, h->n0, h->hist);
     CTR_LAUNCHED(h);
     CTR_CUDA(h, cudaMemsetAsync(h->hist, 0, sizeof(unsigned) * 2048 * Bp, st));
   } else {
-    k_tv_faces<V, ND><<<grid, block, 0, st>>>(d, f, h->n0, h->hist);
+    k_tv_faces<V, ND><<<grid, block, 0, st>>>(d, rows, f, h->n0, h->hist);
     CTR_LAUNCHED(h);
     k_tv_select<<<Bp, 256, 0, st>>>(h->sc, h->hist, 2048, 20, 1, 0, h->sel_k, eps2, rec, Bp);
     CTR_LAUNCHED(h);
-    k_tv_hist<V, ND><<<grid, block, 0, st>>>(d, h->n0, h->hist, h->sc, 10, 1023u, 20);
+    k_tv_hist<V, ND><<<grid, block, 0, st>>>(d, rows, h->n0, h->hist, h->sc, 10, 1023u, 20);
     CTR_LAUNCHED(h);
     k_tv_select<<<Bp, 256, 0, st>>>(h->sc, h->hist, 1024, 10, 0, 0, 0, eps2, rec, Bp);
     CTR_LAUNCHED(h);
-    k_tv_hist<V, ND><<<grid, block, 0, st>>>(d, h->n0, h->hist, h->sc, 0, 1023u, 10);
+    k_tv_hist<V, ND><<<grid, block, 0, st>>>(d, rows, h->n0, h->hist, h->sc, 0, 1023u, 10);
     CTR_LAUNCHED(h);
     k_tv_select<<<Bp, 256, 0, st>>>(h->sc, h->hist, 1024, 0, 0, 1, 0, eps2, rec, Bp);
     CTR_LAUNCHED(h);
   }
-  k_tv_weights<V, ND><<<grid, block, 0, st>>>(d, h->n0, w, h->sc, h->p.weights_mode);
+  k_tv_weights<V, ND><<<grid, block, 0, st>>>(d, rows, h->n0, w, h->sc, h->p.weights_mode);
   CTR_LAUNCHED(h);
   return CTR_OK;
 }
@@ -772,16 +781,18 @@ template <int V, int ND>
 static int tv_sweep_t(ctr_handle* h, float* f, const float* v, const float* w, float lambda, int clamp,
                       int n0_valid, cudaStream_t st) {
   const Dims& d = h->d;
-  const dim3 grid = vox_grid(d), block(32, 4);
+  const int rows = tv_rows(d, 4, 8, 148 * 16);
+  const dim3 grid = vox_grid(d, rows), block(32, 4);
   const TvParams tp = make_tv_params(h, lambda);
   float* g = h->gimg;
   ProfScope prof(h, CTR_PROF_TV, st);
-  if (n0_valid) k_tv_gradient<V, ND, 1><<<grid, block, 0, st>>>(d, f, v, w, h->n0, g, tp, h->sc, h->part, h->counters + 2 * d.G);
-  else k_tv_gradient<V, ND, 0><<<grid, block, 0, st>>>(d, f, v, w, h->n0, g, tp, h->sc, h->part, h->counters + 2 * d.G);
+  if (n0_valid) k_tv_gradient<V, ND, 1><<<grid, block, 0, st>>>(d, rows, f, v, w, h->n0, g, tp, h->sc, h->part, h->counters + 2 * d.G);
+  else k_tv_gradient<V, ND, 0><<<grid, block, 0, st>>>(d, rows, f, v, w, h->n0, g, tp, h->sc, h->part, h->counters + 2 * d.G);
   CTR_LAUNCHED(h);
-  const dim3 tgrid((d.nx + 31) / 32, ((d.ny + 8 * TV_TROWS - 1) / (8 * TV_TROWS)) * d.nz, d.G), tblock(32, 8);
+  const int trows = tv_rows(d, 8, 16, 148 * 8);
+  const dim3 tgrid((d.nx + 31) / 32, ((d.ny + 8 * trows - 1) / (8 * trows)) * d.nz, d.G), tblock(32, 8);
   for (int k0 = 0; k0 < tp.kmax; k0 += TV_KA) {
-    k_tv_trial<V, ND><<<tgrid, tblock, 0, st>>>(d, f, g, v, w, tp, k0, h->sc, h->part);
+    k_tv_trial<V, ND><<<tgrid, tblock, 0, st>>>(d, trows, f, g, v, w, tp, k0, h->sc, h->part);
     CTR_LAUNCHED(h);
     k_tv_trial_finish<V><<<d.G, 1024, 0, st>>>(h->part, (int)(tgrid.x * tgrid.y), tp, k0, d.ndim, h->sc);
     CTR_LAUNCHED(h);
