@@ -208,13 +208,13 @@ __global__ void __launch_bounds__(256) k_img_update(size_t nl, int LQ, size_t ni
 //   FIN_COEF   N = (NB+1) V: c_i = <b_i, g> (S24) and gamma' = ||g||^2 - sum_i c_i^2 = ||g - sum c_i b_i||^2,
 //                            beta = gamma'/gamma, 1/sqrt(gamma')               (App. I step 4, :432)
 template <int N>
-__global__ void __launch_bounds__(256) k_finish(int mode, const double* __restrict__ part, int nblk, int LQ, int V,
+__global__ void __launch_bounds__(1024) k_finish(int mode, const double* __restrict__ part, int nblk, int LQ, int V,
                                                 int i0, int nb, int Bp, int first, Scal sc) {
-  __shared__ double sm[256];
+  __shared__ double sm[1024];
   __shared__ double tot[N];
   const int q = blockIdx.x, gs = blockIdx.y, t = threadIdx.x;
   const int n = t % N, b0 = t / N;
-  constexpr int NB0 = 256 / N;
+  constexpr int NB0 = 1024 / N;  // block rows: 1024 threads keep the chain of dependent loads short
   double acc = 0.0;
   const double* p = part + ((size_t)gs * nblk * LQ + q) * N + n;
   if (b0 < NB0) {
@@ -257,10 +257,10 @@ int reduce_finish(ctr_handle* h, int mode, int N, int nblk, int i0, int nb, int 
   dim3 grid(d.LQ, d.GS);
   const int Bp = d.G * d.V;
   switch (N) {
-    case 1: k_finish<1><<<grid, 256, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
-    case 4: k_finish<4><<<grid, 256, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
-    case 5: k_finish<5><<<grid, 256, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
-    default: k_finish<20><<<grid, 256, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
+    case 1: k_finish<1><<<grid, 1024, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
+    case 4: k_finish<4><<<grid, 1024, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
+    case 5: k_finish<5><<<grid, 1024, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
+    default: k_finish<20><<<grid, 1024, 0, st>>>(mode, h->part, nblk, d.LQ, d.V, i0, nb, Bp, first, h->sc); break;
   }
   CTR_LAUNCHED(h);
   return CTR_OK;
