@@ -535,7 +535,7 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
     size_t nblk = nblk_tv > nblk_p ? nblk_tv : nblk_p;
     h->part_len = (size_t)d.G * nblk * 8 * d.V;
     // Armijo trial pass: [G][blocks of 32 x 8 voxels][16 V + 3 V]
-    size_t need_t = (size_t)d.G * ((size_t)((d.nx + 31) / 32) * ((d.ny + 7) / 8) * d.nz) * 19 * d.V;
+    size_t need_t = (size_t)d.G * ((size_t)((d.nx + 31) / 32) * ((d.ny + 3) / 4) * d.nz) * 19 * d.V;  // >= 4 rows per block
     if (need_t > h->part_len) h->part_len = need_t;
     // segmented reductions of the CGLS kernels: [GS][blocks][LQ][N] with N <= 8 * V
     size_t nblk_f = ((size_t)d.nray + 8 * (32 / d.LQ) - 1) / (8 * (32 / d.LQ));

@@ -466,14 +466,20 @@ __device__ __forceinline__ void face_forms2(const Window<V, ND>& wf, const Windo
 
 // block (32, 8); partials part[g][blk][NV], NV = TV_KA * V (TV energies, fp32 sums of one block's voxels
 // widened to fp64) + 3 * V (D0, D1, D2 in fp64)
+#ifndef TV_TW
+#define TV_TW 4 /* warps (rows of 32 voxels) per block of the trial kernel; (4, 3) measured best of (4,3) (4,4) (8,2) */
+#endif
+#ifndef TV_TMINB
+#define TV_TMINB 3
+#endif
 template <int V, int ND>
-__global__ void __launch_bounds__(256, 2) k_tv_trial(Dims d, int rows, const float* __restrict__ f, const float* __restrict__ gin,
+__global__ void __launch_bounds__(32 * TV_TW, TV_TMINB) k_tv_trial(Dims d, int rows, const float* __restrict__ f, const float* __restrict__ gin,
                                                   const float* __restrict__ v, const float* __restrict__ w, TvParams tp,
                                                   int k0, Scal sc, double* part) {
   constexpr int NE = TV_KA * V, NV = NE + 3 * V;
-  __shared__ float colsum[8][32][33];
-  __shared__ double wsum[8][NV];
-  const int nby = (d.ny + 8 * rows - 1) / (8 * rows);
+  __shared__ float colsum[TV_TW][32][33];
+  __shared__ double wsum[TV_TW][NV];
+  const int nby = (d.ny + TV_TW * rows - 1) / (TV_TW * rows);
   const int i = blockIdx.x * 32 + threadIdx.x;
   const int k = blockIdx.y / nby;
   const int g = blockIdx.z;
@@ -490,7 +496,7 @@ __global__ void __launch_bounds__(256, 2) k_tv_trial(Dims d, int rows, const flo
 #pragma unroll
   for (int q = 0; q < 3 * V; ++q) dd[q] = 0.0;
   for (int rr = 0; rr < rows; ++rr) {  // a block sweeps `rows` groups of 8 rows: one reduction for all
-  const int j = ((blockIdx.y - k * nby) * rows + rr) * 8 + threadIdx.y;
+  const int j = ((blockIdx.y - k * nby) * rows + rr) * TV_TW + threadIdx.y;
   const bool active = i < d.nx && j < d.ny;
   if (active) {
     Window<V, ND> wf, wg;
@@ -623,7 +629,7 @@ __global__ void __launch_bounds__(256, 2) k_tv_trial(Dims d, int rows, const flo
   if (tid < NV) {
     double t = 0.0;
 #pragma unroll
-    for (int ww = 0; ww < 8; ++ww) t += wsum[ww][tid];
+    for (int ww = 0; ww < TV_TW; ++ww) t += wsum[ww][tid];
     part[((size_t)g * nblk + blk) * NV + tid] = t;
   }
 }
@@ -789,8 +795,8 @@ static int tv_sweep_t(ctr_handle* h, float* f, const float* v, const float* w, f
   if (n0_valid) k_tv_gradient<V, ND, 1><<<grid, block, 0, st>>>(d, rows, f, v, w, h->n0, g, tp, h->sc, h->part, h->counters + 2 * d.G);
   else k_tv_gradient<V, ND, 0><<<grid, block, 0, st>>>(d, rows, f, v, w, h->n0, g, tp, h->sc, h->part, h->counters + 2 * d.G);
   CTR_LAUNCHED(h);
-  const int trows = tv_rows(d, 8, 16, 148 * 8);
-  const dim3 tgrid((d.nx + 31) / 32, ((d.ny + 8 * trows - 1) / (8 * trows)) * d.nz, d.G), tblock(32, 8);
+  const int trows = tv_rows(d, TV_TW, 16, 148 * 8);
+  const dim3 tgrid((d.nx + 31) / 32, ((d.ny + TV_TW * trows - 1) / (TV_TW * trows)) * d.nz, d.G), tblock(32, TV_TW);
   for (int k0 = 0; k0 < tp.kmax; k0 += TV_KA) {
     k_tv_trial<V, ND><<<tgrid, tblock, 0, st>>>(d, trows, f, g, v, w, tp, k0, h->sc, h->part);
     CTR_LAUNCHED(h);
