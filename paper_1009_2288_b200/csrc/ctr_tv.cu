@@ -11,6 +11,13 @@
 
 namespace ctr {
 
+#ifndef TV_GMINB
+#define TV_GMINB 8 /* min blocks per SM of k_tv_gradient (register budget) */
+#endif
+#ifndef TV_FMINB
+#define TV_FMINB 6 /* same for k_tv_faces */
+#endif
+
 
 // ---------------------------------------------------------------------------------------------
 // Neighbourhood access. The stencil of A2/A3 around voxel p needs f at p + {-1,0,1}^ndim minus
@@ -147,7 +154,7 @@ __device__ __forceinline__ void hist_add(unsigned* hist_s, unsigned bits, int sh
 }
 
 template <int V, int ND>
-__global__ void __launch_bounds__(128) k_tv_faces(Dims d, int rows, const float* __restrict__ f, float* __restrict__ n0,
+__global__ void __launch_bounds__(128, TV_FMINB) k_tv_faces(Dims d, int rows, const float* __restrict__ f, float* __restrict__ n0,
                                                   unsigned* __restrict__ hist) {
   __shared__ unsigned hs[V][2048];
   const int tid0 = threadIdx.y * 32 + threadIdx.x;
@@ -314,7 +321,7 @@ __global__ void __launch_bounds__(128) k_tv_weights(Dims d, int rows, const floa
 // update of the same sweep has just produced them); N0ST = 0: recomputed from the window (ctr_eptv_step,
 // where the caller's x need not be the image of the last weight update).
 template <int V, int ND, int N0ST>
-__global__ void __launch_bounds__(128) k_tv_gradient(Dims d, int rows, const float* __restrict__ f, const float* __restrict__ v,
+__global__ void __launch_bounds__(128, TV_GMINB) k_tv_gradient(Dims d, int rows, const float* __restrict__ f, const float* __restrict__ v,
                                                      const float* __restrict__ w, const float* __restrict__ n0st,
                                                      float* __restrict__ gout, TvParams tp, Scal sc, double* part,
                                                      unsigned* counter) {
