@@ -12,7 +12,9 @@ namespace ctr {
 #define CTR_MAX_ARMIJO 32
 #define CTR_STAT_SWEEPS 4096 /* ring capacity, in sweeps */
 #define CTR_PROF_MAX 32768
+#ifndef CTR_MAX_BASIS
 #define CTR_MAX_BASIS 4 /* stored unit gradients b_0..b_3 used for re-orthogonalisation (S24) */
+#endif
 #define CTR_NCOUNTERS 8
 #define CTR_REDUCE_BLOCKS 1184 /* grid cap of the grid-stride reduction kernels: 148 SMs x 8 */
 
