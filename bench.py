@@ -259,8 +259,8 @@ def main():
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the batched kernels at c4, from the committed
-# ncu --set full captures (profiles/r1h_ncu_full_c4.md); None for workloads that were not captured
-NCU_TRAFFIC_C4 = {"forward": 170.1e6, "back": 559.9e6}
+# ncu --set full captures (profiles/r1i_ncu_full_c4.md); None for workloads that were not captured
+NCU_TRAFFIC_C4 = {"forward": 170.5e6, "back": 559.0e6}
 
 
 def roofline(cfg, batch, prof, peaks):
