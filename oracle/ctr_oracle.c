@@ -14,8 +14,10 @@
  * Pins (tests/test_oracle_pins.py): P against box chords, a brute-force dense
  * matrix and analytic ellipse integrals; P^T against the dense transpose and the
  * adjoint identity; CGLS against numpy.linalg.lstsq, hand iterations and the Krylov-subspace
- * minimiser built without a CG recurrence; A2/A3 against a hand-evaluated
- * 4x4 example and invariants; sigma against a sort; Armijo against its inequality.
+ * minimiser built without a CG recurrence; A2/A3 against hand-evaluated 4x4 (2D) and
+ * 3x3x3 (3D, all three face axes) examples, direct numpy restatements of A3 on every face axis,
+ * central differences of the energy along columns of every axis (strides, 1/ndim at 3), axis
+ * permutations and invariants; sigma against a sort; Armijo against its inequality.
  * PARITY UNPINNED: A2 (orc_gradient) beyond those special cases -- it is a
  * definition, not a theorem -- and the composed orc_reconstruct result.
  *

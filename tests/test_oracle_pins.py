@@ -450,6 +450,124 @@ def test_face_mag2_3d_against_direct_numpy(orc):
     assert np.all(n0[0, :, :, -1] == 0)
 
 
+def test_hand_evaluated_3x3x3(orc):
+    """3D A2/A3 (reading S22) on a 3x3x3 volume evaluated by hand: all three face axes, both faces of every
+    axis at the centre voxel, one border-plane face, TV and EP-TV gradient at the interior voxel."""
+    gold = json.loads((GOLD / "a2_a3_3x3x3.json").read_text())
+    f = np.array(gold["volume_planes_k_then_rows_j_then_cols_i"], dtype=np.float64)   # [k, j, i]
+    assert f[1, 1, 1] == 4 and f[1, 1, 0] == 1 and f[1, 1, 2] == 2 and f[1, 0, 1] == 7 and f[0, 1, 1] == 5
+    axis = {"x": 0, "y": 1, "z": 2}
+    n0 = orc.face_mag2(f, 3)                                 # [axis, k, j, i]
+    for key, val in gold["n0sq"].items():
+        ax, i, j, k = key.split("_")
+        assert n0[axis[ax], int(k), int(j), int(i)] == pytest.approx(val, abs=1e-13), key
+    g_tv = orc.gradient(f, f, orc.weights(n0, 1.0, mode=1), lam=0.0, eps=0.0, ndim=3)
+    assert g_tv[1, 1, 1] == pytest.approx(gold["a2_tv_at_1_1_1"], abs=5e-8)
+    w = orc.weights(n0, gold["sigma"], mode=0)
+    for key, val in gold["omega"].items():
+        ax, i, j, k = key.split("_")
+        assert w[axis[ax], int(k), int(j), int(i)] == pytest.approx(val, abs=5e-9), key
+    g_ep = orc.gradient(f, f, w, lam=0.0, eps=0.0, ndim=3)
+    assert g_ep[1, 1, 1] == pytest.approx(gold["a2_eptv_at_1_1_1"], abs=5e-8)
+
+
+def _face_mag2_numpy(f, A):
+    """N0^2 of the +A faces of a volume f[k, j, i] written out directly from A3 with numpy
+    edge padding (S12); numpy axis of image axis A (0 = x, 1 = y, 2 = z) is 2 - A. Border faces excluded."""
+    na = 2 - A
+    fp = np.pad(f, 1, mode="edge")
+    lo = np.take(fp, range(0, fp.shape[na] - 1), axis=na)
+    hi = np.take(fp, range(1, fp.shape[na]), axis=na)
+    m = 0.5 * (hi + lo)                                      # face means, padded transversally
+    d = hi - lo
+    inner = [slice(1, -1)] * 3
+    inner[na] = slice(1, -1)                                 # faces between voxel p and p+1, p = 0..n-2
+    want = d[tuple(inner)] ** 2
+    c = m[tuple(inner)]
+    for T in range(3):
+        if T == A:
+            continue
+        nt = 2 - T
+        up, dn = list(inner), list(inner)
+        up[nt], dn[nt] = slice(2, None), slice(0, -2)
+        want = want + 0.5 * (m[tuple(up)] - c) ** 2 + 0.5 * (c - m[tuple(dn)]) ** 2
+    return want
+
+
+@pytest.mark.parametrize("A", [0, 1, 2])
+def test_face_mag2_3d_every_axis_against_direct_numpy(orc, A):
+    """x-, y- AND z-faces of the 3D A3 (S22): a wrong transverse axis or stride on any face axis fails here."""
+    rng = np.random.default_rng(19 + A)
+    f = rng.random((4, 5, 6))                                # [nz, ny, nx], all different
+    n0 = orc.face_mag2(f, 3)
+    want = _face_mag2_numpy(f, A)
+    sl = [slice(None)] * 3
+    sl[2 - A] = slice(0, -1)
+    assert np.allclose(n0[A][tuple(sl)], want, atol=1e-14)
+    sl[2 - A] = -1
+    assert np.all(n0[A][tuple(sl)] == 0)
+    # and the 2D routine is the 3D one on a single plane (no z terms)
+    n2 = orc.face_mag2(f[:1], 2)
+    assert np.allclose(n2[0, 0, :, :-1], _face_mag2_2d(f[0], 0), atol=1e-14)
+    assert np.allclose(n2[1, 0, :-1, :], _face_mag2_2d(f[0], 1), atol=1e-14)
+
+
+def _face_mag2_2d(f, A):
+    fp = np.pad(f, 1, mode="edge")
+    if A == 1:
+        return _face_mag2_2d(f.T, 0).T
+    m = 0.5 * (fp[:, 1:] + fp[:, :-1])[:, 1:-1]
+    d = f[:, 1:] - f[:, :-1]
+    return d ** 2 + 0.5 * (m[2:] - m[1:-1]) ** 2 + 0.5 * (m[1:-1] - m[:-2]) ** 2
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_gradient_matches_energy_derivative_on_3d_columns(orc, axis):
+    """A column along one axis of a 3D volume: the transverse terms of A3 vanish (clamped indices), so A2 is
+    the derivative of the discrete energy times ndim = 3 (E carries 1/ndim, O9/S22). Pins the stride of every
+    axis, the sign of the flux difference and the 1/ndim factor at 3."""
+    rng = np.random.default_rng(24 + axis)
+    n = 9
+    shape = [1, 1, 1]
+    shape[axis] = n                                          # numpy axes [k, j, i]
+    f, v = rng.standard_normal(shape), rng.standard_normal(shape)
+    A = 2 - axis                                             # image axis of the column
+    n0 = orc.face_mag2(f, 3)
+    assert np.allclose(np.delete(n0, A, axis=0), 0.0)
+    assert np.allclose(n0[A].ravel()[:-1], np.diff(f.ravel()) ** 2, atol=1e-15)
+    w = orc.weights(n0, 1.3, mode=0)
+    eps, lam = 0.05, 0.7
+    g = orc.gradient(f, v, w, lam, eps, ndim=3).ravel()
+    g_fid = np.float32(lam) * (f - v).ravel()
+    h = 1e-6
+    for i in range(n):
+        e = np.zeros(n)
+        e[i] = h
+        e = e.reshape(shape)
+        dE_tv = (orc.energy(f + e, v, w, 0.0, eps, ndim=3) - orc.energy(f - e, v, w, 0.0, eps, ndim=3)) / (2 * h)
+        dE_fid = (orc.energy(f + e, v, 0 * w, lam, eps, ndim=3) - orc.energy(f - e, v, 0 * w, lam, eps, ndim=3)) / (2 * h)
+        assert g[i] - g_fid[i] == pytest.approx(3 * dE_tv, abs=1e-6)
+        assert g_fid[i] == pytest.approx(dE_fid, abs=1e-6)
+
+
+def test_axis_permutation_equivariance_3d(orc):
+    """Permuting the axes of the volume permutes the face planes and the gradient accordingly (S8/S22)."""
+    rng = np.random.default_rng(27)
+    f, v = rng.random((4, 5, 6)), rng.random((4, 5, 6))
+    w, sig = orc.update_weights(f, 0.9, 1e-4, 0, ndim=3)
+    g = orc.gradient(f, v, w, 0.3, 1e-4, ndim=3)
+    e0 = orc.energy(f, v, w, 0.3, 1e-4, ndim=3)
+    for perm in ((0, 2, 1), (2, 1, 0), (1, 0, 2), (1, 2, 0)):      # numpy axes [k, j, i] -> permuted
+        fp, vp = np.ascontiguousarray(f.transpose(perm)), np.ascontiguousarray(v.transpose(perm))
+        wp, sp = orc.update_weights(fp, 0.9, 1e-4, 0, ndim=3)
+        assert sp == pytest.approx(sig, rel=1e-14)
+        for A in range(3):
+            # image axis A of the permuted volume is numpy axis 2 - A, which was numpy axis perm[2 - A]
+            assert np.allclose(wp[A], w[2 - perm[2 - A]].transpose(perm), atol=1e-14)
+        assert np.allclose(orc.gradient(fp, vp, wp, 0.3, 1e-4, ndim=3), g.transpose(perm), atol=1e-13)
+        assert orc.energy(fp, vp, wp, 0.3, 1e-4, ndim=3) == pytest.approx(e0, rel=1e-13)
+
+
 # ---------------------------------------------------------------- O6: sigma
 @pytest.mark.parametrize("q", [0.5, 0.9, 0.95, 1.0, 1e-9])
 def test_sigma_is_order_statistic(orc, q):
