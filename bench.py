@@ -29,8 +29,15 @@ sys.path.insert(0, str(ROOT))
 
 from ctr_inputs import get_config, make_case, scaled_config  # noqa: E402
 
-METRIC = "EP-TV outer iters/sec at 512^2 x 60 views (slice-iterations/s: slices x outer iterations / s)"
 UNIT = "slice-iters/s"
+
+
+def metric_name(cfg):
+    if cfg.ndim == 3:
+        return (f"EP-TV outer iters/sec at {cfg.nx}x{cfg.ny}x{cfg.nz} x {cfg.nviews} views (one volume counts as one "
+                "slice: outer iterations / s)")
+    return (f"EP-TV outer iters/sec at {cfg.nx}^2 x {cfg.nviews} views (slice-iterations/s: slices x outer "
+            "iterations / s)")
 
 
 def parse():
@@ -87,31 +94,58 @@ class ClockSampler:
 
 
 def oracle_step_seconds(cfg, sino_slice, n_steps):
-    """Time the oracle AS IT STANDS on one slice: n_steps outer iterations (full n_cgls / n_gd)."""
+    """Time the oracle AS IT STANDS. 2D: n_steps outer iterations (full n_cgls / n_gd) of ONE slice; returns
+    (seconds per step of one slice, threads, description). 3D (c5: one outer iteration is ~10-20 minutes of CPU):
+    a bounded sample of the same step - P and P^T over 2 of the views of the full volume, one weight update + GD
+    sweep on 8 of the z-planes - scaled to (n_cgls + 1) applications of all views and n_gd sweeps of all planes."""
     from oracle import ctr_oracle as orc
     orc.build()
-    one = scaled_config(cfg.name, batch=1, n_outer=n_steps)
+    if cfg.ndim == 2:
+        one = scaled_config(cfg.name, batch=1, n_outer=n_steps)
+        t0 = time.perf_counter()
+        orc.reconstruct(one, sino_slice.astype(np.float64), one)
+        secs = (time.perf_counter() - t0) / n_steps
+        return secs, orc.num_threads(), (f"one slice of {cfg.batch}, {n_steps} outer iteration(s) from f = 0 at the full "
+                                         f"per-iteration schedule (n_cgls={cfg.n_cgls}, n_gd={cfg.n_gd}), {secs * n_steps:.1f} s")
+    nv_s, nz_s = 2, 8
+    sub = scaled_config(cfg.name, nviews=nv_s)             # same scanner and volume, nv_s equally spaced views
+    g = sub.geometry_dict() | {"angles": [cfg.theta0 + k * cfg.dtheta * (cfg.nviews // nv_s) for k in range(nv_s)]}
+    rng = np.random.default_rng(0)
+    x = rng.random(cfg.img_shape)
     t0 = time.perf_counter()
-    orc.reconstruct(one, sino_slice.astype(np.float64), one)
-    return time.perf_counter() - t0, orc.num_threads()
+    for _ in range(n_steps):
+        y = orc.forward(g, x)
+        orc.back(g, y)
+    t_op = (time.perf_counter() - t0) / n_steps * (cfg.nviews / nv_s) * (cfg.n_cgls + 1)
+    f = 0.02 * rng.random((nz_s, cfg.ny, cfg.nx))
+    t0 = time.perf_counter()
+    for _ in range(n_steps):
+        w, _ = orc.update_weights(f, cfg.sigma_quantile, cfg.eps, 0, ndim=3)
+        orc.eptv_step(f, f, w, cfg.lam, cfg, ndim=3)
+    t_tv = (time.perf_counter() - t0) / n_steps * (cfg.nz / nz_s) * cfg.n_gd
+    return t_op + t_tv, orc.num_threads(), (
+        f"bounded sample of one outer iteration: P + P^T over {nv_s} of {cfg.nviews} views (x{cfg.nviews // nv_s} x "
+        f"{cfg.n_cgls + 1} applications) and one weight update + GD sweep on {nz_s} of {cfg.nz} planes (x{cfg.nz // nz_s} x "
+        f"{cfg.n_gd}), extrapolated to {t_op + t_tv:.0f} s per step")
 
 
 def run_reference(args):
     """--impl reference: the oracle on the host cores, each step = one outer iteration of ONE slice of
-    the workload (a bounded sample: 1/batch of a real step)."""
+    the workload (a bounded sample: 1/batch of a real step; c5: see oracle_step_seconds)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     cfg = get_config(args.workload)
-    sino = make_case(scaled_config(args.workload, batch=1), raster=False)["sino"][0]
-    if args.warmup > 0:
-        oracle_step_seconds(cfg, sino, args.warmup)
-    secs, cores = oracle_step_seconds(cfg, sino, args.steps)
-    value = args.steps / secs
-    sample = f"1 of {cfg.batch} slices per step, full schedule per step (n_cgls={cfg.n_cgls}, n_gd={cfg.n_gd})"
+    sino = None
+    if cfg.ndim == 2:
+        sino = make_case(scaled_config(args.workload, batch=1), raster=False)["sino"][0]
+        if args.warmup > 0:
+            oracle_step_seconds(cfg, sino, args.warmup)
+    secs, cores, sample = oracle_step_seconds(cfg, sino, args.steps)
+    value = 1.0 / secs
     print(json.dumps({
-        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps,
+        "impl": "reference", "metric": metric_name(cfg), "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": workload_config(cfg, cfg.batch) | {"sample": sample},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
@@ -120,10 +154,21 @@ def run_reference(args):
 
 
 def workload_config(cfg, batch):
-    return {"workload": f"{cfg.name}: {batch} slices x {cfg.ny}x{cfg.nx} @ {cfg.dx:.2f} mm, {cfg.nviews} views x "
-                        f"{cfg.nu} bins, flat detector, dso {cfg.dso:.0f} / dsd {cfg.dsd:.0f} mm",
+    if cfg.ndim == 3:
+        what = (f"{cfg.name}: cone beam, volume {cfg.nz}x{cfg.ny}x{cfg.nx} @ {cfg.dx:.2f} mm, {cfg.nviews} views x "
+                f"{cfg.nv}x{cfg.nu} bins @ {cfg.du:.2f} mm")
+        nbytes = 4.0 * (9 * cfg.n_pix + 4 * cfg.n_rays)
+    else:
+        what = (f"{cfg.name}: {batch} slice{'s' if batch > 1 else ''} x {cfg.ny}x{cfg.nx} @ {cfg.dx:.2f} mm, "
+                f"{cfg.nviews} views x {cfg.nu} bins")
+        nbytes = 4.0 * batch * (9 * cfg.nx * cfg.ny + 4 * cfg.nviews * cfg.nu)
+    big = nbytes > 126e6
+    return {"workload": what + f", flat detector, dso {cfg.dso:.0f} / dsd {cfg.dsd:.0f} mm",
             "n_cgls": cfg.n_cgls, "n_gd": cfg.n_gd, "lambda": cfg.lam, "I0": cfg.I0, "slices_per_gpu": batch,
-            "l2_policy": "working set (~2.3 GB per GPU at c4) is larger than the 126 MB L2; no explicit flush"}
+            "l2_policy": (f"working set of one step (~{nbytes / 1e6:.0f} MB of vectors + tables) is larger than the 126 MB L2; "
+                          "no explicit flush") if big else
+                         (f"working set of one step (~{nbytes / 1e6:.1f} MB of vectors) is L2-resident by nature of this small "
+                          "workload; the stored matrices (if any) stream from HBM every application; no explicit flush")}
 
 
 # ----------------------------------------------------------------------------------------------
@@ -152,7 +197,10 @@ def main():
     case = make_case(cfg, slices=shard.slice_range(rank, world, batch), raster=False)
     sino_host = torch.from_numpy(case["sino"]).pin_memory()
     sino = sino_host.cuda(non_blocking=True)
+    # on-chip peaks of THIS device, measured before anything is timed (roofline denominators)
+    dev_peaks = ctr.ctr_measure_peaks(5)
     h = ctr.ctr_create(cfg)
+    path = h.ctr_path_info()
     img = torch.zeros(h.img_shape, device="cuda")
     img_host = torch.empty(h.img_shape, dtype=torch.float32).pin_memory()
 
@@ -237,7 +285,7 @@ def main():
         except Exception:
             pass
         out = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "metric": metric_name(cfg), "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic", "config": workload_config(cfg, batch),
             "clocks": clocks, "gpu_launches": int(launches),
@@ -246,69 +294,115 @@ def main():
             "kernel_ms_per_step": {k: v[0] / K for k, v in prof.items()},
             "kernel_launch_groups_per_step": {k: v[1] / K for k, v in prof.items()},
         }
-        out["roofline"] = roofline(cfg, batch, prof, peaks)
+        out["roofline"] = roofline(cfg, batch, prof, peaks, dev_peaks, path)
+        out["hbm_bound_parts"] = hbm_kinds(cfg, batch, prof, peaks, K)
+        out["measured_peaks_this_run"] = dev_peaks
+        out["kernel_path"] = path
         if not args.no_cpu_baseline:
-            secs, cores = oracle_step_seconds(cfg, case["sino"][0], 1)
-            out["cpu_baseline"] = {"value": 1.0 / secs, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                   "sample": f"slice 0 of {batch}, one outer iteration from f = 0 "
-                                             f"(n_cgls={cfg.n_cgls}, n_gd={cfg.n_gd}), {secs:.1f} s"}
+            secs, cores, sample = oracle_step_seconds(cfg, case["sino"][0] if cfg.ndim == 2 else None,
+                                                      5 if cfg.name in ("c3", "c4") else (1 if cfg.ndim == 3 else 20))
+            out["cpu_baseline"] = {"value": 1.0 / secs, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
         print(json.dumps(out))
     h.close()
     if world > 1:
         dist.destroy_process_group()
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the batched kernels at c4, from the committed
-# ncu --set full captures (profiles/r1i_ncu_full_c4.md); None for workloads that were not captured
-NCU_TRAFFIC_C4 = {"forward": 170.5e6, "back": 559.0e6}
+NNZ = {"c1": 2.32e5, "c2": 4.60e6, "c3": 2.95e7, "c4": 2.95e7, "c5": 4.37e9}  # nnz(P) per slice / volume
 
 
-def roofline(cfg, batch, prof, peaks):
-    """Dominant kernel = the slower of the projector pair (a1 / a2). Both are bound by on-chip work, not HBM
-    (DESIGN.md section 6): algorithmic work per application = one FMA (2 flop) per non-zero of P, i.e. per
-    ray-pixel intersection, per slice; nnz(P) per slice is counted from the geometry (2.95e7
-    for the 512^2 / 60 x 888 geometry). Peak = fp32 FMA peak of the chip, 148 SMs x 128 lanes x 2 flop x
-    sm_max_mhz (B200_PROFILING.md unit counts, MEASURED_PEAKS.json clock). The HBM view of the same launch
-    (compulsory image + sinogram bytes against the measured copy bandwidth) is reported beside it, as
-    BASELINE.json's metric asks, with the ncu-measured DRAM traffic."""
-    nnz = {"c1": 2.32e5, "c2": 4.60e6, "c3": 2.95e7, "c4": 2.95e7, "c5": 4.37e9}[cfg.name]
+def ncu_traffic(cfg, batch, kernel_substr):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture of this
+    workload (profiles/dram_traffic.csv: workload,batch,kernel,dram_bytes_per_launch,source), or (None, None)."""
+    try:
+        for line in (ROOT / "profiles" / "dram_traffic.csv").read_text().splitlines()[1:]:
+            wl, b, kern, nbytes, src = [c.strip() for c in line.split(",", 4)]
+            if wl == cfg.name and int(b) == batch and kern in kernel_substr:
+                return float(nbytes), src
+    except Exception:
+        pass
+    return None, None
+
+
+def roofline(cfg, batch, prof, peaks, dev_peaks, path):
+    """Dominant kernel = the slower of the projector pair (a1 / a2), DESIGN.md section 5.
+
+    Batched (c4): both kernels are bound by the L1 data pipe (ncu: l1tex 80+ % busy; DRAM 5-25 %; FMA pipe 30-45 %):
+    every non-zero of P moves 4 bytes per slice through an L1. achieved = 4 B x nnz(P) x slices / launch time;
+    peak = L1 load bandwidth MEASURED in this run by ctr_measure_peaks (LDG.128 hitting L1 at full occupancy).
+    The fp32-FMA view (2 flop per non-zero and slice over the measured FFMA peak) and the HBM view BASELINE.json's
+    metric asks for (compulsory image + sinogram bytes over MEASURED_PEAKS.json's copy bandwidth) are beside it.
+    Single problems (c1-c3, c5) apply stored matrices: 8 B per non-zero streamed from HBM."""
+    nnz = NNZ[cfg.name]
     kind = max(("forward", "back"), key=lambda k: prof[k][0])
-    names = {"forward": "k_si_forward (P, a1)" if batch > 1 else "k_ell_apply<0> (stored P, a1)",
-             "back": "k_si_back_quad (P^T gather, a2)" if batch > 1 else "k_ell_apply<1> (stored P^T, a2)"}
-    sm_mhz = peaks.get("sm_max_mhz", 1965.0)
-    peak = 148 * 128 * 2 * sm_mhz * 1e6 / 1e12
     hbm = peaks.get("hbm_gbs", 6650.0)
+    hbm_src = "MEASURED_PEAKS.json hbm_gbs (measured)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
     bytes_alg = 4.0 * batch * (cfg.nx * cfg.ny * cfg.nz + cfg.nviews * cfg.nu * cfg.nv)
 
-    def one(k):
+    def launch_s(k):
         ms, n = prof[k]
-        sec = ms / max(n, 1) * 1e-3
-        ach = 2.0 * nnz * batch / sec / 1e12
-        return {"kernel": names[k], "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-                "avg_launch_ms": sec * 1e3, "launches": n,
-                "traffic": NCU_TRAFFIC_C4.get(k) if (cfg.name == "c4" and batch == 64) else None,
-                "compulsory_GBps": bytes_alg / sec / 1e9,
-                "compulsory_GBps_frac_of_measured_hbm": bytes_alg / sec / 1e9 / hbm}
+        return ms / max(n, 1) * 1e-3, n
 
-    # the unit that actually binds both kernels (ncu: l1tex data pipe 78 % busy): every non-zero of P moves
-    # 4 bytes per slice through an L1; peak = 148 SMs x 128 B/clk x sm_max_mhz
-    sec_k = prof[kind][0] / max(prof[kind][1], 1) * 1e-3
-    l1_peak = 148 * 128 * sm_mhz * 1e6 / 1e12
-    l1 = {"bound": "l1 gather bandwidth", "achieved": 4.0 * nnz * batch / sec_k / 1e12, "peak": l1_peak, "unit": "TB/s",
-          "frac": 4.0 * nnz * batch / sec_k / 1e12 / l1_peak,
-          "note": "algorithmic gather bytes (4 B per non-zero of P per slice) over the L1 data-pipe peak"}
     if batch == 1:
-        # single problems apply stored matrices (DESIGN.md section 4): 8 bytes per non-zero streamed from HBM
-        ms_k, n_k = prof[kind]
-        ach = 8.0 * nnz / (ms_k / max(n_k, 1) * 1e-3) / 1e9
-        return {"bound": "hbm", "kernel": names[kind], "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm,
-                "traffic": None, "avg_launch_ms": ms_k / max(n_k, 1), "launches": n_k,
-                "peak_source": "MEASURED_PEAKS.json hbm_gbs (measured)" if "hbm_gbs" in peaks else "fallback 6650 GB/s",
-                "note": "algorithmic bytes = 8 B x nnz(P) of the stored matrix (index + weight)"}
-    out = {"bound": "alu", **one(kind), "l1_view": l1,
-           "peak_source": "derived: 148 SM x 128 fp32 FMA lanes x 2 flop x sm_max_mhz (MEASURED_PEAKS.json clock); "
-                          "hbm_gbs of measured" if "hbm_gbs" in peaks else "fallback 6650 GB/s",
-           "other": one("back" if kind == "forward" else "forward")}
+        stored = "ell" in path.get(kind, "")
+        sec, n = launch_s(kind)
+        traffic, tsrc = ncu_traffic(cfg, batch, path.get(kind, ""))
+        if stored:
+            ach = 8.0 * nnz / sec / 1e9
+            return {"bound": "hbm", "kernel": f"{path.get(kind)} ({'P, a1' if kind == 'forward' else 'P^T, a2'})",
+                    "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm, "traffic": traffic,
+                    "traffic_source": tsrc, "avg_launch_ms": sec * 1e3, "launches": n, "peak_source": hbm_src,
+                    "note": "algorithmic bytes = 8 B x nnz(P) of the stored matrix (index + weight), streamed once per "
+                            "application; for c1-c3 the vectors are L2-resident"}
+        ach = 2.0 * nnz / sec / 1e12
+        return {"bound": "alu", "kernel": path.get(kind), "achieved": ach, "peak": dev_peaks["fma_tflops"],
+                "unit": "TFLOP/s", "frac": ach / dev_peaks["fma_tflops"], "traffic": traffic, "traffic_source": tsrc,
+                "avg_launch_ms": sec * 1e3, "launches": n,
+                "peak_source": "fp32 FFMA rate measured in this run (ctr_measure_peaks)",
+                "note": "on-the-fly kernel (lookup tables not built): 2 flop per non-zero of P"}
+
+    def view(k):
+        sec, n = launch_s(k)
+        traffic, tsrc = ncu_traffic(cfg, batch, path.get(k, ""))
+        l1 = 4.0 * nnz * batch / sec / 1e9
+        fma = 2.0 * nnz * batch / sec / 1e12
+        return {"kernel": f"{path.get(k)} ({'P, a1' if k == 'forward' else 'P^T gather, a2'})",
+                "achieved": l1, "peak": dev_peaks["l1_tbs"] * 1e3, "unit": "GB/s", "frac": l1 / (dev_peaks["l1_tbs"] * 1e3),
+                "traffic": traffic, "traffic_source": tsrc, "avg_launch_ms": sec * 1e3, "launches": n,
+                "fma_view": {"achieved": fma, "peak": dev_peaks["fma_tflops"], "unit": "TFLOP/s",
+                             "frac": fma / dev_peaks["fma_tflops"]},
+                "hbm_view": {"achieved": bytes_alg / sec / 1e9, "peak": hbm, "unit": "GB/s",
+                             "frac": bytes_alg / sec / 1e9 / hbm, "peak_source": hbm_src,
+                             "note": "compulsory bytes (image + sinogram once) of one application"}}
+
+    return {"bound": "l1", **view(kind),
+            "peak_source": "L1 load bandwidth measured in this run by ctr_measure_peaks (LDG.128 hitting L1, full "
+                           "occupancy); fma_view: measured FFMA rate; hbm_view: " + hbm_src,
+            "note": "algorithmic bytes = 4 B per non-zero of P per slice through the L1 data pipe, the unit ncu shows "
+                    "busiest for this kernel (profiles/)",
+            "other": view("back" if kind == "forward" else "forward")}
+
+
+def hbm_kinds(cfg, batch, prof, peaks, steps):
+    """The HBM-bound parts of a step: CGLS vector work (a3) and the TV sweeps (a4-a7),
+    algorithmic bytes per unit over the measured copy bandwidth."""
+    hbm = peaks.get("hbm_gbs", 6650.0)
+    npix, nray = cfg.nx * cfg.ny * cfg.nz * batch, cfg.nviews * cfg.nu * cfg.nv * batch
+    out = {}
+    ms_v = prof["vector"][0] / steps
+    by_v = (20.0 * npix + 12.0 * nray) * cfg.n_cgls
+    out["cgls_vector"] = {"ms_per_step": ms_v, "algorithmic_bytes_per_step": by_v,
+                          "achieved_GBps": by_v / (ms_v * 1e-3) / 1e9 if ms_v > 0 else None,
+                          "frac_of_measured_hbm": by_v / (ms_v * 1e-3) / 1e9 / hbm if ms_v > 0 else None,
+                          "note": "20 B/pixel + 12 B/ray per CGLS iteration (SURVEY.md 8(d) a3); the S24 "
+                                  "re-orthogonalisation reads are extra traffic, not algorithmic bytes"}
+    ms_t = prof["tv"][0] / steps
+    by_t = 44.0 * npix * cfg.n_gd
+    out["tv_sweeps"] = {"ms_per_step": ms_t, "ms_per_sweep": ms_t / max(cfg.n_gd, 1), "algorithmic_bytes_per_step": by_t,
+                        "achieved_GBps": by_t / (ms_t * 1e-3) / 1e9 if ms_t > 0 else None,
+                        "frac_of_measured_hbm": by_t / (ms_t * 1e-3) / 1e9 / hbm if ms_t > 0 else None,
+                        "note": "44 B/pixel per sweep, the lower figure of SURVEY.md 8(d) a4-a7 (60 B/pixel would "
+                                "read 1.36x higher)"}
     return out
 
 

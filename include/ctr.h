@@ -25,6 +25,8 @@
  * - Return value: CTR_OK (0) or a negative ctr_status. No exceptions, no exit(), nothing printed.
  *   On error nothing has been enqueued unless the code is CTR_ECUDA.
  * - A handle must not be used from two host threads at once (its scratch is shared by all calls).
+ * - Inputs must be finite. A NaN/Inf in a sinogram bin reaches every pixel of the 2 x 2 pixel quads its ray
+ *   touches in the batched P^T (0 * Inf), not only the pixels the ray crosses.
  */
 #ifndef CTR_H_
 #define CTR_H_
@@ -67,7 +69,15 @@ typedef struct {
   float dso, dsd;         /* source-isocentre and source-detector distances, mm                                  */
   int32_t det_type;       /* 0 = FLAT, 1 = ARC                                                    */
   int32_t batch;          /* independent 2D slices sharing this geometry (>= 1); must be 1 when ndim = 3          */
+  int32_t flags;          /* bit mask of CTR_GEOM_* below; 0 in every config                                      */
 } ctr_geometry;
+
+/* ctr_geometry.flags */
+enum {
+  CTR_GEOM_NO_TABLES = 1 /* do not build the stored matrices / hit tables (second strategy): every
+                            p_ij is computed on the fly. Same bits either way; a low-memory mode and the tests' way
+                            of checking that the tables hold exactly what the on-the-fly kernels compute. */
+};
 
 /* Iteration schedule and the constants the paper leaves open (readings S13, S14). */
 typedef struct {
@@ -143,8 +153,27 @@ int ctr_get_stats(ctr_handle* h, ctr_sweep_stat* buf, size_t n_records);
 enum { CTR_PROF_FORWARD = 0, CTR_PROF_BACK = 1, CTR_PROF_VECTOR = 2, CTR_PROF_TV = 3, CTR_PROF_LAYOUT = 4, CTR_PROF_KINDS = 5 };
 int ctr_profile_enable(ctr_handle* h, int on);
 int ctr_profile_read(ctr_handle* h, double* ms_by_kind, long long* count_by_kind);
+/* Which kernels this handle applies P and P^T with, as "forward=<kernel>;back=<kernel>;tables_mb=<MB of lookup
+ * tables built>;graphs=<0|1>" (the lookup tables of PAPER.md:193 are built best effort at ctr_create). Valid
+ * for the life of the handle. */
+const char* ctr_path_info(const ctr_handle* h);
 /* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
 long long ctr_launch_count(const ctr_handle* h);
+
+/* Measured peaks of the on-chip units that bound the projector kernels (bench.py's roofline denominators; not part
+ * of the reconstruction path). Each figure is the best of `reps` runs of a microbenchmark kernel at full occupancy on
+ * the CURRENT device, timed with CUDA events on the legacy default stream; synchronous; allocates and frees ~2 GiB. */
+typedef struct {
+  double fma_tflops;    /* fp32 FMA (FFMA), 2 flop each                                                        */
+  double fma2_tflops;   /* packed fp32x2 FMA (FFMA2, sm_100), 4 flop each                                       */
+  double issue_gwinst;  /* warp instructions issued per second / 1e9 (FFMA and integer ALU interleaved)         */
+  double l1_tbs;        /* L1 data pipe: LDG.128 that hit in L1, TB/s (128 bytes per wavefront)                 */
+  double smem_tbs;      /* shared memory: conflict-free LDS.128, TB/s                                           */
+  double hbm_copy_gbs;  /* device-memory copy of 1 GiB, read + write bytes, GB/s                                */
+  int32_t sm_count;
+  int32_t pad;
+} ctr_peaks;
+int ctr_measure_peaks(ctr_peaks* out, int reps);
 
 const char* ctr_strerror(int status);
 /* Text of the last error on this handle ("" if none); valid until the next call on the handle. */

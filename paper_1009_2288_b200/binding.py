@@ -34,7 +34,10 @@ class ctr_geometry(C.Structure):
                 ("angles", C.POINTER(C.c_float)),
                 ("nu", C.c_int32), ("nv", C.c_int32), ("du", C.c_float), ("dv", C.c_float),
                 ("u_off", C.c_float), ("v_off", C.c_float), ("dso", C.c_float), ("dsd", C.c_float),
-                ("det_type", C.c_int32), ("batch", C.c_int32)]
+                ("det_type", C.c_int32), ("batch", C.c_int32), ("flags", C.c_int32)]
+
+
+CTR_GEOM_NO_TABLES = 1
 
 
 class ctr_params(C.Structure):
@@ -50,10 +53,16 @@ class ctr_sweep_stat(C.Structure):
                 ("k", C.c_int32), ("pad", C.c_int32)]
 
 
+class ctr_peaks(C.Structure):
+    _fields_ = [("fma_tflops", C.c_double), ("fma2_tflops", C.c_double), ("issue_gwinst", C.c_double),
+                ("l1_tbs", C.c_double), ("smem_tbs", C.c_double), ("hbm_copy_gbs", C.c_double),
+                ("sm_count", C.c_int32), ("pad", C.c_int32)]
+
+
 EXPORTS = ["ctr_default_params", "ctr_create", "ctr_destroy", "ctr_forward", "ctr_back", "ctr_back_pixel", "ctr_cgls",
            "ctr_update_weights", "ctr_eptv_step", "ctr_reconstruct", "ctr_reconstruct_w",
            "ctr_set_params", "ctr_get_stats", "ctr_launch_count", "ctr_strerror", "ctr_last_error",
-           "ctr_profile_enable", "ctr_profile_read"]
+           "ctr_profile_enable", "ctr_profile_read", "ctr_measure_peaks", "ctr_path_info"]
 
 
 def load_library():
@@ -83,12 +92,15 @@ def load_library():
     L.ctr_get_stats.argtypes = [H, C.POINTER(ctr_sweep_stat), C.c_size_t]
     L.ctr_profile_enable.argtypes = [H, C.c_int]
     L.ctr_profile_read.argtypes = [H, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+    L.ctr_measure_peaks.argtypes = [C.POINTER(ctr_peaks), C.c_int]
     L.ctr_launch_count.argtypes = [H]
     L.ctr_launch_count.restype = C.c_longlong
     L.ctr_strerror.argtypes = [C.c_int]
     L.ctr_strerror.restype = C.c_char_p
     L.ctr_last_error.argtypes = [H]
     L.ctr_last_error.restype = C.c_char_p
+    L.ctr_path_info.argtypes = [H]
+    L.ctr_path_info.restype = C.c_char_p
     _lib = L
     return L
 
@@ -105,7 +117,7 @@ def make_geometry(g) -> ctr_geometry:
     d = g.geometry_dict() if hasattr(g, "geometry_dict") else dict(g)
     cg = ctr_geometry()
     defaults = dict(ndim=2, nz=1, nv=1, dz=1.0, dv=1.0, cx=0.0, cy=0.0, cz=0.0, theta0=0.0, dtheta=0.0,
-                    u_off=0.0, v_off=0.0, det_type=0, batch=1)
+                    u_off=0.0, v_off=0.0, det_type=0, batch=1, flags=0)
     defaults.update({k: v for k, v in d.items() if k != "angles"})
     for name, ctype in ctr_geometry._fields_:
         if name == "angles":
@@ -151,9 +163,10 @@ def _stream():
 class Handle:
     """Owns a ctr_handle*. Methods mirror the C entry points one to one."""
 
-    def __init__(self, geometry):
+    def __init__(self, geometry, flags: int = 0):
         self._L = load_library()
         self.geom = make_geometry(geometry)
+        self.geom.flags |= int(flags)
         self._h = C.c_void_p()
         rc = self._L.ctr_create(C.byref(self.geom), C.byref(self._h))
         if rc != CTR_OK:
@@ -236,12 +249,25 @@ class Handle:
         kinds = ["forward", "back", "vector", "tv", "layout"]
         return {k: (ms[i], int(cnt[i])) for i, k in enumerate(kinds)}
 
+    def ctr_path_info(self) -> dict:
+        return dict(kv.split("=", 1) for kv in self._L.ctr_path_info(self._h).decode().split(";") if kv)
+
     def ctr_launch_count(self) -> int:
         return int(self._L.ctr_launch_count(self._h))
 
 
-def ctr_create(geometry) -> Handle:
-    return Handle(geometry)
+def ctr_measure_peaks(reps: int = 5) -> dict:
+    """Synchronous microbenchmarks on the current device (include/ctr.h); returns the ctr_peaks fields."""
+    pk = ctr_peaks()
+    rc = load_library().ctr_measure_peaks(C.byref(pk), int(reps))
+    if rc != CTR_OK:
+        raise CtrError(rc, "ctr_measure_peaks")
+    return {n: getattr(pk, n) for n, _ in ctr_peaks._fields_ if n != "pad"}
+
+
+def ctr_create(geometry, flags: int = 0) -> Handle:
+    """flags: ctr_geometry.flags bits (CTR_GEOM_NO_TABLES) OR-ed into the geometry."""
+    return Handle(geometry, flags)
 
 
 def ctr_destroy(h: Handle) -> None:

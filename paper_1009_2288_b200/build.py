@@ -12,10 +12,11 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libctr.so"
-SOURCES = ["ctr_api.cu", "ctr_fan.cu", "ctr_si.cu", "ctr_tv.cu", "ctr_cone.cu"]
+SOURCES = ["ctr_api.cu", "ctr_fan.cu", "ctr_si.cu", "ctr_tv.cu", "ctr_cone.cu", "ctr_peaks.cu"]
 HEADERS = ["ctr_common.cuh", "ctr_internal.h", "ctr_fan_geom.cuh", "ctr_ell.cuh", "../../include/ctr.h"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-              "-Xcompiler", "-fPIC", "-shared"]
+              "-Xcompiler", "-fPIC"]
+OBJ = PKG / "build"  # object files (git-ignored); one nvcc per source, in parallel
 
 
 def _nvcc() -> str:
@@ -35,14 +36,32 @@ def needs_build() -> bool:
 def build(force: bool = False, verbose: bool = False) -> Path:
     if not force and not needs_build():
         return LIB
+    from concurrent.futures import ThreadPoolExecutor
+    OBJ.mkdir(exist_ok=True)
+    hdr_t = max((CSRC / f).stat().st_mtime for f in HEADERS)
+
+    def compile_one(src: str):
+        obj = OBJ / (src.replace(".cu", f".{os.getpid()}.o") if force else src.replace(".cu", ".o"))
+        final = OBJ / src.replace(".cu", ".o")
+        if not force and final.exists() and final.stat().st_mtime > max((CSRC / src).stat().st_mtime, hdr_t):
+            return final, ""
+        cmd = [_nvcc(), *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-c", "-o", str(obj), str(CSRC / src)]
+        res = subprocess.run(cmd, capture_output=True, text=True)
+        if res.returncode != 0:
+            raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + res.stdout + res.stderr)
+        if obj != final:
+            os.replace(obj, final)
+        return final, res.stderr
+
+    with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
+        done = list(ex.map(compile_one, SOURCES))
+    if verbose:
+        print("".join(err for _, err in done))
     tmp = LIB.with_name(f"libctr.tmp{os.getpid()}.so")
-    cmd = [_nvcc(), *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", str(tmp),
-           *[str(CSRC / f) for f in SOURCES]]
+    cmd = [_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", str(tmp), *[str(o) for o, _ in done]]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if res.returncode != 0:
-        raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + res.stdout + res.stderr)
-    if verbose:
-        print(res.stderr)
+        raise RuntimeError("link failed:\n" + " ".join(cmd) + "\n" + res.stdout + res.stderr)
     os.replace(tmp, LIB)
     return LIB
 

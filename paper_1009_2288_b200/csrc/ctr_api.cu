@@ -132,6 +132,8 @@ __global__ void __launch_bounds__(256) k_img_uupdate(size_t nl, int LQ, float* _
 //                           sums over a thread's elements, everything above that in fp64)
 //   pass 2 (k_reorth_sub) : g <- g - sum_i c_i b_i, gamma' = ||g||^2, beta = gamma'/gamma (:432)
 #define REORTH_NB 4   /* basis vectors per k_reorth_dots launch (= CTR_MAX_BASIS: one launch) */
+static_assert(CTR_MAX_BASIS >= 1 && CTR_MAX_BASIS <= REORTH_NB,
+              "CTR_MAX_BASIS must be 1..4: k_reorth_dots / k_finish handle REORTH_NB = 4 basis vectors per launch");
 template <int V>
 __global__ void __launch_bounds__(256) k_reorth_dots(size_t nl, int LQ, size_t nimg, const float* __restrict__ gi,
                                                      const float* __restrict__ basis, int i0, int nb, int Bp, Scal sc,
@@ -317,27 +319,12 @@ static int op_back(ctr_handle* h, const float* sino, float* out, int mode, const
   return h->d.ndim == 3 ? cone_back(h, sino, out, mode, s, u, st) : fan_back(h, sino, out, mode, s, u, st);
 }
 
-// storage for the unit gradients; grows (synchronously) only when a longer CGLS run is requested
-static int ensure_basis(ctr_handle* h, int n_iter) {
-  int need = n_iter < CTR_MAX_BASIS ? n_iter : CTR_MAX_BASIS;
-  if (need <= h->basis_cap) return CTR_OK;
-  CTR_CUDA(h, cudaDeviceSynchronize());
-  if (h->basis) cudaFree(h->basis);
-  h->basis = nullptr;
-  h->basis_cap = 0;
-  cudaError_t e = cudaMalloc((void**)&h->basis, (size_t)need * h->nimg * sizeof(float));
-  if (e != cudaSuccess) { cudaGetLastError(); return set_err(h, CTR_ENOMEM, "CGLS basis allocation failed"); }
-  h->basis_cap = need;
-  return CTR_OK;
-}
-
 // CGLS on internal-layout arrays (gradients re-orthogonalised, S24). u: in x0 /
 // out u^(M). The last iteration only needs u (its P^T r and s are never used, O4), so it ends with a
 // plain u += a s.
 static int cgls_internal(ctr_handle* h, const float* b, float* u, int n_iter, bool x0_zero, cudaStream_t st) {
   if (n_iter <= 0) return CTR_OK;
   int rc;
-  if ((rc = ensure_basis(h, n_iter))) return rc;
   if (x0_zero) {
     CTR_CUDA(h, cudaMemcpyAsync(h->r, b, h->nsino * sizeof(float), cudaMemcpyDeviceToDevice, st));  // r0 = y
   } else if ((rc = op_forward(h, u, h->r, 1, b, st))) return rc;                                    // r0 = y - P u0
@@ -348,7 +335,7 @@ static int cgls_internal(ctr_handle* h, const float* b, float* u, int n_iter, bo
     if (m == n_iter - 1) return vec_img_uupdate(h, u, h->s, st);         // u += a s
     if ((rc = vec_sino_axpy(h, h->r, h->q, st))) return rc;              // r -= a q
     if ((rc = op_back(h, h->r, h->gimg, 2, h->s, u, st))) return rc;     // g = P^T r, u += a s
-    float* bnew = (m + 1 < h->basis_cap) ? h->basis + (size_t)(m + 1) * h->nimg : nullptr;
+    float* bnew = (m + 1 < CTR_MAX_BASIS) ? h->basis + (size_t)(m + 1) * h->nimg : nullptr;
     if ((rc = vec_direction(h, h->gimg, m + 1, 0, bnew, st))) return rc;  // g' _|_ b_0.., gamma', beta, s = g' + beta s, b_{m+1}
   }
   return CTR_OK;
@@ -413,6 +400,7 @@ const char* ctr_strerror(int status) {
 }
 
 const char* ctr_last_error(const ctr_handle* h) { return h ? h->err : ""; }
+const char* ctr_path_info(const ctr_handle* h) { return h ? h->path_info : ""; }
 long long ctr_launch_count(const ctr_handle* h) { return h ? h->launches : 0; }
 
 void ctr_destroy(ctr_handle* h) {
@@ -442,6 +430,7 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
   if (!(g->dx > 0) || !(g->dy > 0) || !(g->du > 0) || !(g->dso > 0) || !(g->dsd > g->dso)) return CTR_EINVAL;
   if (g->ndim == 3 && (!(g->dz > 0) || !(g->dv > 0))) return CTR_EINVAL;
   if (g->det_type != 0 && g->det_type != 1) return CTR_EINVAL;
+  if (g->flags & ~CTR_GEOM_NO_TABLES) return CTR_EINVAL;
   if ((long long)g->nx * g->ny * g->nz >= (1ll << 31) || (long long)g->nviews * g->nu * g->nv >= (1ll << 31)) return CTR_EINVAL;
   // source and detector must lie outside the circle circumscribing the grid (plus one voxel)
   {
@@ -528,6 +517,7 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
   A((void**)&h->v, h->nimg * fb);
   A((void**)&h->w, h->nimg * fb * d.ndim);
   A((void**)&h->n0, h->nimg * fb * d.ndim);
+  A((void**)&h->basis, h->nimg * fb * CTR_MAX_BASIS);  // unit CGLS gradients b_0..b_3 (S24)
   // partial sums: the largest user is the TV trial kernel (TV_KC * V slots per block)
   {
     size_t nblk_tv = (size_t)((d.nx + 31) / 32) * ((d.ny + 3) / 4) * d.nz;
@@ -586,6 +576,21 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
   int rc = d.ndim == 3 ? cone_build_tables(h) : fan_build_tables(h);
   if (rc == CTR_OK && d.ndim == 2 && d.V == 4) rc = si_build_hits(h);
   if (rc != CTR_OK) { ctr_destroy(h); return rc; }
+  {
+    // which kernels ctr_forward / ctr_back launch on this handle (the tables are built best effort)
+    const char *fw, *bk;
+    double table_mb = 0.0;
+    if (d.V == 4) {
+      fw = "k_si_forward";
+      bk = h->qwts ? "k_si_back_quad" : "k_si_back";
+      if (h->qwts) table_mb = (double)((d.nx + 1) / 2) * ((d.ny + 1) / 2) * h->hits_cap * 20.0 / 1e6;
+    } else {
+      fw = h->ell_p.tab ? "k_ell_apply<P>" : (d.ndim == 3 ? "k_cone_forward" : "k_fan_forward");
+      bk = h->ell_pt.tab ? "k_ell_apply<PT>" : (d.ndim == 3 ? "k_cone_back" : "k_fan_back");
+      table_mb = (double)(h->ell_p.tab ? h->ell_p.bytes : 0) / 1e6 + (double)(h->ell_pt.tab ? h->ell_pt.bytes : 0) / 1e6;
+    }
+    snprintf(h->path_info, sizeof(h->path_info), "forward=%s;back=%s;tables_mb=%.1f;graphs=%d", fw, bk, table_mb, 0);
+  }
   *out = h;
   return CTR_OK;
 }
@@ -659,9 +664,9 @@ int ctr_update_weights(ctr_handle* h, const float* d_x, float* d_w, float quanti
   if (h->d.V == 1) {
     rc = tv_update_weights(h, d_x, d_w, st);
   } else {
-    if ((rc = pack(h, d_x, h->ximg, h->d.npix, 1, st))) return rc;
-    if ((rc = tv_update_weights(h, h->ximg, h->w, st))) return rc;
-    rc = unpack(h, h->w, d_w, h->d.npix, h->d.ndim, st);
+    rc = pack(h, d_x, h->ximg, h->d.npix, 1, st);
+    if (!rc) rc = tv_update_weights(h, h->ximg, h->w, st);
+    if (!rc) rc = unpack(h, h->w, d_w, h->d.npix, h->d.ndim, st);
   }
   set_quantile(h, q_saved);
   if (rc) return rc;
@@ -711,7 +716,6 @@ int ctr_reconstruct_w(ctr_handle* h, const float* d_sino, float* d_img, float* d
     if ((rc = si_from_abi(h, d_sino, h->bsino, h->d.nray, st))) return rc;  // slice-interleaved
     b = h->bsino;
   }
-  if ((rc = ensure_basis(h, P.n_cgls))) return rc;
   if (!P.warm_start) CTR_CUDA(h, cudaMemsetAsync(f, 0, h->nimg * sizeof(float), st));            // f^(0) = 0 (:171)
   else if (!direct && (rc = pack(h, d_img, h->ximg, h->d.npix, 1, st))) return rc;
   for (int it = 0; it < P.n_outer; ++it) {

@@ -103,11 +103,11 @@ __global__ void __launch_bounds__(128) k_ell_apply(size_t nrows, const int* __re
 }
 
 // Build a table for `nrows` rows. Best effort: leaves t.tab == nullptr (the caller then uses the on-the-fly
-// kernel) when the table does not fit in free device memory or CTR_NO_TABLES is set in the environment.
+// kernel) when the table does not fit in free device memory or ctr_geometry.flags has CTR_GEOM_NO_TABLES.
 template <class Hits>
 static int ell_build(ctr_handle* h, Hits hits, size_t nrows, EllTable& t) {
   t.tab = nullptr; t.cap = nullptr; t.off = nullptr; t.nrows = nrows;
-  if (getenv("CTR_NO_TABLES")) return CTR_OK;
+  if (h->g.flags & CTR_GEOM_NO_TABLES) return CTR_OK;
   const size_t nwarp = (nrows + 31) / 32;
   const unsigned nblk = (unsigned)((nrows + 127) / 128);
   if (cudaMalloc((void**)&t.cap, sizeof(int) * nwarp) != cudaSuccess) { cudaGetLastError(); t.cap = nullptr; return CTR_OK; }

@@ -13,7 +13,7 @@ namespace ctr {
 #define CTR_STAT_SWEEPS 4096 /* ring capacity, in sweeps */
 #define CTR_PROF_MAX 32768
 #ifndef CTR_MAX_BASIS
-#define CTR_MAX_BASIS 4 /* stored unit gradients b_0..b_3 used for re-orthogonalisation (S24) */
+#define CTR_MAX_BASIS 4 /* stored unit gradients b_0..b_3 used for re-orthogonalisation (S24); valid: 1..4 */
 #endif
 #define CTR_NCOUNTERS 8
 #define CTR_REDUCE_BLOCKS 1184 /* grid cap of the grid-stride reduction kernels: 148 SMs x 8 */
@@ -95,8 +95,7 @@ struct ctr_handle {
   int hits_cap;
   ctr::EllTable ell_p, ell_pt;  // stored P (rows = rays) and P^T (rows = voxels), batch = 1 only; tab == NULL: on the fly
   float* usi;           // CGLS iterate in the slice-interleaved layout (batch > 1)
-  float* basis;         // [basis_cap][nimg] unit CGLS gradients (S24)
-  int basis_cap;
+  float* basis;         // [CTR_MAX_BASIS][nimg] unit CGLS gradients (S24), allocated in ctr_create
   int dots_blocks;      // resident blocks of k_reorth_dots on this device (its grid size)
   double* part;
   size_t part_len;
@@ -116,6 +115,7 @@ struct ctr_handle {
   cudaEvent_t* prof_ev;       // [2 * CTR_PROF_MAX]
   unsigned char* prof_kind;   // [CTR_PROF_MAX]
   char err[256];
+  char path_info[160];
 };
 
 namespace ctr {

@@ -246,7 +246,8 @@ __global__ void __launch_bounds__(256) k_si_back(Dims d, const float4* __restric
 // qidx[quad][e] = ray index * LQ (or -1: padding), qwts[quad][e] = p_ij of that ray in pixels
 // (i0,j0), (i0+1,j0), (i0,j0+1), (i0+1,j0+1); views ascending, bins ascending. The weights are the values
 // fan_pixel_weight() returns (0 where the ray misses the pixel), so P^T stays the bit-exact transpose of P
-// and every pixel adds its non-zero terms in the same order as the single-slice kernel.
+// and every pixel adds its non-zero terms in the same order as the single-slice kernel (a ray that misses a
+// pixel of the quad adds 0 * y: the inputs must be finite, include/ctr.h).
 // (A 2 x 4 tile was measured too: 6.3 ms per step against 4.2 ms - 32 accumulators per lane cost more in
 // occupancy than the extra sharing saves.)
 // ------------------------------------------------------------------------------------------------
@@ -397,7 +398,7 @@ int si_build_hits(ctr_handle* h) {
   h->qidx = nullptr;
   h->qwts = nullptr;
   h->hits_cap = 0;
-  if (getenv("CTR_NO_TABLES")) return CTR_OK;
+  if (h->g.flags & CTR_GEOM_NO_TABLES) return CTR_OK;
   const int nqx = (d.nx + 1) / 2, nqy = (d.ny + 1) / 2, nquad = nqx * nqy;
   if (cudaMalloc((void**)&h->qcnt, sizeof(int) * (size_t)nquad) != cudaSuccess) { cudaGetLastError(); h->qcnt = nullptr; return CTR_OK; }
   dim3 grid((nqx + 31) / 32, (nqy + 3) / 4), block(32, 4);

@@ -57,7 +57,7 @@ def test_ctypes_structs_match_header():
     import paper_1009_2288_b200 as ctr
     kinds = {"int32_t": C.c_int32, "float": C.c_float, "double": C.c_double, "constfloat*": C.POINTER(C.c_float)}
     for name, struct in (("ctr_geometry", ctr.ctr_geometry), ("ctr_params", ctr.ctr_params),
-                         ("ctr_sweep_stat", ctr.ctr_sweep_stat)):
+                         ("ctr_sweep_stat", ctr.ctr_sweep_stat), ("ctr_peaks", ctr.ctr_peaks)):
         hdr = _struct_fields(name)
         got = [(n, t) for n, t in struct._fields_]
         assert len(hdr) == len(got), name

@@ -172,9 +172,72 @@ def test_c5_full_size_operators(ctr, torch_cuda, orc):
     assert rel(pty, orc.back(cfg, case["sino"].astype(np.float64))) <= 1e-5
 
 
+# ------------------------------------------------------------------ configs[4] at FULL size, whole path
+GOLD = __import__("pathlib").Path(__file__).resolve().parent / "golden"
+
+
+def _c5_golden():
+    """tests/golden/c5_full_oracle.npz, written by tests/golden/make_c5_golden.py (oracle only): the oracle's
+    image after outer iterations 1..n_done of the full-size config, at 131072 seeded voxels + plane norms."""
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("make_c5_golden", GOLD / "make_c5_golden.py")
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    z = np.load(GOLD / "c5_full_oracle.npz")
+    assert str(z["oracle_sha"]) == mod.oracle_fingerprint(), "oracle code changed: rerun tests/golden/make_c5_golden.py"
+    cfg = get_config("c5")
+    assert (int(z["n_cgls"]), int(z["n_gd"])) == (cfg.n_cgls, cfg.n_gd)
+    assert np.array_equal(z["positions"], mod.sample_positions(cfg.nx * cfg.ny * cfg.nz))
+    return z
+
+
+def _c5_reconstruct_vs_golden(ctr, torch, n_outer):
+    z = _c5_golden()
+    assert int(z["n_done"]) >= n_outer
+    cfg = scaled_config("c5", n_outer=n_outer)
+    case = make_case(cfg, raster=False)
+    h = ctr.ctr_create(cfg)
+    img = torch.full(h.img_shape, float("nan"), device="cuda")
+    h.ctr_reconstruct(to_gpu(torch, case["sino"]), img, ctr.make_params(cfg))
+    torch.cuda.synchronize()
+    stats = h.ctr_get_stats()
+    h.close()
+    got = img.cpu().numpy().astype(np.float64)
+    log = z["log"][: n_outer * cfg.n_gd]
+    want_s, got_s = z[f"samples_{n_outer}"], got.ravel()[z["positions"]]
+    planes = np.sqrt((got.reshape(cfg.nz, -1) ** 2).sum(axis=1))
+    err = rel(got_s, want_s)
+    err_max = float(np.max(np.abs(got_s - want_s)) / np.max(np.abs(want_s)))
+    err_pl = float(np.max(np.abs(planes - z[f"planes_{n_outer}"]) / z[f"planes_{n_outer}"]))
+    ks = [r["k"] for r in stats]
+    sig = np.array([r["sigma"] for r in stats])
+    print(f"[parity] c5 full size {n_outer}x({cfg.n_cgls}+{cfg.n_gd}): sampled rel-L2 {err:.3e}, max-abs/max {err_max:.3e}, "
+          f"plane norms {err_pl:.3e}, |f| {np.linalg.norm(got):.6e} vs {float(z[f'norm_{n_outer}']):.6e}, ks {ks}")
+    assert got.min() >= 0.0 and np.isfinite(got).all()
+    assert ks == list(log[:, 1].astype(int))
+    assert float(np.max(np.abs(sig - log[:, 0]) / log[:, 0])) <= 2e-3
+    assert err <= 1e-3                      # north_star: final image within 1e-3 (on the seeded sample of voxels)
+    assert err_max <= 2e-3                  # no single sampled voxel far off
+    assert err_pl <= 1e-3                   # every z-plane's norm (all voxels enter)
+    assert abs(np.linalg.norm(got) - float(z[f"norm_{n_outer}"])) <= 1e-3 * float(z[f"norm_{n_outer}"])
+
+
+def test_c5_full_size_reconstruct_two_outer_iterations(ctr, torch_cuda):
+    """configs[4] at 512x512x128 / 60 x 384x512, 2 outer iterations at the config's schedule (10 CGLS + 5 GD)."""
+    _c5_reconstruct_vs_golden(ctr, torch_cuda, 2)
+
+
+@pytest.mark.slow
+def test_c5_full_size_reconstruct_all_stored_iterations(ctr, torch_cuda):
+    """as above for as many outer iterations as the stored oracle run reached (20 = BASELINE.json's full schedule)."""
+    n = int(_c5_golden()["n_done"])
+    if n <= 2:
+        pytest.skip("the stored oracle run holds 2 outer iterations only")
+    _c5_reconstruct_vs_golden(ctr, torch_cuda, n)
+
+
 def test_stored_matrices_equal_on_the_fly_kernels_3d(ctr, torch_cuda):
     """3D lookup tables (sliced ELL) vs the on-the-fly cone kernels: identical bits."""
-    import os
     torch = torch_cuda
     cfg = small3d()
     rng = np.random.default_rng(43)
@@ -182,12 +245,7 @@ def test_stored_matrices_equal_on_the_fly_kernels_3d(ctr, torch_cuda):
     y = rng.random((cfg.nviews, cfg.nv, cfg.nu)).astype(np.float32)
     res = []
     for no_tables in (False, True):
-        if no_tables:
-            os.environ["CTR_NO_TABLES"] = "1"
-        try:
-            h = ctr.ctr_create(cfg)
-        finally:
-            os.environ.pop("CTR_NO_TABLES", None)
+        h = ctr.ctr_create(cfg, flags=ctr.CTR_GEOM_NO_TABLES if no_tables else 0)
         sino = torch.full(h.sino_shape, float("nan"), device="cuda")
         img = torch.full(h.img_shape, float("nan"), device="cuda")
         h.ctr_forward(to_gpu(torch, x), sino)

@@ -30,8 +30,8 @@ def rel(a, b):
     return float(np.linalg.norm(np.asarray(a, np.float64) - b) / np.linalg.norm(b))
 
 
-def gpu_forward(ctr, torch, cfg, img):
-    h = ctr.ctr_create(cfg)
+def gpu_forward(ctr, torch, cfg, img, flags=0):
+    h = ctr.ctr_create(cfg, flags=flags)
     x = torch.from_numpy(np.ascontiguousarray(img, dtype=np.float32)).cuda()
     y = torch.full(h.sino_shape, float("nan"), dtype=torch.float32, device="cuda")
     h.ctr_forward(x, y)
@@ -40,8 +40,8 @@ def gpu_forward(ctr, torch, cfg, img):
     return y.cpu().numpy()
 
 
-def gpu_back(ctr, torch, cfg, sino):
-    h = ctr.ctr_create(cfg)
+def gpu_back(ctr, torch, cfg, sino, flags=0):
+    h = ctr.ctr_create(cfg, flags=flags)
     y = torch.from_numpy(np.ascontiguousarray(sino, dtype=np.float32)).cuda()
     x = torch.full(h.img_shape, float("nan"), dtype=torch.float32, device="cuda")
     h.ctr_back(y, x)
@@ -234,15 +234,9 @@ def test_sub_warp_widths(ctr, torch_cuda, orc, batch):
 # ------------------------------------------------------------------ stored matrices (single slice)
 def _both_ways(ctr, torch, cfg, x, y):
     """(P x, P^T y) with the stored sliced-ELL matrices and with the on-the-fly kernels."""
-    import os
     out = []
-    for no_tables in (False, True):
-        if no_tables:
-            os.environ["CTR_NO_TABLES"] = "1"
-        try:
-            out.append((gpu_forward(ctr, torch, cfg, x), gpu_back(ctr, torch, cfg, y)))
-        finally:
-            os.environ.pop("CTR_NO_TABLES", None)
+    for flags in (0, ctr.CTR_GEOM_NO_TABLES):
+        out.append((gpu_forward(ctr, torch, cfg, x, flags), gpu_back(ctr, torch, cfg, y, flags)))
     return out
 
 

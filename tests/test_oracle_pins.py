@@ -656,6 +656,27 @@ def test_reconstruct_positivity_and_restarted_cgls(orc):
     assert np.array_equal(w1, ww[:, 0])
 
 
+def test_composed_outer_loop_is_orc_reconstruct(orc):
+    """tests/golden/make_c5_golden.py composes O10 from the oracle's own steps so that it can checkpoint a long
+    run: the composition must be orc_reconstruct itself, bit for bit (2D and 3D)."""
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("make_c5_golden", GOLD / "make_c5_golden.py")
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    cfg2 = scaled_config("c1", n_outer=2, n_cgls=4, n_gd=3)
+    cfg3 = tiny3d(nx=10, ny=9, nz=6, nviews=8, nu=14, nv=10, n_outer=2, n_cgls=3, n_gd=2, lam=0.02)
+    rng = np.random.default_rng(12)
+    for cfg, sino in ((cfg2, make_case(cfg2)["sino"][0].astype(np.float64)),
+                      (cfg3, rng.random((cfg3.nviews, cfg3.nv, cfg3.nu)))):
+        want, _, log = orc.reconstruct(cfg, sino, cfg)
+        seen = []
+        got, glog = mod.composed_reconstruct(orc, cfg, sino, cfg.n_outer, lambda n, f, lg: seen.append(n))
+        assert np.array_equal(got.reshape(want.shape), want)
+        assert np.array_equal(glog[:, 1], log[:, 1])                       # Armijo indices
+        assert np.allclose(glog, log, rtol=1e-12, atol=0)                  # E0 is an OpenMP reduction: order may differ
+        assert seen == [1, 2]
+
+
 def test_reconstruct_c1_reduces_error_and_stays_positive(orc):
     """Sanity on the seeded c1 workload: positivity after every outer iteration
     and a reconstruction closer to the truth than the zero image."""
