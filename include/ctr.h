@@ -74,9 +74,11 @@ typedef struct {
 
 /* ctr_geometry.flags */
 enum {
-  CTR_GEOM_NO_TABLES = 1 /* do not build the stored matrices / hit tables (second strategy): every
+  CTR_GEOM_NO_TABLES = 1, /* do not build the stored matrices / hit tables (second strategy): every
                             p_ij is computed on the fly. Same bits either way; a low-memory mode and the tests' way
                             of checking that the tables hold exactly what the on-the-fly kernels compute. */
+  CTR_GEOM_NO_GRAPHS = 2  /* ctr_reconstruct launches every kernel itself instead of replaying a CUDA graph of the
+                            steady-state outer iteration (batch = 1 only; same kernels, same results). */
 };
 
 /* Iteration schedule and the constants the paper leaves open (readings S13, S14). */
@@ -166,7 +168,8 @@ long long ctr_launch_count(const ctr_handle* h);
 typedef struct {
   double fma_tflops;    /* fp32 FMA (FFMA), 2 flop each                                                        */
   double fma2_tflops;   /* packed fp32x2 FMA (FFMA2, sm_100), 4 flop each                                       */
-  double issue_gwinst;  /* warp instructions issued per second / 1e9 (FFMA and integer ALU interleaved)         */
+  double issue_gwinst;  /* warp instructions issued per second / 1e9 (the FFMA kernel: one pipe, 1 per clock and scheduler) */
+  double mixed_gwinst;  /* the same for FFMA and integer ALU instructions interleaved 1:1 (the integer pipe is slower) */
   double l1_tbs;        /* L1 data pipe: LDG.128 that hit in L1, TB/s (128 bytes per wavefront)                 */
   double smem_tbs;      /* shared memory: conflict-free LDS.128, TB/s                                           */
   double hbm_copy_gbs;  /* device-memory copy of 1 GiB, read + write bytes, GB/s                                */

@@ -53,6 +53,11 @@ struct Scal {
   unsigned* sel_rank;
   float* ginv;     // 1/||g|| of the newest CGLS gradient (0 when g = 0)
   float* coef;     // [CTR_MAX_BASIS][Bp] projections of g on the stored unit gradients
+  // fused sigma selection (ctr_tv.cu): candidate lists of the first radix pass
+  int* pred;            // top-11-bit bin of sigma^2 found by the previous sweep (the prediction; < 0: none)
+  unsigned* cand_cnt;   // entries appended to the slice's candidate list by the current first pass
+  unsigned* ovf;        // a block's staging buffer overflowed: the list is incomplete
+  int* hit;             // 1: the winning bin is covered by the list, passes 2 and 3 run on the list
 };
 
 // stored system matrix, sliced ELL (ctr_ell.cuh)
@@ -63,6 +68,18 @@ struct EllTable {
   size_t nrows, bytes;
 };
 
+// Ring of sweep records (ctr_get_stats). The slot of the CURRENT sweep is taken from a device-side sweep counter
+// (advanced by k_tv_apply), not from a host value baked into the launch, so that a captured CUDA graph of one outer
+// iteration writes consecutive records when it is replayed.
+struct StatRing {
+  ctr_sweep_stat* base;             // [CTR_STAT_SWEEPS][Bp]
+  unsigned long long* sweep;        // device counter: sweeps finished since the last reset
+  int Bp;
+#ifdef __CUDACC__
+  __device__ __forceinline__ ctr_sweep_stat* slot() const { return base + (size_t)(__ldcg(sweep) % CTR_STAT_SWEEPS) * Bp; }
+#endif
+};
+
 struct TvParams {
   float lambda, eps, c_armijo;
   int kmax;
@@ -70,6 +87,16 @@ struct TvParams {
   float t[CTR_MAX_ARMIJO];
 };
 
+}  // namespace ctr
+
+namespace ctr {
+// what a captured outer iteration has baked in (ctr_reconstruct)
+struct GraphKey {
+  const float* sino;
+  float* img;
+  ctr_params p;   // n_outer and warm_start zeroed
+  unsigned long long sel_k;
+};
 }  // namespace ctr
 
 struct ctr_handle {
@@ -94,6 +121,8 @@ struct ctr_handle {
   int* qcnt;            // [nquad] entries used per quad
   int hits_cap;
   ctr::EllTable ell_p, ell_pt;  // stored P (rows = rays) and P^T (rows = voxels), batch = 1 only; tab == NULL: on the fly
+  unsigned* cand;       // [Bp][cand_cap] candidate lists (bit patterns of N0^2 near the predicted sigma^2)
+  unsigned cand_cap;
   float* usi;           // CGLS iterate in the slice-interleaved layout (batch > 1)
   float* basis;         // [CTR_MAX_BASIS][nimg] unit CGLS gradients (S24), allocated in ctr_create
   int dots_blocks;      // resident blocks of k_reorth_dots on this device (its grid size)
@@ -104,11 +133,17 @@ struct ctr_handle {
   ctr::Scal sc;
   void* scal_block;
   ctr_sweep_stat* stats;     // device ring [CTR_STAT_SWEEPS][Bp]
+  unsigned long long* d_sweep;  // device copy of sweep_count (StatRing)
   long long sweep_count;     // sweeps recorded since the last reset
   unsigned long long sel_k;  // rank of the sigma order statistic (1-based), from the current quantile
   float sel_q;
   cudaStream_t last_stream;
   long long launches;
+  // CUDA graph of the steady-state outer iteration (batch = 1)
+  cudaStream_t gstream;       // capture stream (never executes anything)
+  cudaGraphExec_t graph_exec;
+  ctr::GraphKey graph_key;
+  long long graph_launches;   // kernels per replay
   // optional event profiler (ctr_profile_*)
   int prof_on;
   int prof_n;                 // intervals recorded
@@ -181,6 +216,7 @@ int cone_back(ctr_handle* h, const float* sino, float* out, int mode, const floa
 int tv_update_weights(ctr_handle* h, const float* f, float* w, cudaStream_t st);
 int tv_sweep(ctr_handle* h, float* f, const float* v, const float* w, float lambda, int clamp, int n0_valid,
              cudaStream_t st);  // n0_valid: h->n0 holds the face magnitudes of THIS f (tv_update_weights just ran)
+int tv_sweep_fused(ctr_handle* h, float* f, const float* v, float lambda, int clamp, cudaStream_t st);  // weights + sweep, no planes
 int tv_clamp(ctr_handle* h, float* f, cudaStream_t st);
 // implemented in ctr_api.cu: finishing pass of a segmented reduction (block partials in h->part)
 enum { CTR_FIN_ALPHA = 0, CTR_FIN_COEF = 1 };

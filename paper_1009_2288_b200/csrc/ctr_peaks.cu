@@ -61,28 +61,27 @@ __global__ void __launch_bounds__(PK_THREADS) k_peak_fma2(int iters, float seed,
 }
 
 // 2. warp-instruction issue: FFMA (FMA pipe) and LOP3 / IADD3 (ALU pipe) interleaved, all independent:
-// 8 FFMA + 8 integer instructions per group
+// 8 FFMA + 8 integer instructions per group (a ring of data-dependent xor / add so that ptxas cannot fold them)
 __global__ void __launch_bounds__(PK_THREADS) k_peak_issue(int iters, float seed, float* sink) {
   float a0 = seed + threadIdx.x, a1 = a0 + 1.f, a2 = a0 + 2.f, a3 = a0 + 3.f, a4 = a0 + 4.f, a5 = a0 + 5.f, a6 = a0 + 6.f,
         a7 = a0 + 7.f;
   unsigned b0 = threadIdx.x, b1 = b0 + 1, b2 = b0 + 2, b3 = b0 + 3, b4 = b0 + 4, b5 = b0 + 5, b6 = b0 + 6, b7 = b0 + 7;
   const float m = 0.999f, c = 0.001f;
-  const unsigned k = 0x9e3779b9u;
   for (int i = 0; i < iters; ++i) {
 #pragma unroll
     for (int u = 0; u < 8; ++u) {
       asm volatile(
-          "fma.rn.f32 %0, %0, %16, %17;\n\txor.b32 %8, %8, %18;\n\t"
-          "fma.rn.f32 %1, %1, %16, %17;\n\tadd.u32 %9, %9, %18;\n\t"
-          "fma.rn.f32 %2, %2, %16, %17;\n\txor.b32 %10, %10, %18;\n\t"
-          "fma.rn.f32 %3, %3, %16, %17;\n\tadd.u32 %11, %11, %18;\n\t"
-          "fma.rn.f32 %4, %4, %16, %17;\n\txor.b32 %12, %12, %18;\n\t"
-          "fma.rn.f32 %5, %5, %16, %17;\n\tadd.u32 %13, %13, %18;\n\t"
-          "fma.rn.f32 %6, %6, %16, %17;\n\txor.b32 %14, %14, %18;\n\t"
-          "fma.rn.f32 %7, %7, %16, %17;\n\tadd.u32 %15, %15, %18;"
+          "fma.rn.f32 %0, %0, %16, %17;\n\txor.b32 %8, %8, %9;\n\t"
+          "fma.rn.f32 %1, %1, %16, %17;\n\tadd.u32 %9, %9, %10;\n\t"
+          "fma.rn.f32 %2, %2, %16, %17;\n\txor.b32 %10, %10, %11;\n\t"
+          "fma.rn.f32 %3, %3, %16, %17;\n\tadd.u32 %11, %11, %12;\n\t"
+          "fma.rn.f32 %4, %4, %16, %17;\n\txor.b32 %12, %12, %13;\n\t"
+          "fma.rn.f32 %5, %5, %16, %17;\n\tadd.u32 %13, %13, %14;\n\t"
+          "fma.rn.f32 %6, %6, %16, %17;\n\txor.b32 %14, %14, %15;\n\t"
+          "fma.rn.f32 %7, %7, %16, %17;\n\tadd.u32 %15, %15, %8;"
           : "+f"(a0), "+f"(a1), "+f"(a2), "+f"(a3), "+f"(a4), "+f"(a5), "+f"(a6), "+f"(a7), "+r"(b0), "+r"(b1), "+r"(b2),
             "+r"(b3), "+r"(b4), "+r"(b5), "+r"(b6), "+r"(b7)
-          : "f"(m), "f"(c), "r"(k));
+          : "f"(m), "f"(c));
     }
   }
   const float s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
@@ -120,7 +119,7 @@ __global__ void __launch_bounds__(PK_THREADS) k_peak_smem(int iters, float* sink
     for (int u = 0; u < 8; ++u) {
       float4 v;
       const unsigned addr = (unsigned)__cvta_generic_to_shared(&sm[idx & 511u]);
-      asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+      asm volatile("ld.volatile.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
       acc += (v.x + v.y) + (v.z + v.w);
       idx += 32u;
     }
@@ -183,10 +182,11 @@ extern "C" int ctr_measure_peaks(ctr_peaks* out, int reps) {
   out->sm_count = sms;
   if (e == cudaSuccess) e = best_ms([&] { k_peak_fma<<<blocks, PK_THREADS>>>(iters, 1.0f, sink); }, reps, &ms);
   out->fma_tflops = threads * iters * 64.0 * 2.0 / (ms * 1e-3) / 1e12;
+  out->issue_gwinst = threads / 32.0 * iters * 64.0 / (ms * 1e-3) / 1e9;
   if (e == cudaSuccess) e = best_ms([&] { k_peak_fma2<<<blocks, PK_THREADS>>>(iters, 1.0f, sink); }, reps, &ms);
   out->fma2_tflops = threads * iters * 64.0 * 4.0 / (ms * 1e-3) / 1e12;
   if (e == cudaSuccess) e = best_ms([&] { k_peak_issue<<<blocks, PK_THREADS>>>(iters, 1.0f, sink); }, reps, &ms);
-  out->issue_gwinst = threads / 32.0 * iters * 128.0 / (ms * 1e-3) / 1e9;
+  out->mixed_gwinst = threads / 32.0 * iters * 128.0 / (ms * 1e-3) / 1e9;
   if (e == cudaSuccess) e = best_ms([&] { k_peak_l1<<<blocks, PK_THREADS>>>(iters, buf, sink); }, reps, &ms);
   out->l1_tbs = threads * iters * 8.0 * 16.0 / (ms * 1e-3) / 1e12;
   if (e == cudaSuccess) e = best_ms([&] { k_peak_smem<<<blocks, PK_THREADS>>>(iters, sink); }, reps, &ms);

@@ -49,24 +49,34 @@ __device__ __forceinline__ void fma4(float (&acc)[4], float w, const float4 f) {
 #define SI_FWD_WARPS 8 /* warps per block (16 adjacent rays at LQ = 16); 4, 16 and 32 measured slower */
 #endif
 
-template <int LQ, int MODE>
+// H = float4 slice quads per lane: a sub-warp has SW = LQ / H lanes. With 64 slices (LQ = 16) H = 2: a ray is
+// carried by 8 lanes that read the pixel as two contiguous 128-byte halves (quads l and l + 8), so a warp holds
+// four rays and one broadcast record read serves twice as many FMAs. ncu (round 1, H = 1) had the L1 data pipe
+// as the busiest unit at 78 %, a third of its wavefronts being the record traffic through shared memory; the
+// global wavefronts are already the algorithmic minimum (one per 128 bytes gathered).
+template <int LQ, int H, int MODE>
 __global__ void __launch_bounds__(SI_FWD_WARPS * 32, SI_FWD_MINB) k_si_forward(Dims d, const float4* __restrict__ rays,
                                                     const float4* __restrict__ img, float4* __restrict__ out,
                                                     const float4* __restrict__ bs, Scal sc, double* part,
                                                     unsigned* counter) {
-  constexpr int RW = 32 / LQ;  // rays per warp
+  constexpr int SW = LQ / H;   // lanes per ray
+  constexpr int RW = 32 / SW;  // rays per warp
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int q = lane % LQ, sub = lane / LQ;
+  const int q = lane % SW, sub = lane / SW;
   const int r = (blockIdx.x * SI_FWD_WARPS + warp) * RW + sub;
   const int gs = blockIdx.y;
   const bool live = r < d.nray;
-  float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+  float acc[H][4];
+#pragma unroll
+  for (int hh = 0; hh < H; ++hh)
+#pragma unroll
+    for (int c = 0; c < 4; ++c) acc[hh][c] = 0.0f;
   // per-slab records {pa, wa, pb, wb} of the sub-warp's ray, written by the lane that evaluated the slab
   // and read back as one broadcast LDS.128 per slab (a shuffle costs an L1 data-pipe wavefront each; four
   // of them per slab were 40 % of the pipe, measured in round 1). Rows are padded by one entry so that the
   // sub-warps of a warp hit different banks. (Interleaving the two rays' records per slab, and 8-byte
   // records with the second length recomputed as L - wa, were measured: no gain / 50 % slower.)
-  __shared__ float4 slab[SI_FWD_WARPS][RW][LQ + 1];
+  __shared__ float4 slab[SI_FWD_WARPS][RW][SW + 1];
   float4* myslab = slab[warp][sub];
 
   float x0 = 0.0f, m = 0.0f, L = 0.0f, K = 0.0f;
@@ -101,7 +111,7 @@ __global__ void __launch_bounds__(SI_FWD_WARPS * 32, SI_FWD_MINB) k_si_forward(D
   const int st_drv = (xdrv ? 1 : d.nx) * LQ;  // float4 stride of one slab step
   const int st_oth = (xdrv ? d.nx : 1) * LQ;  // float4 stride of one cell of the other axis
 
-  for (int sb = w_lo; sb < w_hi; sb += LQ) {
+  for (int sb = w_lo; sb < w_hi; sb += SW) {
     const int s = sb + q;
     int pa = 0, pb = 0;
     float wa = 0.0f, wb = 0.0f;
@@ -125,25 +135,47 @@ __global__ void __launch_bounds__(SI_FWD_WARPS * 32, SI_FWD_MINB) k_si_forward(D
     myslab[q] = make_float4(__int_as_float(pa), wa, __int_as_float(pb), wb);
     __syncwarp();
 #pragma unroll
-    for (int t = 0; t < LQ; ++t) {
+    for (int t = 0; t < SW; ++t) {
       const float4 rec = myslab[t];
-      if (rec.y != 0.0f) fma4(acc, rec.y, __ldg(base + __float_as_int(rec.x)));
-      if (rec.w != 0.0f) fma4(acc, rec.w, __ldg(base + __float_as_int(rec.z)));
+      if (rec.y != 0.0f) {
+        const float4* pa4 = base + __float_as_int(rec.x);
+#pragma unroll
+        for (int hh = 0; hh < H; ++hh) fma4(acc[hh], rec.y, __ldg(pa4 + hh * SW));
+      }
+      if (rec.w != 0.0f) {
+        const float4* pb4 = base + __float_as_int(rec.z);
+#pragma unroll
+        for (int hh = 0; hh < H; ++hh) fma4(acc[hh], rec.w, __ldg(pb4 + hh * SW));
+      }
     }
   }
   if (live) {
-    const size_t e = ((size_t)gs * d.nray + r) * LQ + q;
-    if (MODE == 1) {
-      const float4 b = __ldg(bs + e);
-      acc[0] = b.x - acc[0]; acc[1] = b.y - acc[1]; acc[2] = b.z - acc[2]; acc[3] = b.w - acc[3];
+#pragma unroll
+    for (int hh = 0; hh < H; ++hh) {
+      const size_t e = ((size_t)gs * d.nray + r) * LQ + q + hh * SW;
+      if (MODE == 1) {
+        const float4 b = __ldg(bs + e);
+        acc[hh][0] = b.x - acc[hh][0]; acc[hh][1] = b.y - acc[hh][1]; acc[hh][2] = b.z - acc[hh][2]; acc[hh][3] = b.w - acc[hh][3];
+      }
+      out[e] = make_float4(acc[hh][0], acc[hh][1], acc[hh][2], acc[hh][3]);
     }
-    out[e] = make_float4(acc[0], acc[1], acc[2], acc[3]);
   }
   if (MODE == 2) {
-    double v[4];
+    // ||out||^2 per slice: the thread's 4 H sums belong to slice quads q + hh SW
+    double v[4 * H];
 #pragma unroll
-    for (int c = 0; c < 4; ++c) v[c] = live ? (double)acc[c] * (double)acc[c] : 0.0;
-    block_partials_q<4, SI_FWD_WARPS>(v, LQ, part + (size_t)gs * gridDim.x * LQ * 4, blockIdx.x, threadIdx.x);
+    for (int hh = 0; hh < H; ++hh)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) v[hh * 4 + c] = live ? (double)acc[hh][c] * (double)acc[hh][c] : 0.0;
+    __shared__ double sm[4 * H][SI_FWD_WARPS][16];
+    block_sum_q<4 * H, SI_FWD_WARPS>(v, sm, SW, threadIdx.x);
+    if (threadIdx.x < SW) {
+      double* dst = part + ((size_t)gs * gridDim.x + blockIdx.x) * LQ * 4;
+#pragma unroll
+      for (int hh = 0; hh < H; ++hh)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) dst[(threadIdx.x + hh * SW) * 4 + c] = v[hh * 4 + c];
+    }
   }
 }
 
@@ -521,18 +553,22 @@ int si_to_planar(ctr_handle* h, const float* src, float* dst, size_t n, cudaStre
 // ------------------------------------------------------------------------------------------------
 // host side: dispatch on LQ (1, 2, 4, 8, 16)
 // ------------------------------------------------------------------------------------------------
+#ifndef SI_FWD_H
+#define SI_FWD_H 1 /* float4 slice quads per lane of k_si_forward at LQ = 16 (1: a ray per 16 lanes, 2: per 8 lanes) */
+#endif
 template <int LQ>
 static int si_forward_t(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st) {
   const Dims& d = h->d;
-  const int rays_per_block = SI_FWD_WARPS * (32 / LQ), nt = SI_FWD_WARPS * 32;
+  constexpr int H = LQ == 16 ? SI_FWD_H : 1;
+  const int rays_per_block = SI_FWD_WARPS * (32 / (LQ / H)), nt = SI_FWD_WARPS * 32;
   dim3 grid((d.nray + rays_per_block - 1) / rays_per_block, d.GS);
   unsigned* cnt = h->counters + 0 * d.G;
   const float4 *im = (const float4*)img, *b4 = (const float4*)bs;
   float4* o4 = (float4*)out;
   ProfScope prof(h, CTR_PROF_FORWARD, st);
-  if (mode == 0) k_si_forward<LQ, 0><<<grid, nt, 0, st>>>(d, h->rays, im, o4, b4, h->sc, h->part, cnt);
-  else if (mode == 1) k_si_forward<LQ, 1><<<grid, nt, 0, st>>>(d, h->rays, im, o4, b4, h->sc, h->part, cnt);
-  else k_si_forward<LQ, 2><<<grid, nt, 0, st>>>(d, h->rays, im, o4, b4, h->sc, h->part, cnt);
+  if (mode == 0) k_si_forward<LQ, H, 0><<<grid, nt, 0, st>>>(d, h->rays, im, o4, b4, h->sc, h->part, cnt);
+  else if (mode == 1) k_si_forward<LQ, H, 1><<<grid, nt, 0, st>>>(d, h->rays, im, o4, b4, h->sc, h->part, cnt);
+  else k_si_forward<LQ, H, 2><<<grid, nt, 0, st>>>(d, h->rays, im, o4, b4, h->sc, h->part, cnt);
   CTR_LAUNCHED(h);
   if (mode == 2) return reduce_finish(h, CTR_FIN_ALPHA, 4, (int)grid.x, 0, 0, 0, st);  // a = gamma/||P s||^2
   return CTR_OK;

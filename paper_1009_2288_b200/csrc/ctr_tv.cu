@@ -12,7 +12,7 @@
 namespace ctr {
 
 #ifndef TV_GMINB
-#define TV_GMINB 8 /* min blocks per SM of k_tv_gradient (register budget) */
+#define TV_GMINB 5 /* min blocks per SM of k_tv_gradient (register budget) */
 #endif
 #ifndef TV_FMINB
 #define TV_FMINB 6 /* same for k_tv_faces */
@@ -22,7 +22,10 @@ namespace ctr {
 // ---------------------------------------------------------------------------------------------
 // Neighbourhood access. The stencil of A2/A3 around voxel p needs f at p + {-1,0,1}^ndim minus
 // the far corners; we load the full 3x3 (2D) or 3x3x3 (3D) window with per-axis clamped indices
-// (replicate border, S12) so the formulas below need no special cases.
+// (replicate border, S12) so the formulas below need no special cases. The loads go through L1 (ld.global.nc):
+// neighbouring threads share eight of the nine cells, and with cache-bypassing loads every one of them went to
+// L2 (round 1: k_tv_faces at 0 % L1 hits and 19 % of DRAM peak). The image is never written by a kernel that
+// reads it through a window.
 // ---------------------------------------------------------------------------------------------
 template <int V, int ND>
 struct Window {
@@ -43,12 +46,12 @@ __device__ __forceinline__ void load_window(const Dims& d, const float* __restri
       for (int b = 0; b < 3; ++b)
 #pragma unroll
         for (int c = 0; c < 3; ++c)
-          Pack<V>::ldcg(base, ((size_t)zk[a] * d.ny + yj[b]) * d.nx + xi[c], w.c[ND == 3 ? a : 0][b][c]);
+          Pack<V>::ld(base, ((size_t)zk[a] * d.ny + yj[b]) * d.nx + xi[c], w.c[ND == 3 ? a : 0][b][c]);
   } else {
 #pragma unroll
     for (int b = 0; b < 3; ++b)
 #pragma unroll
-      for (int c = 0; c < 3; ++c) Pack<V>::ldcg(base, (size_t)yj[b] * d.nx + xi[c], w.c[0][b][c]);
+      for (int c = 0; c < 3; ++c) Pack<V>::ld(base, (size_t)yj[b] * d.nx + xi[c], w.c[0][b][c]);
   }
 }
 
@@ -115,12 +118,12 @@ struct Vox {
   bool active;
   unsigned blk, nblk;
 };
-__device__ __forceinline__ Vox vox_of_thread(const Dims& d, int rr, int rows) {
+__device__ __forceinline__ Vox vox_of_thread(const Dims& d, int rr, int rows, int br = 4) {
   Vox v;
-  const int nby = (d.ny + 4 * rows - 1) / (4 * rows);
+  const int nby = (d.ny + br * rows - 1) / (br * rows);
   v.i = blockIdx.x * 32 + threadIdx.x;
   v.k = blockIdx.y / nby;
-  v.j = ((blockIdx.y - v.k * nby) * rows + rr) * 4 + threadIdx.y;
+  v.j = ((blockIdx.y - v.k * nby) * rows + rr) * br + threadIdx.y;
   v.g = blockIdx.z;
   v.tid = threadIdx.y * 32 + threadIdx.x;
   v.active = v.i < d.nx && v.j < d.ny;
@@ -128,8 +131,8 @@ __device__ __forceinline__ Vox vox_of_thread(const Dims& d, int rr, int rows) {
   v.nblk = gridDim.x * gridDim.y;
   return v;
 }
-static dim3 vox_grid(const Dims& d, int rows) {
-  return dim3((d.nx + 31) / 32, ((d.ny + 4 * rows - 1) / (4 * rows)) * d.nz, d.G);
+static dim3 vox_grid(const Dims& d, int rows, int br = 4) {
+  return dim3((d.nx + 31) / 32, ((d.ny + br * rows - 1) / (br * rows)) * d.nz, d.G);
 }
 // row groups per block: as many as leave at least ~16 blocks per SM (8 for the 256-thread trial kernel)
 static int tv_rows(const Dims& d, int rows_per_group, int max_rows, int min_blocks) {
@@ -246,9 +249,12 @@ __global__ void __launch_bounds__(128) k_tv_hist(Dims d, int rows, const float* 
 
 // a4.3  per slice: find the bin holding the element of rank sel_rank, extend the prefix, clear the
 // histogram. After the last pass the prefix IS the bit pattern of the k-th smallest N0^2 (O6).
+// Fused path (lists != 0): after the first pass the slice is a HIT when the bin found lies within one bin of the
+// prediction (so every value of that bin is in the candidate list), no staging buffer overflowed and the list
+// fits; after the final pass the bin becomes the next sweep's prediction and the list is emptied.
 __global__ void __launch_bounds__(256) k_tv_select(Scal sc, unsigned* __restrict__ hist, int nbins, int shift,
                                                    int first, int final_pass, unsigned long long rank0, float eps2,
-                                                   ctr_sweep_stat* stats, int nslices) {
+                                                   StatRing ring, int lists, unsigned cand_cap) {
   __shared__ unsigned tot[256];
   __shared__ unsigned found_bin, found_before;
   const int sl = blockIdx.x, t = threadIdx.x;
@@ -280,19 +286,195 @@ __global__ void __launch_bounds__(256) k_tv_select(Scal sc, unsigned* __restrict
     const unsigned prefix = (first ? 0u : sc.sel_prefix[sl]) | (found_bin << shift);
     sc.sel_prefix[sl] = prefix;
     sc.sel_rank[sl] = rank - found_before;
+    if (lists && first) {
+      const int dbin = (int)found_bin - sc.pred[sl];
+      sc.hit[sl] = (dbin >= -1 && dbin <= 1 && sc.ovf[sl] == 0u && sc.cand_cnt[sl] <= cand_cap) ? 1 : 0;
+    }
     if (final_pass) {
       const float s2 = fmaxf(__uint_as_float(prefix), eps2);
       sc.sigma2[sl] = s2;
-      if (stats) stats[sl].sigma = sqrt((double)s2);
+      ring.slot()[sl].sigma = sqrt((double)s2);
+      if (lists) {
+        sc.pred[sl] = (int)(prefix >> 20);
+        sc.cand_cnt[sl] = 0u;
+        sc.ovf[sl] = 0u;
+      }
     }
   }
-  (void)nslices;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Fused sigma selection (ctr_reconstruct): no N0^2 planes. The face magnitudes are recomputed from the L1-cached
+// window wherever they are needed (4 B per voxel read instead of 8 B written + 8 B read back per pass), and
+// the second and third radix passes run on a CANDIDATE LIST instead of the image: sigma moves little from one
+// sweep to the next, so the first pass appends every value whose top 11 bits lie within one bin of the bin the
+// previous sweep found (a few per cent of the faces) to a per-slice list - staged per block in shared memory,
+// one global atomicAdd per block and slice - and if the winning bin is indeed covered (k_tv_select: HIT), passes
+// 2 and 3 only filter that list. On a MISS (first sweep, or sigma jumped) the blocks of k_tv_scan23 recompute the
+// magnitudes from the image instead: same counts, so sigma is the exact order statistic either way (O6).
+// ---------------------------------------------------------------------------------------------
+#define TV_SCAP(V) (3072 / (V)) /* staging entries per block and slice (a block sees 32 x 8 x rows voxels x ND faces per slice) */
+#ifndef TV_SMINB
+#define TV_SMINB 3
+#endif
+
+template <int V, int ND>
+__device__ __forceinline__ void own_face_values(const Dims& d, const Window<V, ND>& w, const int (&pos)[3],
+                                                const int (&lim)[3], float (&val)[ND][V]) {
+  const int cz = (ND == 3) ? 1 : 0;
+#pragma unroll
+  for (int A = 0; A < ND; ++A) {
+    if (V % 2 == 0) {
+#pragma unroll
+      for (int hh = 0; hh < V / 2; ++hh) {
+        const float2 t = face_n0sq2<V, ND>(w, A, cz, 1, 1, hh);
+        val[A][2 * hh] = pos[A] < lim[A] ? t.x : 0.0f;
+        val[A][2 * hh + (V > 1)] = pos[A] < lim[A] ? t.y : 0.0f;
+      }
+    } else {
+#pragma unroll
+      for (int s = 0; s < V; ++s) val[A][s] = pos[A] < lim[A] ? face_n0sq<V, ND>(w, A, cz, 1, 1, s) : 0.0f;
+    }
+  }
+  (void)d;
+}
+
+template <int V, int ND>
+__global__ void __launch_bounds__(256, TV_SMINB) k_tv_scan1(Dims d, int rows, const float* __restrict__ f,
+                                                            unsigned* __restrict__ hist, Scal sc,
+                                                            unsigned* __restrict__ cand, unsigned cap) {
+  __shared__ unsigned hs[V][2048];
+  __shared__ unsigned stage[V][TV_SCAP(V)];
+  __shared__ unsigned stage_n[V], stage_base[V];
+  const int tid0 = threadIdx.y * 32 + threadIdx.x;
+  for (int t = tid0; t < V * 2048; t += 256) (&hs[0][0])[t] = 0;
+  if (tid0 < V) stage_n[tid0] = 0;
+  int pred[V];
+#pragma unroll
+  for (int s = 0; s < V; ++s) pred[s] = sc.pred[blockIdx.z * V + s];
+  __syncthreads();
+  const int lim[3] = {d.nx - 1, d.ny - 1, d.nz - 1};
+  for (int rr = 0; rr < rows; ++rr) {
+    const Vox p = vox_of_thread(d, rr, rows, 8);
+    const int pos[3] = {p.i, p.j, p.k};
+    float val[ND][V];
+    if (p.active) {
+      Window<V, ND> w;
+      load_window<V, ND>(d, f, p.g, p.i, p.j, p.k, w);
+      own_face_values<V, ND>(d, w, pos, lim, val);
+    }
+#pragma unroll
+    for (int A = 0; A < ND; ++A) {
+      const bool valid = p.active && pos[A] < lim[A];
+#pragma unroll
+      for (int s = 0; s < V; ++s) {
+        const unsigned bits = valid ? __float_as_uint(val[A][s]) : 0u;
+        hist_add(hs[s], bits, 20, 2047u, valid);
+        const int dbin = (int)(bits >> 20) - pred[s];
+        if (valid && dbin >= -1 && dbin <= 1) {
+          const unsigned at = atomicAdd(&stage_n[s], 1u);
+          if (at < TV_SCAP(V)) stage[s][at] = bits;
+        }
+      }
+    }
+  }
+  __syncthreads();
+  for (int t = tid0; t < V * 2048; t += 256) {
+    const unsigned c = (&hs[0][0])[t];
+    if (c) atomicAdd(&hist[(size_t)(blockIdx.z * V + t / 2048) * 2048 + (t & 2047)], c);
+  }
+  if (tid0 < V) {
+    const int sl = blockIdx.z * V + tid0;
+    unsigned n = stage_n[tid0];
+    if (n > TV_SCAP(V)) { atomicOr(&sc.ovf[sl], 1u); n = TV_SCAP(V); }
+    stage_n[tid0] = n;
+    stage_base[tid0] = n ? atomicAdd(&sc.cand_cnt[sl], n) : 0u;
+  }
+  __syncthreads();
+#pragma unroll
+  for (int s = 0; s < V; ++s) {
+    const unsigned n = stage_n[s], base = stage_base[s];
+    unsigned* dst = cand + (size_t)(blockIdx.z * V + s) * cap;
+    for (unsigned t = tid0; t < n; t += 256)
+      if (base + t < cap) dst[base + t] = stage[s][t];
+  }
+}
+
+// passes 2 and 3 of the fused selection: histogram of the next bits of the values that carry the prefix found
+// so far; from the candidate lists when every slice of the group was a hit, from the image otherwise
+template <int V, int ND>
+__global__ void __launch_bounds__(256, TV_SMINB) k_tv_scan23(Dims d, int rows, const float* __restrict__ f,
+                                                             unsigned* __restrict__ hist, Scal sc,
+                                                             const unsigned* __restrict__ cand, unsigned cap, int shift,
+                                                             unsigned mask, int prefix_shift) {
+  __shared__ unsigned hs[V][1024];
+  const int tid0 = threadIdx.y * 32 + threadIdx.x;
+  bool hit = true;
+  unsigned pre[V], cnt[V], maxc = 0;
+#pragma unroll
+  for (int s = 0; s < V; ++s) {
+    const int sl = blockIdx.z * V + s;
+    hit = hit && sc.hit[sl] != 0;
+    pre[s] = sc.sel_prefix[sl] >> prefix_shift;
+    cnt[s] = sc.cand_cnt[sl];
+    maxc = max(maxc, cnt[s]);
+  }
+  const unsigned blk = blockIdx.y * gridDim.x + blockIdx.x, nblk = gridDim.x * gridDim.y;
+  if (hit && blk * 256u >= maxc) return;  // nothing of the lists falls to this block
+  for (int t = tid0; t < V * 1024; t += 256) (&hs[0][0])[t] = 0;
+  __syncthreads();
+  if (hit) {
+#pragma unroll
+    for (int s = 0; s < V; ++s) {
+      const unsigned* src = cand + (size_t)(blockIdx.z * V + s) * cap;
+      for (unsigned e = blk * 256u + tid0; e < cnt[s]; e += nblk * 256u) {
+        const unsigned bits = __ldcg(src + e);
+        if ((bits >> prefix_shift) == pre[s]) atomicAdd(&hs[s][(bits >> shift) & mask], 1u);
+      }
+    }
+  } else {
+    const int lim[3] = {d.nx - 1, d.ny - 1, d.nz - 1};
+    for (int rr = 0; rr < rows; ++rr) {
+      const Vox p = vox_of_thread(d, rr, rows, 8);
+      const int pos[3] = {p.i, p.j, p.k};
+      float val[ND][V];
+      if (p.active) {
+        Window<V, ND> w;
+        load_window<V, ND>(d, f, p.g, p.i, p.j, p.k, w);
+        own_face_values<V, ND>(d, w, pos, lim, val);
+      }
+#pragma unroll
+      for (int A = 0; A < ND; ++A) {
+        const bool inside = p.active && pos[A] < lim[A];
+        unsigned bits[V];
+        bool valid[V], anyv = false;
+#pragma unroll
+        for (int s = 0; s < V; ++s) {
+          bits[s] = inside ? __float_as_uint(val[A][s]) : 0u;
+          valid[s] = inside && (bits[s] >> prefix_shift) == pre[s];
+          anyv |= valid[s];
+        }
+        if (!__any_sync(0xffffffffu, anyv)) continue;
+#pragma unroll
+        for (int s = 0; s < V; ++s) hist_add(hs[s], bits[s], shift, mask, valid[s]);
+      }
+    }
+  }
+  __syncthreads();
+  for (int t = tid0; t < V * 1024; t += 256) {
+    const unsigned c = (&hs[0][0])[t];
+    if (c) atomicAdd(&hist[(size_t)(blockIdx.z * V + t / 1024) * 2048 + (t & 1023)], c);
+  }
 }
 
 // a4.4  w = exp(-N0^2/sigma^2) on interior faces, 0 on border faces; TV mode: 1
 template <int V, int ND>
 __global__ void __launch_bounds__(128) k_tv_weights(Dims d, int rows, const float* __restrict__ n0, float* __restrict__ w,
-                                                    Scal sc, int mode) {
+                                                    Scal sc, int mode, StatRing ring) {
+  if (mode == 1 && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0 && threadIdx.y == 0) {
+#pragma unroll
+    for (int s = 0; s < V; ++s) ring.slot()[blockIdx.z * V + s].sigma = 0.0;  // plain TV: no sigma (documented as 0)
+  }
   float inv[V];
 #pragma unroll
   for (int s = 0; s < V; ++s) inv[s] = -1.0f / sc.sigma2[blockIdx.z * V + s];
@@ -317,17 +499,31 @@ __global__ void __launch_bounds__(128) k_tv_weights(Dims d, int rows, const floa
 // a5  gradient g = lambda (f - v) - sum_A (flux_A(p) - flux_A(p - e_A)),
 //     flux_A = w_A d_A / sqrt(N0^2 + eps^2) (A2), plus G = ||g||^2 and E0 (O9).
 // ---------------------------------------------------------------------------------------------
-// N0ST = 1: the N0^2 planes written by k_tv_faces for THIS f are read back (ctr_reconstruct: the weight
-// update of the same sweep has just produced them); N0ST = 0: recomputed from the window (ctr_eptv_step,
-// where the caller's x need not be the image of the last weight update).
-template <int V, int ND, int N0ST>
+// WSRC = 0: the weights come from the caller's planes w (ctr_eptv_step: they need not belong to this x);
+// WSRC = 1: fused path of ctr_reconstruct, w = exp(-N0^2/sigma^2) (A3) is evaluated on the fly
+// from the magnitudes of THIS f and the sigma^2 the selection has just left in sc.sigma2 (TV mode: w = 1): no
+// weight planes, no magnitude planes. Either way N0^2 of the four (six) faces of a voxel is recomputed from its
+// window: all their stencils lie inside it.
+__device__ __forceinline__ float edge_weight(float n0sq, float neg_inv_s2) { return __expf(n0sq * neg_inv_s2); }
+// one MUFU.RSQ, no denormal fix-up: the arguments are N0^2 + eps^2 (1e-8 with the default eps); callers treat
+// anything below 1e-30 as a flat face
+__device__ __forceinline__ float rsqrt_fast(float x) {
+  float r;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+
+template <int V, int ND, int WSRC>
 __global__ void __launch_bounds__(128, TV_GMINB) k_tv_gradient(Dims d, int rows, const float* __restrict__ f, const float* __restrict__ v,
-                                                     const float* __restrict__ w, const float* __restrict__ n0st,
-                                                     float* __restrict__ gout, TvParams tp, Scal sc, double* part,
-                                                     unsigned* counter) {
+                                                     const float* __restrict__ w, float* __restrict__ gout, TvParams tp,
+                                                     Scal sc, double* part, unsigned* counter, StatRing ring) {
   double red[2 * V];
 #pragma unroll
   for (int s = 0; s < 2 * V; ++s) red[s] = 0.0;
+  float nis2[V];
+#pragma unroll
+  for (int s = 0; s < V; ++s) nis2[s] = WSRC ? -1.0f / sc.sigma2[blockIdx.z * V + s] : 0.0f;
+  const int lim[3] = {d.nx - 1, d.ny - 1, d.nz - 1};
   for (int rr = 0; rr < rows; ++rr) {
   const Vox p = vox_of_thread(d, rr, rows);
   if (p.active) {
@@ -349,33 +545,45 @@ __global__ void __launch_bounds__(128, TV_GMINB) k_tv_gradient(Dims d, int rows,
 #pragma unroll
     for (int A = 0; A < ND; ++A) {
       float wp[V], wm[V];
-      Pack<V>::ldcg(w + A * plane, e, wp);  // border faces store 0
-      if (pos[A] > 0) Pack<V>::ldcg(w + A * plane, e - stride[A], wm);
-      else {
-#pragma unroll
-        for (int s = 0; s < V; ++s) wm[s] = 0.0f;
-      }
-      const int ez = (A == 2), ey = (A == 1), ex = (A == 0);
-      float sp[V], sm_[V];
-      if (N0ST) {
-        Pack<V>::ldcg(n0st + A * plane, e, sp);
-        if (pos[A] > 0) Pack<V>::ldcg(n0st + A * plane, e - stride[A], sm_);
+      if (!WSRC) {
+        Pack<V>::ldcg(w + A * plane, e, wp);  // border faces store 0
+        if (pos[A] > 0) Pack<V>::ldcg(w + A * plane, e - stride[A], wm);
         else {
 #pragma unroll
-          for (int s = 0; s < V; ++s) sm_[s] = 0.0f;
+          for (int s = 0; s < V; ++s) wm[s] = 0.0f;
+        }
+      }
+      const int ez = (A == 2), ey = (A == 1), ex = (A == 0);
+      float rp[V], rm[V];  // raw N0^2 of the face towards +A (owned by this voxel) and towards -A (owned by the neighbour)
+      if (V % 2 == 0) {
+#pragma unroll
+        for (int hh = 0; hh < V / 2; ++hh) {
+          const float2 a = face_n0sq2<V, ND>(win, A, cz, 1, 1, hh), b = face_n0sq2<V, ND>(win, A, cz - ez, 1 - ey, 1 - ex, hh);
+          rp[2 * hh] = a.x; rp[2 * hh + (V > 1)] = a.y;
+          rm[2 * hh] = b.x; rm[2 * hh + (V > 1)] = b.y;
+        }
+      } else {
+#pragma unroll
+        for (int s = 0; s < V; ++s) {
+          rp[s] = face_n0sq<V, ND>(win, A, cz, 1, 1, s);
+          rm[s] = face_n0sq<V, ND>(win, A, cz - ez, 1 - ey, 1 - ex, s);
         }
       }
 #pragma unroll
       for (int s = 0; s < V; ++s) {
-        // face towards +A (owned by this voxel) and face towards -A (owned by the neighbour)
-        const float n0p = (N0ST ? sp[s] : face_n0sq<V, ND>(win, A, cz, 1, 1, s)) + eps2;
-        const float n0m = (N0ST ? sm_[s] : face_n0sq<V, ND>(win, A, cz - ez, 1 - ey, 1 - ex, s)) + eps2;
+        if (WSRC) {
+          wp[s] = pos[A] < lim[A] ? (tp.weights_mode == 1 ? 1.0f : edge_weight(rp[s], nis2[s])) : 0.0f;
+          wm[s] = pos[A] > 0 ? (tp.weights_mode == 1 ? 1.0f : edge_weight(rm[s], nis2[s])) : 0.0f;
+        }
+        const float n0p = rp[s] + eps2, n0m = rm[s] + eps2;
         const float dp = win.c[cz + ez][1 + ey][1 + ex][s] - win.c[cz][1][1][s];
         const float dm = win.c[cz][1][1][s] - win.c[cz - ez][1 - ey][1 - ex][s];
-        const float fp = (wp[s] != 0.0f && n0p > 0.0f) ? wp[s] * dp * rsqrtf(n0p) : 0.0f;
-        const float fm = (wm[s] != 0.0f && n0m > 0.0f) ? wm[s] * dm * rsqrtf(n0m) : 0.0f;
+        // sqrt(x) = x rsqrt(x): one special-function instruction per face serves both the flux and the energy
+        const float ip = n0p > 1e-30f ? rsqrt_fast(n0p) : 0.0f, im = n0m > 1e-30f ? rsqrt_fast(n0m) : 0.0f;
+        const float fp = wp[s] * dp * ip;
+        const float fm = wm[s] * dm * im;
         gv[s] -= fp - fm;
-        etv[s] = fmaf(wp[s], sqrtf(n0p) - tp.eps, etv[s]);
+        etv[s] = fmaf(wp[s], fmaf(n0p, ip, -tp.eps), etv[s]);
       }
     }
     Pack<V>::st(gout, e, gv);
@@ -397,6 +605,7 @@ __global__ void __launch_bounds__(128, TV_GMINB) k_tv_gradient(Dims d, int rows,
                          sc.e0[sl] = sum[V + s];
                          sc.kacc[sl] = -1;
                          sc.tacc[sl] = 0.0f;
+                         if (WSRC && tp.weights_mode == 1) ring.slot()[sl].sigma = 0.0;  // plain TV: no sigma
                        }
                      });
 }
@@ -479,7 +688,9 @@ __device__ __forceinline__ void face_forms2(const Window<V, ND>& wf, const Windo
 #ifndef TV_TMINB
 #define TV_TMINB 3
 #endif
-template <int V, int ND>
+// WSRC as in k_tv_gradient: 0 = weight planes of the caller, 1 = w = exp(-N0^2(f)/sigma^2) on the fly (N0^2(f) is
+// the form `a` below: the same stencil as face_n0sq(), differences taken in another order)
+template <int V, int ND, int WSRC>
 __global__ void __launch_bounds__(32 * TV_TW, TV_TMINB) k_tv_trial(Dims d, int rows, const float* __restrict__ f, const float* __restrict__ gin,
                                                   const float* __restrict__ v, const float* __restrict__ w, TvParams tp,
                                                   int k0, Scal sc, double* part) {
@@ -496,6 +707,10 @@ __global__ void __launch_bounds__(32 * TV_TW, TV_TMINB) k_tv_trial(Dims d, int r
 #pragma unroll
   for (int s = 0; s < V; ++s) { todo[s] = sc.kacc[g * V + s] < 0; any |= todo[s]; }
   if (!any) return;
+  float nis2[V];
+#pragma unroll
+  for (int s = 0; s < V; ++s) nis2[s] = WSRC ? -1.0f / sc.sigma2[g * V + s] : 0.0f;
+  const int lim[3] = {d.nx - 1, d.ny - 1, d.nz - 1};
   float et[NE];
   double dd[3 * V];
 #pragma unroll
@@ -513,6 +728,7 @@ __global__ void __launch_bounds__(32 * TV_TW, TV_TMINB) k_tv_trial(Dims d, int r
     const size_t e = (size_t)g * d.npix + ((size_t)k * d.ny + j) * d.nx + i;
     const size_t plane = (size_t)d.G * d.npix * V;
     const float eps = tp.eps, eps2 = tp.eps * tp.eps;
+    const int pos[3] = {i, j, k};
     float vv[V];
     Pack<V>::ldcg(v, e, vv);
 #pragma unroll
@@ -530,11 +746,16 @@ __global__ void __launch_bounds__(32 * TV_TW, TV_TMINB) k_tv_trial(Dims d, int r
 #pragma unroll
       for (int A = 0; A < ND; ++A) {
         float wv[V];
-        Pack<V>::ldcg(w + A * plane, e, wv);  // border faces store 0
+        if (!WSRC) Pack<V>::ldcg(w + A * plane, e, wv);  // border faces store 0
 #pragma unroll
         for (int hh = 0; hh < H; ++hh) {
           float2 a, b, c;
           face_forms2<V, ND>(wf, wg, A, hh, a, b, c);
+          if (WSRC) {
+            const bool in = pos[A] < lim[A];
+            wv[2 * hh] = in ? (tp.weights_mode == 1 ? 1.0f : edge_weight(a.x, nis2[2 * hh])) : 0.0f;
+            wv[2 * hh + (V > 1)] = in ? (tp.weights_mode == 1 ? 1.0f : edge_weight(a.y, nis2[2 * hh + (V > 1)])) : 0.0f;
+          }
           fa[A][hh] = __fadd2_rn(a, eps22);
           fb[A][hh] = __fmul2_rn(m2, b);
           fc[A][hh] = c;
@@ -574,11 +795,12 @@ __global__ void __launch_bounds__(32 * TV_TW, TV_TMINB) k_tv_trial(Dims d, int r
       float fa[ND][V], fb[ND][V], fc[ND][V], wA[ND][V];
   #pragma unroll
       for (int A = 0; A < ND; ++A) {
-        Pack<V>::ldcg(w + A * plane, e, wA[A]);  // border faces store 0
+        if (!WSRC) Pack<V>::ldcg(w + A * plane, e, wA[A]);  // border faces store 0
   #pragma unroll
         for (int s = 0; s < V; ++s) {
           float a, b, c;
           face_forms<V, ND>(wf, wg, A, s, a, b, c);
+          if (WSRC) wA[A][s] = pos[A] < lim[A] ? (tp.weights_mode == 1 ? 1.0f : edge_weight(a, nis2[s])) : 0.0f;
           fa[A][s] = a + eps2;
           fb[A][s] = -2.0f * b;
           fc[A][s] = c;
@@ -690,17 +912,19 @@ __global__ void __launch_bounds__(1024) k_tv_trial_finish(const double* __restri
 // a6.2 + a7  f <- f - t g for slices that accepted a step; optional positivity clamp; sweep record.
 template <int V>
 __global__ void __launch_bounds__(256) k_tv_apply(Dims d, float* __restrict__ f, const float* __restrict__ gin, Scal sc,
-                                                  int clamp, ctr_sweep_stat* stats) {
+                                                  int clamp, StatRing ring) {
   const int g = blockIdx.y;
   const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
-  if (idx == 0 && stats) {
-#pragma unroll
-    for (int s = 0; s < V; ++s) {
-      const int sl = g * V + s;
-      stats[sl].e0 = sc.e0[sl];
-      stats[sl].g2 = sc.g2[sl];
-      stats[sl].k = sc.kacc[sl];
+  if (blockIdx.x == 0 && g == 0) {
+    // the sweep record of every slice, then the sweep counter moves on (one block: no other block reads it)
+    ctr_sweep_stat* rec = ring.slot();
+    for (int sl = threadIdx.x; sl < ring.Bp; sl += 256) {
+      rec[sl].e0 = sc.e0[sl];
+      rec[sl].g2 = sc.g2[sl];
+      rec[sl].k = sc.kacc[sl];
     }
+    __syncthreads();
+    if (threadIdx.x == 0) *ring.sweep = *ring.sweep + 1ull;
   }
   if (idx >= (size_t)d.npix) return;
   const size_t e = (size_t)g * d.npix + idx;
@@ -732,11 +956,16 @@ __global__ void __launch_bounds__(256) k_clamp(Dims d, float* __restrict__ f) {
 // ---------------------------------------------------------------------------------------------
 // host drivers
 // ---------------------------------------------------------------------------------------------
-static ctr_sweep_stat* stat_slot(ctr_handle* h) {
-  const int Bp = h->d.G * h->d.V;
-  return h->stats + (size_t)(h->sweep_count % CTR_STAT_SWEEPS) * Bp;
+static StatRing stat_slot(ctr_handle* h) {
+  StatRing r;
+  r.base = h->stats;
+  r.sweep = h->d_sweep;
+  r.Bp = h->d.G * h->d.V;
+  return r;
 }
 
+// weight planes for the caller (ctr_update_weights, and the last sweep of ctr_reconstruct_w): magnitudes to
+// h->n0, three radix passes over them, w = exp(-N0^2/sigma^2)
 template <int V, int ND>
 static int tv_update_weights_t(ctr_handle* h, const float* f, float* w, cudaStream_t st) {
   const Dims& d = h->d;
@@ -744,28 +973,26 @@ static int tv_update_weights_t(ctr_handle* h, const float* f, float* w, cudaStre
   const dim3 grid = vox_grid(d, rows), block(32, 4);
   const int Bp = d.G * d.V;
   const float eps2 = h->p.eps * h->p.eps;
-  ctr_sweep_stat* rec = stat_slot(h);
+  const StatRing rec = stat_slot(h);
   ProfScope prof(h, CTR_PROF_TV, st);
+  k_tv_faces<V, ND><<<grid, block, 0, st>>>(d, rows, f, h->n0, h->hist);
+  CTR_LAUNCHED(h);
   if (h->p.weights_mode == 1) {
-    // plain TV: weights are 1; sigma is not needed (reported as 0)
-    k_tv_faces<V, ND><<<grid, block, 0, st>>>(d, rows, f, h->n0, h->hist);
-    CTR_LAUNCHED(h);
+    // plain TV: weights are 1, sigma is not needed (the record says 0)
     CTR_CUDA(h, cudaMemsetAsync(h->hist, 0, sizeof(unsigned) * 2048 * Bp, st));
   } else {
-    k_tv_faces<V, ND><<<grid, block, 0, st>>>(d, rows, f, h->n0, h->hist);
-    CTR_LAUNCHED(h);
-    k_tv_select<<<Bp, 256, 0, st>>>(h->sc, h->hist, 2048, 20, 1, 0, h->sel_k, eps2, rec, Bp);
+    k_tv_select<<<Bp, 256, 0, st>>>(h->sc, h->hist, 2048, 20, 1, 0, h->sel_k, eps2, rec, 0, 0u);
     CTR_LAUNCHED(h);
     k_tv_hist<V, ND><<<grid, block, 0, st>>>(d, rows, h->n0, h->hist, h->sc, 10, 1023u, 20);
     CTR_LAUNCHED(h);
-    k_tv_select<<<Bp, 256, 0, st>>>(h->sc, h->hist, 1024, 10, 0, 0, 0, eps2, rec, Bp);
+    k_tv_select<<<Bp, 256, 0, st>>>(h->sc, h->hist, 1024, 10, 0, 0, 0, eps2, rec, 0, 0u);
     CTR_LAUNCHED(h);
     k_tv_hist<V, ND><<<grid, block, 0, st>>>(d, rows, h->n0, h->hist, h->sc, 0, 1023u, 10);
     CTR_LAUNCHED(h);
-    k_tv_select<<<Bp, 256, 0, st>>>(h->sc, h->hist, 1024, 0, 0, 1, 0, eps2, rec, Bp);
+    k_tv_select<<<Bp, 256, 0, st>>>(h->sc, h->hist, 1024, 0, 0, 1, 0, eps2, rec, 0, 0u);
     CTR_LAUNCHED(h);
   }
-  k_tv_weights<V, ND><<<grid, block, 0, st>>>(d, rows, h->n0, w, h->sc, h->p.weights_mode);
+  k_tv_weights<V, ND><<<grid, block, 0, st>>>(d, rows, h->n0, w, h->sc, h->p.weights_mode, rec);
   CTR_LAUNCHED(h);
   return CTR_OK;
 }
@@ -790,22 +1017,21 @@ static TvParams make_tv_params(const ctr_handle* h, float lambda) {
   return tp;
 }
 
-template <int V, int ND>
-static int tv_sweep_t(ctr_handle* h, float* f, const float* v, const float* w, float lambda, int clamp,
-                      int n0_valid, cudaStream_t st) {
+// gradient + Armijo trials + update; WSRC = 0: weights from the planes w, WSRC = 1: weights on the fly from
+// sc.sigma2 (fused path)
+template <int V, int ND, int WSRC>
+static int tv_descend_t(ctr_handle* h, float* f, const float* v, const float* w, float lambda, int clamp, cudaStream_t st) {
   const Dims& d = h->d;
   const int rows = tv_rows(d, 4, 8, 148 * 16);
   const dim3 grid = vox_grid(d, rows), block(32, 4);
   const TvParams tp = make_tv_params(h, lambda);
   float* g = h->gimg;
-  ProfScope prof(h, CTR_PROF_TV, st);
-  if (n0_valid) k_tv_gradient<V, ND, 1><<<grid, block, 0, st>>>(d, rows, f, v, w, h->n0, g, tp, h->sc, h->part, h->counters + 2 * d.G);
-  else k_tv_gradient<V, ND, 0><<<grid, block, 0, st>>>(d, rows, f, v, w, h->n0, g, tp, h->sc, h->part, h->counters + 2 * d.G);
+  k_tv_gradient<V, ND, WSRC><<<grid, block, 0, st>>>(d, rows, f, v, w, g, tp, h->sc, h->part, h->counters + 2 * d.G, stat_slot(h));
   CTR_LAUNCHED(h);
   const int trows = tv_rows(d, TV_TW, 16, 148 * 8);
   const dim3 tgrid((d.nx + 31) / 32, ((d.ny + TV_TW * trows - 1) / (TV_TW * trows)) * d.nz, d.G), tblock(32, TV_TW);
   for (int k0 = 0; k0 < tp.kmax; k0 += TV_KA) {
-    k_tv_trial<V, ND><<<tgrid, tblock, 0, st>>>(d, trows, f, g, v, w, tp, k0, h->sc, h->part);
+    k_tv_trial<V, ND, WSRC><<<tgrid, tblock, 0, st>>>(d, trows, f, g, v, w, tp, k0, h->sc, h->part);
     CTR_LAUNCHED(h);
     k_tv_trial_finish<V><<<d.G, 1024, 0, st>>>(h->part, (int)(tgrid.x * tgrid.y), tp, k0, d.ndim, h->sc);
     CTR_LAUNCHED(h);
@@ -818,9 +1044,43 @@ static int tv_sweep_t(ctr_handle* h, float* f, const float* v, const float* w, f
 
 int tv_sweep(ctr_handle* h, float* f, const float* v, const float* w, float lambda, int clamp, int n0_valid,
              cudaStream_t st) {
-  if (h->d.ndim == 3) return tv_sweep_t<1, 3>(h, f, v, w, lambda, clamp, n0_valid, st);
-  return h->d.V == 1 ? tv_sweep_t<1, 2>(h, f, v, w, lambda, clamp, n0_valid, st)
-                     : tv_sweep_t<4, 2>(h, f, v, w, lambda, clamp, n0_valid, st);
+  (void)n0_valid;
+  ProfScope prof(h, CTR_PROF_TV, st);
+  if (h->d.ndim == 3) return tv_descend_t<1, 3, 0>(h, f, v, w, lambda, clamp, st);
+  return h->d.V == 1 ? tv_descend_t<1, 2, 0>(h, f, v, w, lambda, clamp, st) : tv_descend_t<4, 2, 0>(h, f, v, w, lambda, clamp, st);
+}
+
+// One GD sweep of ctr_reconstruct without any plane: sigma by the fused selection (k_tv_scan1 / k_tv_scan23 above),
+// then gradient, trials and update with the weights evaluated on the fly.
+template <int V, int ND>
+static int tv_sweep_fused_t(ctr_handle* h, float* f, const float* v, float lambda, int clamp, cudaStream_t st) {
+  const Dims& d = h->d;
+  ProfScope prof(h, CTR_PROF_TV, st);
+  if (h->p.weights_mode == 0) {
+    const int rows = tv_rows(d, 8, 8, 148 * 8);
+    const dim3 grid = vox_grid(d, rows, 8), block(32, 8);
+    const int Bp = d.G * d.V;
+    const float eps2 = h->p.eps * h->p.eps;
+    const StatRing rec = stat_slot(h);
+    k_tv_scan1<V, ND><<<grid, block, 0, st>>>(d, rows, f, h->hist, h->sc, h->cand, h->cand_cap);
+    CTR_LAUNCHED(h);
+    k_tv_select<<<Bp, 256, 0, st>>>(h->sc, h->hist, 2048, 20, 1, 0, h->sel_k, eps2, rec, 1, h->cand_cap);
+    CTR_LAUNCHED(h);
+    k_tv_scan23<V, ND><<<grid, block, 0, st>>>(d, rows, f, h->hist, h->sc, h->cand, h->cand_cap, 10, 1023u, 20);
+    CTR_LAUNCHED(h);
+    k_tv_select<<<Bp, 256, 0, st>>>(h->sc, h->hist, 1024, 10, 0, 0, 0, eps2, rec, 1, h->cand_cap);
+    CTR_LAUNCHED(h);
+    k_tv_scan23<V, ND><<<grid, block, 0, st>>>(d, rows, f, h->hist, h->sc, h->cand, h->cand_cap, 0, 1023u, 10);
+    CTR_LAUNCHED(h);
+    k_tv_select<<<Bp, 256, 0, st>>>(h->sc, h->hist, 1024, 0, 0, 1, 0, eps2, rec, 1, h->cand_cap);
+    CTR_LAUNCHED(h);
+  }
+  return tv_descend_t<V, ND, 1>(h, f, v, nullptr, lambda, clamp, st);
+}
+
+int tv_sweep_fused(ctr_handle* h, float* f, const float* v, float lambda, int clamp, cudaStream_t st) {
+  if (h->d.ndim == 3) return tv_sweep_fused_t<1, 3>(h, f, v, lambda, clamp, st);
+  return h->d.V == 1 ? tv_sweep_fused_t<1, 2>(h, f, v, lambda, clamp, st) : tv_sweep_fused_t<4, 2>(h, f, v, lambda, clamp, st);
 }
 
 int tv_clamp(ctr_handle* h, float* f, cudaStream_t st) {

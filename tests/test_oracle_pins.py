@@ -712,6 +712,76 @@ def test_reconstruct_is_reproducible_under_the_S25_constants(orc):
     assert amplification(scaled_config("c1", armijo_c=1e-4, eps=1e-6)) > 1e3
 
 
+def test_S25_amplification_on_c2(orc):
+    """DESIGN.md S25 on configs[1] at its full schedule (20 x (10 CGLS + 5 GD)): the constants first proposed
+    (Armijo c = 1e-4, eps = 1e-6) amplify a 1e-8 perturbation of the data by > 1e3 (DESIGN.md quotes 2e5), the
+    built ones (c = 1/2, eps = 1e-4) by < 100 (quoted: 22)."""
+    rng = np.random.default_rng(5)
+    cfg = get_config("c2")
+    y = make_case(cfg, raster=False)["sino"][0].astype(np.float64)
+    yp = y * (1 + 1e-8 * rng.standard_normal(y.shape))
+
+    def amplification(c):
+        base, _, _ = orc.reconstruct(c, y, c)
+        pert, _, _ = orc.reconstruct(c, yp, c)
+        return np.linalg.norm(pert - base) / np.linalg.norm(base) / 1e-8
+
+    built = amplification(cfg)
+    proposed = amplification(scaled_config("c2", armijo_c=1e-4, eps=1e-6))
+    print(f"[S25] c2 amplification of a 1e-8 perturbation: built constants {built:.1f}, first proposal {proposed:.3g}")
+    assert built < 100
+    assert proposed > 1e3
+
+
+def _cgls_fp32_emulation(orc, cfg, y, M, select):
+    """The CUDA path's arithmetic emulated with the oracle's operators: fp64 recurrence, but P, P^T and every
+    stored vector rounded to fp32; each new gradient is projected against the unit gradients select(n) picks out
+    of the n stored so far (App. I; S24)."""
+    f32 = lambda a: a.astype(np.float32).astype(np.float64)
+    P = lambda x: f32(orc.forward(cfg, x))
+    PT = lambda r: f32(orc.back(cfg, r))
+    u = np.zeros((cfg.ny, cfg.nx))
+    r = y.copy()
+    g = PT(r)
+    gam = (g * g).sum()
+    s = g.copy()
+    B = [g / np.sqrt(gam)]
+    for _ in range(M):
+        q = P(s)
+        a = gam / (q * q).sum()
+        u = f32(u + a * s)
+        r = f32(r - a * q)
+        g = PT(r)
+        for i in select(len(B)):
+            g = g - (B[i] * g).sum() * B[i]
+        g = f32(g)
+        gn = (g * g).sum()
+        s = f32(g + gn / gam * s)
+        gam = gn
+        B.append(g / np.sqrt(gn))
+    return u
+
+
+@pytest.mark.parametrize("name", ["c1", "c2"])
+def test_S24_projecting_against_the_first_four_gradients_tracks_the_full_reorthogonalisation(orc, name):
+    """DESIGN.md S24, table rows "nothing", "first 4", "all": in fp32-rounded arithmetic the printed recurrence
+    drifts from the exact-arithmetic iterate (the oracle's fully re-orthogonalised CGLS) by ~1e-2 after 10
+    iterations, while projecting each new gradient against the FIRST FOUR unit gradients only - what the CUDA
+    path does (CTR_MAX_BASIS = 4) - stays as close to it as projecting against all of them."""
+    cfg = scaled_config(name, batch=1)
+    y = make_case(cfg, raster=False)["sino"][0].astype(np.float64)
+    M = 10
+    ref = orc.cgls(cfg, y, np.zeros((cfg.ny, cfg.nx)), M)
+    rel = lambda a: np.linalg.norm(a - ref) / np.linalg.norm(ref)
+    none = rel(_cgls_fp32_emulation(orc, cfg, y, M, lambda n: []))
+    first4 = rel(_cgls_fp32_emulation(orc, cfg, y, M, lambda n: range(min(4, n))))
+    full = rel(_cgls_fp32_emulation(orc, cfg, y, M, lambda n: range(n)))
+    print(f"[S24] {name}, {M} iterations, fp32-rounded emulation vs the oracle: nothing {none:.2e}, first 4 {first4:.2e}, all {full:.2e}")
+    assert none >= 3e-3
+    assert first4 <= 5e-5 and full <= 5e-5
+    assert first4 <= 3 * full + 1e-6
+
+
 # ------------------------------------------------------------------ NEXT-1: the paper's backprojector Eq. (11)
 def _paper_geometry(**kw):
     """PAPER.md:217: arc detector, 888 units x 1.0239 mm, source-detector 949.075 mm, source-axis 541.0 mm;
