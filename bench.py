@@ -49,6 +49,8 @@ def parse():
     ap.add_argument("--batch", type=int, default=0, help="override the number of slices (debug)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--geom-flags", type=int, default=0,
+                    help="ctr_geometry.flags (1 no tables, 2 no graphs, 4 batched P on the fly): A/B runs")
     return ap.parse_args()
 
 
@@ -199,7 +201,7 @@ def main():
     sino = sino_host.cuda(non_blocking=True)
     # on-chip peaks of THIS device, measured before anything is timed (roofline denominators)
     dev_peaks = ctr.ctr_measure_peaks(5)
-    h = ctr.ctr_create(cfg)
+    h = ctr.ctr_create(cfg, flags=args.geom_flags)
     path = h.ctr_path_info()
     img = torch.zeros(h.img_shape, device="cuda")
     img_host = torch.empty(h.img_shape, dtype=torch.float32).pin_memory()

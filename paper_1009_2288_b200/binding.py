@@ -39,6 +39,7 @@ class ctr_geometry(C.Structure):
 
 CTR_GEOM_NO_TABLES = 1
 CTR_GEOM_NO_GRAPHS = 2
+CTR_GEOM_NO_STORED_P = 4
 
 
 class ctr_params(C.Structure):

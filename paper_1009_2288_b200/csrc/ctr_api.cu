@@ -407,7 +407,7 @@ void ctr_destroy(ctr_handle* h) {
   if (!h) return;
   cudaDeviceSynchronize();
   void* bufs[] = {h->rays, h->rays2, h->views, h->viewsd, h->ximg, h->bsino, h->r, h->q, h->s, h->gimg, h->v, h->w, h->n0,
-                  h->part, h->counters, h->hist, h->scal_block, h->stats, h->d_sweep, h->basis, h->win, h->imgT, h->win2, h->usi, h->cand, h->qidx, h->qwts, h->qcnt, h->ell_p.tab, h->ell_p.cap, h->ell_p.off, h->ell_pt.tab, h->ell_pt.cap, h->ell_pt.off};
+                  h->part, h->counters, h->hist, h->scal_block, h->stats, h->d_sweep, h->basis, h->win, h->imgT, h->win2, h->usi, h->cand, h->rt_tab, h->rt_cnt, h->rt_off, h->qidx, h->qwts, h->qcnt, h->ell_p.tab, h->ell_p.cap, h->ell_p.off, h->ell_pt.tab, h->ell_pt.cap, h->ell_pt.off};
   for (void* b : bufs)
     if (b) cudaFree(b);
   if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
@@ -432,7 +432,7 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
   if (!(g->dx > 0) || !(g->dy > 0) || !(g->du > 0) || !(g->dso > 0) || !(g->dsd > g->dso)) return CTR_EINVAL;
   if (g->ndim == 3 && (!(g->dz > 0) || !(g->dv > 0))) return CTR_EINVAL;
   if (g->det_type != 0 && g->det_type != 1) return CTR_EINVAL;
-  if (g->flags & ~(CTR_GEOM_NO_TABLES | CTR_GEOM_NO_GRAPHS)) return CTR_EINVAL;
+  if (g->flags & ~(CTR_GEOM_NO_TABLES | CTR_GEOM_NO_GRAPHS | CTR_GEOM_NO_STORED_P)) return CTR_EINVAL;
   if ((long long)g->nx * g->ny * g->nz >= (1ll << 31) || (long long)g->nviews * g->nu * g->nv >= (1ll << 31)) return CTR_EINVAL;
   // source and detector must lie outside the circle circumscribing the grid (plus one voxel)
   {
@@ -597,15 +597,17 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
   }
   int rc = d.ndim == 3 ? cone_build_tables(h) : fan_build_tables(h);
   if (rc == CTR_OK && d.ndim == 2 && d.V == 4) rc = si_build_hits(h);
+  if (rc == CTR_OK && d.ndim == 2 && d.V == 4) rc = si_build_raytab(h);
   if (rc != CTR_OK) { ctr_destroy(h); return rc; }
   {
     // which kernels ctr_forward / ctr_back launch on this handle (the tables are built best effort)
     const char *fw, *bk;
     double table_mb = 0.0;
     if (d.V == 4) {
-      fw = "k_si_forward";
+      fw = h->rt_tab ? "k_si_forward_tab" : "k_si_forward";
       bk = h->qwts ? "k_si_back_quad" : "k_si_back";
-      if (h->qwts) table_mb = (double)((d.nx + 1) / 2) * ((d.ny + 1) / 2) * h->hits_cap * 20.0 / 1e6;
+      table_mb = (double)h->rt_bytes / 1e6;
+      if (h->qwts) table_mb += (double)((d.nx + 1) / 2) * ((d.ny + 1) / 2) * h->hits_cap * 20.0 / 1e6;
     } else {
       fw = h->ell_p.tab ? "k_ell_apply<P>" : (d.ndim == 3 ? "k_cone_forward" : "k_fan_forward");
       bk = h->ell_pt.tab ? "k_ell_apply<PT>" : (d.ndim == 3 ? "k_cone_back" : "k_fan_back");

@@ -38,4 +38,41 @@ __device__ __forceinline__ float fan_pixel_weight(const float4 R, float fi, floa
   return (w.ra == tgt ? w.wa : 0.0f) + (w.rb == tgt ? w.wb : 0.0f);
 }
 
+// Row visitor of P: every non-zero (pixel index j nx + i, p_ij) of ray `row`, slab by slab, exactly the entries and
+// the order k_fan_forward adds them in (stored matrices: ctr_ell.cuh for single slices, k_si_forward_tab for batches).
+struct FanRayHits {  // rows of P: ray r = k nu + b; index = pixel j nx + i
+  const float4* rays;
+  template <class Visit>
+  __device__ __forceinline__ void operator()(const Dims& d, size_t row, Visit visit) const {
+    const float4 R = __ldg(&rays[row]);
+    const float x0 = R.x, m = R.y, L = fabsf(R.z), K = R.w;
+    const bool xdrv = R.z < 0.0f;
+    const int n_drv = xdrv ? d.nx : d.ny, n_oth = xdrv ? d.ny : d.nx;
+    const int c_drv = xdrv ? d.c0x : d.c0y, c_oth = xdrv ? d.c0y : d.c0x;
+    int s0 = 0, s1 = n_drv;
+    const float lo = (float)(-c_oth) - 1.0f, hi = (float)(n_oth - c_oth) + 1.0f;
+    if (m != 0.0f) {
+      float t1 = (lo - x0) / m, t2 = (hi - x0) / m;
+      float tmin = fminf(t1, t2), tmax = fmaxf(t1, t2);
+      tmin = fminf(fmaxf(tmin, -1.0e6f), 1.0e6f);
+      tmax = fminf(fmaxf(tmax, -1.0e6f), 1.0e6f);
+      s0 = max(0, (int)floorf(tmin) + c_drv - 2);
+      s1 = min(n_drv, (int)ceilf(tmax) + c_drv + 2);
+    } else if (x0 < lo || x0 > hi) {
+      s1 = 0;
+    }
+    float y = (float)(s0 - c_drv);
+    float oa = fmaf(m, y, x0);
+    for (int s = s0; s < s1; ++s) {
+      const float ob = fmaf(m, y + 1.0f, x0);
+      const SlabW w = slab_weights(oa, ob, L, K);
+      const int ia = cell_of(w.ra) + c_oth, ib = cell_of(w.rb) + c_oth;
+      if (w.wa != 0.0f && (unsigned)ia < (unsigned)n_oth) visit(xdrv ? ia * d.nx + s : s * d.nx + ia, w.wa);
+      if (w.wb != 0.0f && (unsigned)ib < (unsigned)n_oth) visit(xdrv ? ib * d.nx + s : s * d.nx + ib, w.wb);
+      oa = ob;
+      y += 1.0f;
+    }
+  }
+};
+
 }  // namespace ctr

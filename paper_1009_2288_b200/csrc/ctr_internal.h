@@ -120,6 +120,10 @@ struct ctr_handle {
   float4* qwts;         // [nquad][hits_cap] p_ij of that ray in the four pixels of the 2 x 2 quad
   int* qcnt;            // [nquad] entries used per quad
   int hits_cap;
+  float2* rt_tab;       // stored P for batches: per ray (pixel index * LQ, p_ij), padded to chunks of 16 (ctr_si.cu)
+  int* rt_cnt;          // [nray] entries per ray
+  unsigned* rt_off;     // [nray] offset of the ray's entries in rt_tab
+  size_t rt_bytes;
   ctr::EllTable ell_p, ell_pt;  // stored P (rows = rays) and P^T (rows = voxels), batch = 1 only; tab == NULL: on the fly
   unsigned* cand;       // [Bp][cand_cap] candidate lists (bit patterns of N0^2 near the predicted sigma^2)
   unsigned cand_cap;
@@ -204,6 +208,7 @@ int fan_back_eq11(ctr_handle* h, const float* sino, float* img, cudaStream_t st)
 int si_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st);
 int si_back(ctr_handle* h, const float* sino, float* out, int mode, const float* s, float* u, cudaStream_t st);
 int si_build_hits(ctr_handle* h);
+int si_build_raytab(ctr_handle* h);
 int si_from_abi(ctr_handle* h, const float* src, float* dst, size_t n, cudaStream_t st);   // [B][n] -> SI
 int si_to_abi(ctr_handle* h, const float* src, float* dst, size_t n, cudaStream_t st);     // SI -> [B][n]
 int si_from_planar(ctr_handle* h, const float* src, float* dst, size_t n, cudaStream_t st); // [G][n] float4 -> SI

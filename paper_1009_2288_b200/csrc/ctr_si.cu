@@ -180,6 +180,124 @@ __global__ void __launch_bounds__(SI_FWD_WARPS * 32, SI_FWD_MINB) k_si_forward(D
 }
 
 // ------------------------------------------------------------------------------------------------
+// a1 with the stored matrix (NEXT-2; "pre-calculate the projection matrix and save it ... as a lookup
+// table", CGLS by sparse matrix products): P as ONE table shared by all slices - per ray its non-zeros
+// (pixel index * LQ, p_ij) in the order k_si_forward adds them, padded to whole chunks of 16 - applied to the
+// 64 slices at once, i.e. a sparse-matrix x dense-matrix product with the slices as columns. 8 B x nnz(P) =
+// 236 MB at 512^2 / 60 x 888 streamed from HBM per application, against 64 x nnz x 4 B gathered through the L1s.
+// The sub-warp of a ray loads a chunk of 16 entries with one coalesced 128-byte read, hands them round through
+// shared memory two at a time (one LDS.128 = two entries) and every lane does one 16-byte gather and 4 FMAs per
+// entry: no slab arithmetic, no empty slabs, no divergent second-cell branch. Same p_ij bits (the table is
+// filled by the row visitor the on-the-fly kernels share), same order of additions per ray: identical results.
+// ------------------------------------------------------------------------------------------------
+template <int PASS>
+__global__ void __launch_bounds__(128) k_raytab_build(Dims d, const float4* __restrict__ rays, int* __restrict__ cnt,
+                                                      const unsigned* __restrict__ off, float2* __restrict__ tab, int scale) {
+  const int r = blockIdx.x * 128 + threadIdx.x;
+  if (r >= d.nray) return;
+  FanRayHits hits{rays};
+  int n = 0;
+  if (PASS == 0) {
+    hits(d, (size_t)r, [&](int, float) { ++n; });
+    cnt[r] = n;
+  } else {
+    float2* dst = tab + off[r];
+    hits(d, (size_t)r, [&](int idx, float wt) { dst[n++] = make_float2(__int_as_float(idx * scale), wt); });
+    const int padded = (cnt[r] + 15) / 16 * 16;
+    for (; n < padded; ++n) dst[n] = make_float2(0.0f, 0.0f);
+  }
+}
+
+template <int LQ, int MODE>
+__global__ void __launch_bounds__(SI_FWD_WARPS * 32, SI_FWD_MINB) k_si_forward_tab(Dims d, const int* __restrict__ cnt,
+                                                    const unsigned* __restrict__ off, const float2* __restrict__ tab,
+                                                    const float4* __restrict__ img, float4* __restrict__ out,
+                                                    const float4* __restrict__ bs, Scal sc, double* part) {
+  constexpr int RW = 32 / LQ;  // rays per warp
+  constexpr int CH = 16;       // entries per chunk and ray (a 128-byte line of the table)
+  static_assert(LQ <= CH && CH % LQ == 0, "chunk must be a whole number of sub-warp loads");
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int q = lane % LQ, sub = lane / LQ;
+  const int r = (blockIdx.x * SI_FWD_WARPS + warp) * RW + sub;
+  const int gs = blockIdx.y;
+  const bool live = r < d.nray;
+  __shared__ __align__(16) float2 ent[SI_FWD_WARPS][RW][CH + 2];  // rows padded: sub-warps in different banks
+  float2* mine = ent[warp][sub];
+  float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+  const int n = live ? __ldg(&cnt[r]) : 0;
+  const int nmax = __reduce_max_sync(FULL, n);
+  const float2* src = tab + (live ? __ldg(&off[r]) : 0u);
+  const float4* base = img + (size_t)gs * d.npix * LQ + q;
+  asm volatile("" : "+l"(base));
+  for (int e0 = 0; e0 < nmax; e0 += CH) {
+    __syncwarp();
+#pragma unroll
+    for (int c = 0; c < CH / LQ; ++c) {
+      const int e = e0 + c * LQ + q;
+      mine[c * LQ + q] = e < n ? __ldcs(src + e) : make_float2(0.0f, 0.0f);  // streamed once per application
+    }
+    __syncwarp();
+#pragma unroll
+    for (int t = 0; t < CH; t += 2) {
+      const float4 two = *reinterpret_cast<const float4*>(mine + t);  // entries t and t + 1
+      if (two.y != 0.0f) fma4(acc, two.y, __ldg(base + __float_as_int(two.x)));
+      if (two.w != 0.0f) fma4(acc, two.w, __ldg(base + __float_as_int(two.z)));
+    }
+  }
+  if (live) {
+    const size_t e = ((size_t)gs * d.nray + r) * LQ + q;
+    if (MODE == 1) {
+      const float4 b = __ldg(bs + e);
+      acc[0] = b.x - acc[0]; acc[1] = b.y - acc[1]; acc[2] = b.z - acc[2]; acc[3] = b.w - acc[3];
+    }
+    out[e] = make_float4(acc[0], acc[1], acc[2], acc[3]);
+  }
+  if (MODE == 2) {
+    double v[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) v[c] = live ? (double)acc[c] * (double)acc[c] : 0.0;
+    block_partials_q<4, SI_FWD_WARPS>(v, LQ, part + (size_t)gs * gridDim.x * LQ * 4, blockIdx.x, threadIdx.x);
+  }
+}
+
+// built once per handle (ctr_create), best effort: without it k_si_forward computes the entries on the fly
+int si_build_raytab(ctr_handle* h) {
+  const Dims& d = h->d;
+  h->rt_tab = nullptr; h->rt_cnt = nullptr; h->rt_off = nullptr; h->rt_bytes = 0;
+  if (h->g.flags & (CTR_GEOM_NO_TABLES | CTR_GEOM_NO_STORED_P)) return CTR_OK;
+  if ((size_t)d.npix * d.LQ >= (1u << 31)) return CTR_OK;
+  if (cudaMalloc((void**)&h->rt_cnt, sizeof(int) * (size_t)d.nray) != cudaSuccess) { cudaGetLastError(); h->rt_cnt = nullptr; return CTR_OK; }
+  const unsigned nblk = (unsigned)((d.nray + 127) / 128);
+  k_raytab_build<0><<<nblk, 128>>>(d, h->rays, h->rt_cnt, nullptr, nullptr, d.LQ);
+  CTR_LAUNCHED(h);
+  int* cnt = (int*)malloc(sizeof(int) * (size_t)d.nray);
+  unsigned* off = (unsigned*)malloc(sizeof(unsigned) * (size_t)d.nray);
+  if (!cnt || !off) { free(cnt); free(off); return CTR_ENOMEM; }
+  CTR_CUDA(h, cudaMemcpy(cnt, h->rt_cnt, sizeof(int) * (size_t)d.nray, cudaMemcpyDeviceToHost));
+  unsigned long long total = 0;
+  for (int r = 0; r < d.nray; ++r) { off[r] = (unsigned)total; total += (unsigned long long)(cnt[r] + 15) / 16 * 16; }
+  free(cnt);
+  bool ok = total > 0 && total < (1ull << 32);
+  if (ok && cudaMalloc((void**)&h->rt_off, sizeof(unsigned) * (size_t)d.nray) != cudaSuccess) { cudaGetLastError(); h->rt_off = nullptr; ok = false; }
+  if (ok && cudaMalloc((void**)&h->rt_tab, sizeof(float2) * total) != cudaSuccess) { cudaGetLastError(); h->rt_tab = nullptr; ok = false; }
+  if (!ok) {
+    free(off);
+    if (h->rt_off) cudaFree(h->rt_off);
+    cudaFree(h->rt_cnt);
+    h->rt_tab = nullptr; h->rt_cnt = nullptr; h->rt_off = nullptr;
+    return CTR_OK;
+  }
+  cudaError_t ce = cudaMemcpy(h->rt_off, off, sizeof(unsigned) * (size_t)d.nray, cudaMemcpyHostToDevice);
+  free(off);
+  if (ce != cudaSuccess) return cuda_fail(h, ce, "si_build_raytab: offsets");
+  k_raytab_build<1><<<nblk, 128>>>(d, h->rays, h->rt_cnt, h->rt_off, h->rt_tab, d.LQ);
+  CTR_LAUNCHED(h);
+  CTR_CUDA(h, cudaDeviceSynchronize());
+  h->rt_bytes = sizeof(float2) * total;
+  return CTR_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
 // a2  P^T (gather). Sub-warp per pixel; a block is a TX x TY tile of pixels, so the sinogram segments
 // it reads overlap in L1. Views are taken LQ at a time: lane q looks up the bins of view k0+q whose
 // rays cross the pixel (window table win2, or fan_window() when the table is not usable) and evaluates
@@ -566,6 +684,15 @@ static int si_forward_t(ctr_handle* h, const float* img, float* out, int mode, c
   const float4 *im = (const float4*)img, *b4 = (const float4*)bs;
   float4* o4 = (float4*)out;
   ProfScope prof(h, CTR_PROF_FORWARD, st);
+  if (h->rt_tab) {
+    dim3 tgrid((d.nray + SI_FWD_WARPS * (32 / LQ) - 1) / (SI_FWD_WARPS * (32 / LQ)), d.GS);
+    if (mode == 0) k_si_forward_tab<LQ, 0><<<tgrid, nt, 0, st>>>(d, h->rt_cnt, h->rt_off, h->rt_tab, im, o4, b4, h->sc, h->part);
+    else if (mode == 1) k_si_forward_tab<LQ, 1><<<tgrid, nt, 0, st>>>(d, h->rt_cnt, h->rt_off, h->rt_tab, im, o4, b4, h->sc, h->part);
+    else k_si_forward_tab<LQ, 2><<<tgrid, nt, 0, st>>>(d, h->rt_cnt, h->rt_off, h->rt_tab, im, o4, b4, h->sc, h->part);
+    CTR_LAUNCHED(h);
+    if (mode == 2) return reduce_finish(h, CTR_FIN_ALPHA, 4, (int)tgrid.x, 0, 0, 0, st);
+    return CTR_OK;
+  }
   if (mode == 0) k_si_forward<LQ, H, 0><<<grid, nt, 0, st>>>(d, h->rays, im, o4, b4, h->sc, h->part, cnt);
   else if (mode == 1) k_si_forward<LQ, H, 1><<<grid, nt, 0, st>>>(d, h->rays, im, o4, b4, h->sc, h->part, cnt);
   else k_si_forward<LQ, H, 2><<<grid, nt, 0, st>>>(d, h->rays, im, o4, b4, h->sc, h->part, cnt);

@@ -354,29 +354,37 @@ __global__ void __launch_bounds__(256, TV_SMINB) k_tv_scan1(Dims d, int rows, co
   for (int s = 0; s < V; ++s) pred[s] = sc.pred[blockIdx.z * V + s];
   __syncthreads();
   const int lim[3] = {d.nx - 1, d.ny - 1, d.nz - 1};
+  unsigned nzero[V];  // exact zeros (flat regions) are counted in a register instead of hammering bin 0
+#pragma unroll
+  for (int s = 0; s < V; ++s) nzero[s] = 0u;
   for (int rr = 0; rr < rows; ++rr) {
     const Vox p = vox_of_thread(d, rr, rows, 8);
     const int pos[3] = {p.i, p.j, p.k};
+    if (!p.active) continue;
     float val[ND][V];
-    if (p.active) {
-      Window<V, ND> w;
-      load_window<V, ND>(d, f, p.g, p.i, p.j, p.k, w);
-      own_face_values<V, ND>(d, w, pos, lim, val);
-    }
+    Window<V, ND> w;
+    load_window<V, ND>(d, f, p.g, p.i, p.j, p.k, w);
+    own_face_values<V, ND>(d, w, pos, lim, val);
 #pragma unroll
     for (int A = 0; A < ND; ++A) {
-      const bool valid = p.active && pos[A] < lim[A];
+      if (pos[A] >= lim[A]) continue;  // border face
 #pragma unroll
       for (int s = 0; s < V; ++s) {
-        const unsigned bits = valid ? __float_as_uint(val[A][s]) : 0u;
-        hist_add(hs[s], bits, 20, 2047u, valid);
-        const int dbin = (int)(bits >> 20) - pred[s];
-        if (valid && dbin >= -1 && dbin <= 1) {
+        const unsigned bits = __float_as_uint(val[A][s]);
+        const unsigned bin = bits >> 20;
+        if (bin) atomicAdd(&hs[s][bin], 1u);
+        else ++nzero[s];
+        if (bin + 1u - (unsigned)pred[s] <= 2u) {  // |bin - pred| <= 1 (pred < 0 never matches)
           const unsigned at = atomicAdd(&stage_n[s], 1u);
           if (at < TV_SCAP(V)) stage[s][at] = bits;
         }
       }
     }
+  }
+#pragma unroll
+  for (int s = 0; s < V; ++s) {
+    const unsigned z = __reduce_add_sync(0xffffffffu, nzero[s]);
+    if ((threadIdx.x & 31) == 0 && z) atomicAdd(&hs[s][0], z);
   }
   __syncthreads();
   for (int t = tid0; t < V * 2048; t += 256) {
@@ -504,7 +512,14 @@ __global__ void __launch_bounds__(128) k_tv_weights(Dims d, int rows, const floa
 // from the magnitudes of THIS f and the sigma^2 the selection has just left in sc.sigma2 (TV mode: w = 1): no
 // weight planes, no magnitude planes. Either way N0^2 of the four (six) faces of a voxel is recomputed from its
 // window: all their stencils lie inside it.
-__device__ __forceinline__ float edge_weight(float n0sq, float neg_inv_s2) { return __expf(n0sq * neg_inv_s2); }
+// w = exp(-N0^2/sigma^2) = 2^(N0^2 k), k = -log2(e)/sigma^2 formed once per block: one FMUL and one MUFU.EX2 per
+// face (__expf adds a denormal-range fix-up per call; w underflowing to 0 for N0 >> sigma is what is wanted)
+__device__ __forceinline__ float edge_weight(float n0sq, float k) {
+  float r;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(n0sq * k));
+  return r;
+}
+#define CTR_LOG2E 1.4426950408889634f
 // one MUFU.RSQ, no denormal fix-up: the arguments are N0^2 + eps^2 (1e-8 with the default eps); callers treat
 // anything below 1e-30 as a flat face
 __device__ __forceinline__ float rsqrt_fast(float x) {
@@ -517,12 +532,13 @@ template <int V, int ND, int WSRC>
 __global__ void __launch_bounds__(128, TV_GMINB) k_tv_gradient(Dims d, int rows, const float* __restrict__ f, const float* __restrict__ v,
                                                      const float* __restrict__ w, float* __restrict__ gout, TvParams tp,
                                                      Scal sc, double* part, unsigned* counter, StatRing ring) {
-  double red[2 * V];
+  // per-thread sums over its (at most 8) voxels in fp32, everything above that in fp64
+  float acc[2 * V];
 #pragma unroll
-  for (int s = 0; s < 2 * V; ++s) red[s] = 0.0;
+  for (int s = 0; s < 2 * V; ++s) acc[s] = 0.0f;
   float nis2[V];
 #pragma unroll
-  for (int s = 0; s < V; ++s) nis2[s] = WSRC ? -1.0f / sc.sigma2[blockIdx.z * V + s] : 0.0f;
+  for (int s = 0; s < V; ++s) nis2[s] = WSRC ? -CTR_LOG2E / sc.sigma2[blockIdx.z * V + s] : 0.0f;
   const int lim[3] = {d.nx - 1, d.ny - 1, d.nz - 1};
   for (int rr = 0; rr < rows; ++rr) {
   const Vox p = vox_of_thread(d, rr, rows);
@@ -570,31 +586,37 @@ __global__ void __launch_bounds__(128, TV_GMINB) k_tv_gradient(Dims d, int rows,
         }
       }
 #pragma unroll
+      // border faces: the face towards -A of the first voxel has dm = 0 exactly (replicated neighbour), so only
+      // the +A face of the last voxel needs its weight masked (it would otherwise enter the energy)
+      const float maskp = pos[A] < lim[A] ? 1.0f : 0.0f;
+#pragma unroll
       for (int s = 0; s < V; ++s) {
         if (WSRC) {
-          wp[s] = pos[A] < lim[A] ? (tp.weights_mode == 1 ? 1.0f : edge_weight(rp[s], nis2[s])) : 0.0f;
-          wm[s] = pos[A] > 0 ? (tp.weights_mode == 1 ? 1.0f : edge_weight(rm[s], nis2[s])) : 0.0f;
+          wp[s] = tp.weights_mode == 1 ? maskp : maskp * edge_weight(rp[s], nis2[s]);
+          wm[s] = tp.weights_mode == 1 ? 1.0f : edge_weight(rm[s], nis2[s]);
         }
-        const float n0p = rp[s] + eps2, n0m = rm[s] + eps2;
+        const float n0p = fmaxf(rp[s] + eps2, 1e-30f), n0m = fmaxf(rm[s] + eps2, 1e-30f);
         const float dp = win.c[cz + ez][1 + ey][1 + ex][s] - win.c[cz][1][1][s];
         const float dm = win.c[cz][1][1][s] - win.c[cz - ez][1 - ey][1 - ex][s];
         // sqrt(x) = x rsqrt(x): one special-function instruction per face serves both the flux and the energy
-        const float ip = n0p > 1e-30f ? rsqrt_fast(n0p) : 0.0f, im = n0m > 1e-30f ? rsqrt_fast(n0m) : 0.0f;
-        const float fp = wp[s] * dp * ip;
-        const float fm = wm[s] * dm * im;
-        gv[s] -= fp - fm;
-        etv[s] = fmaf(wp[s], fmaf(n0p, ip, -tp.eps), etv[s]);
+        const float ip = rsqrt_fast(n0p), im = rsqrt_fast(n0m);
+        gv[s] -= wp[s] * dp * ip - wm[s] * dm * im;
+        // (a flat face contributes exactly 0: north_star's invariant on a constant image)
+        etv[s] = fmaf(wp[s], rp[s] > 0.0f ? fmaf(n0p, ip, -tp.eps) : 0.0f, etv[s]);
       }
     }
     Pack<V>::st(gout, e, gv);
 #pragma unroll
     for (int s = 0; s < V; ++s) {
       const float df = win.c[cz][1][1][s] - vv[s];
-      red[s] += (double)gv[s] * (double)gv[s];
-      red[V + s] += 0.5 * (double)tp.lambda * (double)df * (double)df + (double)etv[s] / (double)ND;
+      acc[s] = fmaf(gv[s], gv[s], acc[s]);
+      acc[V + s] += fmaf(0.5f * tp.lambda * df, df, etv[s] * (1.0f / (float)ND));
     }
   }
   }  // rr
+  double red[2 * V];
+#pragma unroll
+  for (int s = 0; s < 2 * V; ++s) red[s] = (double)acc[s];
   const Vox p = vox_of_thread(d, 0, rows);
   grid_reduce<2 * V>(red, part + (size_t)p.g * p.nblk * 2 * V, counter + p.g, p.nblk, p.blk, p.tid, 128,
                      [&](double(&sum)[2 * V]) {
@@ -709,7 +731,7 @@ __global__ void __launch_bounds__(32 * TV_TW, TV_TMINB) k_tv_trial(Dims d, int r
   if (!any) return;
   float nis2[V];
 #pragma unroll
-  for (int s = 0; s < V; ++s) nis2[s] = WSRC ? -1.0f / sc.sigma2[g * V + s] : 0.0f;
+  for (int s = 0; s < V; ++s) nis2[s] = WSRC ? -CTR_LOG2E / sc.sigma2[g * V + s] : 0.0f;
   const int lim[3] = {d.nx - 1, d.ny - 1, d.nz - 1};
   float et[NE];
   double dd[3 * V];
@@ -773,7 +795,7 @@ __global__ void __launch_bounds__(32 * TV_TW, TV_TMINB) k_tv_trial(Dims d, int r
           for (int A = 0; A < ND; ++A) {
             float2 rad = __ffma2_rn(t2, __ffma2_rn(t2, fc[A][hh], fb[A][hh]), fa[A][hh]);
             rad.x = fmaxf(rad.x, 1e-30f); rad.y = fmaxf(rad.y, 1e-30f);
-            acc2 = __ffma2_rn(__fmul2_rn(wA2[A][hh], rad), make_float2(rsqrtf(rad.x), rsqrtf(rad.y)), acc2);
+            acc2 = __ffma2_rn(__fmul2_rn(wA2[A][hh], rad), make_float2(rsqrt_fast(rad.x), rsqrt_fast(rad.y)), acc2);
           }
           et[q * V + 2 * hh] += acc2.x;
           et[q * V + 2 * hh + (V > 1)] += acc2.y;
@@ -816,7 +838,7 @@ __global__ void __launch_bounds__(32 * TV_TW, TV_TMINB) k_tv_trial(Dims d, int r
   #pragma unroll
           for (int s = 0; s < V; ++s) {
             const float rad = fmaxf(fmaf(t, fmaf(t, fc[A][s], fb[A][s]), fa[A][s]), 1e-30f);
-            et[q * V + s] = fmaf(wA[A][s] * rad, rsqrtf(rad), et[q * V + s]);
+            et[q * V + s] = fmaf(wA[A][s] * rad, rsqrt_fast(rad), et[q * V + s]);
           }
       }
       {

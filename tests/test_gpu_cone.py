@@ -28,6 +28,21 @@ def rel(a, b):
     return float(np.linalg.norm(np.asarray(a, np.float64) - b) / np.linalg.norm(b))
 
 
+def assert_close(a, b, tol):
+    """relative L2 error <= tol (north_star's norm) AND no single element further off than 10 tol of the largest
+    reference value (30 tol for one operator application): a handful of wrong border pixels or one wrong view would
+    hide under the L2 norm alone. Why 30: a ray almost parallel to a grid axis (slope m -> 0) splits its length in a
+    slab between two neighbouring cells at a crossing whose position is known to ~1e-5 pixel in fp32, i.e. the split
+    moves by ~1e-5 / |m| of the slab length; the SUM over the two cells is exact, single elements of P^T y differ by up
+    to ~2e-4 of the largest value at 512^2 (measured)."""
+    a, b = np.asarray(a, np.float64), np.asarray(b, np.float64)
+    err_l2 = float(np.linalg.norm(a - b) / np.linalg.norm(b))
+    err_max = float(np.max(np.abs(a - b)) / np.max(np.abs(b)))
+    assert err_l2 <= tol, (err_l2, tol)
+    elem = (30 if tol <= 2e-5 else 10) * tol
+    assert err_max <= elem, (err_max, elem)
+
+
 def to_gpu(torch, a):
     return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
 
@@ -61,8 +76,8 @@ def test_forward_back_match_oracle_small(ctr, torch_cuda, orc):
         torch.cuda.synchronize()
         px, pty = sino.cpu().numpy(), img.cpu().numpy()
         h.close()
-        assert rel(px, orc.forward(cfg, x.astype(np.float64))) <= 2e-5
-        assert rel(pty, orc.back(cfg, y.astype(np.float64))) <= 2e-5
+        assert_close(px, orc.forward(cfg, x.astype(np.float64)), 2e-5)
+        assert_close(pty, orc.back(cfg, y.astype(np.float64)), 2e-5)
         lhs, rhs = (px.astype(np.float64) * y).sum(), (x * pty.astype(np.float64)).sum()
         assert abs(lhs - rhs) <= 2e-6 * abs(lhs)
 
@@ -102,14 +117,14 @@ def test_mini_c5_operators_and_reconstruction(ctr, torch_cuda, orc):
     h.ctr_forward(to_gpu(torch, case["truth"]), sino)
     h.ctr_back(to_gpu(torch, case["sino"]), img)
     torch.cuda.synchronize()
-    assert rel(sino.cpu().numpy(), orc.forward(cfg, case["truth"].astype(np.float64))) <= 1e-5
-    assert rel(img.cpu().numpy(), orc.back(cfg, case["sino"].astype(np.float64))) <= 1e-5
+    assert_close(sino.cpu().numpy(), orc.forward(cfg, case["truth"].astype(np.float64)), 1e-5)
+    assert_close(img.cpu().numpy(), orc.back(cfg, case["sino"].astype(np.float64)), 1e-5)
     # CGLS
     x = torch.zeros(h.img_shape, device="cuda")
     h.ctr_cgls(to_gpu(torch, case["sino"]), x, 6)
     torch.cuda.synchronize()
     want = orc.cgls(cfg, case["sino"].astype(np.float64), np.zeros(cfg.img_shape), 6)
-    assert rel(x.cpu().numpy(), want.reshape(cfg.img_shape)) <= 1e-4
+    assert_close(x.cpu().numpy(), want.reshape(cfg.img_shape), 1e-4)
     # full (short) schedule
     h.ctr_reconstruct(to_gpu(torch, case["sino"]), img, ctr.make_params(cfg))
     torch.cuda.synchronize()
@@ -122,7 +137,7 @@ def test_mini_c5_operators_and_reconstruction(ctr, torch_cuda, orc):
     assert ks == list(log[:, 1].astype(int))
     assert max(abs(r["sigma"] - l[0]) / l[0] for r, l in zip(stats, log)) <= 2e-3
     assert got.min() >= 0.0
-    assert rel(got, want) <= 1e-3
+    assert_close(got, want, 1e-3)
 
 
 def test_tv_3d_matches_oracle(ctr, torch_cuda, orc):
@@ -149,7 +164,7 @@ def test_tv_3d_matches_oracle(ctr, torch_cuda, orc):
         f_new, k, E0, G, t = orc.eptv_step(f_ref, v.astype(np.float64), w_ref, cfg.lam, cfg, ndim=3)
         assert st["k"] == k and abs(st["sigma"] - s_ref) <= 1e-5 * s_ref
         assert abs(st["e0"] - E0) <= 1e-5 * abs(E0) and abs(st["g2"] - G) <= 1e-4 * G
-        assert rel(f.cpu().numpy(), f_new) <= 1e-5
+        assert_close(f.cpu().numpy(), f_new, 1e-5)
         f_ref = f_new
     h.close()
 
@@ -168,8 +183,8 @@ def test_c5_full_size_operators(ctr, torch_cuda, orc):
     torch.cuda.synchronize()
     px, pty = sino.cpu().numpy(), img.cpu().numpy()
     h.close()
-    assert rel(px, orc.forward(cfg, case["truth"].astype(np.float64))) <= 1e-5
-    assert rel(pty, orc.back(cfg, case["sino"].astype(np.float64))) <= 1e-5
+    assert_close(px, orc.forward(cfg, case["truth"].astype(np.float64)), 1e-5)
+    assert_close(pty, orc.back(cfg, case["sino"].astype(np.float64)), 1e-5)
 
 
 # ------------------------------------------------------------------ configs[4] at FULL size, whole path

@@ -28,6 +28,21 @@ def rel(a, b):
     return float(np.linalg.norm(np.asarray(a, np.float64) - b) / np.linalg.norm(b))
 
 
+def assert_close(a, b, tol):
+    """relative L2 error <= tol (north_star's norm) AND no single element further off than 10 tol of the largest
+    reference value (30 tol for one operator application): a handful of wrong border pixels or one wrong view would
+    hide under the L2 norm alone. Why 30: a ray almost parallel to a grid axis (slope m -> 0) splits its length in a
+    slab between two neighbouring cells at a crossing whose position is known to ~1e-5 pixel in fp32, i.e. the split
+    moves by ~1e-5 / |m| of the slab length; the SUM over the two cells is exact, single elements of P^T y differ by up
+    to ~2e-4 of the largest value at 512^2 (measured)."""
+    a, b = np.asarray(a, np.float64), np.asarray(b, np.float64)
+    err_l2 = float(np.linalg.norm(a - b) / np.linalg.norm(b))
+    err_max = float(np.max(np.abs(a - b)) / np.max(np.abs(b)))
+    assert err_l2 <= tol, (err_l2, tol)
+    elem = (30 if tol <= 2e-5 else 10) * tol
+    assert err_max <= elem, (err_max, elem)
+
+
 def to_gpu(torch, a):
     return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
 
@@ -48,7 +63,7 @@ def test_cgls_matches_oracle(ctr, torch_cuda, orc, name, batch, n_iter):
     h.close()
     for sl in range(batch):
         want = orc.cgls(cfg, case["sino"][sl].astype(np.float64), x0[sl].astype(np.float64), n_iter)
-        assert rel(got[sl], want) <= 1e-4
+        assert_close(got[sl], want, 1e-4)
 
 
 def test_cgls_single_iteration_by_hand(ctr, torch_cuda, orc):
@@ -63,7 +78,7 @@ def test_cgls_single_iteration_by_hand(ctr, torch_cuda, orc):
     x = torch.zeros(h.img_shape, device="cuda")
     h.ctr_cgls(to_gpu(torch, case["sino"]), x, 1)
     torch.cuda.synchronize()
-    assert rel(x.cpu().numpy()[0], want) <= 1e-5
+    assert_close(x.cpu().numpy()[0], want, 1e-5)
     h.close()
 
 
@@ -143,7 +158,7 @@ def test_eptv_step_matches_oracle(ctr, torch_cuda, orc, name, batch):
             assert abs(st[sl]["sigma"] - s_ref) <= 1e-5 * s_ref
             assert abs(st[sl]["e0"] - E0) <= 1e-5 * abs(E0)
             assert abs(st[sl]["g2"] - G) <= 1e-4 * abs(G)
-            assert rel(got[sl], f_new[0]) <= 1e-5
+            assert_close(got[sl], f_new[0], 1e-5)
             f_ref[sl] = f_new[0]
     h.close()
 
@@ -193,6 +208,7 @@ def compare_with_oracle(orc, cfg, sino_slice, got_img, got_stats, tol=1e-3):
     # agree as well as the iterates do (tol), per sweep on equal inputs it agrees to 1e-5 (test above)
     assert err_sig <= 2 * tol
     assert err_img <= tol
+    assert float(np.max(np.abs(got_img - want)) / np.max(np.abs(want))) <= 10 * tol   # no single pixel far off
     return want, w_ref
 
 
@@ -227,7 +243,7 @@ def test_reconstruct_batched_short_schedule(ctr, torch_cuda, orc):
     one = scaled_config("c4", batch=1, n_outer=2, n_cgls=6)
     # the batched path sums in a different (fixed) order than the single-slice kernels: equal to rounding
     solo, _, _, _ = run_reconstruct(ctr, torch_cuda, one, case["sino"][2:3])
-    assert rel(img[2], solo[0].astype(np.float64)) <= 1e-4
+    assert_close(img[2], solo[0].astype(np.float64), 1e-4)
 
 
 def test_reconstruct_variants(ctr, torch_cuda, orc):
@@ -237,19 +253,19 @@ def test_reconstruct_variants(ctr, torch_cuda, orc):
         case = make_case(cfg)
         img, stats, _, _ = run_reconstruct(ctr, torch_cuda, cfg, case["sino"])
         want, _, log = orc.reconstruct(cfg, case["sino"][0].astype(np.float64), cfg)
-        assert rel(img[0], want) <= 1e-3
+        assert_close(img[0], want, 1e-3)
         if cfg.n_gd:
             assert [r["k"] for r in stats] == list(log[:, 1].astype(int))
 
 
 def test_reconstruct_c4_full_batch_one_step(ctr, torch_cuda, orc):
     """configs[3] in bench.py's launch configuration (64 slices per call), one outer iteration at the full
-    per-iteration schedule (15 CGLS + 5 GD); slices 7 and 50 against the oracle."""
+    per-iteration schedule (15 CGLS + 5 GD); eight slices spread over all four super-group lanes against the oracle."""
     cfg = scaled_config("c4", n_outer=1)
     case = make_case(cfg, raster=False)
     img, stats, _, _ = run_reconstruct(ctr, torch_cuda, cfg, case["sino"])
     assert len(stats) == cfg.n_gd * 64
-    for sl in (7, 50):
+    for sl in (0, 7, 13, 22, 36, 41, 50, 63):
         compare_with_oracle(orc, cfg, case["sino"][sl], img[sl], stats[sl::64])
 
 
