@@ -94,6 +94,13 @@ typedef struct {
   int32_t weights_mode;           /* 0 = EP-TV (Eq. 4-5), 1 = plain TV, w = 1                        */
   int32_t positivity;             /* 1: f <- max(f,0) after the last sweep of every outer iteration  */
   int32_t warm_start;             /* 0: f^(0) = 0 as in the paper (:171); 1: ctr_reconstruct continues from d_img   */
+  /* NEXT rows of SURVEY.md 8(f), off (0) in every config: */
+  int32_t fidelity_mode;          /* Step 1 of ctr_reconstruct: 0 = CGLS; 1 = the plain gradient update
+                                     (P1) of Eq. 8 (:141): v <- v - p1_step P^T (P v - y), n_cgls times from v = f        */
+  float p1_step;                  /* mu/lambda of (P1), the step of that update (>= 0; stable below 2/||P||^2)         */
+  int32_t backprojector;          /* P^T inside ctr_cgls / Step 1: 0 = exact transpose (ctr_back); 1 = the paper's
+                                     pixel-driven Eq. (11) (ctr_back_pixel, 2D only): an UNMATCHED pair, so CGLS then
+                                     runs the recurrence as printed (:420-440), without re-orthogonalisation (S24)      */
 } ctr_params;
 
 /* One record per (GD sweep, slice), in execution order: what steered the iteration. */
@@ -106,7 +113,7 @@ typedef struct {
 } ctr_sweep_stat;
 
 /* Defaults: n_outer 1, n_cgls 10, n_gd 5, lambda 0.01, q 0.90, eps 1e-4, t0 1e-3, rho 0.5, c 0.5 (S25),
- * armijo_max 16, EP-TV, positivity on, warm_start off. */
+ * armijo_max 16, EP-TV, positivity on, warm_start off, fidelity_mode 0 (CGLS), p1_step 0, backprojector 0. */
 void ctr_default_params(ctr_params* p);
 
 /* Build a handle for `g` on the CURRENT CUDA device: validates the geometry, builds the ray table
@@ -120,14 +127,15 @@ int ctr_forward(ctr_handle* h, const float* d_img, float* d_sino, void* stream);
 /* a2: d_img = P^T d_sino, the exact transpose of ctr_forward's matrix (same p_ij, bit for bit), gather
  * form, no atomics (PAPER.md:193 explains why not scatter). d_img is overwritten. */
 int ctr_back(ctr_handle* h, const float* d_sino, float* d_img, void* stream);
-/* NEXT-1 (not on the hot path, not used by ctr_cgls): the paper's own pixel-driven backprojector, Eq. (11)
+/* NEXT-1 (not on the hot path; ctr_cgls uses it only with ctr_params.backprojector = 1): the paper's own pixel-driven backprojector, Eq. (11)
  * (PAPER.md:195-197): d_img(u*,v*) = (dx dy / dbeta) sum_views y(beta*) / l, with y(beta*) linearly interpolated
  * between the two nearest detector units (0 outside the outermost unit centres) and l the source-pixel
  * distance; dbeta = du/dsd (ARC) or du cos^2(beta*)/dsd (FLAT). An APPROXIMATE adjoint of ctr_forward (the paper
  * reports < 1 % mismatch, :493). 2D only (CTR_EINVAL otherwise). Same layouts as ctr_back; d_img is overwritten. */
 int ctr_back_pixel(ctr_handle* h, const float* d_sino, float* d_img, void* stream);
 /* a3: n_iter CGLS iterations on min ||P x - b||^2 from the start value in d_x;
- * d_x is updated in place to u^(n_iter). n_iter = 0 is a no-op. Zero denominators stop the update (S4). */
+ * d_x is updated in place to u^(n_iter). n_iter = 0 is a no-op. Zero denominators stop the update (S4).
+ * With ctr_params.backprojector = 1 (ctr_set_params) every P^T is Eq. (11) instead (2D; CTR_EINVAL in 3D). */
 int ctr_cgls(ctr_handle* h, const float* d_b, float* d_x, int n_iter, void* stream);
 /* a4: d_w[ndim][image] = exp(-N0^2/sigma^2) with N0 the face magnitudes of A3 at d_x and
  * sigma = max(k-th smallest N0, eps), k = ceil(quantile * #interior faces) per slice (exact order

@@ -274,3 +274,70 @@ def reconstruct(g, sino, params):
     if og.ndim == 2:
         return f[0], w[:, 0], log
     return f, w, log
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT rows of SURVEY.md 8(f), composed in numpy from the C steps above (no new arithmetic in C):
+#   NEXT-1  CGLS with the paper's unmatched pair (P by ray tracing, P^T by Eq. (11))
+#   NEXT-4  the plain gradient update (P1) of Eq. 8, that the paper replaced by CGLS
+# Pins (tests/test_oracle_pins.py): cgls_recurrence(back_op=back) equals orc_cgls(reorth=0) - the C transcription
+# of App. I, itself pinned to lstsq / hand iterations; p1_updates equals the dense-matrix iteration on 8x8 and
+# converges to the least-squares solution; reconstruct_steps(step1 = cgls) equals orc_reconstruct bit for bit.
+# ---------------------------------------------------------------------------------------------
+def cgls_recurrence(g, b, x0, n_iter, back_op=None):
+    """App. I as printed, with the backprojector given as a function (default: the exact
+    transpose `back`; `back_eq11` gives the paper's own unmatched pair). Zero denominators stop (S4)."""
+    back_op = back_op or back
+    b = _c64(b)
+    u = _c64(x0).copy()
+    r = b - forward(g, u).reshape(b.shape)           # r = y - P u            (:420)
+    gr = back_op(g, r).reshape(u.shape)              # g = P^T r
+    s = gr.copy()
+    gamma = float(np.sum(gr * gr))
+    for _ in range(int(n_iter)):
+        q = forward(g, s).reshape(b.shape)           # q = P s                (:423)
+        delta = float(np.sum(q * q))
+        if gamma == 0.0 or delta == 0.0:
+            break
+        a = gamma / delta
+        u = u + a * s                                # :426
+        r = r - a * q                                # :429
+        gr = back_op(g, r).reshape(u.shape)
+        gamma_new = float(np.sum(gr * gr))           # :432
+        s = gr + (gamma_new / gamma) * s             # :435
+        gamma = gamma_new
+    return u
+
+
+def p1_updates(g, y, f, n, tau, back_op=None):
+    """(P1) of Eq. 8: f <- f - tau P^T (P f - y), n times; tau = mu/lambda."""
+    back_op = back_op or back
+    y = _c64(y)
+    f = _c64(f).copy()
+    tau = _f32(tau)
+    for _ in range(int(n)):
+        r = y - forward(g, f).reshape(y.shape)
+        f = f + tau * back_op(g, r).reshape(f.shape)
+    return f
+
+
+def reconstruct_steps(g, sino, params, step1=None):
+    """O10 composed from the oracle's steps, with Step 1 given as a function
+    step1(f) -> v (default: CGLS with the config's n_cgls, reading S24). Returns (f, log[n_outer*n_gd, 4])."""
+    og = make_geom(g)
+    d = params.params_dict() if hasattr(params, "params_dict") else dict(params)
+    p = make_params(d)
+    if step1 is None:
+        step1 = lambda f: cgls(g, sino, f, p.n_cgls).reshape(f.shape)  # noqa: E731
+    f = np.zeros((og.nz, og.ny, og.nx))
+    log = []
+    for _ in range(p.n_outer):
+        f = _c64(step1(f)).reshape(f.shape)                            # Step 1 (:171)
+        v = f.copy()
+        for _ in range(p.n_gd):                                        # Step 2 (:172)
+            w, sig = update_weights(f, p.sigma_quantile, p.eps, p.weights_mode, ndim=og.ndim)
+            f, k, e0, g2, _t = eptv_step(f, v, w, p.lam, d, ndim=og.ndim)
+            log.append((sig, k, e0, g2))
+        if p.positivity:                                               # Step 3 (:173)
+            f = np.maximum(f, 0.0)
+    return (f[0] if og.ndim == 2 else f), np.array(log)

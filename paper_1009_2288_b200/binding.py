@@ -47,7 +47,8 @@ class ctr_params(C.Structure):
                 ("lam", C.c_float), ("sigma_quantile", C.c_float), ("eps", C.c_float),
                 ("armijo_t0", C.c_float), ("armijo_rho", C.c_float), ("armijo_c", C.c_float),
                 ("armijo_max", C.c_int32), ("weights_mode", C.c_int32), ("positivity", C.c_int32),
-                ("warm_start", C.c_int32)]
+                ("warm_start", C.c_int32), ("fidelity_mode", C.c_int32), ("p1_step", C.c_float),
+                ("backprojector", C.c_int32)]
 
 
 class ctr_sweep_stat(C.Structure):

@@ -278,6 +278,20 @@ static int vec_sino_axpy(ctr_handle* h, float* r, const float* q, cudaStream_t s
   CTR_LAUNCHED(h);
   return CTR_OK;
 }
+// u <- u + tau g with one step for all slices: the (P1) update of Eq. 8, any layout
+__global__ void __launch_bounds__(256) k_axpy_const(size_t n4, float4* __restrict__ u, const float4* __restrict__ g, float tau) {
+  const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
+  if (idx >= n4) return;
+  float4 uv = __ldcg(u + idx);
+  const float4 gv = __ldcg(g + idx);
+  uv.x = fmaf(tau, gv.x, uv.x); uv.y = fmaf(tau, gv.y, uv.y); uv.z = fmaf(tau, gv.z, uv.z); uv.w = fmaf(tau, gv.w, uv.w);
+  u[idx] = uv;
+}
+__global__ void __launch_bounds__(256) k_axpy_const1(size_t n, float* __restrict__ u, const float* __restrict__ g, float tau) {
+  const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
+  if (idx < n) u[idx] = fmaf(tau, __ldcg(g + idx), u[idx]);
+}
+
 static int vec_img_uupdate(ctr_handle* h, float* u, const float* s, cudaStream_t st) {
   const Dims& d = h->d;
   const size_t nl = (size_t)d.npix * d.LQ;
@@ -319,24 +333,58 @@ static int op_back(ctr_handle* h, const float* sino, float* out, int mode, const
   return h->d.ndim == 3 ? cone_back(h, sino, out, mode, s, u, st) : fan_back(h, sino, out, mode, s, u, st);
 }
 
+// NEXT-1 inside the solvers (ctr_params.backprojector = 1): out = B sino with B the paper's pixel-driven Eq. (11)
+// in place of the exact transpose. k_back_eq11 works on the ABI layouts, so a batch goes
+// SI -> ABI -> Eq. (11) -> SI through h->q and h->n0, which are free whenever a backprojection is due.
+static int op_back_eq11(ctr_handle* h, const float* sino, float* out, cudaStream_t st) {
+  if (h->d.V == 1) return fan_back_eq11(h, sino, out, st);
+  int rc;
+  if ((rc = si_to_abi(h, sino, h->q, h->d.nray, st))) return rc;
+  if ((rc = fan_back_eq11(h, h->q, h->n0, st))) return rc;
+  return si_from_abi(h, h->n0, out, h->d.npix, st);
+}
+
 // CGLS on internal-layout arrays (gradients re-orthogonalised, S24). u: in x0 /
 // out u^(M). The last iteration only needs u (its P^T r and s are never used, O4), so it ends with a
-// plain u += a s.
+// plain u += a s. With the unmatched pair (backprojector = 1) the "gradients" B r are not orthogonal even in
+// exact arithmetic: the recurrence runs as printed, nothing is projected out.
 static int cgls_internal(ctr_handle* h, const float* b, float* u, int n_iter, bool x0_zero, cudaStream_t st) {
   if (n_iter <= 0) return CTR_OK;
   int rc;
+  const bool eq11 = h->p.backprojector == 1;
   if (x0_zero) {
     CTR_CUDA(h, cudaMemcpyAsync(h->r, b, h->nsino * sizeof(float), cudaMemcpyDeviceToDevice, st));  // r0 = y
   } else if ((rc = op_forward(h, u, h->r, 1, b, st))) return rc;                                    // r0 = y - P u0
-  if ((rc = op_back(h, h->r, h->gimg, 0, nullptr, nullptr, st))) return rc;                         // g0 = P^T r0
-  if ((rc = vec_direction(h, h->gimg, 0, 1, h->basis, st))) return rc;                              // gamma0, s0 = g0, b_0
+  if ((rc = eq11 ? op_back_eq11(h, h->r, h->gimg, st) : op_back(h, h->r, h->gimg, 0, nullptr, nullptr, st))) return rc;  // g0 = P^T r0
+  if ((rc = vec_direction(h, h->gimg, 0, 1, eq11 ? nullptr : h->basis, st))) return rc;             // gamma0, s0 = g0, b_0
   for (int m = 0; m < n_iter; ++m) {
     if ((rc = op_forward(h, h->s, h->q, 2, nullptr, st))) return rc;     // q = P s, a = gamma/||q||^2
     if (m == n_iter - 1) return vec_img_uupdate(h, u, h->s, st);         // u += a s
     if ((rc = vec_sino_axpy(h, h->r, h->q, st))) return rc;              // r -= a q
+    if (eq11) {
+      if ((rc = vec_img_uupdate(h, u, h->s, st))) return rc;             // u += a s
+      if ((rc = op_back_eq11(h, h->r, h->gimg, st))) return rc;          // g = B r
+      if ((rc = vec_direction(h, h->gimg, 0, 0, nullptr, st))) return rc;  // gamma', beta, s = g + beta s
+      continue;
+    }
     if ((rc = op_back(h, h->r, h->gimg, 2, h->s, u, st))) return rc;     // g = P^T r, u += a s
     float* bnew = (m + 1 < CTR_MAX_BASIS) ? h->basis + (size_t)(m + 1) * h->nimg : nullptr;
     if ((rc = vec_direction(h, h->gimg, m + 1, 0, bnew, st))) return rc;  // g' _|_ b_0.., gamma', beta, s = g' + beta s, b_{m+1}
+  }
+  return CTR_OK;
+}
+
+// (P1) of Eq. 8 (NEXT-4): n plain gradient updates u <- u - tau P^T (P u - y) on internal-layout arrays
+static int p1_internal(ctr_handle* h, const float* b, float* u, int n, float tau, cudaStream_t st) {
+  int rc;
+  const bool eq11 = h->p.backprojector == 1;
+  for (int m = 0; m < n; ++m) {
+    if ((rc = op_forward(h, u, h->r, 1, b, st))) return rc;                                          // r = y - P u
+    if ((rc = eq11 ? op_back_eq11(h, h->r, h->gimg, st) : op_back(h, h->r, h->gimg, 0, nullptr, nullptr, st))) return rc;
+    ProfScope prof(h, CTR_PROF_VECTOR, st);
+    if (h->d.V == 1) k_axpy_const1<<<(unsigned)((h->nimg + 255) / 256), 256, 0, st>>>(h->nimg, u, h->gimg, tau);
+    else k_axpy_const<<<(unsigned)((h->nimg / 4 + 255) / 256), 256, 0, st>>>(h->nimg / 4, (float4*)u, (const float4*)h->gimg, tau);
+    CTR_LAUNCHED(h);
   }
   return CTR_OK;
 }
@@ -356,6 +404,9 @@ static int check_params(const ctr_params* p) {
   if (!(p->eps >= 0.0f) || !(p->armijo_t0 > 0.0f) || !(p->armijo_rho > 0.0f && p->armijo_rho < 1.0f)) return CTR_EINVAL;
   if (!(p->armijo_c >= 0.0f) || p->armijo_max < 1 || p->armijo_max > CTR_MAX_ARMIJO) return CTR_EINVAL;
   if (p->weights_mode != 0 && p->weights_mode != 1) return CTR_EINVAL;
+  if (p->fidelity_mode != 0 && p->fidelity_mode != 1) return CTR_EINVAL;
+  if (p->backprojector != 0 && p->backprojector != 1) return CTR_EINVAL;
+  if (!(p->p1_step >= 0.0f)) return CTR_EINVAL;
   return CTR_OK;
 }
 
@@ -385,6 +436,7 @@ void ctr_default_params(ctr_params* p) {
   p->lambda = 0.01f; p->sigma_quantile = 0.90f; p->eps = 1e-4f;
   p->armijo_t0 = 1e-3f; p->armijo_rho = 0.5f; p->armijo_c = 0.5f; p->armijo_max = 16;
   p->weights_mode = 0; p->positivity = 1; p->warm_start = 0;
+  p->fidelity_mode = 0; p->p1_step = 0.0f; p->backprojector = 0;
 }
 
 const char* ctr_strerror(int status) {
@@ -624,6 +676,7 @@ int ctr_set_params(ctr_handle* h, const ctr_params* p) {
   if (!h) return CTR_EINVAL;
   int rc = check_params(p);
   if (rc) return set_err(h, rc, "ctr_set_params: parameter out of range");
+  if (p->backprojector == 1 && h->d.ndim != 2) return set_err(h, CTR_EINVAL, "ctr_set_params: Eq. (11) backprojector is 2D only");
   h->p = *p;
   set_quantile(h, p->sigma_quantile);
   return CTR_OK;
@@ -747,13 +800,17 @@ int ctr_reconstruct_w(ctr_handle* h, const float* d_sino, float* d_img, float* d
   // one outer iteration (Steps 1-3 of the algorithm box), enqueued on stream s
   auto outer = [&](int it, bool x0_zero, bool want_w, cudaStream_t s_) -> int {
     int rc_;
+    // Step 1 (:171): CGLS, or the (P1) gradient updates it replaced (fidelity_mode = 1)
+    auto step1 = [&](float* u) -> int {
+      return P.fidelity_mode == 1 ? p1_internal(h, b, u, P.n_cgls, P.p1_step, s_) : cgls_internal(h, b, u, P.n_cgls, x0_zero, s_);
+    };
     if (direct) {
-      if ((rc_ = cgls_internal(h, b, f, P.n_cgls, x0_zero, s_))) return rc_;                       // Step 1 (:171)
+      if ((rc_ = step1(f))) return rc_;
     } else if (P.n_cgls > 0) {
-      // batched: CGLS runs in the slice-interleaved layout, the TV sweeps in the group-planar one
+      // batched: Step 1 runs in the slice-interleaved layout, the TV sweeps in the group-planar one
       if (x0_zero) CTR_CUDA(h, cudaMemsetAsync(h->usi, 0, h->nimg * sizeof(float), s_));
       else if ((rc_ = si_from_planar(h, f, h->usi, h->d.npix, s_))) return rc_;
-      if ((rc_ = cgls_internal(h, b, h->usi, P.n_cgls, x0_zero, s_))) return rc_;                  // Step 1 (:171)
+      if ((rc_ = step1(h->usi))) return rc_;
       if ((rc_ = si_to_planar(h, h->usi, f, h->d.npix, s_))) return rc_;
     }
     if (P.n_gd > 0)

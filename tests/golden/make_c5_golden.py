@@ -17,7 +17,8 @@ gives orc_reconstruct's result bit for bit.
     python tests/golden/make_c5_golden.py [--n-outer 20] [--threads 6]
 
 About 20 minutes per outer iteration on 8 cores. The file is rewritten (atomically) after every outer
-iteration; a rerun continues from nothing (the oracle has no warm start), so let it finish.
+iteration (checkpoints KEEP and the last one reached stay in it); a rerun continues from nothing (the oracle
+has no warm start), so let it finish.
 """
 from __future__ import annotations
 
@@ -36,6 +37,7 @@ sys.path.insert(0, str(ROOT))
 
 N_SAMPLES = 131072
 SAMPLE_SEED = 10092288 + 5000 + 77
+KEEP = (1, 2, 3, 5, 10, 15, 20)  # checkpoints kept in the file besides the last one reached (1 MB each)
 
 
 def oracle_fingerprint() -> str:
@@ -92,6 +94,9 @@ def main():
         store[f"norm_{n}"] = np.linalg.norm(f)
         store["log"] = log
         store["n_done"] = n
+        if n - 1 not in KEEP:
+            for key in ("samples", "planes", "norm"):
+                store.pop(f"{key}_{n - 1}", None)
         tmp = args.out + f".tmp{os.getpid()}.npz"
         np.savez_compressed(tmp, **store)
         os.replace(tmp, args.out)

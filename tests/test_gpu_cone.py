@@ -270,3 +270,13 @@ def test_stored_matrices_equal_on_the_fly_kernels_3d(ctr, torch_cuda):
         h.close()
     assert np.array_equal(res[0][0], res[1][0])
     assert np.array_equal(res[0][1], res[1][1])
+
+
+def test_eq11_backprojector_is_rejected_in_3d(ctr, torch_cuda):
+    """ctr_params.backprojector = 1 (Eq. 11) is a 2D fan-beam formula: CTR_EINVAL on a cone-beam handle."""
+    cfg = small3d()
+    h = ctr.ctr_create(cfg)
+    with pytest.raises(ctr.CtrError):
+        h.ctr_set_params(ctr.make_params(cfg, backprojector=1))
+    h.ctr_set_params(ctr.make_params(cfg, fidelity_mode=1, p1_step=1e-4))   # (P1) itself is dimension-agnostic
+    h.close()

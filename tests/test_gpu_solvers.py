@@ -304,3 +304,108 @@ def test_warm_start_continues_the_iteration(ctr, torch_cuda, batch):
     torch.cuda.synchronize()
     assert torch.equal(a, b)
     h.close()
+
+
+# ------------------------------------------------------------------ NEXT-1 / NEXT-4: the paper's own Step-1 variants
+def _arc_config(batch=1, **kw):
+    """The paper's scanner (arc detector, 949.075 / 541.0 mm) on a reduced grid."""
+    base = dict(name="arc", index=92, ndim=2, nx=96, ny=80, nz=1, dx=3.2, dy=3.2, dz=1.0, nviews=24, nu=160, nv=1,
+                du=1.0239 * 888 / 160, dv=1.0, dso=541.0, dsd=949.075, det_type=1, batch=batch)
+    base.update(kw)
+    return Config(**base)
+
+
+def _blobs(cfg, batch, seed):
+    rng = np.random.default_rng(seed)
+    jj, ii = np.mgrid[0:cfg.ny, 0:cfg.nx]
+    out = np.zeros((batch, cfg.ny, cfg.nx))
+    for sl in range(batch):
+        for _ in range(4):
+            cx, cy = rng.uniform(0.3, 0.7) * cfg.nx, rng.uniform(0.3, 0.7) * cfg.ny
+            s = rng.uniform(0.05, 0.12) * cfg.nx
+            out[sl] += rng.uniform(0.005, 0.02) * np.exp(-((ii - cx) ** 2 + (jj - cy) ** 2) / (2 * s * s))
+    return out
+
+
+@pytest.mark.parametrize("cfg,batch", [(_arc_config(), 1), (_arc_config(batch=5), 5), (scaled_config("c1", batch=1), 1)],
+                         ids=["arc", "arc x5", "c1 flat"])
+def test_cgls_with_the_papers_unmatched_pair_matches_oracle(ctr, torch_cuda, orc, cfg, batch):
+    """NEXT-1 as a CGLS mode (ctr_params.backprojector = 1): P by ray tracing, P^T by the
+    pixel-driven Eq. (11), recurrence as printed (App. I). Against the oracle's numpy transcription with
+    orc.back_eq11, 6 iterations from a random start: relative L2 <= 1e-4, element check as everywhere."""
+    torch = torch_cuda
+    truth = _blobs(cfg, batch, 5)
+    rng = np.random.default_rng(32)
+    x0 = (0.002 * rng.random((batch, cfg.ny, cfg.nx))).astype(np.float32)
+    one = scaled_cfg_batch1(cfg)
+    y = np.stack([orc.forward(one, truth[sl]) for sl in range(batch)]).astype(np.float32)
+    h = ctr.ctr_create(cfg)
+    h.ctr_set_params(ctr.make_params(cfg, backprojector=1))
+    b, x = to_gpu(torch, y), to_gpu(torch, x0)
+    h.ctr_cgls(b, x, 6)
+    torch.cuda.synchronize()
+    got = x.cpu().numpy()
+    # and the matched pair on the same handle afterwards: the mode is a parameter, not a property of the handle
+    h.ctr_set_params(ctr.make_params(cfg, backprojector=0))
+    xm = to_gpu(torch, x0)
+    h.ctr_cgls(b, xm, 6)
+    torch.cuda.synchronize()
+    got_m = xm.cpu().numpy()
+    h.close()
+    for sl in sorted({0, batch - 1}):
+        want = orc.cgls_recurrence(one, y[sl].astype(np.float64), x0[sl].astype(np.float64), 6, back_op=orc.back_eq11)
+        assert_close(got[sl], want, 1e-4)
+        want_m = orc.cgls(one, y[sl].astype(np.float64), x0[sl].astype(np.float64), 6)
+        assert_close(got_m[sl], want_m, 1e-4)
+        # the two pairs give different iterates (the mode does something) that stay close (the paper's "< 1 %")
+        d = rel(got[sl], want_m)
+        assert 1e-5 < d < 0.2, d
+
+
+def scaled_cfg_batch1(cfg):
+    return Config(**{**cfg.__dict__, "batch": 1})
+
+
+@pytest.mark.parametrize("batch,backprojector", [(1, 0), (3, 0), (3, 1)])
+def test_reconstruct_with_the_p1_gradient_update_matches_oracle(ctr, torch_cuda, orc, batch, backprojector):
+    """NEXT-4: Step 1 as the plain gradient update (P1) of Eq. 8, v <- v - tau P^T (P v - y), n_cgls
+    times per outer iteration (fidelity_mode = 1), followed by the usual GD sweeps and the clamp. tau = 1/||P||^2
+    from a power iteration on the oracle's operators. Final image within 1e-3, Armijo indices identical."""
+    torch = torch_cuda
+    cfg = scaled_config("c1", batch=batch, n_outer=3, n_cgls=5, n_gd=2)
+    one = scaled_cfg_batch1(cfg)
+    case = make_case(cfg)
+    z = np.random.default_rng(1).random((cfg.ny, cfg.nx))
+    for _ in range(12):
+        z = orc.back(one, orc.forward(one, z))
+        nrm = np.linalg.norm(z)
+        z /= nrm
+    tau = float(np.float32(1.0 / nrm))
+    back_op = orc.back_eq11 if backprojector else orc.back
+    h = ctr.ctr_create(cfg)
+    img = torch.full(h.img_shape, float("nan"), device="cuda")
+    h.ctr_reconstruct(to_gpu(torch, case["sino"]), img, ctr.make_params(cfg, fidelity_mode=1, p1_step=tau, backprojector=backprojector))
+    torch.cuda.synchronize()
+    stats = h.ctr_get_stats()
+    got = img.cpu().numpy().astype(np.float64)
+    h.close()
+    for sl in sorted({0, batch - 1}):
+        y = case["sino"][sl].astype(np.float64)
+        want, log = orc.reconstruct_steps(one, y, cfg, step1=lambda f: orc.p1_updates(one, y, f[0], cfg.n_cgls, tau, back_op))
+        ks = [r["k"] for r in stats][sl::batch]
+        assert ks == list(log[:, 1].astype(int)), (ks, log[:, 1])
+        assert_close(got[sl], want, 1e-3)
+        assert got[sl].min() >= 0.0
+    # (P1) with this step is far from converged where CGLS is not: the modification the paper reports as "more efficient"
+    cg, _ = orc.reconstruct_steps(one, case["sino"][0].astype(np.float64), cfg)
+    res = lambda f: np.linalg.norm(orc.forward(one, f) - case["sino"][0])
+    assert res(cg) < res(got[0])
+
+
+def test_invalid_variant_parameters_are_rejected(ctr, torch_cuda):
+    cfg = scaled_config("c1")
+    h = ctr.ctr_create(cfg)
+    for bad in (dict(fidelity_mode=2), dict(backprojector=-1), dict(p1_step=-1.0), dict(p1_step=float("nan"))):
+        with pytest.raises(ctr.CtrError):
+            h.ctr_set_params(ctr.make_params(cfg, **bad))
+    h.close()

@@ -849,3 +849,74 @@ def test_eq11_pixels_outside_the_fan_get_nothing(orc):
     # view 0: source on the -x axis, central ray along +x; the 16-unit fan covers |y| < ~9 mm at the isocentre
     assert img[32, 32] > 0 and img[0, 32] == 0 and img[63, 32] == 0
     assert np.all(img >= 0)
+
+
+# ------------------------------------------------------------------ NEXT-1 / NEXT-4 compositions (oracle/ctr_oracle.py)
+def test_cgls_recurrence_in_numpy_is_the_printed_recurrence_of_the_c_oracle(orc):
+    """cgls_recurrence() is App. I typed a second time, in numpy, with the backprojector as a
+    parameter; with the exact transpose it must reproduce orc_cgls(reorth=0) - the C transcription that the lstsq,
+    hand-iteration and Krylov pins above hold in place."""
+    cfg = scaled_config("c1")
+    d = make_case(cfg)
+    y = d["sino"][0].astype(np.float64)
+    rng = np.random.default_rng(3)
+    for x0 in (np.zeros((cfg.ny, cfg.nx)), 0.01 * rng.random((cfg.ny, cfg.nx))):
+        for n in (1, 4):
+            want = orc.cgls(cfg, y, x0, n, reorth=False)
+            got = orc.cgls_recurrence(cfg, y, x0, n)
+            assert np.linalg.norm(got - want) <= 1e-12 * np.linalg.norm(want)
+
+
+def test_cgls_with_the_unmatched_pair_still_reduces_the_residual(orc):
+    """NEXT-1: the paper runs CGLS with P by ray tracing and P^T by Eq. (11). On its scanner
+    geometry (arc detector) the unmatched pair must behave like the matched one over the first iterations - the
+    residual ||P u - y|| falls, and stays within a few per cent of the matched pair's - which is the paper's
+    argument for accepting a < 1 % adjoint mismatch."""
+    cfg = _paper_geometry(nx=128, ny=128, dx=500.0 / 128, dy=500.0 / 128, nu=222, du=1.0239 * 4, nviews=30)
+    f, _ = _smooth_pair(cfg)
+    y = orc.forward(cfg, f)
+    x0 = np.zeros_like(f)
+    res = {}
+    for name, op in (("matched", orc.back), ("eq11", orc.back_eq11)):
+        res[name] = [np.linalg.norm(orc.forward(cfg, orc.cgls_recurrence(cfg, y, x0, n, back_op=op)) - y) for n in (1, 3, 6)]
+    r0 = np.linalg.norm(y)
+    assert res["eq11"][0] < 0.6 * r0 and res["eq11"][2] < res["eq11"][1] < res["eq11"][0]
+    for a, b in zip(res["matched"], res["eq11"]):
+        assert b <= 1.5 * a + 1e-3 * r0
+
+
+def test_p1_updates_equal_the_dense_matrix_iteration_and_its_svd_closed_form(orc):
+    """(P1) of Eq. 8: v = f - tau P^T (P f - y). On 8x8 with the brute-force dense matrix the
+    n-step result is the Landweber iterate written with that matrix, and from f = 0 it has the textbook closed form
+    in the SVD A = U S V^T:  f_n = sum_i (1 - (1 - tau s_i^2)^n) / s_i (u_i . y) v_i, which tends to the minimum-norm
+    least-squares solution for tau < 2/||A||^2 (the residual falls monotonically on the way)."""
+    cfg = tiny2d()
+    A = brute_matrix(cfg)
+    rng = np.random.default_rng(5)
+    y = A @ rng.random(A.shape[1]) + 0.01 * rng.standard_normal(A.shape[0])
+    tau = float(np.float32(1.0 / np.linalg.norm(A, 2) ** 2))
+    f = rng.random(A.shape[1])
+    want = f.copy()
+    for _ in range(7):
+        want = want - tau * (A.T @ (A @ want - y))
+    got = orc.p1_updates(cfg, y.reshape(cfg.nviews, cfg.nu), f.reshape(cfg.ny, cfg.nx), 7, tau)
+    assert np.linalg.norm(got.ravel() - want) <= 1e-12 * np.linalg.norm(want)
+    U, S, Vt = np.linalg.svd(A, full_matrices=False)
+    keep = S > 1e-10 * S[0]
+    res = []
+    for n in (1, 20, 150):
+        fn = orc.p1_updates(cfg, y.reshape(cfg.nviews, cfg.nu), np.zeros((cfg.ny, cfg.nx)), n, tau).ravel()
+        closed = Vt[keep].T @ ((1.0 - (1.0 - tau * S[keep] ** 2) ** n) / S[keep] * (U[:, keep].T @ y))
+        assert np.linalg.norm(fn - closed) <= 1e-10 * np.linalg.norm(closed)
+        res.append(np.linalg.norm(A @ fn - y))
+    assert res[2] < res[1] < res[0] < np.linalg.norm(y)
+
+
+def test_reconstruct_steps_with_cgls_is_orc_reconstruct(orc):
+    """reconstruct_steps() composes O10 with Step 1 as a parameter; with the default Step 1 it is orc_reconstruct."""
+    cfg = scaled_config("c1", n_outer=2, n_cgls=4, n_gd=3)
+    sino = make_case(cfg)["sino"][0].astype(np.float64)
+    want, _, log = orc.reconstruct(cfg, sino, cfg)
+    got, glog = orc.reconstruct_steps(cfg, sino, cfg)
+    assert np.array_equal(got, want)
+    assert np.array_equal(glog[:, 1], log[:, 1]) and np.allclose(glog, log, rtol=1e-12, atol=0)
