@@ -50,7 +50,7 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--geom-flags", type=int, default=0,
-                    help="ctr_geometry.flags (1 no tables, 2 no graphs, 4 batched P on the fly): A/B runs")
+                    help="ctr_geometry.flags (1 no tables, 2 no graphs, 4 batched P on the fly, 8 CGLS re-orthogonalisation in image space only): A/B runs")
     return ap.parse_args()
 
 

@@ -79,8 +79,11 @@ enum {
                             of checking that the tables hold exactly what the on-the-fly kernels compute. */
   CTR_GEOM_NO_GRAPHS = 2, /* ctr_reconstruct launches every kernel itself instead of replaying a CUDA graph of the
                             steady-state outer iteration (batch = 1 only; same kernels, same results). */
-  CTR_GEOM_NO_STORED_P = 4 /* batched slices: apply P on the fly (k_si_forward) instead of from the stored matrix
+  CTR_GEOM_NO_STORED_P = 4, /* batched slices: apply P on the fly (k_si_forward) instead of from the stored matrix
                             shared by all slices (k_si_forward_tab); the other tables are still built. */
+  CTR_GEOM_NO_LAZY_CGLS = 8 /* CGLS projects every gradient against the stored unit gradients in image space in all
+                            iterations (S24) instead of moving that work to the sinogram side after the
+                            first four: the same iteration in exact arithmetic; for A/B runs and tests. */
 };
 
 /* Iteration schedule and the constants the paper leaves open (readings S13, S14). */
@@ -182,6 +185,7 @@ typedef struct {
   double mixed_gwinst;  /* the same for FFMA and integer ALU instructions interleaved 1:1 (the integer pipe is slower) */
   double l1_tbs;        /* L1 data pipe: LDG.128 that hit in L1, TB/s (128 bytes per wavefront)                 */
   double smem_tbs;      /* shared memory: conflict-free LDS.128, TB/s                                           */
+  double l2_tbs;        /* L2 -> SM fabric: LDG.128 (cache-global) over a 32 MiB window resident in L2, TB/s    */
   double hbm_copy_gbs;  /* device-memory copy of 1 GiB, read + write bytes, GB/s                                */
   int32_t sm_count;
   int32_t pad;

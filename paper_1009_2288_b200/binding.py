@@ -40,6 +40,7 @@ class ctr_geometry(C.Structure):
 CTR_GEOM_NO_TABLES = 1
 CTR_GEOM_NO_GRAPHS = 2
 CTR_GEOM_NO_STORED_P = 4
+CTR_GEOM_NO_LAZY_CGLS = 8
 
 
 class ctr_params(C.Structure):
@@ -58,7 +59,7 @@ class ctr_sweep_stat(C.Structure):
 
 class ctr_peaks(C.Structure):
     _fields_ = [("fma_tflops", C.c_double), ("fma2_tflops", C.c_double), ("issue_gwinst", C.c_double), ("mixed_gwinst", C.c_double),
-                ("l1_tbs", C.c_double), ("smem_tbs", C.c_double), ("hbm_copy_gbs", C.c_double),
+                ("l1_tbs", C.c_double), ("smem_tbs", C.c_double), ("l2_tbs", C.c_double), ("hbm_copy_gbs", C.c_double),
                 ("sm_count", C.c_int32), ("pad", C.c_int32)]
 
 

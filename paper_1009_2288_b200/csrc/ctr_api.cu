@@ -235,7 +235,10 @@ __global__ void __launch_bounds__(1024) k_finish(int mode, const double* __restr
   const int c = n % V, sl = (gs * LQ + q) * V + c;
   if (mode == CTR_FIN_ALPHA) {
     const double gamma = sc.gamma[sl];
-    sc.a[sl] = (sum > 0.0 && gamma > 0.0) ? (float)(gamma / sum) : 0.0f;  // S4
+    const float a = (sum > 0.0 && gamma > 0.0) ? (float)(gamma / sum) : 0.0f;  // S4
+    sc.a[sl] = a;
+    // lazy phase: u_hat += a s_hat leaves out a sum_i e_i b_i; remember it per slice (nb = coefficients in use)
+    for (int i = 0; i < nb; ++i) sc.dco[(size_t)i * Bp + sl] = fmaf(a, sc.eco[(size_t)i * Bp + sl], sc.dco[(size_t)i * Bp + sl]);
   } else {
     const int qb = n / V, NBV = N / V - 1;
     if (qb < nb) sc.coef[(size_t)(i0 + qb) * Bp + sl] = (float)sum;
@@ -266,6 +269,181 @@ int reduce_finish(ctr_handle* h, int mode, int N, int nblk, int i0, int nb, int 
   }
   CTR_LAUNCHED(h);
   return CTR_OK;
+}
+
+
+// ---------------------------------------------------------------------------------------------
+// Lazy phase of the re-orthogonalised CGLS (S24, section 5). Once the CTR_MAX_BASIS unit gradients b_i
+// exist, projecting every new gradient against them in image space costs two passes over 4 image-size vectors
+// per iteration (most of the CGLS vector traffic at 64 slices). Both passes move to the sinogram side, which is
+// 5 x smaller:
+//   c_i = <b_i, P^T r> = <P b_i, r>, and P b_i comes for free: s_i = g'_i + beta_i s_(i-1) gives
+//         P b_i = (q_i - beta_i q_(i-1)) / ||g'_i|| from the q = P s that CGLS forms anyway;
+//   the projected direction is never materialised: the kernels carry s_hat = g + beta s_hat (the recurrence as
+//         printed) and per-slice coefficients e_i <- c_i + beta e_i with s = s_hat - sum_i e_i b_i, hence
+//         q = P s = P s_hat - sum_i e_i P b_i (sinogram side), and u = u_hat - sum_i d_i b_i with d_i += a e_i is
+//         materialised once, after the last iteration.
+// In exact arithmetic this is the iteration of vec_direction() term for term; in fp32 it tracks the oracle as
+// closely (tests/test_oracle_pins.py emulates both).
+// ---------------------------------------------------------------------------------------------
+// explicit phase, iteration m < CTR_MAX_BASIS: P b_m = (q - beta q_prev) / ||g'_m|| (first: q / ||g'_0||); q_prev <- q
+template <int V>
+__global__ void __launch_bounds__(256) k_sino_pb(size_t nl, int LQ, const float* __restrict__ q, float* __restrict__ qprev,
+                                                 float* __restrict__ pbm, int first, Scal sc) {
+  const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
+  const int gs = blockIdx.y;
+  if (idx >= nl) return;
+  const int sl0 = (gs * LQ + (int)(idx % LQ)) * V;
+  const size_t e = (size_t)gs * nl + idx;
+  float qv[V], pv[V], o[V];
+  Pack<V>::ldcg(q, e, qv);
+  if (!first) Pack<V>::ldcg(qprev, e, pv);
+#pragma unroll
+  for (int c = 0; c < V; ++c) o[c] = (first ? qv[c] : fmaf(-sc.beta[sl0 + c], pv[c], qv[c])) * sc.ginv[sl0 + c];
+  Pack<V>::st(pbm, e, o);
+  Pack<V>::st(qprev, e, qv);
+}
+
+// lazy phase: q <- q_hat - sum_i e_i P b_i, and delta = ||q||^2 (block partials, N = V)
+template <int V>
+__global__ void __launch_bounds__(256) k_sino_correct(size_t nl, int LQ, size_t nsino, float* __restrict__ q,
+                                                      const float* __restrict__ pb, int nb, int Bp, Scal sc, double* part) {
+  const int gs = blockIdx.y;
+  float acc[V];
+#pragma unroll
+  for (int c = 0; c < V; ++c) acc[c] = 0.0f;
+  for (size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x; idx < nl; idx += (size_t)gridDim.x * 256) {
+    const int sl0 = (gs * LQ + (int)(idx % LQ)) * V;
+    const size_t e = (size_t)gs * nl + idx;
+    float qv[V];
+    Pack<V>::ldcg(q, e, qv);
+#pragma unroll 4
+    for (int i = 0; i < nb; ++i) {
+      float pv[V];
+      Pack<V>::ldcg(pb + (size_t)i * nsino, e, pv);
+#pragma unroll
+      for (int c = 0; c < V; ++c) qv[c] = fmaf(-sc.eco[(size_t)i * Bp + sl0 + c], pv[c], qv[c]);
+    }
+    Pack<V>::st(q, e, qv);
+#pragma unroll
+    for (int c = 0; c < V; ++c) acc[c] = fmaf(qv[c], qv[c], acc[c]);
+  }
+  double red[V];
+#pragma unroll
+  for (int c = 0; c < V; ++c) red[c] = (double)acc[c];
+  block_partials_q<V, 8>(red, LQ, part + (size_t)gs * gridDim.x * LQ * V, blockIdx.x, threadIdx.x);
+}
+
+// lazy phase: r <- r - a q (App. I step 3, :429) and c_i = <P b_i, r> for the new r (block partials, N = REORTH_NB V)
+template <int V>
+__global__ void __launch_bounds__(256) k_sino_axpy_dots(size_t nl, int LQ, size_t nsino, float* __restrict__ r,
+                                                        const float* __restrict__ q, const float* __restrict__ pb, int nb,
+                                                        Scal sc, double* part) {
+  const int gs = blockIdx.y;
+  float acc[REORTH_NB * V];
+#pragma unroll
+  for (int t = 0; t < REORTH_NB * V; ++t) acc[t] = 0.0f;
+  for (size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x; idx < nl; idx += (size_t)gridDim.x * 256) {
+    const int sl0 = (gs * LQ + (int)(idx % LQ)) * V;
+    const size_t e = (size_t)gs * nl + idx;
+    float rv[V], qv[V];
+    Pack<V>::ldcg(r, e, rv);
+    Pack<V>::ldcg(q, e, qv);
+#pragma unroll
+    for (int c = 0; c < V; ++c) rv[c] = fmaf(-sc.a[sl0 + c], qv[c], rv[c]);
+    Pack<V>::st(r, e, rv);
+#pragma unroll
+    for (int i = 0; i < REORTH_NB; ++i) {
+      if (i < nb) {
+        float pv[V];
+        Pack<V>::ldcg(pb + (size_t)i * nsino, e, pv);
+#pragma unroll
+        for (int c = 0; c < V; ++c) acc[i * V + c] = fmaf(pv[c], rv[c], acc[i * V + c]);
+      }
+    }
+  }
+  double red[REORTH_NB * V];
+#pragma unroll
+  for (int t = 0; t < REORTH_NB * V; ++t) red[t] = (double)acc[t];
+  block_partials_q<REORTH_NB * V, 8>(red, LQ, part + (size_t)gs * gridDim.x * LQ * REORTH_NB * V, blockIdx.x, threadIdx.x);
+}
+
+// lazy phase, scalar step after P^T: block (q, gs) sums ||g||^2 and the c_i (partials of k_sino_axpy_dots), then gamma' = ||g||^2 - sum c_i^2, beta = gamma'/gamma
+// (:432) and e_i <- c_i + beta e_i
+template <int V>
+__global__ void __launch_bounds__(1024) k_finish_lazy(const double* __restrict__ part, int nblk, int N1, int off1,
+                                                     const double* __restrict__ part2, int nblk2, int LQ, int nb, int Bp,
+                                                     Scal sc) {
+  // ||g||^2: value off1 + c of the N1 values per (block, segment) in `part` (k_reorth_dots with nb = 0: N1 =
+  // (REORTH_NB + 1) V, off1 = REORTH_NB V; k_si_back_quad<.., 3>: N1 = V, off1 = 0)
+  constexpr int N2 = REORTH_NB * V, NT = V + N2;  // values wanted: ||g||^2 [V], c [NB][V]
+  constexpr int ROWS = 1024 / NT;
+  __shared__ double sm[ROWS][NT];
+  __shared__ double tot[NT];
+  const int q = blockIdx.x, gs = blockIdx.y, t = threadIdx.x;
+  const int n = t % NT, row = t / NT;
+  if (row < ROWS) {
+    double acc = 0.0;
+    if (n < V) {
+      const double* p = part + ((size_t)gs * nblk * LQ + q) * N1 + off1 + n;
+#pragma unroll 4
+      for (int b = row; b < nblk; b += ROWS) acc += __ldcg(p + (size_t)b * LQ * N1);
+    } else {
+      const double* p = part2 + ((size_t)gs * nblk2 * LQ + q) * N2 + (n - V);
+#pragma unroll 4
+      for (int b = row; b < nblk2; b += ROWS) acc += __ldcg(p + (size_t)b * LQ * N2);
+    }
+    sm[row][n] = acc;
+  }
+  __syncthreads();
+  if (t < NT) {
+    double acc = 0.0;
+    for (int r = 0; r < ROWS; ++r) acc += sm[r][t];
+    tot[t] = acc;
+  }
+  __syncthreads();
+  if (t >= V) return;
+  const int sl = (gs * LQ + q) * V + t;
+  double g2 = tot[t];
+  float cf[REORTH_NB];
+#pragma unroll
+  for (int i = 0; i < REORTH_NB; ++i) {
+    cf[i] = i < nb ? (float)tot[V + i * V + t] : 0.0f;
+    g2 -= (double)cf[i] * (double)cf[i];  // the coefficients act in fp32: Pythagoras with their rounded values
+  }
+  if (g2 < 0.0) g2 = 0.0;
+  const double gamma = sc.gamma[sl];
+  const float beta = gamma > 0.0 ? (float)(g2 / gamma) : 0.0f;  // S4
+  sc.beta[sl] = beta;
+  sc.gamma[sl] = g2;
+  sc.ginv[sl] = g2 > 0.0 ? (float)(1.0 / sqrt(g2)) : 0.0f;
+#pragma unroll
+  for (int i = 0; i < REORTH_NB; ++i)
+    if (i < nb) {
+      sc.coef[(size_t)i * Bp + sl] = cf[i];
+      sc.eco[(size_t)i * Bp + sl] = fmaf(beta, sc.eco[(size_t)i * Bp + sl], cf[i]);
+    }
+}
+
+// after the last iteration: u <- u_hat - sum_i d_i b_i
+template <int V>
+__global__ void __launch_bounds__(256) k_img_fixup(size_t nl, int LQ, size_t nimg, float* __restrict__ u,
+                                                   const float* __restrict__ basis, int nb, int Bp, Scal sc) {
+  const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
+  const int gs = blockIdx.y;
+  if (idx >= nl) return;
+  const int sl0 = (gs * LQ + (int)(idx % LQ)) * V;
+  const size_t e = (size_t)gs * nl + idx;
+  float uv[V];
+  Pack<V>::ldcg(u, e, uv);
+#pragma unroll 4
+  for (int i = 0; i < nb; ++i) {
+    float bv[V];
+    Pack<V>::ldcg(basis + (size_t)i * nimg, e, bv);
+#pragma unroll
+    for (int c = 0; c < V; ++c) uv[c] = fmaf(-sc.dco[(size_t)i * Bp + sl0 + c], bv[c], uv[c]);
+  }
+  Pack<V>::st(u, e, uv);
 }
 
 static int vec_sino_axpy(ctr_handle* h, float* r, const float* q, cudaStream_t st) {
@@ -326,6 +504,87 @@ static int vec_direction(ctr_handle* h, const float* g, int nb, int first, float
   return CTR_OK;
 }
 
+// lazy phase helpers (kernels above)
+static int vec_sino_pb(ctr_handle* h, int m, cudaStream_t st) {
+  const Dims& d = h->d;
+  const size_t nl = (size_t)d.nray * d.LQ;
+  dim3 grid((unsigned)((nl + 255) / 256), d.GS);
+  ProfScope prof(h, CTR_PROF_VECTOR, st);
+  float* pbm = h->pbasis + (size_t)m * h->nsino;
+  if (d.V == 1) k_sino_pb<1><<<grid, 256, 0, st>>>(nl, d.LQ, h->q, h->qprev, pbm, m == 0, h->sc);
+  else k_sino_pb<4><<<grid, 256, 0, st>>>(nl, d.LQ, h->q, h->qprev, pbm, m == 0, h->sc);
+  CTR_LAUNCHED(h);
+  return CTR_OK;
+}
+static dim3 sino_reduce_grid(const ctr_handle* h) {
+  const Dims& d = h->d;
+  const size_t nl = (size_t)d.nray * d.LQ;
+  const unsigned want = (unsigned)((nl + 255) / 256);
+  unsigned cap = (unsigned)(CTR_REDUCE_BLOCKS / d.GS);
+  if (cap < 1) cap = 1;
+  return dim3(want < cap ? want : cap, d.GS);
+}
+// q <- q_hat - sum e_i P b_i, a = gamma/||q||^2, d_i += a e_i
+static int vec_sino_correct(ctr_handle* h, cudaStream_t st) {
+  const Dims& d = h->d;
+  const size_t nl = (size_t)d.nray * d.LQ;
+  const dim3 grid = sino_reduce_grid(h);
+  const int Bp = d.G * d.V;
+  ProfScope prof(h, CTR_PROF_VECTOR, st);
+  if (d.V == 1) k_sino_correct<1><<<grid, 256, 0, st>>>(nl, d.LQ, h->nsino, h->q, h->pbasis, CTR_MAX_BASIS, Bp, h->sc, h->part);
+  else k_sino_correct<4><<<grid, 256, 0, st>>>(nl, d.LQ, h->nsino, h->q, h->pbasis, CTR_MAX_BASIS, Bp, h->sc, h->part);
+  CTR_LAUNCHED(h);
+  return reduce_finish(h, CTR_FIN_ALPHA, d.V, (int)grid.x, 0, CTR_MAX_BASIS, 0, st);
+}
+// r <- r - a q and the partials of c_i = <P b_i, r>; returns the block count of the partials in *nblk2
+static int vec_sino_axpy_dots(ctr_handle* h, int* nblk2, cudaStream_t st) {
+  const Dims& d = h->d;
+  const size_t nl = (size_t)d.nray * d.LQ;
+  const dim3 grid = sino_reduce_grid(h);
+  ProfScope prof(h, CTR_PROF_VECTOR, st);
+  if (d.V == 1) k_sino_axpy_dots<1><<<grid, 256, 0, st>>>(nl, d.LQ, h->nsino, h->r, h->q, h->pbasis, CTR_MAX_BASIS, h->sc, h->part2);
+  else k_sino_axpy_dots<4><<<grid, 256, 0, st>>>(nl, d.LQ, h->nsino, h->r, h->q, h->pbasis, CTR_MAX_BASIS, h->sc, h->part2);
+  CTR_LAUNCHED(h);
+  *nblk2 = (int)grid.x;
+  return CTR_OK;
+}
+// ||g||^2, then gamma', beta, e_i, then s_hat <- g + beta s_hat
+static int vec_direction_lazy(ctr_handle* h, const float* g, int nblk2, cudaStream_t st) {
+  const Dims& d = h->d;
+  const size_t nl = (size_t)d.npix * d.LQ;
+  const int Bp = d.G * d.V;
+  const unsigned want = (unsigned)((nl + 255) / 256);
+  unsigned dcap = (unsigned)(h->dots_blocks / d.GS);
+  if (dcap < 1) dcap = 1;
+  dim3 grid(want, d.GS), dgrid(want < dcap ? want : dcap, d.GS), fgrid(d.LQ, d.GS);
+  ProfScope prof(h, CTR_PROF_VECTOR, st);
+  if (d.V == 1) {
+    k_reorth_dots<1><<<dgrid, 256, 0, st>>>(nl, d.LQ, h->nimg, g, h->basis, 0, 0, Bp, h->sc, h->part, h->counters + 4 * d.G);
+    CTR_LAUNCHED(h);
+    k_finish_lazy<1><<<fgrid, 1024, 0, st>>>(h->part, (int)dgrid.x, REORTH_NB + 1, REORTH_NB, h->part2, nblk2, d.LQ, CTR_MAX_BASIS, Bp, h->sc);
+    CTR_LAUNCHED(h);
+    k_img_supdate<1><<<grid, 256, 0, st>>>(nl, d.LQ, h->s, g, nullptr, h->sc, 0);
+  } else {
+    k_reorth_dots<4><<<dgrid, 256, 0, st>>>(nl, d.LQ, h->nimg, g, h->basis, 0, 0, Bp, h->sc, h->part, h->counters + 4 * d.G);
+    CTR_LAUNCHED(h);
+    k_finish_lazy<4><<<fgrid, 1024, 0, st>>>(h->part, (int)dgrid.x, (REORTH_NB + 1) * 4, REORTH_NB * 4, h->part2, nblk2, d.LQ, CTR_MAX_BASIS, Bp, h->sc);
+    CTR_LAUNCHED(h);
+    k_img_supdate<4><<<grid, 256, 0, st>>>(nl, d.LQ, h->s, g, nullptr, h->sc, 0);
+  }
+  CTR_LAUNCHED(h);
+  return CTR_OK;
+}
+static int vec_img_fixup(ctr_handle* h, float* u, cudaStream_t st) {
+  const Dims& d = h->d;
+  const size_t nl = (size_t)d.npix * d.LQ;
+  dim3 grid((unsigned)((nl + 255) / 256), d.GS);
+  ProfScope prof(h, CTR_PROF_VECTOR, st);
+  if (d.V == 1) k_img_fixup<1><<<grid, 256, 0, st>>>(nl, d.LQ, h->nimg, u, h->basis, CTR_MAX_BASIS, d.G * d.V, h->sc);
+  else k_img_fixup<4><<<grid, 256, 0, st>>>(nl, d.LQ, h->nimg, u, h->basis, CTR_MAX_BASIS, d.G * d.V, h->sc);
+  CTR_LAUNCHED(h);
+  return CTR_OK;
+}
+
 static int op_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st) {
   return h->d.ndim == 3 ? cone_forward(h, img, out, mode, bs, st) : fan_forward(h, img, out, mode, bs, st);
 }
@@ -357,9 +616,44 @@ static int cgls_internal(ctr_handle* h, const float* b, float* u, int n_iter, bo
   } else if ((rc = op_forward(h, u, h->r, 1, b, st))) return rc;                                    // r0 = y - P u0
   if ((rc = eq11 ? op_back_eq11(h, h->r, h->gimg, st) : op_back(h, h->r, h->gimg, 0, nullptr, nullptr, st))) return rc;  // g0 = P^T r0
   if ((rc = vec_direction(h, h->gimg, 0, 1, eq11 ? nullptr : h->basis, st))) return rc;             // gamma0, s0 = g0, b_0
+  // lazy phase (see k_sino_pb ...): from iteration CTR_MAX_BASIS on, if the solve is long enough to get there
+  // (only where the image-size vectors stream from HBM: for a single slice everything is L2-resident and the extra
+  // launches cost more than the traffic they save - c3: 1.93 -> 2.00 ms per outer iteration, measured)
+  const bool lazy = !eq11 && !(h->g.flags & CTR_GEOM_NO_LAZY_CGLS) && n_iter > CTR_MAX_BASIS + 1 &&
+                    h->nimg * sizeof(float) >= ((size_t)32 << 20);
+  // (Folding the sinogram-side correction into k_si_forward_tab's epilogue and ||g||^2 into k_si_back_quad's was built
+  // and measured at c4: forward +0.21, back +0.14, vector -0.26 ms per step - a net loss of 0.1 ms against the
+  // separate 12-15 us passes used here: a block-wide reduction at the end of a projector block costs as much.)
+  if (lazy) {
+    const size_t nco = sizeof(float) * (size_t)h->d.G * h->d.V * CTR_MAX_BASIS;
+    CTR_CUDA(h, cudaMemsetAsync(h->sc.eco, 0, nco, st));
+    CTR_CUDA(h, cudaMemsetAsync(h->sc.dco, 0, nco, st));
+  }
   for (int m = 0; m < n_iter; ++m) {
+    if (lazy && m >= CTR_MAX_BASIS) {
+      if ((rc = op_forward(h, h->s, h->q, 0, nullptr, st))) return rc;   // q_hat = P s_hat
+      if ((rc = vec_sino_correct(h, st))) return rc;                     // q = P s, a = gamma/||q||^2, d += a e
+      if (m == n_iter - 1) {
+        if ((rc = vec_img_uupdate(h, u, h->s, st))) return rc;           // u_hat += a s_hat
+        return vec_img_fixup(h, u, st);                                  // u = u_hat - sum d_i b_i
+      }
+      int nblk2 = 0;
+      if ((rc = vec_sino_axpy_dots(h, &nblk2, st))) return rc;           // r -= a q, c_i = <P b_i, r>
+      if ((rc = op_back(h, h->r, h->gimg, 2, h->s, u, st))) return rc;   // g = P^T r, u_hat += a s_hat
+      if ((rc = vec_direction_lazy(h, h->gimg, nblk2, st))) return rc;   // ||g||^2, gamma', beta, e_i, s_hat = g + beta s_hat
+      continue;
+    }
     if ((rc = op_forward(h, h->s, h->q, 2, nullptr, st))) return rc;     // q = P s, a = gamma/||q||^2
     if (m == n_iter - 1) return vec_img_uupdate(h, u, h->s, st);         // u += a s
+    if (lazy && (rc = vec_sino_pb(h, m, st))) return rc;                 // P b_m from q_m and q_(m-1)
+    if (lazy && m == CTR_MAX_BASIS - 1) {
+      // the gradient of the next iteration is the first one projected on the sinogram side
+      int nblk2 = 0;
+      if ((rc = vec_sino_axpy_dots(h, &nblk2, st))) return rc;
+      if ((rc = op_back(h, h->r, h->gimg, 2, h->s, u, st))) return rc;
+      if ((rc = vec_direction_lazy(h, h->gimg, nblk2, st))) return rc;
+      continue;
+    }
     if ((rc = vec_sino_axpy(h, h->r, h->q, st))) return rc;              // r -= a q
     if (eq11) {
       if ((rc = vec_img_uupdate(h, u, h->s, st))) return rc;             // u += a s
@@ -459,7 +753,7 @@ void ctr_destroy(ctr_handle* h) {
   if (!h) return;
   cudaDeviceSynchronize();
   void* bufs[] = {h->rays, h->rays2, h->views, h->viewsd, h->ximg, h->bsino, h->r, h->q, h->s, h->gimg, h->v, h->w, h->n0,
-                  h->part, h->counters, h->hist, h->scal_block, h->stats, h->d_sweep, h->basis, h->win, h->imgT, h->win2, h->usi, h->cand, h->rt_tab, h->rt_cnt, h->rt_off, h->qidx, h->qwts, h->qcnt, h->ell_p.tab, h->ell_p.cap, h->ell_p.off, h->ell_pt.tab, h->ell_pt.cap, h->ell_pt.off};
+                  h->part, h->part2, h->counters, h->hist, h->scal_block, h->stats, h->d_sweep, h->basis, h->pbasis, h->qprev, h->win, h->imgT, h->win2, h->usi, h->cand, h->rt_tab, h->rt_cnt, h->rt_off, h->qidx, h->qwts, h->qcnt, h->ell_p.tab, h->ell_p.cap, h->ell_p.off, h->ell_pt.tab, h->ell_pt.cap, h->ell_pt.off};
   for (void* b : bufs)
     if (b) cudaFree(b);
   if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
@@ -484,7 +778,7 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
   if (!(g->dx > 0) || !(g->dy > 0) || !(g->du > 0) || !(g->dso > 0) || !(g->dsd > g->dso)) return CTR_EINVAL;
   if (g->ndim == 3 && (!(g->dz > 0) || !(g->dv > 0))) return CTR_EINVAL;
   if (g->det_type != 0 && g->det_type != 1) return CTR_EINVAL;
-  if (g->flags & ~(CTR_GEOM_NO_TABLES | CTR_GEOM_NO_GRAPHS | CTR_GEOM_NO_STORED_P)) return CTR_EINVAL;
+  if (g->flags & ~(CTR_GEOM_NO_TABLES | CTR_GEOM_NO_GRAPHS | CTR_GEOM_NO_STORED_P | CTR_GEOM_NO_LAZY_CGLS)) return CTR_EINVAL;
   if ((long long)g->nx * g->ny * g->nz >= (1ll << 31) || (long long)g->nviews * g->nu * g->nv >= (1ll << 31)) return CTR_EINVAL;
   // source and detector must lie outside the circle circumscribing the grid (plus one voxel)
   {
@@ -572,6 +866,9 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
   A((void**)&h->w, h->nimg * fb * d.ndim);
   A((void**)&h->n0, h->nimg * fb * d.ndim);
   A((void**)&h->basis, h->nimg * fb * CTR_MAX_BASIS);  // unit CGLS gradients b_0..b_3 (S24)
+  A((void**)&h->pbasis, h->nsino * fb * CTR_MAX_BASIS);  // P b_i, and q of the previous iteration (lazy CGLS phase)
+  A((void**)&h->qprev, h->nsino * fb);
+  A((void**)&h->part2, sizeof(double) * (size_t)CTR_REDUCE_BLOCKS * 16 * REORTH_NB * 4);  // [GS][blocks <= cap/GS][LQ][NB V]
   // partial sums: the largest user is the TV trial kernel (TV_KC * V slots per block)
   {
     size_t nblk_tv = (size_t)((d.nx + 31) / 32) * ((d.ny + 3) / 4) * d.nz;
@@ -592,7 +889,7 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
   A((void**)&h->hist, sizeof(unsigned) * 2048 * Bp);
   A((void**)&h->stats, sizeof(ctr_sweep_stat) * (size_t)CTR_STAT_SWEEPS * Bp);
   A((void**)&h->d_sweep, 16);
-  const size_t scal_bytes = (size_t)Bp * (3 * sizeof(double) + (5 + CTR_MAX_BASIS) * sizeof(float) + 7 * sizeof(unsigned) + 16);
+  const size_t scal_bytes = (size_t)Bp * (3 * sizeof(double) + (5 + 3 * CTR_MAX_BASIS) * sizeof(float) + 7 * sizeof(unsigned) + 16);
   {
     // candidate lists of the fused sigma selection: a quarter of the faces of a slice / volume each
     unsigned long long S = (unsigned long long)(d.nx - 1) * d.ny * d.nz + (unsigned long long)d.nx * (d.ny - 1) * d.nz;
@@ -628,6 +925,8 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
     h->sc.sel_rank = (unsigned*)p; p += sizeof(unsigned) * Bp;
     h->sc.ginv = (float*)p; p += sizeof(float) * Bp;
     h->sc.coef = (float*)p; p += sizeof(float) * Bp * CTR_MAX_BASIS;
+    h->sc.eco = (float*)p; p += sizeof(float) * Bp * CTR_MAX_BASIS;
+    h->sc.dco = (float*)p; p += sizeof(float) * Bp * CTR_MAX_BASIS;
     h->sc.pred = (int*)p; p += sizeof(int) * Bp;
     h->sc.cand_cnt = (unsigned*)p; p += sizeof(unsigned) * Bp;
     h->sc.ovf = (unsigned*)p; p += sizeof(unsigned) * Bp;

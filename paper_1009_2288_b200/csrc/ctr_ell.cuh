@@ -95,10 +95,19 @@ __global__ void __launch_bounds__(128) k_ell_apply(size_t nrows, const int* __re
   }
   if (ROLE == 0 && MODE == 2) {
     double v[1] = {(double)acc * (double)acc};
-    grid_reduce<1>(v, part, counter, gridDim.x, blockIdx.x, threadIdx.x, 128, [&](double(&sum)[1]) {
-      const double gamma = sc.gamma[0];
-      sc.a[0] = (sum[0] > 0.0 && gamma > 0.0) ? (float)(gamma / sum[0]) : 0.0f;  // S4
-    });
+    if (counter) {
+      // few blocks (a 2D slice): the block that arrives last adds the partials and forms a = gamma/delta here
+      grid_reduce<1>(v, part, counter, gridDim.x, blockIdx.x, threadIdx.x, 128, [&](double(&sum)[1]) {
+        const double gamma = sc.gamma[0];
+        sc.a[0] = (sum[0] > 0.0 && gamma > 0.0) ? (float)(gamma / sum[0]) : 0.0f;  // S4
+      });
+    } else {
+      // many blocks (c5: 92 000, where that single finishing block took ~0.6 ms): block partials only, k_finish
+      // adds them with 1024 threads
+      __shared__ double sm[1][32];
+      block_sum<1>(v, sm, threadIdx.x, 128);
+      if (threadIdx.x == 0) part[blockIdx.x] = v[0];
+    }
   }
 }
 
@@ -150,8 +159,10 @@ static int ell_forward(ctr_handle* h, const EllTable& t, const float* img, float
   unsigned* cnt = h->counters;
   if (mode == 0) k_ell_apply<0, 0, SPLIT><<<nblk, 128, 0, st>>>(t.nrows, t.cap, t.off, t.tab, img, out, bs, nullptr, h->sc, h->part, cnt);
   else if (mode == 1) k_ell_apply<0, 1, SPLIT><<<nblk, 128, 0, st>>>(t.nrows, t.cap, t.off, t.tab, img, out, bs, nullptr, h->sc, h->part, cnt);
-  else k_ell_apply<0, 2, SPLIT><<<nblk, 128, 0, st>>>(t.nrows, t.cap, t.off, t.tab, img, out, bs, nullptr, h->sc, h->part, cnt);
+  else k_ell_apply<0, 2, SPLIT><<<nblk, 128, 0, st>>>(t.nrows, t.cap, t.off, t.tab, img, out, bs, nullptr, h->sc, h->part,
+                                                      nblk > 8192 ? nullptr : cnt);
   CTR_LAUNCHED(h);
+  if (mode == 2 && nblk > 8192) return reduce_finish(h, CTR_FIN_ALPHA, 1, (int)nblk, 0, 0, 0, st);  // a = gamma/||P s||^2
   return CTR_OK;
 }
 

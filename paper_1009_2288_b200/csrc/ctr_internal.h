@@ -53,6 +53,8 @@ struct Scal {
   unsigned* sel_rank;
   float* ginv;     // 1/||g|| of the newest CGLS gradient (0 when g = 0)
   float* coef;     // [CTR_MAX_BASIS][Bp] projections of g on the stored unit gradients
+  float* eco;      // [CTR_MAX_BASIS][Bp] lazy phase of CGLS: the true direction is s = s_hat - sum_i eco_i b_i
+  float* dco;      // [CTR_MAX_BASIS][Bp] lazy phase of CGLS: the true iterate is u = u_hat - sum_i dco_i b_i
   // fused sigma selection (ctr_tv.cu): candidate lists of the first radix pass
   int* pred;            // top-11-bit bin of sigma^2 found by the previous sweep (the prediction; < 0: none)
   unsigned* cand_cnt;   // entries appended to the slice's candidate list by the current first pass
@@ -129,6 +131,9 @@ struct ctr_handle {
   unsigned cand_cap;
   float* usi;           // CGLS iterate in the slice-interleaved layout (batch > 1)
   float* basis;         // [CTR_MAX_BASIS][nimg] unit CGLS gradients (S24), allocated in ctr_create
+  float* pbasis;        // [CTR_MAX_BASIS][nsino] their projections P b_i (lazy phase of CGLS, ctr_api.cu)
+  float* qprev;         // [nsino] P s of the previous CGLS iteration while the P b_i are being formed
+  double* part2;        // block partials of the sinogram-side dot products <P b_i, r>
   int dots_blocks;      // resident blocks of k_reorth_dots on this device (its grid size)
   double* part;
   size_t part_len;

@@ -107,6 +107,26 @@ __global__ void __launch_bounds__(PK_THREADS) k_peak_l1(int iters, const float4*
   if (acc == 123.456f) sink[0] = acc;
 }
 
+// 3b. L2 -> SM fabric: the same LDG.128 stream, but cache-global (ld.global.cg: not kept in L1) over a window of
+// 2^21 float4 = 32 MiB that stays resident in the 126 MB L2; every warp reads 512 contiguous bytes (4 sectors
+// of 4 lines) at a rotating, warp-dependent offset, like the 256-byte gathers of the projector kernels
+__global__ void __launch_bounds__(PK_THREADS) k_peak_l2(int iters, const float4* __restrict__ buf, float* sink) {
+  const unsigned lane = threadIdx.x & 31u;
+  unsigned w = (blockIdx.x * (PK_THREADS / 32) + (threadIdx.x >> 5)) * 2654435761u;  // warp-dependent start chunk
+  float acc = 0.0f;
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      float4 v;
+      const float4* p = buf + ((size_t)(w & 0xffffu) * 32u + lane);  // chunk of 32 float4 out of 65536 chunks
+      asm volatile("ld.global.cg.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+      acc += (v.x + v.y) + (v.z + v.w);
+      w = w * 1664525u + 1013904223u;
+    }
+  }
+  if (acc == 123.456f) sink[0] = acc;
+}
+
 // 4. shared memory: LDS.128 per thread (4 wavefronts per warp), conflict-free
 __global__ void __launch_bounds__(PK_THREADS) k_peak_smem(int iters, float* sink) {
   __shared__ float4 sm[512];
@@ -189,6 +209,8 @@ extern "C" int ctr_measure_peaks(ctr_peaks* out, int reps) {
   out->mixed_gwinst = threads / 32.0 * iters * 128.0 / (ms * 1e-3) / 1e9;
   if (e == cudaSuccess) e = best_ms([&] { k_peak_l1<<<blocks, PK_THREADS>>>(iters, buf, sink); }, reps, &ms);
   out->l1_tbs = threads * iters * 8.0 * 16.0 / (ms * 1e-3) / 1e12;
+  if (e == cudaSuccess) e = best_ms([&] { k_peak_l2<<<blocks, PK_THREADS>>>(iters / 8, src, sink); }, reps, &ms);
+  out->l2_tbs = threads * (iters / 8) * 8.0 * 16.0 / (ms * 1e-3) / 1e12;
   if (e == cudaSuccess) e = best_ms([&] { k_peak_smem<<<blocks, PK_THREADS>>>(iters, sink); }, reps, &ms);
   out->smem_tbs = threads * iters * 8.0 * 16.0 / (ms * 1e-3) / 1e12;
   if (e == cudaSuccess) e = best_ms([&] { k_peak_copy<<<sms * 16, PK_THREADS>>>(src, dst, ncopy); }, reps, &ms);

@@ -208,8 +208,11 @@ __global__ void __launch_bounds__(128) k_raytab_build(Dims d, const float4* __re
   }
 }
 
+#ifndef SI_TAB_MINB
+#define SI_TAB_MINB SI_FWD_MINB
+#endif
 template <int LQ, int MODE>
-__global__ void __launch_bounds__(SI_FWD_WARPS * 32, SI_FWD_MINB) k_si_forward_tab(Dims d, const int* __restrict__ cnt,
+__global__ void __launch_bounds__(SI_FWD_WARPS * 32, SI_TAB_MINB) k_si_forward_tab(Dims d, const int* __restrict__ cnt,
                                                     const unsigned* __restrict__ off, const float2* __restrict__ tab,
                                                     const float4* __restrict__ img, float4* __restrict__ out,
                                                     const float4* __restrict__ bs, Scal sc, double* part) {

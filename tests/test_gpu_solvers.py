@@ -409,3 +409,30 @@ def test_invalid_variant_parameters_are_rejected(ctr, torch_cuda):
         with pytest.raises(ctr.CtrError):
             h.ctr_set_params(ctr.make_params(cfg, **bad))
     h.close()
+
+
+@pytest.mark.parametrize("name,batch,n_iter", [("c2", 1, 15), ("c2", 5, 15), ("c1", 3, 6)])
+def test_cgls_lazy_phase_against_image_space_projection_and_oracle(ctr, torch_cuda, orc, name, batch, n_iter):
+    """DESIGN.md S24: after the first four iterations ctr_cgls projects the gradients on the sinogram side and
+    carries the direction implicitly (the lazy phase); CTR_GEOM_NO_LAZY_CGLS keeps the image-space projection of
+    round 1 throughout. Same iteration in exact arithmetic: both must meet the oracle's tolerance and agree with
+    one another at that level."""
+    torch = torch_cuda
+    cfg = scaled_config(name, batch=batch)
+    case = make_case(cfg)
+    rng = np.random.default_rng(33)
+    x0 = (0.01 * rng.random((batch, cfg.ny, cfg.nx))).astype(np.float32)
+    got = {}
+    for flags in (0, ctr.CTR_GEOM_NO_LAZY_CGLS):
+        h = ctr.ctr_create(cfg, flags=flags)
+        b, x = to_gpu(torch, case["sino"]), to_gpu(torch, x0)
+        h.ctr_cgls(b, x, n_iter)
+        torch.cuda.synchronize()
+        got[flags] = x.cpu().numpy()
+        h.close()
+    one = scaled_config(name, batch=1)
+    for sl in sorted({0, batch - 1}):
+        want = orc.cgls(one, case["sino"][sl].astype(np.float64), x0[sl].astype(np.float64), n_iter)
+        for flags in got:
+            assert_close(got[flags][sl], want, 1e-4)
+        assert rel(got[0][sl], got[ctr.CTR_GEOM_NO_LAZY_CGLS][sl].astype(np.float64)) <= 2e-4   # each within 1e-4 of the oracle

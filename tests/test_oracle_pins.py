@@ -782,6 +782,73 @@ def test_S24_projecting_against_the_first_four_gradients_tracks_the_full_reortho
     assert first4 <= 3 * full + 1e-6
 
 
+def _cgls_fp32_lazy_emulation(orc, cfg, y, M, NB=4):
+    """The CUDA path's LAZY phase (ctr_api.cu, S24) emulated the same way: the first NB iterations project
+    in image space as above; from then on the coefficients c_i = <P b_i, r> are taken on the sinogram side, with
+    P b_i = (q_i - beta_i q_(i-1)) / ||g'_i|| from the q = P s of the first iterations, the direction is carried as
+    s_hat = g + beta s_hat with s = s_hat - sum e_i b_i, e_i <- c_i + beta e_i, q = P s_hat - sum e_i P b_i, and
+    u = u_hat - sum d_i b_i (d_i += a e_i) is formed once at the end. Scalars are rounded to fp32 as on the device."""
+    f32 = lambda a: np.asarray(a).astype(np.float32).astype(np.float64)
+    P = lambda x: f32(orc.forward(cfg, x))
+    PT = lambda r: f32(orc.back(cfg, r))
+    u = np.zeros((cfg.ny, cfg.nx))
+    r = y.copy()
+    g = PT(r)
+    gam = (g * g).sum()
+    s = g.copy()
+    ginv = 1.0 / np.sqrt(gam)
+    B, PB = [f32(g * ginv)], []
+    e, dacc = np.zeros(NB), np.zeros(NB)
+    qprev, beta = None, 0.0
+    for m in range(M):
+        q = P(s)
+        if m < NB:
+            PB.append(f32(q * ginv if m == 0 else (q - beta * qprev) * ginv))
+            qprev = q
+        else:
+            q = f32(q - sum(ei * pb for ei, pb in zip(e, PB)))
+        a = float(np.float32(gam / (q * q).sum()))
+        u = f32(u + a * s)
+        dacc = dacc + a * e
+        r = f32(r - a * q)
+        g = PT(r)
+        g2 = (g * g).sum()
+        if m + 1 < NB:
+            c = [float(np.float32((b * g).sum())) for b in B]
+            g2 -= sum(ci * ci for ci in c)
+            gp = g - sum(ci * b for ci, b in zip(c, B))
+            beta = float(np.float32(g2 / gam))
+            s = f32(gp + beta * s)
+            ginv = 1.0 / np.sqrt(g2)
+            B.append(f32(gp * ginv))
+        else:
+            c = np.array([float(np.float32((pb * r).sum())) for pb in PB])
+            g2 -= (c * c).sum()
+            beta = float(np.float32(g2 / gam))
+            e = f32(c + beta * e)
+            s = f32(g + beta * s)
+        gam = g2
+    return f32(u - sum(di * b for di, b in zip(dacc, B)))
+
+
+@pytest.mark.parametrize("name,M", [("c1", 10), ("c2", 15)])
+def test_S24_sinogram_side_projection_tracks_the_full_reorthogonalisation(orc, name, M):
+    """DESIGN.md S24, lazy phase: moving the projection against the first four unit gradients to the sinogram side
+    (<b_i, P^T r> = <P b_i, r>) and carrying the projected direction implicitly is the same iteration in exact
+    arithmetic; in fp32-rounded arithmetic it stays as close to the oracle's fully re-orthogonalised CGLS as the
+    image-space projection does."""
+    cfg = scaled_config(name, batch=1)
+    y = make_case(cfg, raster=False)["sino"][0].astype(np.float64)
+    ref = orc.cgls(cfg, y, np.zeros((cfg.ny, cfg.nx)), M)
+    rel = lambda a: np.linalg.norm(a - ref) / np.linalg.norm(ref)
+    first4 = rel(_cgls_fp32_emulation(orc, cfg, y, M, lambda n: range(min(4, n))))
+    lazy = rel(_cgls_fp32_lazy_emulation(orc, cfg, y, M))
+    print(f"[S24] {name}, {M} iterations, fp32-rounded emulation vs the oracle: first 4 in image space {first4:.2e}, "
+          f"lazy (sinogram side) {lazy:.2e}")
+    assert lazy <= 5e-5
+    assert lazy <= 3 * first4 + 1e-6
+
+
 # ------------------------------------------------------------------ NEXT-1: the paper's backprojector Eq. (11)
 def _paper_geometry(**kw):
     """PAPER.md:217: arc detector, 888 units x 1.0239 mm, source-detector 949.075 mm, source-axis 541.0 mm;
