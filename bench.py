@@ -297,7 +297,7 @@ def main():
             "kernel_launch_groups_per_step": {k: v[1] / K for k, v in prof.items()},
         }
         out["roofline"] = roofline(cfg, batch, prof, peaks, dev_peaks, path)
-        out["hbm_bound_parts"] = hbm_kinds(cfg, batch, prof, peaks, K)
+        out["hbm_bound_parts"] = hbm_kinds(cfg, batch, prof, peaks, K, dev_peaks)
         out["measured_peaks_this_run"] = dev_peaks
         out["kernel_path"] = path
         if not args.no_cpu_baseline:
@@ -313,17 +313,23 @@ def main():
 NNZ = {"c1": 2.32e5, "c2": 4.60e6, "c3": 2.95e7, "c4": 2.95e7, "c5": 4.37e9}  # nnz(P) per slice / volume
 
 
-def ncu_traffic(cfg, batch, kernel_substr):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture of this
-    workload (profiles/dram_traffic.csv: workload,batch,kernel,dram_bytes_per_launch,source), or (None, None)."""
+def ncu_row(cfg, batch, kernel_substr):
+    """Per-launch figures of a kernel from the committed `ncu --set full` capture of this workload
+    (profiles/ncu_per_launch.csv: workload,batch,kernel,dram_bytes,l2_to_l1_bytes,warp_insts,source), or None."""
     try:
-        for line in (ROOT / "profiles" / "dram_traffic.csv").read_text().splitlines()[1:]:
-            wl, b, kern, nbytes, src = [c.strip() for c in line.split(",", 4)]
+        for line in (ROOT / "profiles" / "ncu_per_launch.csv").read_text().splitlines()[1:]:
+            wl, b, kern, dram, l2, inst, src = [c.strip() for c in line.split(",", 6)]
             if wl == cfg.name and int(b) == batch and kern in kernel_substr:
-                return float(nbytes), src
+                num = lambda x: float(x) if x else None  # noqa: E731
+                return {"dram": num(dram), "l2": num(l2), "inst": num(inst), "src": src}
     except Exception:
         pass
-    return None, None
+    return None
+
+
+def ncu_traffic(cfg, batch, kernel_substr):
+    row = ncu_row(cfg, batch, kernel_substr)
+    return (row["dram"], row["src"]) if row else (None, None)
 
 
 def roofline(cfg, batch, prof, peaks, dev_peaks, path):
@@ -365,17 +371,23 @@ def roofline(cfg, batch, prof, peaks, dev_peaks, path):
 
     def view(k):
         sec, n = launch_s(k)
-        traffic, tsrc = ncu_traffic(cfg, batch, path.get(k, ""))
+        row = ncu_row(cfg, batch, path.get(k, "")) or {}
         l1 = 4.0 * nnz * batch / sec / 1e9
         fma = 2.0 * nnz * batch / sec / 1e12
-        return {"kernel": f"{path.get(k)} ({'P, a1' if k == 'forward' else 'P^T gather, a2'})",
-                "achieved": l1, "peak": dev_peaks["l1_tbs"] * 1e3, "unit": "GB/s", "frac": l1 / (dev_peaks["l1_tbs"] * 1e3),
-                "traffic": traffic, "traffic_source": tsrc, "avg_launch_ms": sec * 1e3, "launches": n,
-                "fma_view": {"achieved": fma, "peak": dev_peaks["fma_tflops"], "unit": "TFLOP/s",
-                             "frac": fma / dev_peaks["fma_tflops"]},
-                "hbm_view": {"achieved": bytes_alg / sec / 1e9, "peak": hbm, "unit": "GB/s",
-                             "frac": bytes_alg / sec / 1e9 / hbm, "peak_source": hbm_src,
-                             "note": "compulsory bytes (image + sinogram once) of one application"}}
+        out = {"kernel": f"{path.get(k)} ({'P, a1' if k == 'forward' else 'P^T gather, a2'})",
+               "achieved": l1, "peak": dev_peaks["l1_tbs"] * 1e3, "unit": "GB/s", "frac": l1 / (dev_peaks["l1_tbs"] * 1e3),
+               "traffic": row.get("dram"), "traffic_source": row.get("src"), "avg_launch_ms": sec * 1e3, "launches": n,
+               "fma_view": {"achieved": fma, "peak": dev_peaks["fma_tflops"], "unit": "TFLOP/s",
+                            "frac": fma / dev_peaks["fma_tflops"]},
+               "hbm_view": {"achieved": bytes_alg / sec / 1e9, "peak": hbm, "unit": "GB/s",
+                            "frac": bytes_alg / sec / 1e9 / hbm, "peak_source": hbm_src,
+                            "note": "compulsory bytes (image + sinogram once) of one application"}}
+        if row.get("l2") and dev_peaks.get("l2_tbs"):
+            l2 = row["l2"] / sec / 1e9
+            out["l2_view"] = {"achieved": l2, "peak": dev_peaks["l2_tbs"] * 1e3, "unit": "GB/s", "frac": l2 / (dev_peaks["l2_tbs"] * 1e3),
+                              "note": "bytes that cross the L2 -> SM fabric per launch (ncu, profiles/ncu_per_launch.csv) over this "
+                                      "run's launch time; peak = LDG.128 cache-global over an L2-resident window, measured in this run"}
+        return out
 
     return {"bound": "l1", **view(kind),
             "peak_source": "L1 load bandwidth measured in this run by ctr_measure_peaks (LDG.128 hitting L1, full "
@@ -385,7 +397,7 @@ def roofline(cfg, batch, prof, peaks, dev_peaks, path):
             "other": view("back" if kind == "forward" else "forward")}
 
 
-def hbm_kinds(cfg, batch, prof, peaks, steps):
+def hbm_kinds(cfg, batch, prof, peaks, steps, dev_peaks=None):
     """The HBM-bound parts of a step: CGLS vector work (a3) and the TV sweeps (a4-a7),
     algorithmic bytes per unit over the measured copy bandwidth."""
     hbm = peaks.get("hbm_gbs", 6650.0)
@@ -404,7 +416,18 @@ def hbm_kinds(cfg, batch, prof, peaks, steps):
                         "achieved_GBps": by_t / (ms_t * 1e-3) / 1e9 if ms_t > 0 else None,
                         "frac_of_measured_hbm": by_t / (ms_t * 1e-3) / 1e9 / hbm if ms_t > 0 else None,
                         "note": "44 B/pixel per sweep, the lower figure of SURVEY.md 8(d) a4-a7 (60 B/pixel would "
-                                "read 1.36x higher)"}
+                                "read 1.36x higher); the fused sweep moves 40 B/pixel"}
+    row = ncu_row(cfg, batch, "tv_sweep")
+    if row and row.get("inst") and dev_peaks and ms_t > 0 and cfg.n_gd > 0:
+        # the sweep is bound by instruction issue, not by HBM (profiles/): warp instructions of one sweep (ncu) over this
+        # run's time per sweep, against the issue rate measured in this run
+        rate = row["inst"] / (ms_t / cfg.n_gd * 1e-3) / 1e9
+        out["tv_sweeps"]["issue_view"] = {"warp_insts_per_sweep": row["inst"], "source": row["src"], "achieved_gwinst": rate,
+                                          "peak_gwinst": dev_peaks["issue_gwinst"], "frac": rate / dev_peaks["issue_gwinst"],
+                                          "peak_mixed_gwinst": dev_peaks["mixed_gwinst"],
+                                          "frac_of_mixed": rate / dev_peaks["mixed_gwinst"],
+                                          "note": "peak = one warp instruction per clock and scheduler (FFMA stream); mixed = FFMA and "
+                                                  "integer instructions 1:1"}
     return out
 
 

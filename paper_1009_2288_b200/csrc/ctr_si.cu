@@ -484,7 +484,7 @@ __global__ void __launch_bounds__(256, SI_BACK_MINB) k_si_back_quad(Dims d, cons
   // chunk of LQ table entries per quad, handed round through shared memory (broadcast reads; rows padded
   // so that the sub-warps of a warp use different banks)
   __shared__ float4 chw[PB][LQ + 1];
-  __shared__ int chi[PB][LQ + 1];
+  __shared__ __align__(16) int chi[PB][LQ + 4];  // rows 16-byte aligned: four indices per LDS.128
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int q = lane % LQ, sub = lane / LQ;
   const int pl = warp * (32 / LQ) + sub;
@@ -512,16 +512,37 @@ __global__ void __launch_bounds__(256, SI_BACK_MINB) k_si_back_quad(Dims d, cons
     chi[pl][q] = id;
     chw[pl][q] = w4;
     __syncwarp();
+    if (LQ % 4 == 0) {
+      // the ray indices four at a time: a broadcast LDS.128 per four entries instead of an LDS.32 per entry (shared
+      // memory and the gathers share the L1 data pipe, which bounds this kernel)
 #pragma unroll
-    for (int t = 0; t < LQ; ++t) {
-      const int it = chi[pl][t];
-      if (it >= 0) {
-        const float4 w = chw[pl][t];
-        const float4 y = __ldg(sg + it);
-        fma4(acc[0], w.x, y);
-        fma4(acc[1], w.y, y);
-        fma4(acc[2], w.z, y);
-        fma4(acc[3], w.w, y);
+      for (int t4 = 0; t4 < LQ / 4; ++t4) {
+        const int4 i4 = *reinterpret_cast<const int4*>(&chi[pl][4 * t4]);
+        const int its[4] = {i4.x, i4.y, i4.z, i4.w};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          if (its[k] >= 0) {
+            const float4 w = chw[pl][4 * t4 + k];
+            const float4 y = __ldg(sg + its[k]);
+            fma4(acc[0], w.x, y);
+            fma4(acc[1], w.y, y);
+            fma4(acc[2], w.z, y);
+            fma4(acc[3], w.w, y);
+          }
+        }
+      }
+    } else {
+#pragma unroll
+      for (int t = 0; t < LQ; ++t) {
+        const int it = chi[pl][t];
+        if (it >= 0) {
+          const float4 w = chw[pl][t];
+          const float4 y = __ldg(sg + it);
+          fma4(acc[0], w.x, y);
+          fma4(acc[1], w.y, y);
+          fma4(acc[2], w.z, y);
+          fma4(acc[3], w.w, y);
+        }
       }
     }
   }
