@@ -33,6 +33,28 @@ __device__ __forceinline__ void fma4(float (&acc)[4], float w, const float4 f) {
   acc[3] = fmaf(w, f.w, acc[3]);
 }
 
+// The 4 x 4 outer product acc[p][c] += w_p y_c of the quad gather with packed fp32x2 instructions (FFMA2, sm_100):
+// A[pp][0] = (acc[2pp][0], acc[2pp+1][1]), A[pp][1] = (acc[2pp][1], acc[2pp+1][0]), A[pp][2] = (acc[2pp][2],
+// acc[2pp+1][3]), A[pp][3] = (acc[2pp][3], acc[2pp+1][2]): the weight pairs (w0,w1), (w2,w3) and the slice pairs
+// (y0,y1), (y2,y3) are the register pairs the 128-bit loads deliver, the swapped slice pairs cost two moves:
+// 8 FFMA2 + moves instead of 16 FFMA per table entry, the same fma per accumulator in the same order (same bits).
+__device__ __forceinline__ void outer16(float2 (&A)[2][4], const float4 w, const float4 y) {
+  const float2 w01 = make_float2(w.x, w.y), w23 = make_float2(w.z, w.w);
+  const float2 y01 = make_float2(y.x, y.y), y10 = make_float2(y.y, y.x);
+  const float2 y23 = make_float2(y.z, y.w), y32 = make_float2(y.w, y.z);
+  A[0][0] = __ffma2_rn(w01, y01, A[0][0]);
+  A[0][1] = __ffma2_rn(w01, y10, A[0][1]);
+  A[0][2] = __ffma2_rn(w01, y23, A[0][2]);
+  A[0][3] = __ffma2_rn(w01, y32, A[0][3]);
+  A[1][0] = __ffma2_rn(w23, y01, A[1][0]);
+  A[1][1] = __ffma2_rn(w23, y10, A[1][1]);
+  A[1][2] = __ffma2_rn(w23, y23, A[1][2]);
+  A[1][3] = __ffma2_rn(w23, y32, A[1][3]);
+}
+#ifndef SI_BACK_FMA2
+#define SI_BACK_FMA2 1
+#endif
+
 // ------------------------------------------------------------------------------------------------
 // a1  P. Sub-warp per ray. The slab loop runs over a warp-uniform range in batches of LQ slabs: lane q
 // evaluates slab_weights() of slab sb+q (closed form per slab, no dependence between slabs), then the
@@ -498,6 +520,11 @@ __global__ void __launch_bounds__(256, SI_BACK_MINB) k_si_back_quad(Dims d, cons
   for (int p = 0; p < 4; ++p)
 #pragma unroll
     for (int c = 0; c < 4; ++c) acc[p][c] = 0.0f;
+  float2 A2[2][4];
+#pragma unroll
+  for (int pp = 0; pp < 2; ++pp)
+#pragma unroll
+    for (int c = 0; c < 4; ++c) A2[pp][c] = make_float2(0.0f, 0.0f);
   const int cnt = live ? __ldg(&qcnt[quad]) : 0;
   const int wmax = __reduce_max_sync(FULL, cnt);
   const float4* sg = sino + (size_t)gs * d.nray * LQ + q;
@@ -524,10 +551,14 @@ __global__ void __launch_bounds__(256, SI_BACK_MINB) k_si_back_quad(Dims d, cons
           if (its[k] >= 0) {
             const float4 w = chw[pl][4 * t4 + k];
             const float4 y = __ldg(sg + its[k]);
-            fma4(acc[0], w.x, y);
-            fma4(acc[1], w.y, y);
-            fma4(acc[2], w.z, y);
-            fma4(acc[3], w.w, y);
+            if (SI_BACK_FMA2) {
+              outer16(A2, w, y);
+            } else {
+              fma4(acc[0], w.x, y);
+              fma4(acc[1], w.y, y);
+              fma4(acc[2], w.z, y);
+              fma4(acc[3], w.w, y);
+            }
           }
         }
       }
@@ -547,6 +578,13 @@ __global__ void __launch_bounds__(256, SI_BACK_MINB) k_si_back_quad(Dims d, cons
     }
   }
   if (!live) return;
+  if (SI_BACK_FMA2 && LQ % 4 == 0) {
+#pragma unroll
+    for (int pp = 0; pp < 2; ++pp) {
+      acc[2 * pp][0] = A2[pp][0].x; acc[2 * pp][1] = A2[pp][1].x; acc[2 * pp][2] = A2[pp][2].x; acc[2 * pp][3] = A2[pp][3].x;
+      acc[2 * pp + 1][0] = A2[pp][1].y; acc[2 * pp + 1][1] = A2[pp][0].y; acc[2 * pp + 1][2] = A2[pp][3].y; acc[2 * pp + 1][3] = A2[pp][2].y;
+    }
+  }
 #pragma unroll
   for (int p = 0; p < 4; ++p) {
     const int i = 2 * qx + (p & 1), j = 2 * qy + (p >> 1);

@@ -585,7 +585,6 @@ __global__ void __launch_bounds__(128, TV_GMINB) k_tv_gradient(Dims d, int rows,
           rm[s] = face_n0sq<V, ND>(win, A, cz - ez, 1 - ey, 1 - ex, s);
         }
       }
-#pragma unroll
       // border faces: the face towards -A of the first voxel has dm = 0 exactly (replicated neighbour), so only
       // the +A face of the last voxel needs its weight masked (it would otherwise enter the energy)
       const float maskp = pos[A] < lim[A] ? 1.0f : 0.0f;
@@ -642,7 +641,9 @@ __global__ void __launch_bounds__(128, TV_GMINB) k_tv_gradient(Dims d, int rows,
 // E(f - t_k g) with w frozen (O9) is assembled in fp64 by k_tv_trial_finish, which takes the first k with
 // E <= E0 - c t_k |g|^2. Slices that accepted a step in an earlier pass are skipped.
 // ---------------------------------------------------------------------------------------------
+#ifndef TV_KA
 #define TV_KA 8 /* candidates per pass; k <= 5 in every sweep seen, a later pass covers the rest (6 measured no faster) */
+#endif
 
 // the linear forms of A3 on the face between the centre cell and its +A neighbour,
 // evaluated on windows wf and wg: returns a = sum c_i Lf_i^2, b = sum c_i Lf_i Lg_i, c = sum c_i Lg_i^2

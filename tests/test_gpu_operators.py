@@ -258,7 +258,7 @@ def _both_ways(ctr, torch, cfg, x, y):
 @pytest.mark.parametrize("cfg", [get_config("c2"), odd2d(), odd2d(det_type=1, du=1.0)], ids=["c2", "odd", "arc"])
 def test_stored_matrices_equal_on_the_fly_kernels(ctr, torch_cuda, cfg):
     """The lookup-table operators hold the very values the on-the-fly kernels compute. P^T adds
-    them in the same order (identical bits); the stored P of a 2D slice splits every ray over 8 threads, so its
+    them in the same order (identical bits); the stored P of a 2D slice splits every ray over 16 threads, so its
     sums agree with the on-the-fly kernel to fp32 rounding."""
     rng = np.random.default_rng(406)
     x = rng.random((1, cfg.ny, cfg.nx), dtype=np.float32)
