@@ -286,6 +286,10 @@ int reduce_finish(ctr_handle* h, int mode, int N, int nblk, int i0, int nb, int 
 // In exact arithmetic this is the iteration of vec_direction() term for term; in fp32 it tracks the oracle as
 // closely (tests/test_oracle_pins.py emulates both).
 // ---------------------------------------------------------------------------------------------
+#ifndef CTR_LAZY_BLOCKS
+#define CTR_LAZY_BLOCKS 592 /* grid cap of the lazy-phase reduction kernels, 4 blocks per SM: their partials are finished by k_finish* (c4 vector work 1.85 / 1.82 / 2.11 ms for 1184 / 592 / 296) */
+#endif
+static_assert(CTR_LAZY_BLOCKS <= CTR_REDUCE_BLOCKS, "part2 is sized for CTR_REDUCE_BLOCKS blocks");
 // explicit phase, iteration m < CTR_MAX_BASIS: P b_m = (q - beta q_prev) / ||g'_m|| (first: q / ||g'_0||); q_prev <- q
 template <int V>
 __global__ void __launch_bounds__(256) k_sino_pb(size_t nl, int LQ, const float* __restrict__ q, float* __restrict__ qprev,
@@ -368,14 +372,34 @@ __global__ void __launch_bounds__(256) k_sino_axpy_dots(size_t nl, int LQ, size_
   block_partials_q<REORTH_NB * V, 8>(red, LQ, part + (size_t)gs * gridDim.x * LQ * REORTH_NB * V, blockIdx.x, threadIdx.x);
 }
 
+// lazy phase: ||g||^2 per slice (block partials, N = V). k_reorth_dots with nb = 0 would do, but its grid is sized for
+// five streams per thread (two blocks per SM): 25 us for the 64-MiB gradient against 12 us here.
+template <int V>
+__global__ void __launch_bounds__(256) k_img_norm(size_t nl, int LQ, const float* __restrict__ gi, double* part) {
+  const int gs = blockIdx.y;
+  float acc[V];
+#pragma unroll
+  for (int c = 0; c < V; ++c) acc[c] = 0.0f;
+#pragma unroll 4
+  for (size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x; idx < nl; idx += (size_t)gridDim.x * 256) {
+    float gv[V];
+    Pack<V>::ldcg(gi, (size_t)gs * nl + idx, gv);
+#pragma unroll
+    for (int c = 0; c < V; ++c) acc[c] = fmaf(gv[c], gv[c], acc[c]);
+  }
+  double red[V];
+#pragma unroll
+  for (int c = 0; c < V; ++c) red[c] = (double)acc[c];
+  block_partials_q<V, 8>(red, LQ, part + (size_t)gs * gridDim.x * LQ * V, blockIdx.x, threadIdx.x);
+}
+
 // lazy phase, scalar step after P^T: block (q, gs) sums ||g||^2 and the c_i (partials of k_sino_axpy_dots), then gamma' = ||g||^2 - sum c_i^2, beta = gamma'/gamma
 // (:432) and e_i <- c_i + beta e_i
 template <int V>
 __global__ void __launch_bounds__(1024) k_finish_lazy(const double* __restrict__ part, int nblk, int N1, int off1,
                                                      const double* __restrict__ part2, int nblk2, int LQ, int nb, int Bp,
                                                      Scal sc) {
-  // ||g||^2: value off1 + c of the N1 values per (block, segment) in `part` (k_reorth_dots with nb = 0: N1 =
-  // (REORTH_NB + 1) V, off1 = REORTH_NB V; k_si_back_quad<.., 3>: N1 = V, off1 = 0)
+  // ||g||^2: value off1 + c of the N1 values per (block, segment) in `part` (k_img_norm: N1 = V, off1 = 0)
   constexpr int N2 = REORTH_NB * V, NT = V + N2;  // values wanted: ||g||^2 [V], c [NB][V]
   constexpr int ROWS = 1024 / NT;
   __shared__ double sm[ROWS][NT];
@@ -520,7 +544,7 @@ static dim3 sino_reduce_grid(const ctr_handle* h) {
   const Dims& d = h->d;
   const size_t nl = (size_t)d.nray * d.LQ;
   const unsigned want = (unsigned)((nl + 255) / 256);
-  unsigned cap = (unsigned)(CTR_REDUCE_BLOCKS / d.GS);
+  unsigned cap = (unsigned)(CTR_LAZY_BLOCKS / d.GS);
   if (cap < 1) cap = 1;
   return dim3(want < cap ? want : cap, d.GS);
 }
@@ -554,20 +578,20 @@ static int vec_direction_lazy(ctr_handle* h, const float* g, int nblk2, cudaStre
   const size_t nl = (size_t)d.npix * d.LQ;
   const int Bp = d.G * d.V;
   const unsigned want = (unsigned)((nl + 255) / 256);
-  unsigned dcap = (unsigned)(h->dots_blocks / d.GS);
-  if (dcap < 1) dcap = 1;
-  dim3 grid(want, d.GS), dgrid(want < dcap ? want : dcap, d.GS), fgrid(d.LQ, d.GS);
+  unsigned ncap = (unsigned)(CTR_LAZY_BLOCKS / d.GS);
+  if (ncap < 1) ncap = 1;
+  dim3 grid(want, d.GS), ngrid(want < ncap ? want : ncap, d.GS), fgrid(d.LQ, d.GS);
   ProfScope prof(h, CTR_PROF_VECTOR, st);
   if (d.V == 1) {
-    k_reorth_dots<1><<<dgrid, 256, 0, st>>>(nl, d.LQ, h->nimg, g, h->basis, 0, 0, Bp, h->sc, h->part, h->counters + 4 * d.G);
+    k_img_norm<1><<<ngrid, 256, 0, st>>>(nl, d.LQ, g, h->part);
     CTR_LAUNCHED(h);
-    k_finish_lazy<1><<<fgrid, 1024, 0, st>>>(h->part, (int)dgrid.x, REORTH_NB + 1, REORTH_NB, h->part2, nblk2, d.LQ, CTR_MAX_BASIS, Bp, h->sc);
+    k_finish_lazy<1><<<fgrid, 1024, 0, st>>>(h->part, (int)ngrid.x, 1, 0, h->part2, nblk2, d.LQ, CTR_MAX_BASIS, Bp, h->sc);
     CTR_LAUNCHED(h);
     k_img_supdate<1><<<grid, 256, 0, st>>>(nl, d.LQ, h->s, g, nullptr, h->sc, 0);
   } else {
-    k_reorth_dots<4><<<dgrid, 256, 0, st>>>(nl, d.LQ, h->nimg, g, h->basis, 0, 0, Bp, h->sc, h->part, h->counters + 4 * d.G);
+    k_img_norm<4><<<ngrid, 256, 0, st>>>(nl, d.LQ, g, h->part);
     CTR_LAUNCHED(h);
-    k_finish_lazy<4><<<fgrid, 1024, 0, st>>>(h->part, (int)dgrid.x, (REORTH_NB + 1) * 4, REORTH_NB * 4, h->part2, nblk2, d.LQ, CTR_MAX_BASIS, Bp, h->sc);
+    k_finish_lazy<4><<<fgrid, 1024, 0, st>>>(h->part, (int)ngrid.x, 4, 0, h->part2, nblk2, d.LQ, CTR_MAX_BASIS, Bp, h->sc);
     CTR_LAUNCHED(h);
     k_img_supdate<4><<<grid, 256, 0, st>>>(nl, d.LQ, h->s, g, nullptr, h->sc, 0);
   }
