@@ -913,7 +913,7 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
   A((void**)&h->hist, sizeof(unsigned) * 2048 * Bp);
   A((void**)&h->stats, sizeof(ctr_sweep_stat) * (size_t)CTR_STAT_SWEEPS * Bp);
   A((void**)&h->d_sweep, 16);
-  const size_t scal_bytes = (size_t)Bp * (3 * sizeof(double) + (5 + 3 * CTR_MAX_BASIS) * sizeof(float) + 7 * sizeof(unsigned) + 16);
+  const size_t scal_bytes = (size_t)Bp * (3 * sizeof(double) + (5 + 3 * CTR_MAX_BASIS) * sizeof(float) + 9 * sizeof(unsigned) + 16);
   {
     // candidate lists of the fused sigma selection: a quarter of the faces of a slice / volume each
     unsigned long long S = (unsigned long long)(d.nx - 1) * d.ny * d.nz + (unsigned long long)d.nx * (d.ny - 1) * d.nz;
@@ -954,8 +954,11 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
     h->sc.pred = (int*)p; p += sizeof(int) * Bp;
     h->sc.cand_cnt = (unsigned*)p; p += sizeof(unsigned) * Bp;
     h->sc.ovf = (unsigned*)p; p += sizeof(unsigned) * Bp;
-    h->sc.hit = (int*)p;
+    h->sc.hit = (int*)p; p += sizeof(int) * Bp;
+    h->sc.lastbin = (int*)p; p += sizeof(int) * Bp;
+    h->sc.jump = (int*)p;
     cudaMemset(h->sc.pred, 0x80, sizeof(int) * Bp);  // a large negative bin: no prediction yet
+    cudaMemset(h->sc.lastbin, 0x80, sizeof(int) * Bp);
   }
   set_quantile(h, h->p.sigma_quantile);
   {
@@ -1144,7 +1147,7 @@ int ctr_reconstruct_w(ctr_handle* h, const float* d_sino, float* d_img, float* d
         // the caller wants the weights of the last sweep: materialise them for this one sweep
         if ((rc_ = tv_update_weights(h, f, h->w, s_))) return rc_;
         if ((rc_ = tv_sweep(h, f, h->v, h->w, P.lambda, clamp, 1, s_))) return rc_;
-      } else if ((rc_ = tv_sweep_fused(h, f, h->v, P.lambda, clamp, s_))) return rc_;
+      } else if ((rc_ = tv_sweep_fused(h, f, h->v, P.lambda, clamp, (sw == 0 ? 1 : 0) | (sw == P.n_gd - 1 ? 2 : 0), s_))) return rc_;
     }
     if (P.n_gd == 0 && P.positivity && (rc_ = tv_clamp(h, f, s_))) return rc_;                     // Step 3 (:173)
     (void)it;

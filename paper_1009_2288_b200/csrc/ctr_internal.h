@@ -60,6 +60,10 @@ struct Scal {
   unsigned* cand_cnt;   // entries appended to the slice's candidate list by the current first pass
   unsigned* ovf;        // a block's staging buffer overflowed: the list is incomplete
   int* hit;             // 1: the winning bin is covered by the list, passes 2 and 3 run on the list
+  int* lastbin;         // bin of sigma^2 in the last sweep of the previous outer iteration (< 0: none)
+  int* jump;            // by how many bins sigma^2 moved across the last Step 1 (CGLS): sigma^2 grows by 1.2-2 x there,
+                        // i.e. 2-9 bins, smoothly from one outer iteration to the next, so the first sweep after CGLS
+                        // predicts lastbin + jump instead of missing its candidate list every time
 };
 
 // stored system matrix, sliced ELL (ctr_ell.cuh)
@@ -226,7 +230,8 @@ int cone_back(ctr_handle* h, const float* sino, float* out, int mode, const floa
 int tv_update_weights(ctr_handle* h, const float* f, float* w, cudaStream_t st);
 int tv_sweep(ctr_handle* h, float* f, const float* v, const float* w, float lambda, int clamp, int n0_valid,
              cudaStream_t st);  // n0_valid: h->n0 holds the face magnitudes of THIS f (tv_update_weights just ran)
-int tv_sweep_fused(ctr_handle* h, float* f, const float* v, float lambda, int clamp, cudaStream_t st);  // weights + sweep, no planes
+// weights + sweep, no planes; pos: bit 0 = first sweep after Step 1, bit 1 = last sweep of the outer iteration
+int tv_sweep_fused(ctr_handle* h, float* f, const float* v, float lambda, int clamp, int pos, cudaStream_t st);
 int tv_clamp(ctr_handle* h, float* f, cudaStream_t st);
 // implemented in ctr_api.cu: finishing pass of a segmented reduction (block partials in h->part)
 enum { CTR_FIN_ALPHA = 0, CTR_FIN_COEF = 1 };

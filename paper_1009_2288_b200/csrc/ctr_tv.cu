@@ -254,7 +254,7 @@ __global__ void __launch_bounds__(128) k_tv_hist(Dims d, int rows, const float* 
 // fits; after the final pass the bin becomes the next sweep's prediction and the list is emptied.
 __global__ void __launch_bounds__(256) k_tv_select(Scal sc, unsigned* __restrict__ hist, int nbins, int shift,
                                                    int first, int final_pass, unsigned long long rank0, float eps2,
-                                                   StatRing ring, int lists, unsigned cand_cap) {
+                                                   StatRing ring, int lists, unsigned cand_cap, int pos = 0) {
   __shared__ unsigned tot[256];
   __shared__ unsigned found_bin, found_before;
   const int sl = blockIdx.x, t = threadIdx.x;
@@ -295,7 +295,12 @@ __global__ void __launch_bounds__(256) k_tv_select(Scal sc, unsigned* __restrict
       sc.sigma2[sl] = s2;
       ring.slot()[sl].sigma = sqrt((double)s2);
       if (lists) {
-        sc.pred[sl] = (int)(prefix >> 20);
+        // prediction for the next sweep: this bin; across Step 1 (pos bit 1: this is the last sweep of the outer
+        // iteration) this bin plus the jump the previous Step 1 caused (measured in the first sweep after it, pos bit 0)
+        const int bin = (int)(prefix >> 20);
+        if ((pos & 1) && sc.lastbin[sl] >= 0) sc.jump[sl] = max(-64, min(64, bin - sc.lastbin[sl]));
+        if (pos & 2) sc.lastbin[sl] = bin;
+        sc.pred[sl] = (pos & 2) ? bin + sc.jump[sl] : bin;
         sc.cand_cnt[sl] = 0u;
         sc.ovf[sl] = 0u;
       }
@@ -1076,7 +1081,7 @@ int tv_sweep(ctr_handle* h, float* f, const float* v, const float* w, float lamb
 // One GD sweep of ctr_reconstruct without any plane: sigma by the fused selection (k_tv_scan1 / k_tv_scan23 above),
 // then gradient, trials and update with the weights evaluated on the fly.
 template <int V, int ND>
-static int tv_sweep_fused_t(ctr_handle* h, float* f, const float* v, float lambda, int clamp, cudaStream_t st) {
+static int tv_sweep_fused_t(ctr_handle* h, float* f, const float* v, float lambda, int clamp, int pos, cudaStream_t st) {
   const Dims& d = h->d;
   ProfScope prof(h, CTR_PROF_TV, st);
   if (h->p.weights_mode == 0) {
@@ -1095,15 +1100,15 @@ static int tv_sweep_fused_t(ctr_handle* h, float* f, const float* v, float lambd
     CTR_LAUNCHED(h);
     k_tv_scan23<V, ND><<<grid, block, 0, st>>>(d, rows, f, h->hist, h->sc, h->cand, h->cand_cap, 0, 1023u, 10);
     CTR_LAUNCHED(h);
-    k_tv_select<<<Bp, 256, 0, st>>>(h->sc, h->hist, 1024, 0, 0, 1, 0, eps2, rec, 1, h->cand_cap);
+    k_tv_select<<<Bp, 256, 0, st>>>(h->sc, h->hist, 1024, 0, 0, 1, 0, eps2, rec, 1, h->cand_cap, pos);
     CTR_LAUNCHED(h);
   }
   return tv_descend_t<V, ND, 1>(h, f, v, nullptr, lambda, clamp, st);
 }
 
-int tv_sweep_fused(ctr_handle* h, float* f, const float* v, float lambda, int clamp, cudaStream_t st) {
-  if (h->d.ndim == 3) return tv_sweep_fused_t<1, 3>(h, f, v, lambda, clamp, st);
-  return h->d.V == 1 ? tv_sweep_fused_t<1, 2>(h, f, v, lambda, clamp, st) : tv_sweep_fused_t<4, 2>(h, f, v, lambda, clamp, st);
+int tv_sweep_fused(ctr_handle* h, float* f, const float* v, float lambda, int clamp, int pos, cudaStream_t st) {
+  if (h->d.ndim == 3) return tv_sweep_fused_t<1, 3>(h, f, v, lambda, clamp, pos, st);
+  return h->d.V == 1 ? tv_sweep_fused_t<1, 2>(h, f, v, lambda, clamp, pos, st) : tv_sweep_fused_t<4, 2>(h, f, v, lambda, clamp, pos, st);
 }
 
 int tv_clamp(ctr_handle* h, float* f, cudaStream_t st) {
