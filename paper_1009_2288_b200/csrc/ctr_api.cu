@@ -913,7 +913,7 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
   A((void**)&h->hist, sizeof(unsigned) * 2048 * Bp);
   A((void**)&h->stats, sizeof(ctr_sweep_stat) * (size_t)CTR_STAT_SWEEPS * Bp);
   A((void**)&h->d_sweep, 16);
-  const size_t scal_bytes = (size_t)Bp * (3 * sizeof(double) + (5 + 3 * CTR_MAX_BASIS) * sizeof(float) + 9 * sizeof(unsigned) + 16);
+  const size_t scal_bytes = (size_t)Bp * (3 * sizeof(double) + (5 + 3 * CTR_MAX_BASIS) * sizeof(float) + 10 * sizeof(unsigned) + 16);
   {
     // candidate lists of the fused sigma selection: a quarter of the faces of a slice / volume each
     unsigned long long S = (unsigned long long)(d.nx - 1) * d.ny * d.nz + (unsigned long long)d.nx * (d.ny - 1) * d.nz;
@@ -956,7 +956,8 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
     h->sc.ovf = (unsigned*)p; p += sizeof(unsigned) * Bp;
     h->sc.hit = (int*)p; p += sizeof(int) * Bp;
     h->sc.lastbin = (int*)p; p += sizeof(int) * Bp;
-    h->sc.jump = (int*)p;
+    h->sc.jump = (int*)p; p += sizeof(int) * Bp;
+    h->sc.fhit = (int*)p;
     cudaMemset(h->sc.pred, 0x80, sizeof(int) * Bp);  // a large negative bin: no prediction yet
     cudaMemset(h->sc.lastbin, 0x80, sizeof(int) * Bp);
   }

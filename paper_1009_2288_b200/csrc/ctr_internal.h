@@ -60,6 +60,7 @@ struct Scal {
   unsigned* cand_cnt;   // entries appended to the slice's candidate list by the current first pass
   unsigned* ovf;        // a block's staging buffer overflowed: the list is incomplete
   int* hit;             // 1: the winning bin is covered by the list, passes 2 and 3 run on the list
+  int* fhit;            // 1: the fast first pass (k_tv_scan1f) found the winning bin inside its three-bin window
   int* lastbin;         // bin of sigma^2 in the last sweep of the previous outer iteration (< 0: none)
   int* jump;            // by how many bins sigma^2 moved across the last Step 1 (CGLS): sigma^2 grows by 1.2-2 x there,
                         // i.e. 2-9 bins, smoothly from one outer iteration to the next, so the first sweep after CGLS

@@ -6,6 +6,8 @@
 //   Armijo       : PAPER.md:149;  clamp: PAPER.md:157, :173
 // Readings: S5/S7/S8 faces, S9/S10 sigma = exact q-quantile, S11 eps, S12 replicate border
 // with zero border flux, S14 Armijo constants, S22 3D generalisation.
+#include <limits.h>
+
 #include "ctr_common.cuh"
 #include "ctr_internal.h"
 
@@ -254,10 +256,16 @@ __global__ void __launch_bounds__(128) k_tv_hist(Dims d, int rows, const float* 
 // fits; after the final pass the bin becomes the next sweep's prediction and the list is emptied.
 __global__ void __launch_bounds__(256) k_tv_select(Scal sc, unsigned* __restrict__ hist, int nbins, int shift,
                                                    int first, int final_pass, unsigned long long rank0, float eps2,
-                                                   StatRing ring, int lists, unsigned cand_cap, int pos = 0) {
+                                                   StatRing ring, int lists, unsigned cand_cap, int pos = 0, int gv = 0) {
   __shared__ unsigned tot[256];
   __shared__ unsigned found_bin, found_before;
   const int sl = blockIdx.x, t = threadIdx.x;
+  if (gv > 0) {
+    // first pass after k_tv_scan1f: the full histogram exists only for groups (gv slices) in which a slice missed
+    bool allhit = true;
+    for (int s = 0; s < gv; ++s) allhit = allhit && sc.fhit[(sl / gv) * gv + s] != 0;
+    if (allhit) return;
+  }
   unsigned* h = hist + (size_t)sl * 2048;
   const int per = nbins / 256;  // 8 or 4
   unsigned loc[8], sum = 0;
@@ -322,6 +330,9 @@ __global__ void __launch_bounds__(256) k_tv_select(Scal sc, unsigned* __restrict
 #ifndef TV_SMINB
 #define TV_SMINB 3
 #endif
+#ifndef TV_FAST_SCAN
+#define TV_FAST_SCAN 1
+#endif
 
 template <int V, int ND>
 __device__ __forceinline__ void own_face_values(const Dims& d, const Window<V, ND>& w, const int (&pos)[3],
@@ -347,7 +358,7 @@ __device__ __forceinline__ void own_face_values(const Dims& d, const Window<V, N
 template <int V, int ND>
 __global__ void __launch_bounds__(256, TV_SMINB) k_tv_scan1(Dims d, int rows, const float* __restrict__ f,
                                                             unsigned* __restrict__ hist, Scal sc,
-                                                            unsigned* __restrict__ cand, unsigned cap) {
+                                                            unsigned* __restrict__ cand, unsigned cap, int after_fast) {
   __shared__ unsigned hs[V][2048];
   __shared__ unsigned stage[V][TV_SCAP(V)];
   __shared__ unsigned stage_n[V], stage_base[V];
@@ -355,8 +366,19 @@ __global__ void __launch_bounds__(256, TV_SMINB) k_tv_scan1(Dims d, int rows, co
   for (int t = tid0; t < V * 2048; t += 256) (&hs[0][0])[t] = 0;
   if (tid0 < V) stage_n[tid0] = 0;
   int pred[V];
+  bool need = !after_fast;
 #pragma unroll
-  for (int s = 0; s < V; ++s) pred[s] = sc.pred[blockIdx.z * V + s];
+  for (int s = 0; s < V; ++s) {
+    pred[s] = sc.pred[blockIdx.z * V + s];
+    if (after_fast) {
+      // after k_tv_scan1f: only groups with a slice that missed need the full histogram, and the slices that hit
+      // keep the candidate lists they have (a prediction that can never match stops a second append)
+      const bool fh = sc.fhit[blockIdx.z * V + s] != 0;
+      need = need || !fh;
+      if (fh) pred[s] = INT_MIN / 2;
+    }
+  }
+  if (!need) return;
   __syncthreads();
   const int lim[3] = {d.nx - 1, d.ny - 1, d.nz - 1};
   unsigned nzero[V];  // exact zeros (flat regions) are counted in a register instead of hammering bin 0
@@ -410,6 +432,108 @@ __global__ void __launch_bounds__(256, TV_SMINB) k_tv_scan1(Dims d, int rows, co
     unsigned* dst = cand + (size_t)(blockIdx.z * V + s) * cap;
     for (unsigned t = tid0; t < n; t += 256)
       if (base + t < cap) dst[base + t] = stage[s][t];
+  }
+}
+
+// Fast first pass (large problems, steady state): the winning bin is almost always within one bin of the prediction,
+// and then all the first pass has to deliver is the number of values BELOW the three-bin window, the counts of the
+// three bins and the candidate list - no 2048-bin histogram, i.e. no shared-memory atomic per value (ncu: half of
+// k_tv_scan1's instructions are the integer and branch work around them). hist[sl][0] = below, [1..3] = the window bins.
+// k_tv_select_f takes the decision; a slice whose rank falls outside the window (or whose list overflowed) is a MISS,
+// and its group then runs the full k_tv_scan1 / k_tv_select pass: sigma is the exact order statistic either way.
+template <int V, int ND>
+__global__ void __launch_bounds__(256, TV_SMINB) k_tv_scan1f(Dims d, int rows, const float* __restrict__ f,
+                                                             unsigned* __restrict__ hist, Scal sc,
+                                                             unsigned* __restrict__ cand, unsigned cap) {
+  __shared__ unsigned cnt_s[V][4];
+  __shared__ unsigned stage[V][TV_SCAP(V)];
+  __shared__ unsigned stage_n[V], stage_base[V];
+  const int tid0 = threadIdx.y * 32 + threadIdx.x;
+  if (tid0 < V * 4) (&cnt_s[0][0])[tid0] = 0;
+  if (tid0 < V) stage_n[tid0] = 0;
+  int lo[V];
+#pragma unroll
+  for (int s = 0; s < V; ++s) lo[s] = sc.pred[blockIdx.z * V + s] - 1;  // no prediction: hugely negative, nothing matches
+  __syncthreads();
+  const int lim[3] = {d.nx - 1, d.ny - 1, d.nz - 1};
+  unsigned nbelow[V];
+#pragma unroll
+  for (int s = 0; s < V; ++s) nbelow[s] = 0u;
+  for (int rr = 0; rr < rows; ++rr) {
+    const Vox p = vox_of_thread(d, rr, rows, 8);
+    const int pos[3] = {p.i, p.j, p.k};
+    if (!p.active) continue;
+    float val[ND][V];
+    Window<V, ND> w;
+    load_window<V, ND>(d, f, p.g, p.i, p.j, p.k, w);
+    own_face_values<V, ND>(d, w, pos, lim, val);
+#pragma unroll
+    for (int A = 0; A < ND; ++A) {
+      if (pos[A] >= lim[A]) continue;  // border face
+#pragma unroll
+      for (int s = 0; s < V; ++s) {
+        const unsigned bits = __float_as_uint(val[A][s]);
+        const int bin = (int)(bits >> 20);
+        nbelow[s] += bin < lo[s] ? 1u : 0u;
+        const unsigned rel = (unsigned)(bin - lo[s]);
+        if (rel < 3u) {
+          atomicAdd(&cnt_s[s][1 + rel], 1u);
+          const unsigned at = atomicAdd(&stage_n[s], 1u);
+          if (at < TV_SCAP(V)) stage[s][at] = bits;
+        }
+      }
+    }
+  }
+#pragma unroll
+  for (int s = 0; s < V; ++s) {
+    const unsigned z = __reduce_add_sync(0xffffffffu, nbelow[s]);
+    if ((threadIdx.x & 31) == 0 && z) atomicAdd(&cnt_s[s][0], z);
+  }
+  __syncthreads();
+  if (tid0 < V * 4) {
+    const unsigned c = (&cnt_s[0][0])[tid0];
+    if (c) atomicAdd(&hist[(size_t)(blockIdx.z * V + tid0 / 4) * 2048 + (tid0 & 3)], c);
+  }
+  if (tid0 < V) {
+    const int sl = blockIdx.z * V + tid0;
+    unsigned n = stage_n[tid0];
+    if (n > TV_SCAP(V)) { atomicOr(&sc.ovf[sl], 1u); n = TV_SCAP(V); }
+    stage_n[tid0] = n;
+    stage_base[tid0] = n ? atomicAdd(&sc.cand_cnt[sl], n) : 0u;
+  }
+  __syncthreads();
+#pragma unroll
+  for (int s = 0; s < V; ++s) {
+    const unsigned n = stage_n[s], base = stage_base[s];
+    unsigned* dst = cand + (size_t)(blockIdx.z * V + s) * cap;
+    for (unsigned t = tid0; t < n; t += 256)
+      if (base + t < cap) dst[base + t] = stage[s][t];
+  }
+}
+
+// decision of the fast first pass, one thread per slice
+__global__ void __launch_bounds__(128) k_tv_select_f(Scal sc, unsigned* __restrict__ hist, int Bp, unsigned long long rank0,
+                                                     unsigned cand_cap) {
+  const int sl = blockIdx.x * 128 + threadIdx.x;
+  if (sl >= Bp) return;
+  unsigned* h = hist + (size_t)sl * 2048;
+  const unsigned below = h[0], c[3] = {h[1], h[2], h[3]};
+  h[0] = 0u; h[1] = 0u; h[2] = 0u; h[3] = 0u;
+  const unsigned rank = (unsigned)rank0;
+  const int lo = sc.pred[sl] - 1;
+  const bool ok = sc.ovf[sl] == 0u && sc.cand_cnt[sl] <= cand_cap && rank > below && rank <= below + c[0] + c[1] + c[2];
+  if (ok) {
+    unsigned cum = below;
+    int j = 0;
+    while (rank > cum + c[j]) { cum += c[j]; ++j; }
+    sc.sel_prefix[sl] = (unsigned)(lo + j) << 20;
+    sc.sel_rank[sl] = rank - cum;
+    sc.hit[sl] = 1;
+    sc.fhit[sl] = 1;
+  } else {
+    sc.fhit[sl] = 0;
+    sc.cand_cnt[sl] = 0u;  // the full pass fills the list again
+    sc.ovf[sl] = 0u;
   }
 }
 
@@ -1090,9 +1214,17 @@ static int tv_sweep_fused_t(ctr_handle* h, float* f, const float* v, float lambd
     const int Bp = d.G * d.V;
     const float eps2 = h->p.eps * h->p.eps;
     const StatRing rec = stat_slot(h);
-    k_tv_scan1<V, ND><<<grid, block, 0, st>>>(d, rows, f, h->hist, h->sc, h->cand, h->cand_cap);
+    // large problems: the fast first pass, and the full one only for the groups in which a slice missed
+    const bool fast = TV_FAST_SCAN && h->nimg * sizeof(float) >= ((size_t)32 << 20);
+    if (fast) {
+      k_tv_scan1f<V, ND><<<grid, block, 0, st>>>(d, rows, f, h->hist, h->sc, h->cand, h->cand_cap);
+      CTR_LAUNCHED(h);
+      k_tv_select_f<<<(Bp + 127) / 128, 128, 0, st>>>(h->sc, h->hist, Bp, h->sel_k, h->cand_cap);
+      CTR_LAUNCHED(h);
+    }
+    k_tv_scan1<V, ND><<<grid, block, 0, st>>>(d, rows, f, h->hist, h->sc, h->cand, h->cand_cap, fast ? 1 : 0);
     CTR_LAUNCHED(h);
-    k_tv_select<<<Bp, 256, 0, st>>>(h->sc, h->hist, 2048, 20, 1, 0, h->sel_k, eps2, rec, 1, h->cand_cap);
+    k_tv_select<<<Bp, 256, 0, st>>>(h->sc, h->hist, 2048, 20, 1, 0, h->sel_k, eps2, rec, 1, h->cand_cap, 0, fast ? V : 0);
     CTR_LAUNCHED(h);
     k_tv_scan23<V, ND><<<grid, block, 0, st>>>(d, rows, f, h->hist, h->sc, h->cand, h->cand_cap, 10, 1023u, 20);
     CTR_LAUNCHED(h);
