@@ -15,8 +15,7 @@ namespace ctr {
 // ABI <-> internal layout. ABI: [B][n] floats. Internal (V = 4): [G][n] float4, lane c = slice 4g+c,
 // missing slices are zero. V = 1 uses the ABI arrays in place (no copies).
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_pack4(const float* __restrict__ src, float* __restrict__ dst, size_t n, int B,
-                                               int planes) {
+__global__ void __launch_bounds__(256) k_pack4(const float* __restrict__ src, float* __restrict__ dst, size_t n, int B) {
   const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
   const int g = blockIdx.y, pl = blockIdx.z, G = gridDim.y;
   if (idx >= n) return;
@@ -27,11 +26,9 @@ __global__ void __launch_bounds__(256) k_pack4(const float* __restrict__ src, fl
     o[c] = sl < B ? __ldg(src + ((size_t)pl * B + sl) * n + idx) : 0.0f;
   }
   reinterpret_cast<float4*>(dst)[((size_t)pl * G + g) * n + idx] = make_float4(o[0], o[1], o[2], o[3]);
-  (void)planes;
 }
 
-__global__ void __launch_bounds__(256) k_unpack4(const float* __restrict__ src, float* __restrict__ dst, size_t n, int B,
-                                                 int planes) {
+__global__ void __launch_bounds__(256) k_unpack4(const float* __restrict__ src, float* __restrict__ dst, size_t n, int B) {
   const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;
   const int g = blockIdx.y, pl = blockIdx.z, G = gridDim.y;
   if (idx >= n) return;
@@ -42,20 +39,19 @@ __global__ void __launch_bounds__(256) k_unpack4(const float* __restrict__ src, 
     const int sl = 4 * g + c;
     if (sl < B) dst[((size_t)pl * B + sl) * n + idx] = o[c];
   }
-  (void)planes;
 }
 
 static int pack(ctr_handle* h, const float* src, float* dst, size_t n, int planes, cudaStream_t st) {
   dim3 grid((unsigned)((n + 255) / 256), h->d.G, planes);
   ProfScope prof(h, CTR_PROF_LAYOUT, st);
-  k_pack4<<<grid, 256, 0, st>>>(src, dst, n, h->d.B, planes);
+  k_pack4<<<grid, 256, 0, st>>>(src, dst, n, h->d.B);
   CTR_LAUNCHED(h);
   return CTR_OK;
 }
 static int unpack(ctr_handle* h, const float* src, float* dst, size_t n, int planes, cudaStream_t st) {
   dim3 grid((unsigned)((n + 255) / 256), h->d.G, planes);
   ProfScope prof(h, CTR_PROF_LAYOUT, st);
-  k_unpack4<<<grid, 256, 0, st>>>(src, dst, n, h->d.B, planes);
+  k_unpack4<<<grid, 256, 0, st>>>(src, dst, n, h->d.B);
   CTR_LAUNCHED(h);
   return CTR_OK;
 }
@@ -1095,12 +1091,12 @@ int ctr_eptv_step(ctr_handle* h, float* d_x, const float* d_v, const float* d_w,
   if (!(lambda >= 0.0f)) return set_err(h, CTR_EINVAL, "ctr_eptv_step: lambda < 0");
   cudaStream_t st = (cudaStream_t)stream;
   h->last_stream = st;
-  if (h->d.V == 1) return tv_sweep(h, d_x, d_v, d_w, lambda, 0, 0, st);
+  if (h->d.V == 1) return tv_sweep(h, d_x, d_v, d_w, lambda, 0, st);
   int rc;
   if ((rc = pack(h, d_x, h->ximg, h->d.npix, 1, st))) return rc;
   if ((rc = pack(h, d_v, h->v, h->d.npix, 1, st))) return rc;
   if ((rc = pack(h, d_w, h->w, h->d.npix, h->d.ndim, st))) return rc;
-  if ((rc = tv_sweep(h, h->ximg, h->v, h->w, lambda, 0, 0, st))) return rc;
+  if ((rc = tv_sweep(h, h->ximg, h->v, h->w, lambda, 0, st))) return rc;
   return unpack(h, h->ximg, d_x, h->d.npix, 1, st);
 }
 
@@ -1147,7 +1143,7 @@ int ctr_reconstruct_w(ctr_handle* h, const float* d_sino, float* d_img, float* d
       if (want_w && sw == P.n_gd - 1) {
         // the caller wants the weights of the last sweep: materialise them for this one sweep
         if ((rc_ = tv_update_weights(h, f, h->w, s_))) return rc_;
-        if ((rc_ = tv_sweep(h, f, h->v, h->w, P.lambda, clamp, 1, s_))) return rc_;
+        if ((rc_ = tv_sweep(h, f, h->v, h->w, P.lambda, clamp, s_))) return rc_;
       } else if ((rc_ = tv_sweep_fused(h, f, h->v, P.lambda, clamp, (sw == 0 ? 1 : 0) | (sw == P.n_gd - 1 ? 2 : 0), s_))) return rc_;
     }
     if (P.n_gd == 0 && P.positivity && (rc_ = tv_clamp(h, f, s_))) return rc_;                     // Step 3 (:173)

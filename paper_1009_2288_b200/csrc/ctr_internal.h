@@ -229,8 +229,7 @@ int cone_forward(ctr_handle* h, const float* img, float* out, int mode, const fl
 int cone_back(ctr_handle* h, const float* sino, float* out, int mode, const float* s, float* u, cudaStream_t st);
 // implemented in ctr_tv.cu
 int tv_update_weights(ctr_handle* h, const float* f, float* w, cudaStream_t st);
-int tv_sweep(ctr_handle* h, float* f, const float* v, const float* w, float lambda, int clamp, int n0_valid,
-             cudaStream_t st);  // n0_valid: h->n0 holds the face magnitudes of THIS f (tv_update_weights just ran)
+int tv_sweep(ctr_handle* h, float* f, const float* v, const float* w, float lambda, int clamp, cudaStream_t st);  // weights from the planes w
 // weights + sweep, no planes; pos: bit 0 = first sweep after Step 1, bit 1 = last sweep of the outer iteration
 int tv_sweep_fused(ctr_handle* h, float* f, const float* v, float lambda, int clamp, int pos, cudaStream_t st);
 int tv_clamp(ctr_handle* h, float* f, cudaStream_t st);

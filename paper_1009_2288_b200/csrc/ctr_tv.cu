@@ -1194,9 +1194,7 @@ static int tv_descend_t(ctr_handle* h, float* f, const float* v, const float* w,
   return CTR_OK;
 }
 
-int tv_sweep(ctr_handle* h, float* f, const float* v, const float* w, float lambda, int clamp, int n0_valid,
-             cudaStream_t st) {
-  (void)n0_valid;
+int tv_sweep(ctr_handle* h, float* f, const float* v, const float* w, float lambda, int clamp, cudaStream_t st) {
   ProfScope prof(h, CTR_PROF_TV, st);
   if (h->d.ndim == 3) return tv_descend_t<1, 3, 0>(h, f, v, w, lambda, clamp, st);
   return h->d.V == 1 ? tv_descend_t<1, 2, 0>(h, f, v, w, lambda, clamp, st) : tv_descend_t<4, 2, 0>(h, f, v, w, lambda, clamp, st);
