@@ -136,6 +136,12 @@ __device__ __forceinline__ Vox vox_of_thread(const Dims& d, int rr, int rows, in
 static dim3 vox_grid(const Dims& d, int rows, int br = 4) {
   return dim3((d.nx + 31) / 32, ((d.ny + br * rows - 1) / (br * rows)) * d.nz, d.G);
 }
+// A volume is ONE group: its blocks' partial sums are finished by a single block and every block pays the fixed
+// costs above, so a 3D block sweeps up to TV_ROWS3D row groups instead of 8 / 16 (c5: 16 384-32 768 blocks otherwise)
+#ifndef TV_ROWS3D
+#define TV_ROWS3D 32 /* c5 TV per outer iteration: 11.0 / 10.0 / 9.7 / 9.9 / 11.2 ms for 8 / 16 / 32 / 48 / 64 */
+#endif
+#define TV_MAXROWS(d, n2d) ((d).ndim == 3 ? TV_ROWS3D : (n2d))
 // row groups per block: as many as leave at least ~16 blocks per SM (8 for the 256-thread trial kernel)
 static int tv_rows(const Dims& d, int rows_per_group, int max_rows, int min_blocks) {
   const long long blocks = (long long)((d.nx + 31) / 32) * ((d.ny + rows_per_group - 1) / rows_per_group) * d.nz * d.G;
@@ -1121,7 +1127,7 @@ static StatRing stat_slot(ctr_handle* h) {
 template <int V, int ND>
 static int tv_update_weights_t(ctr_handle* h, const float* f, float* w, cudaStream_t st) {
   const Dims& d = h->d;
-  const int rows = tv_rows(d, 4, 8, 148 * 16);
+  const int rows = tv_rows(d, 4, TV_MAXROWS(d, 8), 148 * 16);
   const dim3 grid = vox_grid(d, rows), block(32, 4);
   const int Bp = d.G * d.V;
   const float eps2 = h->p.eps * h->p.eps;
@@ -1174,13 +1180,13 @@ static TvParams make_tv_params(const ctr_handle* h, float lambda) {
 template <int V, int ND, int WSRC>
 static int tv_descend_t(ctr_handle* h, float* f, const float* v, const float* w, float lambda, int clamp, cudaStream_t st) {
   const Dims& d = h->d;
-  const int rows = tv_rows(d, 4, 8, 148 * 16);
+  const int rows = tv_rows(d, 4, TV_MAXROWS(d, 8), 148 * 16);
   const dim3 grid = vox_grid(d, rows), block(32, 4);
   const TvParams tp = make_tv_params(h, lambda);
   float* g = h->gimg;
   k_tv_gradient<V, ND, WSRC><<<grid, block, 0, st>>>(d, rows, f, v, w, g, tp, h->sc, h->part, h->counters + 2 * d.G, stat_slot(h));
   CTR_LAUNCHED(h);
-  const int trows = tv_rows(d, TV_TW, 16, 148 * 8);
+  const int trows = tv_rows(d, TV_TW, TV_MAXROWS(d, 16), 148 * 8);
   const dim3 tgrid((d.nx + 31) / 32, ((d.ny + TV_TW * trows - 1) / (TV_TW * trows)) * d.nz, d.G), tblock(32, TV_TW);
   for (int k0 = 0; k0 < tp.kmax; k0 += TV_KA) {
     k_tv_trial<V, ND, WSRC><<<tgrid, tblock, 0, st>>>(d, trows, f, g, v, w, tp, k0, h->sc, h->part);
@@ -1207,7 +1213,7 @@ static int tv_sweep_fused_t(ctr_handle* h, float* f, const float* v, float lambd
   const Dims& d = h->d;
   ProfScope prof(h, CTR_PROF_TV, st);
   if (h->p.weights_mode == 0) {
-    const int rows = tv_rows(d, 8, 8, 148 * 8);
+    const int rows = tv_rows(d, 8, TV_MAXROWS(d, 8), 148 * 8);
     const dim3 grid = vox_grid(d, rows, 8), block(32, 8);
     const int Bp = d.G * d.V;
     const float eps2 = h->p.eps * h->p.eps;
