@@ -246,6 +246,19 @@ def test_reconstruct_batched_short_schedule(ctr, torch_cuda, orc):
     assert_close(img[2], solo[0].astype(np.float64), 1e-4)
 
 
+def test_reconstruct_large_batch_paths_on_a_ragged_batch(ctr, torch_cuda, orc):
+    """The paths that switch on above 32 MiB per vector (the lazy CGLS phase, the fast first radix pass of sigma, the
+    sigma prediction across Step 1) are otherwise only reached at c4 / c5: here 130 slices of the c2 geometry
+    (3 super-groups of 64, the last one ragged: 48 MiB per vector), 3 outer x (7 CGLS + 3 GD), three slices against the
+    oracle, Armijo indices identical."""
+    cfg = scaled_config("c2", batch=130, n_outer=3, n_cgls=7, n_gd=3)
+    case = make_case(cfg, raster=False)
+    img, stats, _, _ = run_reconstruct(ctr, torch_cuda, cfg, case["sino"])
+    assert len(stats) == cfg.n_outer * cfg.n_gd * 130
+    for sl in (0, 77, 129):
+        compare_with_oracle(orc, cfg, case["sino"][sl], img[sl], stats[sl::130])
+
+
 def test_reconstruct_variants(ctr, torch_cuda, orc):
     """n_gd = 0 (restarted CGLS + clamp), plain TV weights, no positivity."""
     for over in (dict(n_gd=0, n_outer=3), dict(weights_mode=1, n_outer=2), dict(positivity=0, n_outer=2)):
