@@ -78,7 +78,7 @@ enum {
                             p_ij is computed on the fly. Same bits either way; a low-memory mode and the tests' way
                             of checking that the tables hold exactly what the on-the-fly kernels compute. */
   CTR_GEOM_NO_GRAPHS = 2, /* ctr_reconstruct launches every kernel itself instead of replaying a CUDA graph of the
-                            steady-state outer iteration (batch = 1 only; same kernels, same results). */
+                            steady-state outer iteration (same kernels, same results). */
   CTR_GEOM_NO_STORED_P = 4, /* batched slices: apply P on the fly (k_si_forward) instead of from the stored matrix
                             shared by all slices (k_si_forward_tab); the other tables are still built. */
   CTR_GEOM_NO_LAZY_CGLS = 8 /* CGLS projects every gradient against the stored unit gradients in image space in all

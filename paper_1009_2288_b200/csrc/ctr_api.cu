@@ -966,7 +966,7 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
     h->dots_blocks = per_sm * prop.multiProcessorCount;
     if (h->dots_blocks > CTR_REDUCE_BLOCKS) h->dots_blocks = CTR_REDUCE_BLOCKS;
   }
-  if (d.V == 1 && cudaStreamCreateWithFlags(&h->gstream, cudaStreamNonBlocking) != cudaSuccess) {
+  if (cudaStreamCreateWithFlags(&h->gstream, cudaStreamNonBlocking) != cudaSuccess) {
     cudaGetLastError();
     h->gstream = nullptr;  // no capture stream: ctr_reconstruct launches kernel by kernel
   }
@@ -989,7 +989,7 @@ int ctr_create(const ctr_geometry* g, ctr_handle** out) {
       table_mb = (double)(h->ell_p.tab ? h->ell_p.bytes : 0) / 1e6 + (double)(h->ell_pt.tab ? h->ell_pt.bytes : 0) / 1e6;
     }
     snprintf(h->path_info, sizeof(h->path_info), "forward=%s;back=%s;tables_mb=%.1f;graphs=%d", fw, bk, table_mb,
-             (d.V == 1 && h->gstream && !(g->flags & CTR_GEOM_NO_GRAPHS)) ? 1 : 0);
+             (h->gstream && !(g->flags & CTR_GEOM_NO_GRAPHS)) ? 1 : 0);
   }
   *out = h;
   return CTR_OK;
@@ -1150,18 +1150,20 @@ int ctr_reconstruct_w(ctr_handle* h, const float* d_sino, float* d_img, float* d
     (void)it;
     return CTR_OK;
   };
-  // Single problems (c1-c3, c5) are bound by launch latency, not by the kernels (~190 launches per outer
-  // iteration of 2.3 ms at c3): the steady-state outer iteration - every steering scalar lives on the device, so
-  // its launch sequence is static - is captured once into a CUDA graph and replayed. The graph is keyed on the
-  // buffers and parameters baked into it; the event profiler (ctr_profile_enable) turns it off.
-  const bool graphs = direct && !h->prof_on && !(h->g.flags & CTR_GEOM_NO_GRAPHS) && h->gstream;
+  // The steady-state outer iteration - every steering scalar lives on the device, so its launch sequence is static -
+  // is captured once into a CUDA graph and replayed: single problems are bound by launch latency (~150 kernels per
+  // outer iteration of 1.9 ms at c3: 2.32 -> 1.92 ms), and 64 slices still gain 3 % (13.73 -> 13.33 ms: ~250 launches,
+  // most of them short). The graph is keyed on the buffers and parameters baked into it; the event profiler
+  // (ctr_profile_enable) turns it off.
+  const bool graphs = !h->prof_on && !(h->g.flags & CTR_GEOM_NO_GRAPHS) && h->gstream;
   for (int it = 0; it < P.n_outer; ++it) {
     const bool x0_zero = it == 0 && !P.warm_start;
     const bool want_w = d_w && it == P.n_outer - 1;
     if (graphs && !x0_zero && !want_w) {
       GraphKey key;
       memset(&key, 0, sizeof(key));
-      key.sino = d_sino; key.img = d_img; key.p = P; key.p.n_outer = 0; key.p.warm_start = 0; key.sel_k = h->sel_k;
+      // (batched slices: the captured work reads and writes the handle's own buffers only)
+      key.sino = direct ? d_sino : h->bsino; key.img = direct ? d_img : h->ximg; key.p = P; key.p.n_outer = 0; key.p.warm_start = 0; key.sel_k = h->sel_k;
       if (!h->graph_exec || memcmp(&key, &h->graph_key, sizeof(key)) != 0) {
         if (h->graph_exec) { cudaGraphExecDestroy(h->graph_exec); h->graph_exec = nullptr; }
         const long long l0 = h->launches, s0 = h->sweep_count;
