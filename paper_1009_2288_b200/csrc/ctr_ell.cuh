@@ -15,6 +15,7 @@
 
 #include "ctr_common.cuh"
 #include "ctr_internal.h"
+#include "ctr_fan_geom.cuh"
 
 namespace ctr {
 
@@ -150,6 +151,21 @@ static int ell_build(ctr_handle* h, Hits hits, size_t nrows, EllTable& t) {
   CTR_CUDA(h, cudaDeviceSynchronize());
   t.bytes = need;
   return CTR_OK;
+}
+
+#ifndef ELL_BLOCKED
+#define ELL_BLOCKED 1
+#endif
+// vol[z][y][x] -> blocked copy (blk_index, ctr_fan_geom.cuh); one thread per element of the blocked array
+static __global__ void __launch_bounds__(256) k_to_blocked(int nx, int ny, int nz, const float* __restrict__ vol, float* __restrict__ out) {
+  const size_t o = (size_t)blockIdx.x * 256 + threadIdx.x;
+  if (o >= (size_t)nx * ny * nz) return;
+  const int xi = (int)(o & 7), yi = (int)((o >> 3) & 3);
+  size_t t = o >> 5;
+  const int tx = (int)(t % (nx >> 3));
+  t /= (nx >> 3);
+  const int ty = (int)(t % (ny >> 2)), z = (int)(t / (ny >> 2));
+  out[o] = __ldg(vol + ((size_t)z * ny + (ty << 2) + yi) * nx + (tx << 3) + xi);
 }
 
 template <int SPLIT>

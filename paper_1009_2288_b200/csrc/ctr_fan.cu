@@ -459,7 +459,9 @@ int fan_build_window(ctr_handle* h) {
   if (d.V == 1) {
     // single slice: stored P and P^T (best effort). A ray's row has ~n entries and a slice has few rays:
     // each ray is dealt to FAN_SPLIT table rows (one thread each; c3: 198 us unsplit, 76 us on the fly, 57 us with 16 rows).
-    int rc = ell_build(h, SplitHits<FAN_SPLIT, FanRayHits>{FanRayHits{h->rays}}, (size_t)d.nray * FAN_SPLIT, h->ell_p);
+    // (the copy is one more launch per application: it pays from 512^2 on - c3 1.90 -> 1.885 ms, c2 0.546 -> 0.555 ms)
+    h->ell_p_blk = (ELL_BLOCKED && blk_ok(d.nx, d.ny) && d.npix >= 512 * 512) ? 1 : 0;
+    int rc = ell_build(h, SplitHits<FAN_SPLIT, FanRayHits>{FanRayHits{h->rays, h->ell_p_blk}}, (size_t)d.nray * FAN_SPLIT, h->ell_p);
     if (rc == CTR_OK) rc = ell_build(h, FanPixelHits{h->rays, h->views, h->win, h->win_ok}, (size_t)d.npix, h->ell_pt);
     return rc;
   }
@@ -487,8 +489,13 @@ static int fan_forward_v(ctr_handle* h, const float* img, float* out, int mode, 
 // batch == 1: the kernels above on the ABI arrays; batch > 1: slice-interleaved kernels of ctr_si.cu
 int fan_forward(ctr_handle* h, const float* img, float* out, int mode, const float* bs, cudaStream_t st) {
   if (h->d.V == 1 && h->ell_p.tab) {
+    const Dims& d = h->d;
     ProfScope prof(h, CTR_PROF_FORWARD, st);
-    return ell_forward<FAN_SPLIT>(h, h->ell_p, img, out, mode, bs, st);
+    if (h->ell_p_blk) {
+      k_to_blocked<<<(unsigned)((h->nimg + 255) / 256), 256, 0, st>>>(d.nx, d.ny, 1, img, h->imgT);
+      CTR_LAUNCHED(h);
+    }
+    return ell_forward<FAN_SPLIT>(h, h->ell_p, h->ell_p_blk ? h->imgT : img, out, mode, bs, st);
   }
   if (h->d.V == 1) return fan_forward_v<1, 1>(h, img, out, mode, bs, st);
   return si_forward(h, img, out, mode, bs, st);

@@ -40,8 +40,18 @@ __device__ __forceinline__ float fan_pixel_weight(const float4 R, float fi, floa
 
 // Row visitor of P: every non-zero (pixel index j nx + i, p_ij) of ray `row`, slab by slab, exactly the entries and
 // the order k_fan_forward adds them in (stored matrices: ctr_ell.cuh for single slices, k_si_forward_tab for batches).
-struct FanRayHits {  // rows of P: ray r = k nu + b; index = pixel j nx + i
+// Blocked copy of an image / volume for the gathers of the stored P of single problems (ctr_ell.cuh): 4 (y) x 8 (x)
+// tiles of 32 floats = one 128-byte line each, [z][ny/4][nx/8][4][8]. The threads of a warp gather from neighbouring
+// rays (3D) or from consecutive slabs of one ray (2D): in the row-major image that is one line per thread whenever
+// the neighbours differ in y, in the blocked copy a handful of lines for either orientation.
+__host__ __device__ __forceinline__ bool blk_ok(int nx, int ny) { return nx % 8 == 0 && ny % 4 == 0; }
+__device__ __forceinline__ int blk_index(int x, int y, int z, int nx, int ny) {
+  return (((z * (ny >> 2) + (y >> 2)) * (nx >> 3) + (x >> 3)) << 5) + ((y & 3) << 3) + (x & 7);
+}
+
+struct FanRayHits {  // rows of P: ray r = k nu + b; index = pixel j nx + i (blk != 0: blk_index of it)
   const float4* rays;
+  int blk = 0;
   template <class Visit>
   __device__ __forceinline__ void operator()(const Dims& d, size_t row, Visit visit) const {
     const float4 R = __ldg(&rays[row]);
@@ -67,8 +77,14 @@ struct FanRayHits {  // rows of P: ray r = k nu + b; index = pixel j nx + i
       const float ob = fmaf(m, y + 1.0f, x0);
       const SlabW w = slab_weights(oa, ob, L, K);
       const int ia = cell_of(w.ra) + c_oth, ib = cell_of(w.rb) + c_oth;
-      if (w.wa != 0.0f && (unsigned)ia < (unsigned)n_oth) visit(xdrv ? ia * d.nx + s : s * d.nx + ia, w.wa);
-      if (w.wb != 0.0f && (unsigned)ib < (unsigned)n_oth) visit(xdrv ? ib * d.nx + s : s * d.nx + ib, w.wb);
+      if (w.wa != 0.0f && (unsigned)ia < (unsigned)n_oth) {
+        const int px = xdrv ? s : ia, py = xdrv ? ia : s;
+        visit(blk ? blk_index(px, py, 0, d.nx, d.ny) : py * d.nx + px, w.wa);
+      }
+      if (w.wb != 0.0f && (unsigned)ib < (unsigned)n_oth) {
+        const int px = xdrv ? s : ib, py = xdrv ? ib : s;
+        visit(blk ? blk_index(px, py, 0, d.nx, d.ny) : py * d.nx + px, w.wb);
+      }
       oa = ob;
       y += 1.0f;
     }

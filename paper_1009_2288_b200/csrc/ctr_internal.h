@@ -132,6 +132,7 @@ struct ctr_handle {
   unsigned* rt_off;     // [nray] offset of the ray's entries in rt_tab
   size_t rt_bytes;
   ctr::EllTable ell_p, ell_pt;  // stored P (rows = rays) and P^T (rows = voxels), batch = 1 only; tab == NULL: on the fly
+  int ell_p_blk;                // stored P indexes the blocked copy of its input (blk_index, ctr_fan_geom.cuh), kept in imgT
   unsigned* cand;       // [Bp][cand_cap] candidate lists (bit patterns of N0^2 near the predicted sigma^2)
   unsigned cand_cap;
   float* usi;           // CGLS iterate in the slice-interleaved layout (batch > 1)
