@@ -270,6 +270,18 @@ def test_stored_matrices_equal_on_the_fly_kernels_3d(ctr, torch_cuda):
         h.close()
     assert np.array_equal(res[0][0], res[1][0])
     assert np.array_equal(res[0][1], res[1][1])
+    # nx % 8 == 0 and ny % 4 == 0: the stored P gathers from the blocked copy of the volume (blk_index): still the same bits
+    cfgb = small3d(nx=40, ny=36)
+    xb = rng.random((cfgb.nz, cfgb.ny, cfgb.nx)).astype(np.float32)
+    outs = []
+    for flags in (0, ctr.CTR_GEOM_NO_TABLES):
+        h = ctr.ctr_create(cfgb, flags=flags)
+        sino = torch.full(h.sino_shape, float("nan"), device="cuda")
+        h.ctr_forward(to_gpu(torch, xb), sino)
+        torch.cuda.synchronize()
+        outs.append(sino.cpu().numpy())
+        h.close()
+    assert np.array_equal(outs[0], outs[1])
 
 
 def test_eq11_backprojector_is_rejected_in_3d(ctr, torch_cuda):
