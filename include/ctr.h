@@ -43,7 +43,9 @@ typedef struct ctr_handle ctr_handle; /* opaque */
 typedef enum {
   CTR_OK = 0,
   CTR_EINVAL = -1, /* NULL / misaligned pointer, non-positive size, dsd <= dso, n_iter < 0, quantile not in (0,1] ... */
-  CTR_EGEOM = -2,  /* source or detector inside the image's circumscribed circle                                   */
+  CTR_EGEOM = -2,  /* source or detector inside the image's circumscribed circle; cone beam also: a ray that advances
+                      more than one voxel in z per in-plane voxel, or a voxel that sees more than 15 detector columns
+                      of a view (limits of the 3D kernels; text in ctr_last_error is not available: *out is NULL)   */
   CTR_ENOMEM = -3, /* device or host allocation failed                                                             */
   CTR_ECUDA = -4,  /* a CUDA runtime call failed; text in ctr_last_error                                           */
   CTR_EARCH = -5   /* current device is not compute capability 10.x (sm_100)                                       */

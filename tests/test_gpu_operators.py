@@ -1,6 +1,8 @@
 """GPU parity of the projector pair through the C ABI (ctr_forward / ctr_back) against the fp64
 oracle, element by element on the same seeded inputs. Tolerance (north_star): relative L2 <= 1e-5
 for one P or P^T application; adjoint identity <= 1e-5; the two kernels' matrices bit-identical."""
+import math
+
 import numpy as np
 import pytest
 
@@ -349,3 +351,48 @@ def test_arc_detector_and_explicit_angles(ctr, torch_cuda, orc, batch):
         assert_close(got_i[sl], orc.back(one, y[sl].astype(np.float64)), TOL_OP)
     # and the angles really were used: a uniform scan gives a different sinogram
     assert rel(gpu_forward(ctr, torch_cuda, base, x)[0], got_s[0].astype(np.float64)) > 1e-2
+
+
+def _random_geometry(rng, batch):
+    """A seeded random scanner: ragged sizes, anisotropic pixels, off-centre grid, shifted detector, either detector type,
+    source and detector outside the grid's circumscribed circle."""
+    nx, ny = int(rng.integers(1, 70)), int(rng.integers(1, 70))
+    dx, dy = float(rng.uniform(0.6, 2.0)), float(rng.uniform(0.6, 2.0))
+    cx, cy = float(rng.uniform(-3, 3)), float(rng.uniform(-3, 3))
+    rad = math.hypot(abs(cx) + 0.5 * nx * dx + dx, abs(cy) + 0.5 * ny * dy + dy)
+    dso = rad * float(rng.uniform(1.3, 6.0))
+    dsd = dso + rad * float(rng.uniform(1.3, 4.0))
+    return Config(name="fuzz", index=94, ndim=2, nx=nx, ny=ny, nz=1, dx=dx, dy=dy, dz=1.0,
+                  nviews=int(rng.integers(1, 40)), nu=int(rng.integers(1, 120)), nv=1,
+                  du=float(rng.uniform(0.5, 3.0)) * dsd / dso, dv=1.0, dso=dso, dsd=dsd, cx=cx, cy=cy,
+                  u_off=float(rng.uniform(-2, 2)), theta0=float(rng.uniform(0, 6.28)),
+                  det_type=int(rng.integers(0, 2)), batch=batch)
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_random_geometries_against_oracle(ctr, torch_cuda, orc, seed):
+    """Seeded random geometries and batch sizes (compute-sanitizer is closed on this pool: ragged sizes against the
+    oracle are the memory-safety net): P and P^T within 2e-5 of the oracle on rough random inputs (first and last slice),
+    tables against on-the-fly kernels, and the adjoint identity on the device."""
+    rng = np.random.default_rng(1000 + seed)
+    batch = int(rng.choice([1, 1, 2, 3, 5, 9, 17, 33]))
+    cfg = _random_geometry(rng, batch)
+    one = Config(**{**cfg.__dict__, "batch": 1})
+    x = rng.random((batch, cfg.ny, cfg.nx)).astype(np.float32)
+    y = rng.random((batch, cfg.nviews, cfg.nu)).astype(np.float32)
+    (s_tab, i_tab), (s_fly, i_fly) = _both_ways(ctr, torch_cuda, cfg, x, y)
+    for sl in sorted({0, batch - 1}):
+        want_s, want_i = orc.forward(one, x[sl].astype(np.float64)), orc.back(one, y[sl].astype(np.float64))
+        if np.linalg.norm(want_s) > 0:
+            assert_close(s_tab[sl], want_s, 2e-5)
+            assert_close(s_fly[sl], want_s, 2e-5)
+        else:
+            assert not s_tab[sl].any() and not s_fly[sl].any()
+        if np.linalg.norm(want_i) > 0:
+            assert_close(i_tab[sl], want_i, 2e-5)
+            assert_close(i_fly[sl], want_i, 2e-5)
+        else:
+            assert not i_tab[sl].any() and not i_fly[sl].any()
+    lhs = float((s_tab.astype(np.float64) * y).sum())
+    rhs = float((x.astype(np.float64) * i_tab).sum())
+    assert abs(lhs - rhs) <= 1e-5 * (np.linalg.norm(s_tab.astype(np.float64)) * np.linalg.norm(y.astype(np.float64)) + 1e-30)
