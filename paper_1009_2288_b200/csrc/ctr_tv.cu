@@ -339,6 +339,9 @@ __global__ void __launch_bounds__(256) k_tv_select(Scal sc, unsigned* __restrict
 #ifndef TV_FAST_SCAN
 #define TV_FAST_SCAN 1
 #endif
+#ifndef TV_SFMINB
+#define TV_SFMINB 5 /* min blocks per SM of k_tv_scan1f (c4 TV per outer iteration: 1.96 / 1.92 / 1.91 / 1.91 ms for 3 / 4 / 5 / 6) */
+#endif
 
 template <int V, int ND>
 __device__ __forceinline__ void own_face_values(const Dims& d, const Window<V, ND>& w, const int (&pos)[3],
@@ -448,7 +451,7 @@ __global__ void __launch_bounds__(256, TV_SMINB) k_tv_scan1(Dims d, int rows, co
 // k_tv_select_f takes the decision; a slice whose rank falls outside the window (or whose list overflowed) is a MISS,
 // and its group then runs the full k_tv_scan1 / k_tv_select pass: sigma is the exact order statistic either way.
 template <int V, int ND>
-__global__ void __launch_bounds__(256, TV_SMINB) k_tv_scan1f(Dims d, int rows, const float* __restrict__ f,
+__global__ void __launch_bounds__(256, TV_SFMINB) k_tv_scan1f(Dims d, int rows, const float* __restrict__ f,
                                                              unsigned* __restrict__ hist, Scal sc,
                                                              unsigned* __restrict__ cand, unsigned cap) {
   __shared__ unsigned cnt_s[V][4];
