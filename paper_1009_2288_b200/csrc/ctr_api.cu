@@ -285,7 +285,10 @@ int reduce_finish(ctr_handle* h, int mode, int N, int nblk, int i0, int nb, int 
 #ifndef CTR_LAZY_BLOCKS
 #define CTR_LAZY_BLOCKS 592 /* grid cap of the lazy-phase reduction kernels, 4 blocks per SM: their partials are finished by k_finish* (c4 vector work 1.85 / 1.82 / 2.11 ms for 1184 / 592 / 296) */
 #endif
-static_assert(CTR_LAZY_BLOCKS <= CTR_REDUCE_BLOCKS, "part2 is sized for CTR_REDUCE_BLOCKS blocks");
+#ifndef CTR_LAZY_V1
+#define CTR_LAZY_V1 4
+#endif
+static_assert(CTR_LAZY_BLOCKS <= CTR_REDUCE_BLOCKS && CTR_LAZY_V1 <= 16, "part2 is sized for CTR_REDUCE_BLOCKS blocks x 16 segments");
 // explicit phase, iteration m < CTR_MAX_BASIS: P b_m = (q - beta q_prev) / ||g'_m|| (first: q / ||g'_0||); q_prev <- q
 template <int V>
 __global__ void __launch_bounds__(256) k_sino_pb(size_t nl, int LQ, const float* __restrict__ q, float* __restrict__ qprev,
@@ -540,7 +543,8 @@ static dim3 sino_reduce_grid(const ctr_handle* h) {
   const Dims& d = h->d;
   const size_t nl = (size_t)d.nray * d.LQ;
   const unsigned want = (unsigned)((nl + 255) / 256);
-  unsigned cap = (unsigned)(CTR_LAZY_BLOCKS / d.GS);
+  // (a single problem loads 4 bytes per thread and stream where a batch loads 16: four times the blocks in flight)
+  unsigned cap = (unsigned)(CTR_LAZY_BLOCKS * (d.V == 1 ? CTR_LAZY_V1 : 1) / d.GS);
   if (cap < 1) cap = 1;
   return dim3(want < cap ? want : cap, d.GS);
 }
@@ -574,7 +578,7 @@ static int vec_direction_lazy(ctr_handle* h, const float* g, int nblk2, cudaStre
   const size_t nl = (size_t)d.npix * d.LQ;
   const int Bp = d.G * d.V;
   const unsigned want = (unsigned)((nl + 255) / 256);
-  unsigned ncap = (unsigned)(CTR_LAZY_BLOCKS / d.GS);
+  unsigned ncap = (unsigned)(CTR_LAZY_BLOCKS * (d.V == 1 ? CTR_LAZY_V1 : 1) / d.GS);
   if (ncap < 1) ncap = 1;
   dim3 grid(want, d.GS), ngrid(want < ncap ? want : ncap, d.GS), fgrid(d.LQ, d.GS);
   ProfScope prof(h, CTR_PROF_VECTOR, st);
