@@ -48,7 +48,8 @@ typedef enum {
                       of a view (limits of the 3D kernels; text in ctr_last_error is not available: *out is NULL)   */
   CTR_ENOMEM = -3, /* device or host allocation failed                                                             */
   CTR_ECUDA = -4,  /* a CUDA runtime call failed; text in ctr_last_error                                           */
-  CTR_EARCH = -5   /* current device is not compute capability 10.x (sm_100)                                       */
+  CTR_EARCH = -5,  /* current device is not compute capability 10.x (sm_100)                                       */
+  CTR_ETOOBIG = -6 /* ctr_forward_noalloc: the problem exceeds the fixed scratch (CTR_NOALLOC_MAX_* below)          */
 } ctr_status;
 
 /* Scanner + grid. Geometry of PAPER.md:85-89, :217 and App. III A6 (:484): at view angle th_k the source
@@ -132,6 +133,21 @@ int ctr_forward(ctr_handle* h, const float* d_img, float* d_sino, void* stream);
 /* a2: d_img = P^T d_sino, the exact transpose of ctr_forward's matrix (same p_ij, bit for bit), gather
  * form, no atomics (PAPER.md:193 explains why not scatter). d_img is overwritten. */
 int ctr_back(ctr_handle* h, const float* d_sino, float* d_img, void* stream);
+/* a1 for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): d_sino = P d_img for ONE 2D fan-beam slice (ndim 2, batch 1, angles NULL, flags 0), no handle needed.
+ * Same kernels and the same bits as ctr_forward on a handle created with CTR_GEOM_NO_TABLES. Calls no cudaMalloc,
+ * cudaFree or allocating library routine: the ray table and the transposed image copy live in one file-scope device
+ * array of CTR_NOALLOC_SCRATCH_BYTES (2.1 MiB) that every GPU which loads the library holds until the process
+ * exits. Limits: nx ny <= CTR_NOALLOC_MAX_PIXELS, nviews nu <= CTR_NOALLOC_MAX_RAYS, nviews <= CTR_NOALLOC_MAX_VIEWS
+ * (BASELINE.json's 512^2 / 60 x 888 slice fits exactly); anything larger returns CTR_ETOOBIG and enqueues nothing.
+ * EVERY call shares that array: calls that overlap on the GPU (different streams or host threads) race - serialise
+ * them. Asynchronous on `stream` like the other calls. The first call on a device looks the array's address up
+ * (cudaGetSymbolAddress): make it outside a stream capture. */
+#define CTR_NOALLOC_MAX_PIXELS (512 * 512)
+#define CTR_NOALLOC_MAX_RAYS 65536
+#define CTR_NOALLOC_MAX_VIEWS 4096
+#define CTR_NOALLOC_SCRATCH_BYTES (16 * CTR_NOALLOC_MAX_RAYS + 4 * CTR_NOALLOC_MAX_PIXELS + 24 * CTR_NOALLOC_MAX_VIEWS)
+int ctr_forward_noalloc(const ctr_geometry* g, const float* d_img, float* d_sino, void* stream);
 /* NEXT-1 (not on the hot path; ctr_cgls uses it only with ctr_params.backprojector = 1): the paper's own pixel-driven backprojector, Eq. (11)
  * (PAPER.md:195-197): d_img(u*,v*) = (dx dy / dbeta) sum_views y(beta*) / l, with y(beta*) linearly interpolated
  * between the two nearest detector units (0 outside the outermost unit centres) and l the source-pixel

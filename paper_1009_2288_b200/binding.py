@@ -14,7 +14,7 @@ import torch
 _LIB_PATH = Path(__file__).resolve().parent / "libctr.so"
 _lib = None
 
-CTR_OK, CTR_EINVAL, CTR_EGEOM, CTR_ENOMEM, CTR_ECUDA, CTR_EARCH = 0, -1, -2, -3, -4, -5
+CTR_OK, CTR_EINVAL, CTR_EGEOM, CTR_ENOMEM, CTR_ECUDA, CTR_EARCH, CTR_ETOOBIG = 0, -1, -2, -3, -4, -5, -6
 
 
 class CtrError(RuntimeError):
@@ -66,7 +66,7 @@ class ctr_peaks(C.Structure):
 EXPORTS = ["ctr_default_params", "ctr_create", "ctr_destroy", "ctr_forward", "ctr_back", "ctr_back_pixel", "ctr_cgls",
            "ctr_update_weights", "ctr_eptv_step", "ctr_reconstruct", "ctr_reconstruct_w",
            "ctr_set_params", "ctr_get_stats", "ctr_launch_count", "ctr_strerror", "ctr_last_error",
-           "ctr_profile_enable", "ctr_profile_read", "ctr_measure_peaks", "ctr_path_info"]
+           "ctr_profile_enable", "ctr_profile_read", "ctr_measure_peaks", "ctr_path_info", "ctr_forward_noalloc"]
 
 
 def load_library():
@@ -86,6 +86,7 @@ def load_library():
     L.ctr_destroy.restype = None
     L.ctr_forward.argtypes = [H, fp, fp, vp]
     L.ctr_back.argtypes = [H, fp, fp, vp]
+    L.ctr_forward_noalloc.argtypes = [C.POINTER(ctr_geometry), fp, fp, vp]
     L.ctr_back_pixel.argtypes = [H, fp, fp, vp]
     L.ctr_cgls.argtypes = [H, fp, fp, C.c_int, vp]
     L.ctr_update_weights.argtypes = [H, fp, fp, C.c_float, fp, vp]
@@ -267,6 +268,18 @@ def ctr_measure_peaks(reps: int = 5) -> dict:
     if rc != CTR_OK:
         raise CtrError(rc, "ctr_measure_peaks")
     return {n: getattr(pk, n) for n, _ in ctr_peaks._fields_ if n != "pad"}
+
+
+def ctr_forward_noalloc(geometry, img: torch.Tensor, sino: torch.Tensor) -> torch.Tensor:
+    """sino = P img for one 2D slice without a handle and without any allocation (include/ctr.h: fixed scratch,
+    CTR_ETOOBIG beyond 512 x 512 pixels / 65536 rays / 4096 views; overlapping calls race)."""
+    L = load_library()
+    cg = make_geometry(geometry)
+    n_img, n_sino = cg.nx * cg.ny, cg.nviews * cg.nu
+    rc = L.ctr_forward_noalloc(C.byref(cg), _ptr(img, n_img, "img"), _ptr(sino, n_sino, "sino"), _stream())
+    if rc != CTR_OK:
+        raise CtrError(rc, "ctr_forward_noalloc")
+    return sino
 
 
 def ctr_create(geometry, flags: int = 0) -> Handle:

@@ -765,6 +765,7 @@ const char* ctr_strerror(int status) {
     case CTR_ENOMEM: return "out of memory";
     case CTR_ECUDA: return "CUDA error";
     case CTR_EARCH: return "device is not sm_100 (B200)";
+    case CTR_ETOOBIG: return "problem exceeds the fixed scratch of ctr_forward_noalloc (max 512 x 512 pixels, 65536 rays, 4096 views)";
     default: return "unknown status";
   }
 }

@@ -528,3 +528,109 @@ int fan_back(ctr_handle* h, const float* sino, float* out, int mode, const float
 }
 
 }  // namespace ctr
+
+// =================================================================================================
+// ctr_forward_noalloc (include/ctr.h): sino = P img for ONE 2D fan-beam slice without a handle and without any
+// allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses
+// that forbid it). The kernels are the on-the-fly ones of ctr_forward (k_fan_build, k_transpose<1>, k_fan_forward<1,1,0>:
+// identical bits); what a handle would own - the ray table and the transposed copy of the image - lives in a file-scope
+// device array of fixed size, CTR_NOALLOC_SCRATCH_BYTES per GPU that loads the library, until the process exits.
+// Every call uses that one array: calls that overlap on the GPU (two streams, two host threads) race. Nothing in
+// it has to start at zero: each call overwrites rays[0, nray), views[0, nviews) and imgT[0, npix) before reading them.
+// =================================================================================================
+namespace {
+
+struct NoallocScratch {
+  float4 rays[CTR_NOALLOC_MAX_RAYS];      // ray table {x0, m, +-L, K}
+  float imgT[CTR_NOALLOC_MAX_PIXELS];     // transposed copy of the image
+  double2 viewsd[CTR_NOALLOC_MAX_VIEWS];  // (cos, sin) per view, written by k_fan_build
+  float2 views[CTR_NOALLOC_MAX_VIEWS];
+};
+static_assert(sizeof(NoallocScratch) <= CTR_NOALLOC_SCRATCH_BYTES, "CTR_NOALLOC_SCRATCH_BYTES in include/ctr.h is too small");
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[CTR_NOALLOC_SCRATCH_BYTES];
+
+// In host code `g_noalloc_scratch` is only a host-side stand-in for the symbol: its device address is looked up once
+// per device, with that device current, and cached here.
+constexpr int NOALLOC_MAX_DEVICES = 64;
+NoallocScratch* g_noalloc_ptr[NOALLOC_MAX_DEVICES];
+
+int noalloc_scratch(int dev, NoallocScratch** out) {
+  if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return CTR_ECUDA;
+  if (!g_noalloc_ptr[dev]) {
+    int major = 0;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) { cudaGetLastError(); return CTR_ECUDA; }
+    if (major != 10) return CTR_EARCH;
+    void* p = nullptr;
+    if (cudaGetSymbolAddress(&p, g_noalloc_scratch) != cudaSuccess || !p) { cudaGetLastError(); return CTR_ECUDA; }
+    g_noalloc_ptr[dev] = (NoallocScratch*)p;
+  }
+  *out = g_noalloc_ptr[dev];
+  return CTR_OK;
+}
+
+}  // namespace
+
+extern "C" int ctr_forward_noalloc(const ctr_geometry* g, const float* d_img, float* d_sino, void* stream) {
+  using namespace ctr;
+  if (!g || !d_img || !d_sino) return CTR_EINVAL;
+  if ((((uintptr_t)d_img) | ((uintptr_t)d_sino)) & 15u) return CTR_EINVAL;
+  if (g->ndim != 2 || g->nz != 1 || g->nv != 1 || g->batch != 1 || g->angles || g->flags) return CTR_EINVAL;
+  if (g->nx < 1 || g->ny < 1 || g->nviews < 1 || g->nu < 1) return CTR_EINVAL;
+  if (!(g->dx > 0) || !(g->dy > 0) || !(g->du > 0) || !(g->dso > 0) || !(g->dsd > g->dso)) return CTR_EINVAL;
+  if (g->det_type != 0 && g->det_type != 1) return CTR_EINVAL;
+  if ((long long)g->nx * g->ny > CTR_NOALLOC_MAX_PIXELS || (long long)g->nviews * g->nu > CTR_NOALLOC_MAX_RAYS ||
+      g->nviews > CTR_NOALLOC_MAX_VIEWS)
+    return CTR_ETOOBIG;
+  {
+    // same rule as ctr_create: source and detector outside the circle circumscribing the grid (plus one pixel)
+    const double hx = fabs((double)g->cx) + 0.5 * g->nx * (double)g->dx + g->dx;
+    const double hy = fabs((double)g->cy) + 0.5 * g->ny * (double)g->dy + g->dy;
+    const double rad = sqrt(hx * hx + hy * hy);
+    if (!(g->dso > rad) || !((double)g->dsd - g->dso > rad)) return CTR_EGEOM;
+  }
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return CTR_ECUDA; }
+  NoallocScratch* S = nullptr;
+  int rc = noalloc_scratch(dev, &S);
+  if (rc != CTR_OK) return rc;
+
+  // problem description, as ctr_create fills it for a single 2D slice
+  Dims d;
+  memset(&d, 0, sizeof(d));
+  d.ndim = 2;
+  d.nx = g->nx; d.ny = g->ny; d.nz = 1;
+  d.nviews = g->nviews; d.nu = g->nu; d.nv = 1;
+  d.c0x = g->nx / 2; d.c0y = g->ny / 2; d.c0z = 0;
+  d.npix = g->nx * g->ny;
+  d.nray = g->nviews * g->nu;
+  d.B = 1; d.V = 1; d.G = 1; d.GS = 1; d.LQ = 1;
+  d.nvp = (g->nviews + 15) / 16 * 16;
+  d.dx = g->dx; d.dy = g->dy; d.dz = 1.0f;
+  d.xlo = (float)((double)g->cx - g->nx * (double)g->dx / 2.0);
+  d.ylo = (float)((double)g->cy - g->ny * (double)g->dy / 2.0);
+  d.zlo = -0.5f;
+  d.dso = g->dso; d.dsd = g->dsd;
+  d.inv_du = 1.0f / g->du; d.inv_dv = 1.0f; d.dvz = 1.0f;
+  d.boff_u = (float)((g->nu - 1) / 2.0 - (double)g->u_off);
+  d.boff_v = 0.0f;
+  d.rvox = 0.5f * sqrtf(d.dx * d.dx + d.dy * d.dy);
+  d.det_type = g->det_type;
+  FanGeomD gd;
+  gd.dso = g->dso; gd.dsd = g->dsd; gd.du = g->du; gd.u_off = g->u_off;
+  gd.theta0 = g->theta0; gd.dtheta = g->dtheta;
+  gd.dx = g->dx; gd.dy = g->dy;
+  gd.xlo = (double)g->cx - g->nx * (double)g->dx / 2.0;
+  gd.ylo = (double)g->cy - g->ny * (double)g->dy / 2.0;
+  gd.nviews = g->nviews; gd.nu = g->nu; gd.c0x = d.c0x; gd.c0y = d.c0y; gd.det_type = g->det_type;
+
+  cudaStream_t st = (cudaStream_t)stream;
+  k_fan_build<<<(d.nray + 127) / 128, 128, 0, st>>>(gd, nullptr, S->rays, S->views, S->viewsd);
+  k_transpose<1><<<dim3((d.nx + 31) / 32, (d.ny + 31) / 32, 1), dim3(32, 8), 0, st>>>(d.nx, d.ny, d_img, S->imgT);
+  Scal none;
+  memset(&none, 0, sizeof(none));
+  k_fan_forward<1, 1, 0><<<dim3((d.nray + 127) / 128, 1), 128, 0, st>>>(d, S->rays, d_img, S->imgT, d_sino, nullptr, none,
+                                                                        nullptr, nullptr);
+  if (cudaPeekAtLastError() != cudaSuccess) { cudaGetLastError(); return CTR_ECUDA; }
+  return CTR_OK;
+}
