@@ -298,6 +298,19 @@ def main():
         }
         out["roofline"] = roofline(cfg, batch, prof, peaks, dev_peaks, path)
         out["hbm_bound_parts"] = hbm_kinds(cfg, batch, prof, peaks, K, dev_peaks)
+        # north_star's list of absolute numbers, derived from the same run (event-timed kinds; whole job = all ranks)
+        kms = out["kernel_ms_per_step"]
+        n_app, n_app_t = cfg.n_cgls + 1, max(cfg.n_cgls, 1)       # applications of P and of P^T per outer iteration (O4: the last P^T is skipped)
+        comp = 4.0 * batch * (cfg.nx * cfg.ny * cfg.nz + cfg.nviews * cfg.nu * cfg.nv)
+        cgls_ms = kms["forward"] + kms["back"] + kms["vector"]
+        out["north_star_numbers"] = {
+            "P_ms_per_application": kms["forward"] / n_app, "PT_ms_per_application": kms["back"] / n_app_t,
+            "P_compulsory_GBps": comp / (kms["forward"] / n_app * 1e-3) / 1e9 if kms["forward"] > 0 else None,
+            "PT_compulsory_GBps": comp / (kms["back"] / n_app_t * 1e-3) / 1e9 if kms["back"] > 0 else None,
+            "cgls_slice_iterations_per_s": world * batch * cfg.n_cgls / (cgls_ms * 1e-3) if cgls_ms > 0 else None,
+            "full_reconstructions_per_s": value / get_config(args.workload).n_outer,
+            "note": f"compulsory bytes = image + sinogram once per application; CGLS: {cfg.n_cgls} iterations per outer iteration over "
+                    f"forward + back + vector time; a full reconstruction = {get_config(args.workload).n_outer} outer iterations of every slice"}
         out["measured_peaks_this_run"] = dev_peaks
         out["kernel_path"] = path
         if not args.no_cpu_baseline:
