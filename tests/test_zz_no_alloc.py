@@ -57,7 +57,7 @@ def test_forward_noalloc_matches_ctr_forward_on_calls_in_a_row(ctr, torch_cuda, 
     for c, x, o in zip(cfgs, xs, outs):                         # four calls in a row on one stream, no sync in between:
         ctr.ctr_forward_noalloc(c, x, o)                        # each finds the scratch as the previous call left it
     torch.cuda.synchronize()
-    assert torch.cuda.mem_get_info()[0] == free0                # nothing was allocated on the device
+    assert torch.cuda.mem_get_info()[0] >= free0                # nothing was allocated on the device
     got = [o.cpu().numpy()[0] for o in outs]
     for c, x, g in zip(cfgs[:3], xs[:3], got[:3]):
         assert np.isfinite(g).all()
